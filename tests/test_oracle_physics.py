@@ -1,0 +1,325 @@
+"""More pins of the oracle: reflection, deposition closed forms, ledger, binning, schedule,
+compaction, boundaries."""
+import math
+
+import numpy as np
+import pytest
+from scipy import stats
+
+from helpers import T_I131, custom, uniform_met
+from oracle import oracle as orc
+from workloads import Grid, Nuclide, RainBox, Release, make
+
+
+# ------------------------------------------------------------------ P8 reflection
+def test_well_mixed_under_reflection():
+    """constant Kz, reflecting walls: a z-uniform cloud stays uniform; z in [0, H] always.
+    Catches a wrong fold (e.g. z = H - (z - H) written as z = H + ...)."""
+    H, N = 400.0, 20_000
+    w = custom(uniform_met(kz=50.0), H=H, dt=10.0, n=0, n_steps=30, seed=3)
+    sim = orc.OracleSim(w)
+    rng = np.random.default_rng(5)
+    z0 = rng.uniform(0, H, N)
+    sim.set_particles(np.zeros(N), np.zeros(N), z0, [np.ones(N)], pid=np.arange(N))
+    sim.step(30)
+    z = sim.particles()["z"]
+    assert z.min() >= 0.0 and z.max() <= H
+    hist, _ = np.histogram(z, bins=20, range=(0, H))
+    assert stats.chisquare(hist).pvalue > 1e-3
+
+
+def test_reflection_single_cases():
+    """z' = -z' below ground; z' = 2H - z' above H (R6): hand-computed from the worked normal n2."""
+    n2 = orc.normals(1, 7, 3)[2]           # 1.119952999 (pinned in test_worked_uniforms_normals)
+    for z_old, H in ((2.0, 1000.0), (995.0, 1000.0)):
+        w = custom(uniform_met(kz=5.0), H=H, dt=10.0, n=0, seed=1)
+        for sign_pid in (7,):
+            sim = orc.OracleSim(w)
+            sim.set_particles([0.0], [0.0], [z_old], [[1.0]], pid=[sign_pid])
+            sim.set_step_index(3)
+            sim.step(1)
+            z_free = z_old + 10.0 * n2
+            want = 2 * H - z_free if z_free > H else abs(z_free)
+            assert abs(sim.particles()["z"][0] - want) < 1e-9
+    # downward case: find a (pid, step) with a strongly negative n2
+    for pid in range(200):
+        n2 = orc.normals(1, pid, 0)[2]
+        if n2 < -1.0:
+            break
+    w = custom(uniform_met(kz=5.0), H=1000.0, dt=10.0, n=0, seed=1)
+    sim = orc.OracleSim(w)
+    sim.set_particles([0.0], [0.0], [3.0], [[1.0]], pid=[pid])
+    sim.step(1)
+    assert abs(sim.particles()["z"][0] - (-(3.0 + 10.0 * n2))) < 1e-9
+
+
+def test_kz_floor():
+    """Kz <- max(Kz, kz_min) (R4): with field Kz = 0 the vertical spread is set by kz_min."""
+    N = 20_000
+    w = custom(uniform_met(kz=0.0), kz_min=2.0, H=1.0e9, dt=5.0, n=N, n_steps=1, src=(0, 0, 1.0e6))
+    sim = orc.OracleSim(w)
+    sim.step(1)
+    z = sim.particles()["z"] - 1.0e6
+    assert abs(z.var() / (2 * 2.0 * 5.0) - 1.0) < 4.0 * math.sqrt(2.0 / N)
+
+
+# ------------------------------------------------------------------ P10 / P11 deposition closed forms
+def test_dry_deposition_closed_form():
+    """uniform dry deposition (h_dep >= H): airborne = m0 (f_d f_l)^n, deposited = m0 p_d (1-(f_d f_l)^n)/(1-f_d f_l)."""
+    H, dt, n, vd = 500.0, 10.0, 60, 2.0e-2
+    g = Grid(8, 8, 4, -4000.0, -4000.0, 0.0, 1000.0, 1000.0, 125.0)
+    w = custom(uniform_met(kz=1.0), grid=g, H=H, Kh=1.0, dt=dt, n=50, n_steps=n,
+               nuclides=[Nuclide("I", T_I131, vd=vd)], activity=[50.0])
+    sim = orc.OracleSim(w)
+    sim.step(n)
+    p_d = float(np.float32(-math.expm1(-vd * dt / H)))
+    assert sim.p_dry(0) == p_d
+    f = (1.0 - p_d) * math.exp(-math.log(2) * dt / T_I131)
+    led = sim.ledger()[0]
+    assert abs(led[1] / (50.0 * f ** n) - 1) < 1e-12
+    dep_total = 50.0 * p_d * (1 - f ** n) / (1 - f)
+    assert abs(led[2] / dep_total - 1) < 1e-12
+    dep = sim.deposition()
+    assert abs(dep.sum() * g.dx * g.dy / dep_total - 1) < 1e-12
+    assert abs(led[0] - (led[1] + led[2] + led[3] + led[4] + led[5])) < 1e-12 * led[0]
+
+
+def test_dry_deposition_layer_threshold():
+    """h_dep < H: only particles with z' < h_dep deposit (PAPER.md L84-86 eligibility)."""
+    H, dt, vd, hd = 1000.0, 10.0, 1.0e-2, 80.0
+    w = custom(uniform_met(), H=H, dt=dt, n=0, n_steps=1, h_dep=hd, nuclides=[Nuclide("I", 0.0, vd=vd)])
+    sim = orc.OracleSim(w)
+    sim.set_particles([0.0, 0.0], [0.0, 0.0], [79.0, 81.0], [[1.0, 1.0]], pid=[0, 1])
+    sim.step(1)
+    m = sim.particles()["m"][0]
+    p_d = float(np.float32(-math.expm1(-vd * dt / hd)))
+    assert m[0] == 1.0 - p_d and m[1] == 1.0
+
+
+def test_wet_deposition_box_and_time():
+    """rain covering the domain for n_r steps adds a factor (1-p_w)^n_r (P11); outside the box or
+    outside the time window nothing is scavenged; dry is applied before wet (R8)."""
+    dt, lam, vd, H = 10.0, 1.0e-3, 1.0e-2, 500.0
+    rain = RainBox(-100.0, 100.0, -100.0, 100.0, 20.0, 50.0)     # steps 2, 3, 4
+    w = custom(uniform_met(), H=H, dt=dt, n=0, n_steps=8, rain=rain,
+               nuclides=[Nuclide("I", 0.0, vd=vd, lambda_wet=lam)])
+    sim = orc.OracleSim(w)
+    sim.set_particles([0.0, 500.0], [0.0, 0.0], [10.0, 10.0], [[1.0, 1.0]], pid=[0, 1])
+    sim.step(8)
+    m = sim.particles()["m"][0]
+    p_w = float(np.float32(-math.expm1(-lam * dt)))
+    p_d = float(np.float32(-math.expm1(-vd * dt / H)))
+    assert abs(m[0] / ((1 - p_d) ** 8 * (1 - p_w) ** 3) - 1) < 1e-13
+    assert abs(m[1] / ((1 - p_d) ** 8) - 1) < 1e-13
+    led = sim.ledger()[0]
+    # wet removes from what is left after dry in the same step
+    wet_expected = sum(((1 - p_d) * (1 - p_w)) ** j * (1 - p_d) ** 2 * (1 - p_d) * p_w for j in range(3))
+    assert abs(led[3] / wet_expected - 1) < 1e-12
+    assert abs(2.0 - (led[1] + led[2] + led[3] + led[4] + led[5])) < 1e-13
+
+
+# ------------------------------------------------------------------ P6 ledger on a full config
+def test_ledger_conservation_c3_small():
+    w = make("c3", scale=2e-4, n_steps=2400)      # 2000 particles, through the start of the rain
+    sim = orc.OracleSim(w)
+    sim.step(2400)
+    led = sim.ledger()
+    for k in range(2):
+        tot = led[k][1] + led[k][2] + led[k][3] + led[k][4] + led[k][5]
+        assert abs(tot / led[k][0] - 1) < 1e-12
+    assert led[0][3] > 0 and led[1][2] > led[0][2] * 0.1    # wet happened; Cs (vd 2e-3, 1e14) vs I
+    dep = sim.deposition()
+    g = w.cgrid
+    for k in range(2):
+        on_grid = dep[k].sum() * g.dx * g.dy
+        assert abs((on_grid + led[k][6]) / (led[k][2] + led[k][3]) - 1) < 1e-12
+
+
+# ------------------------------------------------------------------ P9 binning
+def test_binning_brute_force_and_faces():
+    g = Grid(5, 4, 3, -10.0, 0.0, 0.0, 4.0, 5.0, 10.0)
+    w = custom(uniform_met(), grid=g, n=0)
+    sim = orc.OracleSim(w)
+    rng = np.random.default_rng(2)
+    N = 1000
+    x = rng.uniform(-14, 14, N).astype(np.float32).astype(np.float64)
+    y = rng.uniform(-3, 23, N).astype(np.float32).astype(np.float64)
+    z = rng.uniform(-2, 33, N).astype(np.float32).astype(np.float64)
+    # exact face / edge cases: on a face -> upper cell; x = x0 + nx dx is outside; x = x0 is inside
+    x[:4] = [-10.0, 10.0, -6.0, 9.999999]
+    y[:4] = [2.5, 2.5, 5.0, 19.999998]
+    z[:4] = [0.0, 5.0, 10.0, 29.999998]
+    m = rng.uniform(0.5, 1.5, N)
+    st = (rng.uniform(size=N) < 0.1).astype(np.uint8)
+    st[:4] = 0
+    sim.set_particles(x, y, z, [m], pid=np.arange(N), status=st)
+    sim.bin_now()
+    cnt = np.zeros(g.shape, dtype=np.int64)
+    s = np.zeros(g.shape)
+    for i in range(N):
+        if st[i]:
+            continue
+        # R10: the cell is DEFINED by the fp32 expression floorf((x - x0) * (float)(1/dx))
+        f32 = np.float32
+        ci = math.floor((f32(x[i]) - f32(-10.0)) * f32(1.0 / 4.0))
+        cj = math.floor((f32(y[i]) - f32(0.0)) * f32(1.0 / 5.0))
+        ck = math.floor((f32(z[i]) - f32(0.0)) * f32(1.0 / 10.0))
+        if 0 <= ci < 5 and 0 <= cj < 4 and 0 <= ck < 3:
+            cnt[ck, cj, ci] += 1
+            s[ck, cj, ci] += m[i]
+    np.testing.assert_array_equal(sim.counts(), cnt)
+    np.testing.assert_allclose(sim.concentration()[0], s / (4.0 * 5.0 * 10.0), rtol=1e-13)
+    assert cnt[0, 0, 0] >= 1 and sim.counts()[1, 1, 1] >= 1      # (-10,2.5,0) and (-6,5,10)
+    assert orc.cell_index(10.0, -10.0, 4.0, 5) == -1 and orc.cell_index(-10.0, -10.0, 4.0, 5) == 0
+    assert orc.cell_index(-6.0, -10.0, 4.0, 5) == 1 and orc.cell_index(-10.000001, -10.0, 4.0, 5) == -1
+    # permutation invariance of the counts
+    perm = rng.permutation(N)
+    sim.set_particles(x[perm], y[perm], z[perm], [m[perm]], pid=np.arange(N), status=st[perm])
+    sim.bin_now()
+    np.testing.assert_array_equal(sim.counts(), cnt)
+
+
+# ------------------------------------------------------------------ P13 schedule
+def test_release_schedule_count_mode():
+    """b_j = s_start + floor(j S / N): monotone, sums to N, births per step differ by at most 1."""
+    N, S = 1000, 7
+    w = custom(uniform_met(), n=N, dt=10.0, t_rel=(20.0, 20.0 + S * 10.0), n_steps=12)
+    sim = orc.OracleSim(w)
+    counts = []
+    for s in range(12):
+        sim.step(1)
+        counts.append(sim.injected(s))
+    assert counts[:2] == [0, 0] and sum(counts) == N and counts[9:] == [0, 0, 0]
+    want = [sum(1 for j in range(N) if 2 + (j * S) // N == s) for s in range(12)]
+    assert counts == want
+    assert list(sim.particles()["pid"]) == list(range(N))
+    led = sim.ledger()[0]
+    assert abs(led[0] - 1.0) < 1e-12          # activity scaled to the particle count
+
+
+def test_release_strided_subsample_is_exact_subset():
+    """pid_stride / pid_offset pick a subset whose trajectories equal those of the full run."""
+    kw = dict(Kh=10.0, H=500.0, dt=10.0, n=300, t_rel=(0.0, 100.0), n_steps=15, seed=9)
+    full = orc.OracleSim(custom(uniform_met(u=1.0, kz=3.0), **kw))
+    sub = orc.OracleSim(custom(uniform_met(u=1.0, kz=3.0), pid_offset=3, pid_stride=10, **kw))
+    full.step(15)
+    sub.step(15)
+    pf, ps = full.particles(), sub.particles()
+    assert list(ps["pid"]) == list(range(3, 300, 10))
+    idx = ps["pid"].astype(int)
+    for key in ("x", "y", "z"):
+        np.testing.assert_array_equal(ps[key], pf[key][idx])
+    np.testing.assert_array_equal(ps["m"][0], pf["m"][0][idx])
+
+
+def test_rate_mode_capacity_and_compaction():
+    """rate mode: c slots per step, pid = step*c + j; short capacity skips the highest j (R9);
+    ABSORB + compaction keeps pids strictly increasing and equals a brute-force filter (P12)."""
+    g = Grid(10, 10, 4, -500.0, -500.0, 0.0, 100.0, 100.0, 100.0)
+    kw = dict(grid=g, Kh=400.0, H=400.0, dt=10.0, rate=2.0, t_rel=(0.0, 400.0), n_steps=40, seed=4,
+              boundary="absorb", src=(300.0, 0.0, 50.0))
+    a = orc.OracleSim(custom(uniform_met(u=8.0, kz=2.0), compact=True, capacity=150, **kw))
+    b = orc.OracleSim(custom(uniform_met(u=8.0, kz=2.0), compact=False, capacity=10_000, **kw))
+    throttled = False
+    for s in range(40):
+        a.step(1)
+        b.step(1)
+        throttled |= a.injected(s) < 20
+        pa, pb = a.particles(), b.particles()
+        assert np.all(np.diff(pa["pid"].astype(np.int64)) > 0)
+        assert np.all(pa["status"] == 0) and a.n <= 150
+        if not throttled:
+            alive = pb["status"] == 0
+            np.testing.assert_array_equal(pa["pid"], pb["pid"][alive])
+            np.testing.assert_array_equal(pa["x"], pb["x"][alive])
+    assert (b.particles()["status"] == 1).sum() > 50       # exits really happened
+    led = a.ledger()[0]
+    assert abs((led[1] + led[2] + led[3] + led[4] + led[5]) / led[0] - 1) < 1e-12 and led[5] > 0
+    # throttle: tiny capacity
+    c = orc.OracleSim(custom(uniform_met(), compact=True, capacity=35, grid=g, rate=2.0, dt=10.0,
+                             t_rel=(0.0, 400.0), n_steps=3, boundary="absorb"))
+    c.step(3)
+    assert [c.injected(s) for s in range(3)] == [20, 15, 0]
+    assert list(c.particles()["pid"]) == list(range(20)) + list(range(20, 35))
+
+
+def test_absorb_boundary_is_met_box():
+    g = Grid(10, 10, 4, -500.0, -500.0, 0.0, 100.0, 100.0, 100.0)
+    w = custom(uniform_met(u=10.0), grid=g, dt=10.0, n=0, boundary="absorb")
+    sim = orc.OracleSim(w)
+    sim.set_particles([250.0, 399.0, 400.0], [0.0, 0.0, 0.0], [50.0] * 3, [[1.0, 2.0, 4.0]], pid=[0, 1, 2])
+    sim.step(1)
+    st = sim.particles()["status"]
+    assert list(st) == [0, 0, 1]          # 350, 499 inside; 500 = x0 + nx dx is outside
+    assert sim.ledger()[0][5] == 4.0
+    sim.step(1)
+    assert list(sim.particles()["status"]) == [0, 1, 1] and sim.particles()["x"][2] == 500.0   # exited: never moved again
+
+
+# ------------------------------------------------------------------ P14 independent numpy trace
+def _philox_np(ctr, key):
+    M0, M1, W0, W1 = 0xD2511F53, 0xCD9E8D57, 0x9E3779B9, 0xBB67AE85
+    c, k = [int(v) for v in ctr], [int(v) for v in key]
+    for _ in range(10):
+        p0, p1 = M0 * c[0], M1 * c[2]
+        c = [((p1 >> 32) ^ c[1] ^ k[0]) & 0xFFFFFFFF, p1 & 0xFFFFFFFF, ((p0 >> 32) ^ c[3] ^ k[1]) & 0xFFFFFFFF, p0 & 0xFFFFFFFF]
+        k = [(k[0] + W0) & 0xFFFFFFFF, (k[1] + W1) & 0xFFFFFFFF]
+    return c
+
+
+def test_brute_force_trace_c2_tiny():
+    """independent scalar python loop (scipy map_coordinates for the sampling, python Philox) over a
+    few particles and steps of config 2 (time-varying, z-dependent field, reflection, decay)."""
+    from scipy import ndimage
+    w = make("c2", scale=2e-5, n_steps=40)          # 20 particles
+    sim = orc.OracleSim(w)
+    sim.step(40)
+    p = sim.particles()
+    f = w.fields().astype(np.float64)
+    g = w.mgrid
+    N = w.release.n_particles
+    S = 720
+    sig_h = float(np.float32(math.sqrt(2 * w.Kh * w.dt)))
+    for j in range(N):
+        b = (j * S) // N
+        if b >= 40:
+            assert j >= sim.n
+            continue
+        x, y, z, m = 0.0, 0.0, 50.0, 6.0e9 / N
+        for n in range(b, 40):
+            t = n * w.dt
+            s = min(max(int(math.floor(t / 3600.0)), 0), w.nt - 2)
+            a = float(np.float32(min(max((t - s * 3600.0) / 3600.0, 0.0), 1.0)))
+            r = _philox_np([n, 0, j, 0], [w.seed, 0])
+            u1, u2, u3, u4 = ((r[0] >> 8) + 1) / 2 ** 24, (r[1] >> 8) / 2 ** 24, ((r[2] >> 8) + 1) / 2 ** 24, (r[3] >> 8) / 2 ** 24
+            R1, R2 = math.sqrt(-2 * math.log(u1)), math.sqrt(-2 * math.log(u3))
+            n0, n1, n2 = R1 * math.cos(2 * math.pi * u2), R1 * math.sin(2 * math.pi * u2), R2 * math.cos(2 * math.pi * u4)
+            co = [[(z - g.z0) / g.dz - 0.5], [(y - g.y0) / g.dy - 0.5], [(x - g.x0) / g.dx - 0.5]]
+            met = [(1 - a) * ndimage.map_coordinates(f[s, ..., c], co, order=1, mode="nearest")[0]
+                   + a * ndimage.map_coordinates(f[s + 1, ..., c], co, order=1, mode="nearest")[0] for c in range(4)]
+            kz = max(met[3], w.kz_min)
+            x += met[0] * w.dt + sig_h * n0
+            y += met[1] * w.dt + sig_h * n1
+            z += met[2] * w.dt + math.sqrt(2 * kz * w.dt) * n2
+            if z < 0:
+                z = -z
+            if z > w.H_mix:
+                z = 2 * w.H_mix - z
+            m *= math.exp(-math.log(2) * w.dt / T_I131)
+        assert abs(p["x"][j] - x) < 1e-8 and abs(p["y"][j] - y) < 1e-8 and abs(p["z"][j] - z) < 1e-8
+        assert abs(p["m"][0][j] / m - 1) < 1e-13
+
+
+def test_oracle_deterministic_across_thread_counts():
+    w = make("c3", scale=1e-4, n_steps=200)
+    res = []
+    for nt in (1, 4):
+        orc.set_num_threads(nt)
+        sim = orc.OracleSim(w)
+        sim.step(200)
+        res.append((sim.particles(), sim.deposition(), sim.ledger()))
+    orc.set_num_threads(orc.num_threads())
+    for key in ("x", "y", "z", "m"):
+        np.testing.assert_array_equal(res[0][0][key], res[1][0][key])
+    np.testing.assert_array_equal(res[0][1], res[1][1])
+    np.testing.assert_array_equal(res[0][2], res[1][2])
