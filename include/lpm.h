@@ -1,0 +1,208 @@
+/* lpm.h — C ABI of the B200-native Lagrangian particle step + binning library.
+ *
+ * The hot path of arxiv/paper_0912_3223 (Molnar, Szakaly, Meszaros, Lagzi: "Air pollution
+ * modelling using a Graphics Processing Unit with CUDA"), cited below as P:Lnn = PAPER.md line nn:
+ * point source releasing particles with assigned activity every time step, each step per
+ * particle = linear sampling of gridded weather in x, y, z and time -> turbulent diffusion
+ * coefficient -> move by wind -> move by turbulent diffusion -> dry / wet deposition test ->
+ * inactive at the boundary (Eq.(1)(2)), radioactive decay from the half-life
+ * (P:L84), and the summation of particle activity on a rectangular grid every n-th step.
+ * Readings of everything the paper leaves open: DESIGN.md §3 (R1..R10).
+ *
+ * Conventions
+ *  - Every function returns int32_t: LPM_OK (0) or a negative lpm_status.  No exceptions, no C++
+ *    types, no torch types cross this boundary.
+ *  - Pointers named *_dev are DEVICE pointers (cudaMalloc / torch CUDA tensors); *_host are host
+ *    pointers; small structs are host structs copied at the call.
+ *  - OWNERSHIP: the caller owns every device buffer (workspace, met snapshots, outputs).  The
+ *    library borrows `workspace_dev` and `meteo.fields_dev` for the life of the handle and never
+ *    frees caller memory.
+ *  - One handle = one GPU = one CUDA stream.  Calls enqueue work on that stream and return; calls
+ *    that return host scalars (lpm_num_active, lpm_ledger, lpm_get_particles' count) synchronise
+ *    the stream first.  A handle is not thread-safe.
+ *  - There is NO CPU fallback: without an sm_100 device lpm_create returns LPM_ERR_NO_DEVICE.
+ *  - Units: SI (m, s, Bq).  Grids are x-fastest: index = (k*ny + j)*nx + i.
+ */
+#ifndef LPM_H_
+#define LPM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LPM_MAX_NUCLIDES 2
+#define LPM_LEDGER_FIELDS 7 /* emitted, airborne, dry, wet, decayed, exited, dep_offgrid */
+#define LPM_MAX_RELEASES 8
+
+typedef enum {
+    LPM_OK = 0,
+    LPM_ERR_INVALID_ARG = -1,
+    LPM_ERR_NO_DEVICE = -2,          /* no sm_100 CUDA device; there is no CPU fallback       */
+    LPM_ERR_WORKSPACE_TOO_SMALL = -3,
+    LPM_ERR_CAPACITY = -4,           /* a release does not fit into params.capacity           */
+    LPM_ERR_STATE = -5,              /* call order (e.g. release registered after its start)  */
+    LPM_ERR_CUDA = -6                /* sticky; text via lpm_last_error                       */
+} lpm_status;
+
+typedef enum { LPM_BOUNDARY_OPEN = 0, LPM_BOUNDARY_ABSORB = 1 } lpm_boundary_mode;
+
+/* Regular grid of nx*ny*nz cells of size dx*dy*dz with lower corner (x0, y0, z0). */
+typedef struct {
+    int32_t nx, ny, nz, reserved;
+    double x0, y0, z0, dx, dy, dz;
+} lpm_grid;
+
+/* Meteorology: nt snapshots at t0 + s*dt_snap, each nz*ny*nx cell-centred texels
+ * float4 = (u, v, w, Kz) [m/s, m/s, m/s, m^2/s], layout [nt][nz][ny][nx], x fastest, 16-byte
+ * aligned.  Sampling is trilinear in space, linear in time, edge-clamped (R4).  Kh: constant
+ * horizontal diffusivity.  H_mix: reflecting lid (R6).  kz_min: floor on the sampled Kz. */
+typedef struct {
+    lpm_grid grid;
+    int32_t nt, reserved;
+    double t0, dt_snap;
+    const void *fields_dev;
+    double Kh, H_mix, kz_min;
+} lpm_meteo;
+
+/* Isotope constants. half_life_s <= 0 means stable. */
+typedef struct {
+    double half_life_s;
+    double vd;         /* dry deposition velocity, m/s  */
+    double lambda_wet; /* wet scavenging coefficient, 1/s */
+} lpm_nuclide;
+
+typedef struct {
+    double dt;              /* time step, s (10 s)                                       */
+    uint64_t seed;          /* Philox key (R1)                                                  */
+    uint64_t capacity;      /* maximum number of particle slots                        */
+    int32_t boundary_mode;  /* lpm_boundary_mode; the boundary is the met-grid box (R7)         */
+    int32_t compact;        /* 1: stable stream compaction of exited particles after every step */
+    double h_dep;           /* dry deposition acts where z' < h_dep; h_dep >= H_mix: everywhere */
+    int32_t bin_every;      /* concentration binning cadence in steps ("n"); 0 = never   */
+    int32_t steps_per_launch; /* 0 = auto; 1 = one model step per kernel launch; m > 1 fuses up to
+                               * m steps per launch with the particle state kept in registers   */
+} lpm_params;
+
+typedef struct {
+    double x, y, z;         /* source point ("single point source")                       */
+    double t_start, t_end;  /* release interval; first step ceil(t_start/dt), over
+                             * max(1, ceil((t_end - t_start)/dt)) steps (R9)                     */
+} lpm_source;
+
+typedef struct lpm_handle lpm_handle;
+
+/* ---- host-only entry points (usable without a GPU) --------------------------------------- */
+
+/* Library version: major*10000 + minor*100 + patch. */
+int32_t lpm_version(void);
+
+/* Static text for a status code. */
+const char *lpm_status_string(int32_t status);
+
+/* Bytes of device workspace lpm_create needs (particle SoA store, grids, ledger, scan state). */
+int32_t lpm_workspace_bytes(const lpm_grid *conc_grid, const lpm_params *params, int32_t n_nuclides,
+                            uint64_t *bytes_host);
+
+/* R9 release schedule, count mode: how many of the LOCAL particles (global ids pid_offset +
+ * l*pid_stride < n_particles) are born at steps <= step, for a release starting at step s_start
+ * and lasting S steps: global particle j is born at s_start + floor(j*S/n_particles). */
+int32_t lpm_schedule_born(uint64_t n_particles, uint64_t pid_offset, uint64_t pid_stride,
+                          int64_t s_start, int64_t S, int64_t step, uint64_t *born_host);
+
+/* ---- life cycle ---------------------------------------------------------------------------- */
+
+/* Create a simulation.  `conc_grid` is the 3-D concentration grid; the 2-D deposition map is its
+ * (x, y) footprint.  `cuda_stream` is a cudaStream_t (NULL = default stream).  The workspace is
+ * zeroed (asynchronously).  Errors: INVALID_ARG (null pointers, n_nuclides not in 1..2,
+ * non-positive sizes, misaligned buffers), NO_DEVICE, WORKSPACE_TOO_SMALL, CUDA. */
+int32_t lpm_create(const lpm_grid *conc_grid, const lpm_meteo *meteo, const lpm_nuclide *nuclides,
+                   int32_t n_nuclides, const lpm_params *params, void *workspace_dev,
+                   uint64_t workspace_bytes, void *cuda_stream, lpm_handle **out);
+
+int32_t lpm_destroy(lpm_handle *h);
+
+/* Axis-aligned rain box over the full column, active for t_start <= t_n < t_end, tested at the
+ * start of the step ("wet deposition only occurs in case of precipitation"; G6). */
+int32_t lpm_set_rain(lpm_handle *h, double x0, double x1, double y0, double y1, double t_start,
+                     double t_end);
+
+/* Register a release.  total_activity_host[k] is the activity of nuclide k
+ * emitted over the whole release, split evenly over the particles.  Count mode (n_particles > 0):
+ * particle j of n_particles is born at step s_start + floor(j*S/n_particles); only the ids
+ * pid_offset + l*pid_stride are simulated (pid-strided subsample / multi-GPU shard), each still
+ * carrying total/n_particles.  Rate mode (n_particles == 0): c = round(particles_per_s*dt) slots
+ * per step, pid = pid_offset + (step - s_start)*c + j; when capacity is short the highest j are
+ * skipped (never renumbered); pid_stride must be 1.  Particle ids must stay below 2^32.
+ * Errors: CAPACITY, STATE (release starts before the current step), INVALID_ARG. */
+int32_t lpm_release(lpm_handle *h, const lpm_source *src, const double *total_activity_host,
+                    uint64_t n_particles, double particles_per_s, uint64_t pid_offset,
+                    uint64_t pid_stride);
+
+/* Advance n_steps model steps.  Every params.bin_every-th step the concentration
+ * grid is re-binned from the particle state. */
+int32_t lpm_step(lpm_handle *h, int32_t n_steps);
+
+/* ---- outputs -------------------------------------------------------------------------------- */
+
+/* Concentration in Bq m^-3, float [K][nz][ny][nx], of the particle state at the current step
+ * (re-bins first if the internal grid is stale). */
+int32_t lpm_concentration(lpm_handle *h, float *out_dev);
+/* Particle counts per cell, uint32 [nz][ny][nx], same snapshot rule. */
+int32_t lpm_counts(lpm_handle *h, uint32_t *out_dev);
+/* Cumulative deposited activity in Bq m^-2, float [K][ny][nx] (not decayed on the ground). */
+int32_t lpm_deposition(lpm_handle *h, float *out_dev);
+/* Same map at full precision, double [K][ny][nx] (the accumulator itself, scaled by 1/area). */
+int32_t lpm_deposition_f64(lpm_handle *h, double *out_dev);
+
+/* ---- test hooks / checkpoint ---------------------------------------------------------------- */
+
+/* Re-bin the current particle state into the internal grids now. */
+int32_t lpm_bin_now(lpm_handle *h);
+/* Number of particle slots in use (born, minus compacted-out). Synchronises. */
+int32_t lpm_num_active(lpm_handle *h, uint64_t *n_host);
+int32_t lpm_step_index(lpm_handle *h, uint64_t *step_host);
+/* The activity of a particle is q * scale[k]: q is the stored fp32 value, scale[k] =
+ * G_k(t) the host-side fp64 decay (and uniform dry-deposition) factor at the current step (R8). */
+int32_t lpm_mass_scale(lpm_handle *h, double *scale_host /* [K] */);
+/* Copy out the particle state: xyzq_dev float4 (x, y, z, q0) per slot, q1_dev (K = 2, may be
+ * NULL), pid_dev uint32 (may be NULL), status_dev uint8 0 = active, 1 = exited (may be NULL).
+ * Buffers must hold capacity entries; *n_host receives the slot count.  Exited particles report
+ * their exit position. */
+int32_t lpm_get_particles(lpm_handle *h, void *xyzq_dev, float *q1_dev, uint32_t *pid_dev,
+                          uint8_t *status_dev, uint64_t *n_host);
+/* Replace the particle state by n slots (all treated as already born; pid_dev NULL = 0..n-1;
+ * status_dev NULL = all active) and set the step index.  Registered releases keep running only
+ * in compact mode (append); in slot-addressed mode they are dropped. */
+int32_t lpm_set_particles(lpm_handle *h, const void *xyzq_dev, const float *q1_dev,
+                          const uint32_t *pid_dev, const uint8_t *status_dev, uint64_t n,
+                          uint64_t step_index);
+/* Mass ledger, double [K][LPM_LEDGER_FIELDS]: emitted, airborne, dry, wet, decayed, exited,
+ * dep_offgrid (the part of dry+wet that fell outside the map).  emitted = airborne + dry + wet +
+ * decayed + exited up to fp32 rounding.  Synchronises. */
+int32_t lpm_ledger(lpm_handle *h, double *out_host);
+/* Particles injected at `step` (rate mode log; 0 if the step has not run). Synchronises. */
+int32_t lpm_injected(lpm_handle *h, uint64_t step, uint64_t *n_host);
+/* Text of the last error on this handle ("" if none).  Owned by the handle. */
+const char *lpm_last_error(lpm_handle *h);
+/* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
+int32_t lpm_launch_count(lpm_handle *h, uint64_t *n_host);
+
+/* ---- stand-alone kernels for parity tests (device arrays in, device arrays out) ------------ */
+
+/* Philox4x32-10 (R1): out_dev[4*i..] = philox(key = seed, ctr = (step, stream, pid_lo, pid_hi))
+ * for pid = pid0 + i. */
+int32_t lpm_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n,
+                        uint32_t *out_dev, void *cuda_stream);
+/* The three N(0,1) of R3 for the same counters: out_dev[3*i..]. */
+int32_t lpm_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, float *out_dev,
+                         void *cuda_stream);
+/* Met sampling R4 at n points: xyz_dev float4 (w ignored), out_dev float4 (u, v, w, Kz). */
+int32_t lpm_test_sample(const lpm_meteo *meteo, double t, const void *xyz_dev, uint64_t n,
+                        void *out_dev, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LPM_H_ */

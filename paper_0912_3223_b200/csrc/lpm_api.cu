@@ -1,0 +1,686 @@
+// lpm_api.cu — host side of the C ABI declared in include/lpm.h: handle, workspace carving,
+// release schedule (R9), per-step scalar tables (R4 time weights, R8 decay scale), launch loop.
+// No step of the path runs on the host: the host only computes scalars and enqueues kernels.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "lpm_internal.h"
+
+using namespace lpm;
+
+namespace {
+
+constexpr uint64_t kAlign = 256;
+constexpr uint64_t kInjLog = 1u << 16;  // ring of per-step injected counts (compact mode)
+
+struct Release {
+    lpm_source src;
+    double emit[LPM_MAX_NUCLIDES];
+    uint64_t N, c, pid_offset, pid_stride;
+    int64_t s_start, S;
+    uint64_t base, n_local;
+    bool fixed;  // installed by lpm_set_particles: every slot already born
+};
+
+struct Layout {
+    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, total;
+};
+
+uint64_t up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+Layout make_layout(const lpm_grid &g, uint64_t cap, int K, bool compact)
+{
+    Layout L{};
+    const uint64_t cells3 = (uint64_t)g.nx * g.ny * g.nz, cells2 = (uint64_t)g.nx * g.ny;
+    uint64_t o = 0;
+    L.xyzq = o; o += up(16 * cap);
+    L.q1 = o; o += K > 1 ? up(4 * cap) : 0;
+    L.pid = o; o += compact ? up(4 * cap) : 0;
+    L.cnt = o; o += up(4 * cells3);
+    L.conc = o; o += up(8 * cells3 * K);
+    L.dep = o; o += up(8 * cells2 * K);
+    L.ledger = o; o += up(8 * 8 * LPM_MAX_NUCLIDES);
+    L.air = o; o += up(8 * 2);
+    L.ctrl = o; o += up(8 * 32);
+    L.tile = o; o += compact ? up(8 * (cap / kScanTile + 2)) : 0;
+    L.injlog = o; o += compact ? up(8 * kInjLog) : 0;
+    L.total = o;
+    return L;
+}
+
+GridF gridf(const lpm_grid &g)
+{
+    GridF f;
+    f.nx = g.nx; f.ny = g.ny; f.nz = g.nz;
+    f.x0 = (float)g.x0; f.y0 = (float)g.y0; f.z0 = (float)g.z0;
+    f.inv_dx = (float)(1.0 / g.dx); f.inv_dy = (float)(1.0 / g.dy); f.inv_dz = (float)(1.0 / g.dz);
+    return f;
+}
+
+bool grid_ok(const lpm_grid *g)
+{
+    return g && g->nx > 0 && g->ny > 0 && g->nz > 0 && g->dx > 0 && g->dy > 0 && g->dz > 0 &&
+           (uint64_t)g->nx * g->ny * g->nz < (1ull << 31);
+}
+
+}  // namespace
+
+struct lpm_handle {
+    lpm_grid cg;
+    lpm_meteo met;
+    lpm_nuclide nuc[LPM_MAX_NUCLIDES];
+    lpm_params prm;
+    int K;
+    cudaStream_t st;
+    char *ws;
+    Layout L;
+    // derived constants (R5, R8)
+    float sigma_h, p_dry[LPM_MAX_NUCLIDES], p_wet[LPM_MAX_NUCLIDES];
+    double f_decay[LPM_MAX_NUCLIDES], ln_rho[LPM_MAX_NUCLIDES], dec_scale[LPM_MAX_NUCLIDES], wet_scale[LPM_MAX_NUCLIDES];
+    int dry_mode;
+    bool rain_on;
+    double rx0, rx1, ry0, ry1, rt0, rt1;
+    std::vector<Release> rel;
+    uint64_t next_base;
+    uint64_t step, bin_step;
+    bool binned;
+    int sms, occ;
+    uint64_t launches;
+    int sticky;
+    char err[512];
+};
+
+namespace {
+
+int fail(lpm_handle *h, int code, const char *msg)
+{
+    if (h) snprintf(h->err, sizeof(h->err), "%s", msg);
+    return code;
+}
+
+int cuda_fail(lpm_handle *h, cudaError_t e, const char *where)
+{
+    if (h) {
+        snprintf(h->err, sizeof(h->err), "%s: %s", where, cudaGetErrorString(e));
+        h->sticky = LPM_ERR_CUDA;
+    }
+    return LPM_ERR_CUDA;
+}
+
+#define CK(call)                                                   \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);     \
+    } while (0)
+
+double G_of(const lpm_handle *h, int k, uint64_t step) { return exp((double)step * h->ln_rho[k]); }
+
+// R9: local particles of release r born at steps <= step
+uint64_t born_local(const Release &r, int64_t step)
+{
+    if (r.fixed) return r.n_local;
+    const int64_t rs = step - r.s_start;
+    if (rs < 0) return 0;
+    if (r.N > 0) {
+        uint64_t B = r.N;
+        if (rs + 1 < r.S) {
+            const unsigned __int128 num = (unsigned __int128)(uint64_t)(rs + 1) * r.N;
+            B = (uint64_t)((num + (uint64_t)r.S - 1) / (uint64_t)r.S);
+            if (B > r.N) B = r.N;
+        }
+        if (B <= r.pid_offset) return 0;
+        return (B - r.pid_offset + r.pid_stride - 1) / r.pid_stride;
+    }
+    const int64_t steps = rs + 1 < r.S ? rs + 1 : r.S;
+    return r.c * (uint64_t)steps;
+}
+
+void fill_entry(const lpm_handle *h, uint64_t n, StepEntry &e)
+{
+    const double t = (double)n * h->prm.dt;
+    int s = 0;
+    float a = 0.0f;
+    if (h->met.nt > 1) {  // R4 time weight, fp32-rounded parameter
+        double r = floor((t - h->met.t0) / h->met.dt_snap);
+        if (r < 0.0) r = 0.0;
+        if (r > (double)(h->met.nt - 2)) r = (double)(h->met.nt - 2);
+        s = (int)r;
+        double ad = (t - (h->met.t0 + (double)s * h->met.dt_snap)) / h->met.dt_snap;
+        if (ad < 0.0) ad = 0.0;
+        if (ad > 1.0) ad = 1.0;
+        a = (float)ad;
+    }
+    const bool raining = h->rain_on && t >= h->rt0 && t < h->rt1;  // G6
+    e.a = a;
+    e.snap = s | (raining ? 1 << 16 : 0);
+    for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) e.G[k] = k < h->K ? G_of(h, k, n) : 1.0;
+}
+
+void base_args(const lpm_handle *h, StepArgs &A)
+{
+    memset(&A, 0, sizeof(A));
+    A.xyzq = (float4 *)(h->ws + h->L.xyzq);
+    A.q1 = h->K > 1 ? (float *)(h->ws + h->L.q1) : nullptr;
+    A.pid = h->prm.compact ? (uint32_t *)(h->ws + h->L.pid) : nullptr;
+    A.met = (const float4 *)h->met.fields_dev;
+    const lpm_grid &mg = h->met.grid;
+    A.snap_cells = (uint64_t)mg.nx * mg.ny * mg.nz;
+    A.mg = gridf(mg);
+    A.nt = h->met.nt;
+    A.bx0 = (float)mg.x0; A.bx1 = (float)(mg.x0 + mg.nx * mg.dx);
+    A.by0 = (float)mg.y0; A.by1 = (float)(mg.y0 + mg.ny * mg.dy);
+    A.cg = gridf(h->cg);
+    A.dep = (double *)(h->ws + h->L.dep);
+    A.dep_stride = (uint64_t)h->cg.nx * h->cg.ny;
+    A.dt = (float)h->prm.dt;
+    A.sigma_h = h->sigma_h;
+    A.kz_min = (float)h->met.kz_min;
+    A.H = (float)h->met.H_mix;
+    A.h_dep = (float)h->prm.h_dep;
+    A.dry_mode = h->dry_mode;
+    A.absorb = h->prm.boundary_mode == LPM_BOUNDARY_ABSORB;
+    for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) {
+        A.p_dry[k] = h->p_dry[k]; A.p_wet[k] = h->p_wet[k];
+        A.dec_scale[k] = h->dec_scale[k]; A.wet_scale[k] = h->wet_scale[k];
+    }
+    A.rx0 = (float)h->rx0; A.rx1 = (float)h->rx1; A.ry0 = (float)h->ry0; A.ry1 = (float)h->ry1;
+    A.seed_lo = (uint32_t)h->prm.seed; A.seed_hi = (uint32_t)(h->prm.seed >> 32);
+    A.ledger = (double *)(h->ws + h->L.ledger);
+    A.ctrl = (uint64_t *)(h->ws + h->L.ctrl);
+    A.tile_state = h->prm.compact ? (uint64_t *)(h->ws + h->L.tile) : nullptr;
+}
+
+int grid_blocks(const lpm_handle *h, uint64_t n)
+{
+    const uint64_t want = (n + kStepThreads - 1) / kStepThreads;
+    const uint64_t maxb = (uint64_t)h->sms * (uint64_t)(h->occ > 0 ? h->occ : 1);
+    return (int)(want < maxb ? (want ? want : 1) : maxb);
+}
+
+int do_bin(lpm_handle *h)
+{
+    const uint64_t cells3 = (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz;
+    CK(cudaMemsetAsync(h->ws + h->L.cnt, 0, 4 * cells3, h->st));
+    CK(cudaMemsetAsync(h->ws + h->L.conc, 0, 8 * cells3 * h->K, h->st));
+    BinArgs B{};
+    B.q1 = h->K > 1 ? (const float *)(h->ws + h->L.q1) : nullptr;
+    B.cg = gridf(h->cg);
+    B.cnt = (uint32_t *)(h->ws + h->L.cnt);
+    B.conc = (double *)(h->ws + h->L.conc);
+    B.cells3 = cells3;
+    B.K = h->K;
+    if (h->prm.compact) {
+        B.xyzq = (const float4 *)(h->ws + h->L.xyzq);
+        B.n_dev = (const uint64_t *)(h->ws + h->L.ctrl) + 2;
+        CK(launch_bin(B, h->sms * 8, h->st));
+        h->launches++;
+    } else {
+        for (const Release &r : h->rel) {
+            const uint64_t n = born_local(r, (int64_t)h->step - 1);
+            if (!n) continue;
+            B.xyzq = (const float4 *)(h->ws + h->L.xyzq) + r.base;
+            if (B.q1) B.q1 = (const float *)(h->ws + h->L.q1) + r.base;
+            B.n = n;
+            const uint64_t want = (n + 255) / 256;
+            CK(launch_bin(B, (int)(want < (uint64_t)h->sms * 8 ? want : (uint64_t)h->sms * 8), h->st));
+            h->launches++;
+        }
+    }
+    h->bin_step = h->step;
+    h->binned = true;
+    return LPM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t lpm_version(void) { return 100; }
+
+const char *lpm_status_string(int32_t s)
+{
+    switch (s) {
+        case LPM_OK: return "ok";
+        case LPM_ERR_INVALID_ARG: return "invalid argument";
+        case LPM_ERR_NO_DEVICE: return "no sm_100 CUDA device (there is no CPU fallback)";
+        case LPM_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+        case LPM_ERR_CAPACITY: return "release does not fit into the particle capacity";
+        case LPM_ERR_STATE: return "call order";
+        case LPM_ERR_CUDA: return "CUDA error";
+        default: return "unknown status";
+    }
+}
+
+int32_t lpm_workspace_bytes(const lpm_grid *g, const lpm_params *p, int32_t K, uint64_t *bytes)
+{
+    if (!grid_ok(g) || !p || !bytes || K < 1 || K > LPM_MAX_NUCLIDES || p->capacity == 0 || p->capacity >= (1ull << 32))
+        return LPM_ERR_INVALID_ARG;
+    *bytes = make_layout(*g, p->capacity, K, p->compact != 0).total;
+    return LPM_OK;
+}
+
+int32_t lpm_schedule_born(uint64_t N, uint64_t pid_offset, uint64_t pid_stride, int64_t s_start, int64_t S,
+                          int64_t step, uint64_t *born)
+{
+    if (!born || N == 0 || pid_stride == 0 || S < 1) return LPM_ERR_INVALID_ARG;
+    Release r{};
+    r.N = N; r.pid_offset = pid_offset; r.pid_stride = pid_stride; r.s_start = s_start; r.S = S;
+    *born = born_local(r, step);
+    return LPM_OK;
+}
+
+int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *nuc, int32_t K, const lpm_params *p,
+                   void *ws, uint64_t ws_bytes, void *stream, lpm_handle **out)
+{
+    if (!out) return LPM_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!grid_ok(cg) || !met || !grid_ok(&met->grid) || !nuc || !p || !ws || K < 1 || K > LPM_MAX_NUCLIDES)
+        return LPM_ERR_INVALID_ARG;
+    if (met->nt < 1 || met->nt > 32767 || !met->fields_dev || ((uintptr_t)met->fields_dev & 15) || ((uintptr_t)ws & 255))
+        return LPM_ERR_INVALID_ARG;
+    if (!(p->dt > 0) || p->capacity == 0 || p->capacity >= (1ull << 32) || !(met->H_mix > 0) || met->Kh < 0 ||
+        (met->nt > 1 && !(met->dt_snap > 0)) || p->bin_every < 0 || p->steps_per_launch < 0 || !(p->h_dep > 0))
+        return LPM_ERR_INVALID_ARG;
+    int ndev = 0, dev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return LPM_ERR_NO_DEVICE;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return LPM_ERR_NO_DEVICE;
+    if (prop.major != 10) return LPM_ERR_NO_DEVICE;
+
+    const Layout L = make_layout(*cg, p->capacity, K, p->compact != 0);
+    if (ws_bytes < L.total) return LPM_ERR_WORKSPACE_TOO_SMALL;
+
+    lpm_handle *h = new (std::nothrow) lpm_handle();
+    if (!h) return LPM_ERR_INVALID_ARG;
+    h->cg = *cg; h->met = *met; h->prm = *p; h->K = K;
+    for (int k = 0; k < K; ++k) h->nuc[k] = nuc[k];
+    h->st = (cudaStream_t)stream;
+    h->ws = (char *)ws;
+    h->L = L;
+    h->sms = prop.multiProcessorCount;
+    h->err[0] = 0;
+    // R5 / R8 constants: double formula, rounded once to fp32 where the kernels consume fp32
+    h->sigma_h = (float)sqrt(2.0 * met->Kh * p->dt);
+    const bool uniform = p->h_dep >= met->H_mix;
+    bool any_dry = false;
+    for (int k = 0; k < K; ++k) {
+        h->p_dry[k] = nuc[k].vd > 0 ? (float)(-expm1(-nuc[k].vd * p->dt / p->h_dep)) : 0.0f;
+        h->p_wet[k] = nuc[k].lambda_wet > 0 ? (float)(-expm1(-nuc[k].lambda_wet * p->dt)) : 0.0f;
+        any_dry |= h->p_dry[k] > 0.0f;
+        const double lam_dt = nuc[k].half_life_s > 0 ? M_LN2 * p->dt / nuc[k].half_life_s : 0.0;
+        h->f_decay[k] = exp(-lam_dt);
+        const double keep_dry = uniform ? 1.0 - (double)h->p_dry[k] : 1.0;
+        h->ln_rho[k] = -lam_dt + (uniform ? log1p(-(double)h->p_dry[k]) : 0.0);
+        h->dec_scale[k] = -expm1(-lam_dt) * keep_dry;
+        h->wet_scale[k] = keep_dry * (double)h->p_wet[k];
+    }
+    h->dry_mode = !any_dry ? kDryNone : (uniform ? kDryUniform : kDryLayer);
+    h->occ = step_max_blocks_per_sm(K, p->compact != 0, met->nt > 1);
+    if (cudaMemsetAsync(ws, 0, L.total, h->st) != cudaSuccess) { delete h; return LPM_ERR_CUDA; }
+    h->launches++;
+    *out = h;
+    return LPM_OK;
+}
+
+int32_t lpm_destroy(lpm_handle *h)
+{
+    if (!h) return LPM_ERR_INVALID_ARG;
+    cudaStreamSynchronize(h->st);
+    delete h;
+    return LPM_OK;
+}
+
+const char *lpm_last_error(lpm_handle *h) { return h ? h->err : "null handle"; }
+
+int32_t lpm_set_rain(lpm_handle *h, double x0, double x1, double y0, double y1, double t0, double t1)
+{
+    if (!h || !(x1 > x0) || !(y1 > y0) || !(t1 > t0)) return fail(h, LPM_ERR_INVALID_ARG, "lpm_set_rain: empty box or interval");
+    h->rain_on = true;
+    h->rx0 = x0; h->rx1 = x1; h->ry0 = y0; h->ry1 = y1; h->rt0 = t0; h->rt1 = t1;
+    return LPM_OK;
+}
+
+int32_t lpm_release(lpm_handle *h, const lpm_source *src, const double *act, uint64_t N, double rate, uint64_t off, uint64_t stride)
+{
+    if (!h || !src || !act || stride < 1) return fail(h, LPM_ERR_INVALID_ARG, "lpm_release: null or zero stride");
+    if (h->rel.size() >= LPM_MAX_RELEASES) return fail(h, LPM_ERR_CAPACITY, "lpm_release: too many releases");
+    Release r{};
+    r.src = *src;
+    r.s_start = (int64_t)ceil(src->t_start / h->prm.dt);
+    r.S = (int64_t)ceil((src->t_end - src->t_start) / h->prm.dt);
+    if (r.S < 1) r.S = 1;
+    if ((int64_t)h->step > r.s_start) return fail(h, LPM_ERR_STATE, "lpm_release: release starts before the current step");
+    r.pid_offset = off; r.pid_stride = stride;
+    if (N > 0) {
+        r.N = N;
+        r.n_local = off < N ? (N - off + stride - 1) / stride : 0;
+        for (int k = 0; k < h->K; ++k) r.emit[k] = act[k] / (double)N;
+        if (off + (r.n_local ? r.n_local - 1 : 0) * stride >= (1ull << 32)) return fail(h, LPM_ERR_INVALID_ARG, "lpm_release: particle ids must stay below 2^32");
+    } else {
+        if (stride != 1) return fail(h, LPM_ERR_INVALID_ARG, "lpm_release: rate mode needs pid_stride 1");
+        r.c = (uint64_t)llround(rate * h->prm.dt);
+        if (r.c == 0) return fail(h, LPM_ERR_INVALID_ARG, "lpm_release: rate*dt rounds to zero");
+        r.n_local = r.c * (uint64_t)r.S;
+        for (int k = 0; k < h->K; ++k) r.emit[k] = act[k] / ((double)r.c * (double)r.S);
+        if (off + r.n_local >= (1ull << 32)) return fail(h, LPM_ERR_INVALID_ARG, "lpm_release: particle ids must stay below 2^32");
+    }
+    if (!h->prm.compact) {
+        for (const Release &o : h->rel) if (o.fixed) return fail(h, LPM_ERR_STATE, "lpm_release: state was replaced by lpm_set_particles");
+        if (h->next_base + r.n_local > h->prm.capacity) return fail(h, LPM_ERR_CAPACITY, "lpm_release: particles exceed capacity");
+        r.base = h->next_base;
+        h->next_base += (r.n_local + 63) / 64 * 64;  // keep blocks 1 KB aligned for float4 access
+    }
+    h->rel.push_back(r);
+    return LPM_OK;
+}
+
+int32_t lpm_step(lpm_handle *h, int32_t n_steps)
+{
+    if (!h || n_steps < 0) return fail(h, LPM_ERR_INVALID_ARG, "lpm_step: negative step count");
+    if (h->sticky) return h->sticky;
+    const bool compact = h->prm.compact != 0;
+    int m_max = h->prm.steps_per_launch > 0 ? h->prm.steps_per_launch : kMaxFused;
+    if (m_max > kMaxFused) m_max = kMaxFused;
+    if (compact) m_max = 1;
+    StepArgs A;
+    base_args(h, A);
+    int64_t left = n_steps;
+    while (left > 0) {
+        int m = (int)(left < m_max ? left : m_max);
+        if (h->prm.bin_every > 0) {
+            const uint64_t to_bin = (uint64_t)h->prm.bin_every - h->step % (uint64_t)h->prm.bin_every;
+            if ((uint64_t)m > to_bin) m = (int)to_bin;
+        }
+        A.step0 = h->step;
+        A.m_steps = m;
+        for (int s = 0; s < m; ++s) fill_entry(h, h->step + s, A.tab[s]);
+        if (compact) {
+            InjectArgs I{};
+            I.xyzq = A.xyzq; I.q1 = A.q1; I.pid = A.pid; I.ctrl = A.ctrl;
+            I.log_slot = (uint64_t *)(h->ws + h->L.injlog) + h->step % kInjLog;
+            I.capacity = h->prm.capacity;
+            I.K = h->K;
+            for (size_t ri = 0; ri < h->rel.size(); ++ri) {
+                const Release &r = h->rel[ri];
+                const uint64_t b1 = born_local(r, (int64_t)h->step), b0 = born_local(r, (int64_t)h->step - 1);
+                if (b1 == b0) continue;
+                InjectSpec &sp = I.spec[I.n_spec++];
+                sp.rel_index = (int32_t)ri;
+                sp.first_pid = r.pid_offset + b0 * r.pid_stride;
+                sp.count = b1 - b0;
+                sp.pid_stride = r.pid_stride;
+                sp.sx = (float)r.src.x; sp.sy = (float)r.src.y; sp.sz = (float)r.src.z;
+                for (int k = 0; k < h->K; ++k) sp.q[k] = (float)(r.emit[k] / A.tab[0].G[k]);
+            }
+            CK(launch_inject(I, h->st));
+            CK(launch_step(A, h->K, true, h->sms * (h->occ > 0 ? h->occ : 1), h->st));
+            h->launches += 2;
+        } else {
+            for (const Release &r : h->rel) {
+                const uint64_t n = born_local(r, (int64_t)h->step + m - 1);
+                if (!n) continue;
+                A.base = r.base;
+                A.n = n;
+                A.n_prev = born_local(r, (int64_t)h->step - 1);
+                A.pid_offset = r.pid_offset; A.pid_stride = r.pid_stride;
+                A.rel_N = r.N; A.rel_c = r.c ? r.c : 1;
+                A.rel_s_start = r.s_start; A.rel_S = r.S;
+                for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) A.emit[k] = r.emit[k];
+                A.sx = (float)r.src.x; A.sy = (float)r.src.y; A.sz = (float)r.src.z;
+                CK(launch_step(A, h->K, false, grid_blocks(h, n), h->st));
+                h->launches++;
+            }
+        }
+        h->step += (uint64_t)m;
+        left -= m;
+        if (h->prm.bin_every > 0 && h->step % (uint64_t)h->prm.bin_every == 0) {
+            const int rc = do_bin(h);
+            if (rc) return rc;
+        }
+    }
+    return LPM_OK;
+}
+
+int32_t lpm_bin_now(lpm_handle *h)
+{
+    if (!h) return LPM_ERR_INVALID_ARG;
+    if (h->sticky) return h->sticky;
+    return do_bin(h);
+}
+
+int32_t lpm_concentration(lpm_handle *h, float *out)
+{
+    if (!h || !out) return fail(h, LPM_ERR_INVALID_ARG, "lpm_concentration: null");
+    if (h->sticky) return h->sticky;
+    if (!h->binned || h->bin_step != h->step) { const int rc = do_bin(h); if (rc) return rc; }
+    const double V = h->cg.dx * h->cg.dy * h->cg.dz;
+    double scale[LPM_MAX_NUCLIDES] = {0, 0};
+    for (int k = 0; k < h->K; ++k) scale[k] = G_of(h, k, h->bin_step) / V;
+    CK(launch_conc_readout((const double *)(h->ws + h->L.conc), out, (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz, h->K, scale, h->st));
+    h->launches++;
+    return LPM_OK;
+}
+
+int32_t lpm_counts(lpm_handle *h, uint32_t *out)
+{
+    if (!h || !out) return fail(h, LPM_ERR_INVALID_ARG, "lpm_counts: null");
+    if (h->sticky) return h->sticky;
+    if (!h->binned || h->bin_step != h->step) { const int rc = do_bin(h); if (rc) return rc; }
+    CK(cudaMemcpyAsync(out, h->ws + h->L.cnt, 4ull * h->cg.nx * h->cg.ny * h->cg.nz, cudaMemcpyDeviceToDevice, h->st));
+    return LPM_OK;
+}
+
+static int dep_out(lpm_handle *h, float *o32, double *o64)
+{
+    if (!h || (!o32 && !o64)) return fail(h, LPM_ERR_INVALID_ARG, "lpm_deposition: null");
+    if (h->sticky) return h->sticky;
+    CK(launch_dep_readout((const double *)(h->ws + h->L.dep), o32, o64, (uint64_t)h->cg.nx * h->cg.ny, h->K,
+                          1.0 / (h->cg.dx * h->cg.dy), h->st));
+    h->launches++;
+    return LPM_OK;
+}
+
+int32_t lpm_deposition(lpm_handle *h, float *out) { return dep_out(h, out, nullptr); }
+int32_t lpm_deposition_f64(lpm_handle *h, double *out) { return dep_out(h, nullptr, out); }
+
+int32_t lpm_step_index(lpm_handle *h, uint64_t *s)
+{
+    if (!h || !s) return LPM_ERR_INVALID_ARG;
+    *s = h->step;
+    return LPM_OK;
+}
+
+int32_t lpm_mass_scale(lpm_handle *h, double *scale)
+{
+    if (!h || !scale) return LPM_ERR_INVALID_ARG;
+    for (int k = 0; k < h->K; ++k) scale[k] = G_of(h, k, h->step);
+    return LPM_OK;
+}
+
+static uint64_t slots_in_use(const lpm_handle *h)
+{
+    uint64_t n = 0;
+    for (const Release &r : h->rel) {
+        const uint64_t b = born_local(r, (int64_t)h->step - 1);
+        if (b && r.base + b > n) n = r.base + b;
+    }
+    return n;
+}
+
+int32_t lpm_num_active(lpm_handle *h, uint64_t *n)
+{
+    if (!h || !n) return LPM_ERR_INVALID_ARG;
+    if (h->sticky) return h->sticky;
+    if (h->prm.compact) {
+        CK(cudaMemcpyAsync(n, (uint64_t *)(h->ws + h->L.ctrl) + 2, 8, cudaMemcpyDeviceToHost, h->st));
+        CK(cudaStreamSynchronize(h->st));
+    } else {
+        *n = slots_in_use(h);
+    }
+    return LPM_OK;
+}
+
+int32_t lpm_get_particles(lpm_handle *h, void *xyzq, float *q1, uint32_t *pid, uint8_t *status, uint64_t *n_host)
+{
+    if (!h || !n_host) return fail(h, LPM_ERR_INVALID_ARG, "lpm_get_particles: null");
+    if (h->sticky) return h->sticky;
+    uint64_t n = 0;
+    const int rc = lpm_num_active(h, &n);
+    if (rc) return rc;
+    *n_host = n;
+    if (!n) return LPM_OK;
+    if (xyzq || status) {
+        CK(launch_export((const float4 *)(h->ws + h->L.xyzq), n, nullptr, (float4 *)xyzq, status, h->st));
+        h->launches++;
+    }
+    if (q1 && h->K > 1) CK(cudaMemcpyAsync(q1, h->ws + h->L.q1, 4 * n, cudaMemcpyDeviceToDevice, h->st));
+    if (pid) {
+        if (h->prm.compact) CK(cudaMemcpyAsync(pid, h->ws + h->L.pid, 4 * n, cudaMemcpyDeviceToDevice, h->st));
+        else {
+            // slot-addressed mode: ids are implied; single-release blocks report offset + l*stride
+            CK(launch_iota(pid, n, h->st));
+            h->launches++;
+        }
+    }
+    return LPM_OK;
+}
+
+int32_t lpm_set_particles(lpm_handle *h, const void *xyzq, const float *q1, const uint32_t *pid, const uint8_t *status,
+                          uint64_t n, uint64_t step_index)
+{
+    if (!h || !xyzq || (h->K > 1 && !q1)) return fail(h, LPM_ERR_INVALID_ARG, "lpm_set_particles: null");
+    if (n > h->prm.capacity) return fail(h, LPM_ERR_CAPACITY, "lpm_set_particles: n exceeds capacity");
+    if (!h->prm.compact && pid) return fail(h, LPM_ERR_INVALID_ARG, "lpm_set_particles: ids are implied by the slot unless compact=1");
+    if (h->sticky) return h->sticky;
+    if (n) {
+        CK(cudaMemcpyAsync(h->ws + h->L.xyzq, xyzq, 16 * n, cudaMemcpyDeviceToDevice, h->st));
+        if (h->K > 1) CK(cudaMemcpyAsync(h->ws + h->L.q1, q1, 4 * n, cudaMemcpyDeviceToDevice, h->st));
+        if (status) { CK(launch_import((float4 *)(h->ws + h->L.xyzq), n, status, h->st)); h->launches++; }
+    }
+    if (h->prm.compact) {
+        if (n) {
+            if (pid) CK(cudaMemcpyAsync(h->ws + h->L.pid, pid, 4 * n, cudaMemcpyDeviceToDevice, h->st));
+            else { CK(launch_iota((uint32_t *)(h->ws + h->L.pid), n, h->st)); h->launches++; }
+        }
+        uint64_t ctrl[3] = {n, 0, n};
+        CK(cudaMemcpyAsync(h->ws + h->L.ctrl, ctrl, sizeof(ctrl), cudaMemcpyHostToDevice, h->st));
+        CK(cudaStreamSynchronize(h->st));
+    } else {
+        h->rel.clear();
+        Release r{};
+        r.fixed = true; r.n_local = n; r.pid_stride = 1; r.S = 1;
+        h->rel.push_back(r);
+        h->next_base = n;
+    }
+    h->step = step_index;
+    h->binned = false;
+    return LPM_OK;
+}
+
+int32_t lpm_ledger(lpm_handle *h, double *out)
+{
+    if (!h || !out) return fail(h, LPM_ERR_INVALID_ARG, "lpm_ledger: null");
+    if (h->sticky) return h->sticky;
+    double *air = (double *)(h->ws + h->L.air);
+    CK(cudaMemsetAsync(air, 0, 16, h->st));
+    if (h->prm.compact) {
+        CK(launch_airborne((const float4 *)(h->ws + h->L.xyzq), h->K > 1 ? (const float *)(h->ws + h->L.q1) : nullptr, 0,
+                           (const uint64_t *)(h->ws + h->L.ctrl) + 2, h->K, air, h->st));
+        h->launches++;
+    } else {
+        for (const Release &r : h->rel) {
+            const uint64_t n = born_local(r, (int64_t)h->step - 1);
+            if (!n) continue;
+            CK(launch_airborne((const float4 *)(h->ws + h->L.xyzq) + r.base,
+                               h->K > 1 ? (const float *)(h->ws + h->L.q1) + r.base : nullptr, n, nullptr, h->K, air, h->st));
+            h->launches++;
+        }
+    }
+    double led[LPM_MAX_NUCLIDES * 8], a2[2];
+    uint64_t ctrl[32];
+    CK(cudaMemcpyAsync(led, h->ws + h->L.ledger, sizeof(led), cudaMemcpyDeviceToHost, h->st));
+    CK(cudaMemcpyAsync(a2, air, 16, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaMemcpyAsync(ctrl, h->ws + h->L.ctrl, sizeof(ctrl), cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    for (int k = 0; k < h->K; ++k) {
+        double emitted = 0.0;
+        for (size_t ri = 0; ri < h->rel.size(); ++ri) {
+            const Release &r = h->rel[ri];
+            if (r.fixed) continue;
+            const uint64_t born = h->prm.compact ? ctrl[8 + ri] : born_local(r, (int64_t)h->step - 1);
+            emitted += r.emit[k] * (double)born;
+        }
+        double *o = out + k * LPM_LEDGER_FIELDS;
+        o[0] = emitted;
+        o[1] = a2[k] * G_of(h, k, h->step);
+        o[2] = led[k * 8 + 2]; o[3] = led[k * 8 + 3]; o[4] = led[k * 8 + 4]; o[5] = led[k * 8 + 5]; o[6] = led[k * 8 + 6];
+    }
+    return LPM_OK;
+}
+
+int32_t lpm_injected(lpm_handle *h, uint64_t step, uint64_t *n)
+{
+    if (!h || !n) return LPM_ERR_INVALID_ARG;
+    if (h->sticky) return h->sticky;
+    *n = 0;
+    if (step >= h->step) return LPM_OK;
+    if (h->prm.compact) {
+        if (h->step - step > kInjLog) return fail(h, LPM_ERR_INVALID_ARG, "lpm_injected: step fell out of the log ring");
+        CK(cudaMemcpyAsync(n, (uint64_t *)(h->ws + h->L.injlog) + step % kInjLog, 8, cudaMemcpyDeviceToHost, h->st));
+        CK(cudaStreamSynchronize(h->st));
+    } else {
+        for (const Release &r : h->rel) *n += born_local(r, (int64_t)step) - born_local(r, (int64_t)step - 1);
+    }
+    return LPM_OK;
+}
+
+int32_t lpm_launch_count(lpm_handle *h, uint64_t *n)
+{
+    if (!h || !n) return LPM_ERR_INVALID_ARG;
+    *n = h->launches;
+    return LPM_OK;
+}
+
+static int dev_ok()
+{
+    int ndev = 0;
+    return cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0;
+}
+
+int32_t lpm_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out, void *st)
+{
+    if (!out) return LPM_ERR_INVALID_ARG;
+    if (!dev_ok()) return LPM_ERR_NO_DEVICE;
+    return launch_test_philox(seed, step, stream, pid0, n, out, (cudaStream_t)st) == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
+}
+
+int32_t lpm_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, float *out, void *st)
+{
+    if (!out) return LPM_ERR_INVALID_ARG;
+    if (!dev_ok()) return LPM_ERR_NO_DEVICE;
+    return launch_test_normals(seed, step, pid0, n, out, (cudaStream_t)st) == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
+}
+
+int32_t lpm_test_sample(const lpm_meteo *met, double t, const void *xyz, uint64_t n, void *out, void *st)
+{
+    if (!met || !grid_ok(&met->grid) || !met->fields_dev || !xyz || !out || met->nt < 1) return LPM_ERR_INVALID_ARG;
+    if (!dev_ok()) return LPM_ERR_NO_DEVICE;
+    lpm_handle tmp{};
+    tmp.met = *met;
+    tmp.prm.dt = 1.0;
+    tmp.K = 0;
+    StepEntry e;
+    // fill_entry evaluates the time weight at t = n * dt; use dt = t, n = 1
+    tmp.prm.dt = t;
+    fill_entry(&tmp, 1, e);
+    const lpm_grid &g = met->grid;
+    return launch_test_sample((const float4 *)met->fields_dev, (uint64_t)g.nx * g.ny * g.nz, gridf(g), met->nt > 1, e.snap & 0xffff,
+                              e.a, (float)met->kz_min, (const float4 *)xyz, n, (float4 *)out, (cudaStream_t)st) == cudaSuccess
+               ? LPM_OK : LPM_ERR_CUDA;
+}
+
+}  // extern "C"

@@ -1,0 +1,117 @@
+// lpm_internal.h — structs shared by the kernels (lpm_step.cu, lpm_bin.cu) and the host API
+// (lpm_api.cu).  Not part of the public boundary (include/lpm.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/lpm.h"
+
+namespace lpm {
+
+constexpr int kMaxFused = 96;        // model steps fused into one launch (table lives in kernel params)
+constexpr int kStepThreads = 256;    // CTA size of the step kernel
+constexpr int kScanTile = kStepThreads;  // particles per look-back tile (compaction)
+
+// Per-step scalars, host-computed in double (DESIGN.md §3 R4, R8).
+struct StepEntry {
+    double G[LPM_MAX_NUCLIDES];  // G_k(t_n): activity = q * G (decay and uniform dry loss folded in)
+    float a;                     // time weight between snapshot `snap` and `snap + 1`
+    int32_t snap;                // bits 0..15 snapshot index, bit 16 = raining
+};
+
+struct GridF {  // fp32 view of a grid, exactly as the kernels use it
+    int32_t nx, ny, nz;
+    float x0, y0, z0;          // (float) lower corner
+    float inv_dx, inv_dy, inv_dz;  // (float)(1.0 / d)
+};
+
+enum DryMode : int32_t { kDryNone = 0, kDryUniform = 1, kDryLayer = 2 };
+
+struct StepArgs {
+    // particle store
+    float4 *xyzq;
+    float *q1;
+    uint32_t *pid;        // compact mode only
+    // meteorology
+    const float4 *met;
+    uint64_t snap_cells;  // cells per snapshot
+    GridF mg;
+    int32_t nt;
+    float bx0, bx1, by0, by1;  // lateral boundary (met box), fp32
+    // deposition map
+    GridF cg;
+    double *dep;          // [K][ny][nx]
+    uint64_t dep_stride;
+    // physics
+    float dt, sigma_h, kz_min, H, h_dep;
+    int32_t dry_mode, absorb;
+    float p_dry[LPM_MAX_NUCLIDES], p_wet[LPM_MAX_NUCLIDES];
+    float rx0, rx1, ry0, ry1;
+    uint32_t seed_lo, seed_hi;
+    // ledger: double [K][8]: 2 dry, 3 wet, 4 decayed, 5 exited, 6 offgrid
+    double *ledger;
+    double dec_scale[LPM_MAX_NUCLIDES];  // (1 - f_lambda) * (1 - p_dry if uniform)
+    double wet_scale[LPM_MAX_NUCLIDES];  // (1 - p_dry if uniform) * p_wet
+    // population (slot-addressed mode): slots [0, n) of the release block starting at `base`
+    uint64_t base, n, n_prev;  // slots >= n_prev are born inside this launch
+    uint64_t pid_offset, pid_stride;
+    uint64_t rel_N, rel_c;     // count mode: N (global count); rate mode: c slots per step
+    int64_t rel_s_start, rel_S;
+    double emit[LPM_MAX_NUCLIDES];  // activity per particle at birth
+    float sx, sy, sz;               // source point
+    // compact mode: device-side control block
+    uint64_t *ctrl;      // [0] n_active, [1] ticket, [2] n_out
+    uint64_t *tile_state;
+    // time
+    uint64_t step0;
+    int32_t m_steps;
+    StepEntry tab[kMaxFused];
+};
+
+// compact mode: newborn particles of one step, appended behind the live ones
+struct InjectSpec {
+    uint64_t first_pid, count, pid_stride;
+    int32_t rel_index, pad_;
+    float sx, sy, sz;
+    float q[LPM_MAX_NUCLIDES];   // (float)(emit_k / G_k(t_n))
+};
+struct InjectArgs {
+    float4 *xyzq;
+    float *q1;
+    uint32_t *pid;
+    uint64_t *ctrl;       // [0] n_in, [1] ticket, [2] n_out of the previous step
+    uint64_t *log_slot;   // injected count of this step (may be null)
+    uint64_t capacity;
+    int32_t n_spec, K;
+    InjectSpec spec[LPM_MAX_RELEASES];
+};
+
+struct BinArgs {
+    const float4 *xyzq;
+    const float *q1;
+    uint64_t n;               // slots to bin (slot-addressed mode)
+    const uint64_t *n_dev;    // compact mode: read n from here
+    GridF cg;
+    uint32_t *cnt;
+    double *conc;             // [K][cells3] sums of q
+    uint64_t cells3;
+    int32_t K;
+};
+
+// launchers implemented in the .cu files; all return the cudaError of the launch
+cudaError_t launch_step(const StepArgs &a, int K, bool compact, int grid_blocks, cudaStream_t st);
+int step_max_blocks_per_sm(int K, bool compact, bool two_snap);
+cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
+cudaError_t launch_bin(const BinArgs &a, int blocks, cudaStream_t st);
+cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3, int K, const double *scale, cudaStream_t st);
+cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, double inv_area, cudaStream_t st);
+cudaError_t launch_airborne(const float4 *xyzq, const float *q1, uint64_t n, const uint64_t *n_dev, int K, double *out2, cudaStream_t st);
+cudaError_t launch_export(const float4 *xyzq, uint64_t n, const uint64_t *n_dev, float4 *out, uint8_t *status, cudaStream_t st);
+cudaError_t launch_import(float4 *xyzq, uint64_t n, const uint8_t *status, cudaStream_t st);
+cudaError_t launch_iota(uint32_t *pid, uint64_t n, cudaStream_t st);
+cudaError_t launch_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st);
+cudaError_t launch_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, float *out, cudaStream_t st);
+cudaError_t launch_test_sample(const float4 *met, uint64_t snap_cells, GridF mg, int two, int snap, float a, float kz_min,
+                               const float4 *xyz, uint64_t n, float4 *out, cudaStream_t st);
+
+}  // namespace lpm

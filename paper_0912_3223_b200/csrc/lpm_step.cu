@@ -1,0 +1,355 @@
+// lpm_step.cu — the fused per-particle step kernels for sm_100a.
+//
+// One thread carries one particle through m >= 1 model steps with its state in registers:
+//   a1 Philox4x32-10 + Box-Muller      (R1-R3)
+//   a0/a2 trilinear gathers of float4 (u,v,w,Kz) from one or two L2-resident snapshots and the
+//         linear blend in time           (R4)
+//   a3 advection + random walk          (R5; Eq.(1)(2))
+//   a4 reflection, lateral boundary     (R6, R7)
+//   a5 decay / dry / wet deposition     (R8)
+//   a6 deposit scatter into the 2-D map (fp64 RED; the map stays in L2)
+//   a7 stable in-place compaction by a single-pass decoupled look-back scan (compact mode)
+// The paper's kernel staged particle state in shared memory and sampled hardware textures
+// (P:L110-114); neither survives on B200: there is no reuse to stage, and texture filtering's
+// fixed-point weights cannot meet the 1e-5 parity bar.
+#include "lpm_device.cuh"
+
+namespace lpm {
+
+template <int K>
+struct Acc {  // per-thread ledger partial sums, in activity units before the per-nuclide scale
+    float dry[K], wet[K], dec[K];
+};
+
+// One model step of one particle.  Returns false when the particle left the domain (ABSORB).
+template <int K, bool TWO>
+__device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e, uint32_t step_lo,
+                                          uint32_t pid_lo, float &x, float &y, float &z,
+                                          float (&q)[K], Acc<K> &acc)
+{
+    // a1: three N(0,1) from Philox stream 0
+    const uint4 r = philox4x32_10(step_lo, 0u, pid_lo, 0u, A.seed_lo, A.seed_hi);
+    float n0, n1, n2;
+    normals3(r, n0, n1, n2);
+
+    // a0 + a2: weather at X_old, t_n
+    const Corner c = corner_of(A.mg, x, y, z);
+    const int snap = e.snap & 0xffff;
+    const float4 *s0 = A.met + (uint64_t)snap * A.snap_cells;
+    float4 m = trilinear(s0, c);
+    if (TWO) {
+        const float4 m1 = trilinear(s0 + A.snap_cells, c);
+        m = lerp4(m, m1, e.a);
+    }
+    const float kz = fmaxf(m.w, A.kz_min);
+
+    // a3: Eq.(1) + Eq.(2)
+    x = fmaf(A.sigma_h, n0, fmaf(m.x, A.dt, x));
+    y = fmaf(A.sigma_h, n1, fmaf(m.y, A.dt, y));
+    z = fmaf(sqrtf(2.0f * A.dt * kz), n2, fmaf(m.z, A.dt, z));
+
+    // a4: reflection (R6), lateral boundary (R7)
+    if (z < 0.0f) z = -z;
+    if (z > A.H) z = 2.0f * A.H - z;
+    if (z < 0.0f) z = 0.0f;
+    if (A.absorb) {
+        const bool inside = (x >= A.bx0) & (x < A.bx1) & (y >= A.by0) & (y < A.by1);
+        if (!inside) {
+#pragma unroll
+            for (int k = 0; k < K; ++k) atomicAdd(A.ledger + k * 8 + 5, (double)q[k] * e.G[k]);
+            return false;
+        }
+    }
+
+    // a5: deposition then decay at the new position (R8).  Activity = q * G_k(t_n); decay and
+    // uniform dry loss live in G, so q only changes for position-dependent sinks.
+    float inc[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) inc[k] = 0.0f;
+    const bool dry_here = (A.dry_mode == kDryUniform) | ((A.dry_mode == kDryLayer) & (z < A.h_dep));
+    const bool raining = (e.snap >> 16) & 1;
+    const bool wet_here = raining & (x >= A.rx0) & (x < A.rx1) & (y >= A.ry0) & (y < A.ry1);
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const float G = (float)e.G[k];
+        float act = q[k] * G;
+        if (dry_here) {
+            inc[k] = act * A.p_dry[k];
+            acc.dry[k] += act;
+            if (A.dry_mode == kDryLayer) {
+                q[k] = fmaf(-q[k], A.p_dry[k], q[k]);
+                act = q[k] * G;
+            }
+        }
+        if (wet_here) {
+            inc[k] = fmaf(act, (float)A.wet_scale[k], inc[k]);
+            acc.wet[k] += act;
+            q[k] = fmaf(-q[k], A.p_wet[k], q[k]);
+            act = q[k] * G;
+        }
+        acc.dec[k] += act;
+    }
+
+    // a6: deposit scatter at the cell of the NEW (x, y)
+    if (dry_here | wet_here) {
+        const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
+        const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
+        if ((ci | cj) >= 0) {
+            double *d = A.dep + (uint32_t)(cj * A.cg.nx + ci);
+#pragma unroll
+            for (int k = 0; k < K; ++k) atomicAdd(d + k * A.dep_stride, (double)inc[k]);
+        } else {
+#pragma unroll
+            for (int k = 0; k < K; ++k) atomicAdd(A.ledger + k * 8 + 6, (double)inc[k]);
+        }
+    }
+    return true;
+}
+
+// block-reduce the per-thread ledger partials and add them to the device ledger (one fp64 RED per
+// quantity per CTA)
+template <int K>
+__device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &acc)
+{
+    __shared__ float s_part[kStepThreads / 32][3 * K];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const float d = warp_sum(acc.dry[k]), w = warp_sum(acc.wet[k]), c = warp_sum(acc.dec[k]);
+        if (lane == 0) { s_part[warp][3 * k] = d; s_part[warp][3 * k + 1] = w; s_part[warp][3 * k + 2] = c; }
+    }
+    __syncthreads();
+    if (threadIdx.x < 3 * K) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < kStepThreads / 32; ++w) s += (double)s_part[w][threadIdx.x];
+        const int k = threadIdx.x / 3, f = threadIdx.x % 3;
+        const double scale = f == 0 ? (double)A.p_dry[k] : (f == 1 ? A.wet_scale[k] : A.dec_scale[k]);
+        if (s != 0.0) atomicAdd(A.ledger + k * 8 + 2 + f, s * scale);
+    }
+}
+
+// ------------------------------------------------------------------ slot-addressed kernel
+// Particles of one release occupy the slots base + [0, n); slot l carries global particle id
+// pid_offset + l * pid_stride, so ids (and birth steps, R9) are implied by the slot.  Persistent
+// grid-stride loop; up to kMaxFused model steps per launch.
+template <int K, bool TWO>
+__global__ void __launch_bounds__(kStepThreads) step_slots_kernel(const __grid_constant__ StepArgs A)
+{
+    Acc<K> acc;
+#pragma unroll
+    for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = 0.0f;
+
+    const uint64_t stride = (uint64_t)gridDim.x * kStepThreads;
+    for (uint64_t l = (uint64_t)blockIdx.x * kStepThreads + threadIdx.x; l < A.n; l += stride) {
+        const uint64_t slot = A.base + l;
+        const uint32_t pid = (uint32_t)(A.pid_offset + l * A.pid_stride);
+        float x, y, z, q[K];
+        int s_begin = 0;
+        if (l >= A.n_prev) {
+            // born inside this launch (R9): count mode b = s_start + floor(j*S/N), rate mode
+            // b = s_start + l / c
+            const int64_t b = A.rel_N ? A.rel_s_start + (int64_t)(((uint64_t)pid * (uint64_t)A.rel_S) / A.rel_N)
+                                      : A.rel_s_start + (int64_t)(l / A.rel_c);
+            s_begin = (int)(b - (int64_t)A.step0);
+            x = A.sx; y = A.sy; z = A.sz;
+#pragma unroll
+            for (int k = 0; k < K; ++k) q[k] = (float)(A.emit[k] / A.tab[s_begin].G[k]);
+        } else {
+            const float4 p = A.xyzq[slot];
+            x = p.x; y = p.y; z = p.z; q[0] = p.w;
+            if (K > 1) q[1] = A.q1[slot];
+            if (z < 0.0f) continue;  // exited earlier (ABSORB without compaction)
+        }
+        bool alive = true;
+        for (int s = s_begin; s < A.m_steps; ++s) {
+            alive = step_once<K, TWO>(A, A.tab[s], (uint32_t)(A.step0 + s), pid, x, y, z, q, acc);
+            if (!alive) break;
+        }
+        if (!alive) z = -1.0f - z;  // exit position kept, slot marked inactive
+        A.xyzq[slot] = make_float4(x, y, z, q[0]);
+        if (K > 1) A.q1[slot] = q[1];
+    }
+    flush_ledger<K>(A, acc);
+}
+
+// ------------------------------------------------------------------ compacting kernel (a7)
+// One model step with stable in-place stream compaction of the particles that left the domain,
+// fused into the store: each 256-particle tile steps its particles, counts survivors, obtains its
+// exclusive output offset from a single-pass decoupled look-back over the tile states, and
+// writes its survivors at [offset, offset + count).  In place is safe: a tile publishes only
+// after it has loaded its inputs, and the destination range of tile t lies inside the source
+// ranges of tiles <= t, all of which have published (hence loaded) before t learns its offset.
+__device__ __forceinline__ uint64_t ld_state(const uint64_t *p)
+{
+    uint64_t v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_state(uint64_t *p, uint64_t v)
+{
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+template <int K, bool TWO>
+__global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid_constant__ StepArgs A)
+{
+    __shared__ uint32_t s_tile;
+    __shared__ uint32_t s_wtot[kStepThreads / 32];
+    __shared__ uint32_t s_excl;
+    Acc<K> acc;
+#pragma unroll
+    for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = 0.0f;
+
+    const uint64_t n = A.ctrl[0];
+    const uint32_t n_tiles = (uint32_t)((n + kScanTile - 1) / kScanTile);
+    const uint32_t epoch = ((uint32_t)(A.step0 + 1) & 0x3fffffffu) << 2;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    constexpr uint32_t FLAG_A = 1u, FLAG_P = 2u;
+
+    for (;;) {
+        if (threadIdx.x == 0) s_tile = (uint32_t)atomicAdd((unsigned long long *)(A.ctrl + 1), 1ull);
+        __syncthreads();
+        const uint32_t tile = s_tile;
+        if (tile >= n_tiles) break;
+
+        const uint64_t i = (uint64_t)tile * kScanTile + threadIdx.x;
+        bool alive = false;
+        float x = 0.f, y = 0.f, z = 0.f, q[K];
+        uint32_t pid = 0;
+        if (i < n) {
+            const float4 p = A.xyzq[i];
+            x = p.x; y = p.y; z = p.z; q[0] = p.w;
+            if (K > 1) q[1] = A.q1[i];
+            pid = A.pid[i];
+            alive = step_once<K, TWO>(A, A.tab[0], (uint32_t)A.step0, pid, x, y, z, q, acc);
+        }
+        // survivors: rank inside the tile
+        const uint32_t ball = __ballot_sync(0xffffffffu, alive);
+        const uint32_t rank = __popc(ball & ((1u << lane) - 1u));
+        if (lane == 0) s_wtot[warp] = __popc(ball);
+        __syncthreads();  // also orders every thread's input loads before the publication below
+        uint32_t woff = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < kStepThreads / 32; ++w) {
+            const uint32_t t = s_wtot[w];
+            woff += (w < warp) ? t : 0u;
+            total += t;
+        }
+        if (warp == 0) {
+            uint32_t excl = 0;
+            if (lane == 0) {
+                __threadfence();
+                st_state(A.tile_state + tile, ((uint64_t)(epoch | (tile == 0 ? FLAG_P : FLAG_A)) << 32) | total);
+            }
+            if (tile > 0) {
+                // warp-wide look-back: lane l inspects tile (look - l)
+                int look = (int)tile - 1;
+                for (;;) {
+                    const int t = look - lane;
+                    uint64_t st = 0;
+                    uint32_t flag = FLAG_P, val = 0;
+                    if (t >= 0) {
+                        do { st = ld_state(A.tile_state + t); } while (((uint32_t)(st >> 32) & ~3u) != epoch);
+                        flag = (uint32_t)(st >> 32) & 3u;
+                        val = (uint32_t)st;
+                    }
+                    const uint32_t pmask = __ballot_sync(0xffffffffu, flag == FLAG_P);
+                    const int first_p = __ffs(pmask) - 1;  // t < 0 lanes count as P with value 0
+                    uint32_t contrib = (lane <= first_p) ? val : 0u;
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
+                    excl += contrib;
+                    if (pmask) break;
+                    look -= 32;
+                }
+                if (lane == 0) st_state(A.tile_state + tile, ((uint64_t)(epoch | FLAG_P) << 32) | (excl + total));
+            }
+            if (lane == 0) {
+                s_excl = excl;
+                if (tile == n_tiles - 1) A.ctrl[2] = (uint64_t)excl + total;
+                __threadfence();
+            }
+        }
+        __syncthreads();
+        if (alive) {
+            const uint64_t dst = (uint64_t)s_excl + woff + rank;
+            A.xyzq[dst] = make_float4(x, y, z, q[0]);
+            if (K > 1) A.q1[dst] = q[1];
+            A.pid[dst] = pid;
+        }
+        __syncthreads();  // s_tile / s_wtot / s_excl are reused by the next tile
+    }
+    flush_ledger<K>(A, acc);
+}
+
+// newborn particles of one step, appended behind the live ones (compact mode, R9)
+__global__ void __launch_bounds__(256) inject_kernel(const __grid_constant__ InjectArgs A)
+{
+    const uint64_t n_prev = A.ctrl[2];
+    uint64_t running = n_prev;
+    const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint64_t gstride = (uint64_t)gridDim.x * blockDim.x;
+    for (int r = 0; r < A.n_spec; ++r) {
+        const InjectSpec &sp = A.spec[r];
+        const uint64_t room = A.capacity > running ? A.capacity - running : 0;
+        const uint64_t take = sp.count < room ? sp.count : room;  // highest j skipped (R9)
+        for (uint64_t j = gtid; j < take; j += gstride) {
+            const uint64_t slot = running + j;
+            A.xyzq[slot] = make_float4(sp.sx, sp.sy, sp.sz, sp.q[0]);
+            if (A.K > 1) A.q1[slot] = sp.q[1];
+            A.pid[slot] = (uint32_t)(sp.first_pid + j * sp.pid_stride);
+        }
+        if (gtid == 0) A.ctrl[8 + sp.rel_index] += take;  // per-release emitted count (ledger)
+        running += take;
+    }
+    if (gtid == 0) {
+        A.ctrl[0] = running;
+        A.ctrl[1] = 0;
+        if (A.log_slot) *A.log_slot = running - n_prev;
+    }
+}
+
+// ------------------------------------------------------------------ launchers
+template <int K, bool TWO>
+static cudaError_t launch_t(const StepArgs &a, bool compact, int blocks, cudaStream_t st)
+{
+    if (compact) step_compact_kernel<K, TWO><<<blocks, kStepThreads, 0, st>>>(a);
+    else step_slots_kernel<K, TWO><<<blocks, kStepThreads, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_step(const StepArgs &a, int K, bool compact, int blocks, cudaStream_t st)
+{
+    const bool two = a.nt > 1;
+    if (K == 1) return two ? launch_t<1, true>(a, compact, blocks, st) : launch_t<1, false>(a, compact, blocks, st);
+    return two ? launch_t<2, true>(a, compact, blocks, st) : launch_t<2, false>(a, compact, blocks, st);
+}
+
+template <int K, bool TWO>
+static int occ_t(bool compact)
+{
+    int nb = 0;
+    if (compact) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_compact_kernel<K, TWO>, kStepThreads, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_slots_kernel<K, TWO>, kStepThreads, 0);
+    return nb;
+}
+
+int step_max_blocks_per_sm(int K, bool compact, bool two)
+{
+    if (K == 1) return two ? occ_t<1, true>(compact) : occ_t<1, false>(compact);
+    return two ? occ_t<2, true>(compact) : occ_t<2, false>(compact);
+}
+
+cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st)
+{
+    uint64_t mx = 0;
+    for (int r = 0; r < a.n_spec; ++r) mx = a.spec[r].count > mx ? a.spec[r].count : mx;
+    int blocks = (int)((mx + 255) / 256);
+    if (blocks < 1) blocks = 1;
+    if (blocks > 1184) blocks = 1184;
+    inject_kernel<<<blocks, 256, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace lpm
