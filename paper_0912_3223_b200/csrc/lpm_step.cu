@@ -255,7 +255,7 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
                         val = (uint32_t)st;
                     }
                     const uint32_t pmask = __ballot_sync(0xffffffffu, flag == FLAG_P);
-                    const int first_p = __ffs(pmask) - 1;  // t < 0 lanes count as P with value 0
+                    const int first_p = pmask ? __ffs(pmask) - 1 : 31;  // t < 0 lanes count as P with value 0; no P: all 32 aggregates count
                     uint32_t contrib = (lane <= first_p) ? val : 0u;
 #pragma unroll
                     for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
