@@ -189,6 +189,30 @@ const char *lpm_last_error(lpm_handle *h);
 /* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
 int32_t lpm_launch_count(lpm_handle *h, uint64_t *n_host);
 
+/* ---- host-buffer entry points (end-to-end use: weather arrives from, results go to, host memory) */
+
+/* Copy n_snapshots meteorological snapshots from HOST memory (pinned for full PCIe speed) into
+ * the borrowed device array meteo.fields_dev, starting at snapshot index `first` (P:L104-106:
+ * the weather data of the coming interval are loaded before it is simulated).  Asynchronous on
+ * the handle's stream.  Errors: INVALID_ARG (null, range outside [0, nt)), CUDA. */
+int32_t lpm_upload_meteo(lpm_handle *h, int32_t first, int32_t n_snapshots, const void *fields_host);
+/* lpm_concentration / lpm_deposition into HOST buffers: read-out kernel into a staging area of the
+ * workspace, then a device-to-host copy on the handle's stream; returns after the copy has
+ * completed (the stream is synchronised), so out_host is valid on return. */
+int32_t lpm_concentration_host(lpm_handle *h, float *out_host);
+int32_t lpm_deposition_host(lpm_handle *h, float *out_host);
+
+/* ---- timing hooks (bench.py's per-kernel roofline numbers) --------------------------------- */
+
+/* enable != 0: bracket every step-kernel and every binning-kernel launch of this handle with CUDA
+ * events on the handle's stream (two cudaEventRecord per launch); also clears the totals. */
+int32_t lpm_set_timing(lpm_handle *h, int32_t enable);
+/* Synchronises, then returns out_host[0] = total ms in step kernels, [1] = their launch count,
+ * [2] = total ms in binning kernels (memsets of the grids included), [3] = their launch count,
+ * [4] = particle-steps executed by the timed step launches (born particles x steps, host count),
+ * [5] = particles read by the timed binning launches; accumulated since lpm_set_timing. */
+int32_t lpm_get_timing(lpm_handle *h, double *out_host /* [6] */);
+
 /* ---- stand-alone kernels for parity tests (device arrays in, device arrays out) ------------ */
 
 /* Philox4x32-10 (R1): out_dev[4*i..] = philox(key = seed, ctr = (step, stream, pid_lo, pid_hi))

@@ -26,7 +26,8 @@ SYMBOLS = (
     "lpm_set_rain", "lpm_release", "lpm_step", "lpm_concentration", "lpm_counts", "lpm_deposition",
     "lpm_deposition_f64", "lpm_bin_now", "lpm_num_active", "lpm_step_index", "lpm_mass_scale", "lpm_get_particles",
     "lpm_set_particles", "lpm_ledger", "lpm_injected", "lpm_last_error", "lpm_launch_count", "lpm_test_philox",
-    "lpm_test_normals", "lpm_test_sample",
+    "lpm_test_normals", "lpm_test_sample", "lpm_upload_meteo", "lpm_concentration_host", "lpm_deposition_host",
+    "lpm_set_timing", "lpm_get_timing",
 )
 
 
@@ -99,6 +100,11 @@ def load():
     L.lpm_last_error.argtypes = [vp]
     L.lpm_last_error.restype = C.c_char_p
     L.lpm_launch_count.argtypes = [vp, C.POINTER(u64)]
+    L.lpm_upload_meteo.argtypes = [vp, i32, i32, vp]
+    L.lpm_concentration_host.argtypes = [vp, vp]
+    L.lpm_deposition_host.argtypes = [vp, vp]
+    L.lpm_set_timing.argtypes = [vp, i32]
+    L.lpm_get_timing.argtypes = [vp, C.POINTER(dbl)]
     L.lpm_test_philox.argtypes = [u64, u64, C.c_uint32, u64, u64, vp, vp]
     L.lpm_test_normals.argtypes = [u64, u64, u64, u64, vp, vp]
     L.lpm_test_sample.argtypes = [C.POINTER(lpm_meteo), dbl, vp, u64, vp, vp]
@@ -241,6 +247,31 @@ class Simulation:
         fn = self._L.lpm_deposition_f64 if f64 else self._L.lpm_deposition
         self._ck(fn(self._h, out.data_ptr()), "lpm_deposition")
         return out
+
+    # host-buffer entry points: pinned CPU tensors in / out
+    def upload_meteo(self, first: int, fields_host):
+        """fields_host: CPU float32 tensor [n][nz][ny][nx][4] (pinned for full PCIe speed)."""
+        assert fields_host.device.type == "cpu" and fields_host.is_contiguous() and fields_host.dtype == self.torch.float32
+        self._ck(self._L.lpm_upload_meteo(self._h, first, fields_host.shape[0], fields_host.data_ptr()), "lpm_upload_meteo")
+
+    def concentration_host(self, out):
+        assert out.device.type == "cpu" and out.is_contiguous() and out.dtype == self.torch.float32
+        self._ck(self._L.lpm_concentration_host(self._h, out.data_ptr()), "lpm_concentration_host")
+        return out
+
+    def deposition_host(self, out):
+        assert out.device.type == "cpu" and out.is_contiguous() and out.dtype == self.torch.float32
+        self._ck(self._L.lpm_deposition_host(self._h, out.data_ptr()), "lpm_deposition_host")
+        return out
+
+    def set_timing(self, on: bool = True):
+        self._ck(self._L.lpm_set_timing(self._h, 1 if on else 0), "lpm_set_timing")
+
+    def get_timing(self):
+        out = (C.c_double * 6)()
+        self._ck(self._L.lpm_get_timing(self._h, out), "lpm_get_timing")
+        return dict(step_ms=out[0], step_launches=int(out[1]), bin_ms=out[2], bin_launches=int(out[3]),
+                    particle_steps=out[4], binned_particles=out[5])
 
     @property
     def num_active(self) -> int:

@@ -27,7 +27,7 @@ struct Release {
 };
 
 struct Layout {
-    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, total;
+    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, total;
 };
 
 uint64_t up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
@@ -48,6 +48,7 @@ Layout make_layout(const lpm_grid &g, uint64_t cap, int K, bool compact)
     L.ctrl = o; o += up(8 * 32);
     L.tile = o; o += compact ? up(8 * (cap / kScanTile + 2)) : 0;
     L.injlog = o; o += compact ? up(8 * kInjLog) : 0;
+    L.stage = o; o += up(4 * cells3 * K);  // fp32 read-out staging for the *_host entry points
     L.total = o;
     return L;
 }
@@ -90,6 +91,14 @@ struct lpm_handle {
     bool binned;
     int sms, occ;
     uint64_t launches;
+    // timing hooks: event pairs around step / binning launches
+    bool timing;
+    struct Span { cudaEvent_t a, b; int kind; };
+    std::vector<Span> spans;
+    std::vector<cudaEvent_t> ev_pool;
+    double t_ms[2], t_units[2];
+    uint64_t t_base;  // compact mode: device particle-step counter at lpm_set_timing
+    uint64_t t_launches[2];
     int sticky;
     char err[512];
 };
@@ -116,6 +125,40 @@ int cuda_fail(lpm_handle *h, cudaError_t e, const char *where)
         cudaError_t e_ = (call);                                   \
         if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);     \
     } while (0)
+
+cudaEvent_t ev_get(lpm_handle *h)
+{
+    if (!h->ev_pool.empty()) { cudaEvent_t e = h->ev_pool.back(); h->ev_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+
+// open / close a timed span of kind 0 (step kernel) or 1 (binning) on the handle's stream
+int span_open(lpm_handle *h, int kind, double units)
+{
+    if (!h->timing) return -1;
+    lpm_handle::Span sp{ev_get(h), ev_get(h), kind};
+    cudaEventRecord(sp.a, h->st);
+    h->spans.push_back(sp);
+    h->t_units[kind] += units;
+    h->t_launches[kind]++;
+    return (int)h->spans.size() - 1;
+}
+void span_close(lpm_handle *h, int id)
+{
+    if (id >= 0) cudaEventRecord(h->spans[id].b, h->st);
+}
+void spans_collect(lpm_handle *h)
+{
+    for (auto &sp : h->spans) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) h->t_ms[sp.kind] += (double)ms;
+        h->ev_pool.push_back(sp.a);
+        h->ev_pool.push_back(sp.b);
+    }
+    h->spans.clear();
+}
 
 double G_of(const lpm_handle *h, int k, uint64_t step) { return exp((double)step * h->ln_rho[k]); }
 
@@ -204,6 +247,7 @@ int grid_blocks(const lpm_handle *h, uint64_t n)
 int do_bin(lpm_handle *h)
 {
     const uint64_t cells3 = (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz;
+    const int span = span_open(h, 1, 0.0);
     CK(cudaMemsetAsync(h->ws + h->L.cnt, 0, 4 * cells3, h->st));
     CK(cudaMemsetAsync(h->ws + h->L.conc, 0, 8 * cells3 * h->K, h->st));
     BinArgs B{};
@@ -218,6 +262,7 @@ int do_bin(lpm_handle *h)
         B.n_dev = (const uint64_t *)(h->ws + h->L.ctrl) + 2;
         CK(launch_bin(B, h->sms * 8, h->st));
         h->launches++;
+        // the live count is device-side; the host's upper bound is the capacity (labelled so in bench.py)
     } else {
         for (const Release &r : h->rel) {
             const uint64_t n = born_local(r, (int64_t)h->step - 1);
@@ -228,8 +273,10 @@ int do_bin(lpm_handle *h)
             const uint64_t want = (n + 255) / 256;
             CK(launch_bin(B, (int)(want < (uint64_t)h->sms * 8 ? want : (uint64_t)h->sms * 8), h->st));
             h->launches++;
+            if (h->timing) h->t_units[1] += (double)n;
         }
     }
+    span_close(h, span);
     h->bin_step = h->step;
     h->binned = true;
     return LPM_OK;
@@ -330,6 +377,8 @@ int32_t lpm_destroy(lpm_handle *h)
 {
     if (!h) return LPM_ERR_INVALID_ARG;
     cudaStreamSynchronize(h->st);
+    spans_collect(h);
+    for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
     delete h;
     return LPM_OK;
 }
@@ -417,7 +466,9 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                 for (int k = 0; k < h->K; ++k) sp.q[k] = (float)(r.emit[k] / A.tab[0].G[k]);
             }
             CK(launch_inject(I, h->st));
+            const int span = span_open(h, 0, 0.0);
             CK(launch_step(A, h->K, true, h->sms * (h->occ > 0 ? h->occ : 1), h->st));
+            span_close(h, span);
             h->launches += 2;
         } else {
             for (const Release &r : h->rel) {
@@ -431,7 +482,13 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                 A.rel_s_start = r.s_start; A.rel_S = r.S;
                 for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) A.emit[k] = r.emit[k];
                 A.sx = (float)r.src.x; A.sy = (float)r.src.y; A.sz = (float)r.src.z;
+                double units = 0.0;
+                if (h->timing)
+                    for (int s = 0; s < m; ++s) units += (double)born_local(r, (int64_t)h->step + s);
+                CK(cudaMemsetAsync(A.ctrl + 16, 0, 8, h->st));  // tile ticket of the slot kernel
+                const int span = span_open(h, 0, units);
                 CK(launch_step(A, h->K, false, grid_blocks(h, n), h->st));
+                span_close(h, span);
                 h->launches++;
             }
         }
@@ -634,6 +691,70 @@ int32_t lpm_injected(lpm_handle *h, uint64_t step, uint64_t *n)
         CK(cudaStreamSynchronize(h->st));
     } else {
         for (const Release &r : h->rel) *n += born_local(r, (int64_t)step) - born_local(r, (int64_t)step - 1);
+    }
+    return LPM_OK;
+}
+
+int32_t lpm_upload_meteo(lpm_handle *h, int32_t first, int32_t n_snap, const void *src)
+{
+    if (!h || !src || first < 0 || n_snap < 1 || first + n_snap > h->met.nt) return fail(h, LPM_ERR_INVALID_ARG, "lpm_upload_meteo: null or range");
+    if (h->sticky) return h->sticky;
+    const lpm_grid &g = h->met.grid;
+    const uint64_t snap_bytes = 16ull * g.nx * g.ny * g.nz;
+    CK(cudaMemcpyAsync((char *)h->met.fields_dev + (uint64_t)first * snap_bytes, src, snap_bytes * (uint64_t)n_snap,
+                       cudaMemcpyHostToDevice, h->st));
+    return LPM_OK;
+}
+
+int32_t lpm_concentration_host(lpm_handle *h, float *out)
+{
+    if (!h || !out) return fail(h, LPM_ERR_INVALID_ARG, "lpm_concentration_host: null");
+    float *stage = (float *)(h->ws + h->L.stage);
+    const int rc = lpm_concentration(h, stage);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(out, stage, 4ull * h->cg.nx * h->cg.ny * h->cg.nz * h->K, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    return LPM_OK;
+}
+
+int32_t lpm_deposition_host(lpm_handle *h, float *out)
+{
+    if (!h || !out) return fail(h, LPM_ERR_INVALID_ARG, "lpm_deposition_host: null");
+    float *stage = (float *)(h->ws + h->L.stage);
+    const int rc = lpm_deposition(h, stage);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(out, stage, 4ull * h->cg.nx * h->cg.ny * h->K, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    return LPM_OK;
+}
+
+int32_t lpm_set_timing(lpm_handle *h, int32_t enable)
+{
+    if (!h) return LPM_ERR_INVALID_ARG;
+    CK(cudaStreamSynchronize(h->st));
+    spans_collect(h);
+    h->timing = enable != 0;
+    for (int i = 0; i < 2; ++i) { h->t_ms[i] = 0.0; h->t_units[i] = 0.0; h->t_launches[i] = 0; }
+    if (h->prm.compact) {
+        CK(cudaMemcpyAsync(&h->t_base, (uint64_t *)(h->ws + h->L.ctrl) + 3, 8, cudaMemcpyDeviceToHost, h->st));
+        CK(cudaStreamSynchronize(h->st));
+    }
+    return LPM_OK;
+}
+
+int32_t lpm_get_timing(lpm_handle *h, double *out)
+{
+    if (!h || !out) return LPM_ERR_INVALID_ARG;
+    CK(cudaStreamSynchronize(h->st));
+    spans_collect(h);
+    out[0] = h->t_ms[0]; out[1] = (double)h->t_launches[0];
+    out[2] = h->t_ms[1]; out[3] = (double)h->t_launches[1];
+    out[4] = h->t_units[0]; out[5] = h->t_units[1];
+    if (h->prm.compact) {  // the live count is device-side: cumulative particle-steps since lpm_set_timing
+        uint64_t now = 0;
+        CK(cudaMemcpyAsync(&now, (uint64_t *)(h->ws + h->L.ctrl) + 3, 8, cudaMemcpyDeviceToHost, h->st));
+        CK(cudaStreamSynchronize(h->st));
+        out[4] = (double)(now - h->t_base);
     }
     return LPM_OK;
 }

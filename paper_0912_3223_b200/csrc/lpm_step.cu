@@ -19,13 +19,39 @@ namespace lpm {
 template <int K>
 struct Acc {  // per-thread ledger partial sums, in activity units before the per-nuclide scale
     float dry[K], wet[K], dec[K];
+    float off[K];  // deposit that fell off the map (already scaled)
 };
+
+// a6 run-length aggregation: a particle stays in one 2-D map cell for several steps, so its
+// deposit increments are summed in registers and sent to the map (one fp64 RED per nuclide) only
+// when the cell changes or the launch ends.  cell: >= 0 map cell, -1 off the map, -2 empty.
+template <int K>
+struct Dep {
+    int cell;
+    float a[K];
+};
+
+template <int K>
+__device__ __forceinline__ void dep_flush(const StepArgs &A, Dep<K> &d, Acc<K> &acc)
+{
+    if (d.cell >= 0) {
+        double *p = A.dep + (uint32_t)d.cell;
+#pragma unroll
+        for (int k = 0; k < K; ++k) atomicAdd(p + k * A.dep_stride, (double)d.a[k]);
+    } else if (d.cell == -1) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) acc.off[k] += d.a[k];
+    }
+    d.cell = -2;
+#pragma unroll
+    for (int k = 0; k < K; ++k) d.a[k] = 0.0f;
+}
 
 // One model step of one particle.  Returns false when the particle left the domain (ABSORB).
 template <int K, bool TWO>
 __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e, uint32_t step_lo,
                                           uint32_t pid_lo, float &x, float &y, float &z,
-                                          float (&q)[K], Acc<K> &acc)
+                                          float (&q)[K], Acc<K> &acc, Dep<K> &dep)
 {
     // a1: three N(0,1) from Philox stream 0
     const uint4 r = philox4x32_10(step_lo, 0u, pid_lo, 0u, A.seed_lo, A.seed_hi);
@@ -90,18 +116,17 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
         acc.dec[k] += act;
     }
 
-    // a6: deposit scatter at the cell of the NEW (x, y)
+    // a6: deposit at the cell of the NEW (x, y), run-length aggregated in registers
     if (dry_here | wet_here) {
         const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
         const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
-        if ((ci | cj) >= 0) {
-            double *d = A.dep + (uint32_t)(cj * A.cg.nx + ci);
-#pragma unroll
-            for (int k = 0; k < K; ++k) atomicAdd(d + k * A.dep_stride, (double)inc[k]);
-        } else {
-#pragma unroll
-            for (int k = 0; k < K; ++k) atomicAdd(A.ledger + k * 8 + 6, (double)inc[k]);
+        const int c = (ci | cj) >= 0 ? cj * A.cg.nx + ci : -1;
+        if (c != dep.cell) {
+            dep_flush<K>(A, dep, acc);
+            dep.cell = c;
         }
+#pragma unroll
+        for (int k = 0; k < K; ++k) dep.a[k] += inc[k];
     }
     return true;
 }
@@ -111,21 +136,21 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
 template <int K>
 __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &acc)
 {
-    __shared__ float s_part[kStepThreads / 32][3 * K];
+    __shared__ float s_part[kStepThreads / 32][4 * K];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
     for (int k = 0; k < K; ++k) {
-        const float d = warp_sum(acc.dry[k]), w = warp_sum(acc.wet[k]), c = warp_sum(acc.dec[k]);
-        if (lane == 0) { s_part[warp][3 * k] = d; s_part[warp][3 * k + 1] = w; s_part[warp][3 * k + 2] = c; }
+        const float d = warp_sum(acc.dry[k]), w = warp_sum(acc.wet[k]), c = warp_sum(acc.dec[k]), o = warp_sum(acc.off[k]);
+        if (lane == 0) { s_part[warp][4 * k] = d; s_part[warp][4 * k + 1] = w; s_part[warp][4 * k + 2] = c; s_part[warp][4 * k + 3] = o; }
     }
     __syncthreads();
-    if (threadIdx.x < 3 * K) {
+    if (threadIdx.x < 4 * K) {
         double s = 0.0;
 #pragma unroll
         for (int w = 0; w < kStepThreads / 32; ++w) s += (double)s_part[w][threadIdx.x];
-        const int k = threadIdx.x / 3, f = threadIdx.x % 3;
-        const double scale = f == 0 ? (double)A.p_dry[k] : (f == 1 ? A.wet_scale[k] : A.dec_scale[k]);
-        if (s != 0.0) atomicAdd(A.ledger + k * 8 + 2 + f, s * scale);
+        const int k = threadIdx.x / 4, f = threadIdx.x % 4;
+        const double scale = f == 0 ? (double)A.p_dry[k] : (f == 1 ? A.wet_scale[k] : (f == 2 ? A.dec_scale[k] : 1.0));
+        if (s != 0.0) atomicAdd(A.ledger + k * 8 + (f == 3 ? 6 : 2 + f), s * scale);
     }
 }
 
@@ -136,12 +161,28 @@ __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &ac
 template <int K, bool TWO>
 __global__ void __launch_bounds__(kStepThreads) step_slots_kernel(const __grid_constant__ StepArgs A)
 {
+    __shared__ uint32_t s_ticket;
     Acc<K> acc;
 #pragma unroll
-    for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = 0.0f;
+    for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = acc.off[k] = 0.0f;
 
-    const uint64_t stride = (uint64_t)gridDim.x * kStepThreads;
-    for (uint64_t l = (uint64_t)blockIdx.x * kStepThreads + threadIdx.x; l < A.n; l += stride) {
+    // Dynamic, DECORRELATED tile schedule: ticket t -> tile (t % G) * R + t / G, so the CTAs that
+    // are resident together work on tiles spread over the whole slot range (= over all particle
+    // ages, hence over the whole plume) instead of on ~3e5 neighbouring particles that would all
+    // hit the same few deposition-map cells and met lines at the same time.
+    const uint32_t n_tiles = (uint32_t)((A.n + kStepThreads - 1) / kStepThreads);
+    const uint32_t G = min(n_tiles, (uint32_t)gridDim.x);
+    const uint32_t R = (n_tiles + G - 1) / G;
+    const uint32_t n_tickets = G * R;
+    for (;;) {
+        __syncthreads();
+        if (threadIdx.x == 0) s_ticket = (uint32_t)atomicAdd((unsigned long long *)(A.ctrl + 16), 1ull);
+        __syncthreads();
+        const uint32_t t = s_ticket;
+        if (t >= n_tickets) break;
+        const uint32_t tile = (t % G) * R + t / G;
+        const uint64_t l = (uint64_t)tile * kStepThreads + threadIdx.x;
+        if (l >= A.n) continue;
         const uint64_t slot = A.base + l;
         const uint32_t pid = (uint32_t)(A.pid_offset + l * A.pid_stride);
         float x, y, z, q[K];
@@ -161,11 +202,16 @@ __global__ void __launch_bounds__(kStepThreads) step_slots_kernel(const __grid_c
             if (K > 1) q[1] = A.q1[slot];
             if (z < 0.0f) continue;  // exited earlier (ABSORB without compaction)
         }
+        Dep<K> dep;
+        dep.cell = -2;
+#pragma unroll
+        for (int k = 0; k < K; ++k) dep.a[k] = 0.0f;
         bool alive = true;
         for (int s = s_begin; s < A.m_steps; ++s) {
-            alive = step_once<K, TWO>(A, A.tab[s], (uint32_t)(A.step0 + s), pid, x, y, z, q, acc);
+            alive = step_once<K, TWO>(A, A.tab[s], (uint32_t)(A.step0 + s), pid, x, y, z, q, acc, dep);
             if (!alive) break;
         }
+        dep_flush<K>(A, dep, acc);
         if (!alive) z = -1.0f - z;  // exit position kept, slot marked inactive
         A.xyzq[slot] = make_float4(x, y, z, q[0]);
         if (K > 1) A.q1[slot] = q[1];
@@ -199,7 +245,7 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
     __shared__ uint32_t s_excl;
     Acc<K> acc;
 #pragma unroll
-    for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = 0.0f;
+    for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = acc.off[k] = 0.0f;
 
     const uint64_t n = A.ctrl[0];
     const uint32_t n_tiles = (uint32_t)((n + kScanTile - 1) / kScanTile);
@@ -222,7 +268,12 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
             x = p.x; y = p.y; z = p.z; q[0] = p.w;
             if (K > 1) q[1] = A.q1[i];
             pid = A.pid[i];
-            alive = step_once<K, TWO>(A, A.tab[0], (uint32_t)A.step0, pid, x, y, z, q, acc);
+            Dep<K> dep;
+            dep.cell = -2;
+#pragma unroll
+            for (int k = 0; k < K; ++k) dep.a[k] = 0.0f;
+            alive = step_once<K, TWO>(A, A.tab[0], (uint32_t)A.step0, pid, x, y, z, q, acc, dep);
+            dep_flush<K>(A, dep, acc);
         }
         // survivors: rank inside the tile
         const uint32_t ball = __ballot_sync(0xffffffffu, alive);
@@ -306,6 +357,7 @@ __global__ void __launch_bounds__(256) inject_kernel(const __grid_constant__ Inj
     if (gtid == 0) {
         A.ctrl[0] = running;
         A.ctrl[1] = 0;
+        A.ctrl[3] += running;  // cumulative particle-steps (timing hooks)
         if (A.log_slot) *A.log_slot = running - n_prev;
     }
 }
