@@ -16,7 +16,9 @@
  *    pointers; small structs are host structs copied at the call.
  *  - OWNERSHIP: the caller owns every device buffer (workspace, met snapshots, outputs).  The
  *    library borrows `workspace_dev` and `meteo.fields_dev` for the life of the handle and never
- *    frees caller memory.
+ *    frees caller memory.  The library keeps a re-packed copy of the two snapshots of the current
+ *    met interval: snapshot data must be in place before the first step of the interval that uses
+ *    it, and later changes must go through lpm_upload_meteo (which invalidates the copy).
  *  - One handle = one GPU = one CUDA stream.  Calls enqueue work on that stream and return; calls
  *    that return host scalars (lpm_num_active, lpm_ledger, lpm_get_particles' count) synchronise
  *    the stream first.  A handle is not thread-safe.
@@ -101,9 +103,11 @@ int32_t lpm_version(void);
 /* Static text for a status code. */
 const char *lpm_status_string(int32_t status);
 
-/* Bytes of device workspace lpm_create needs (particle SoA store, grids, ledger, scan state). */
-int32_t lpm_workspace_bytes(const lpm_grid *conc_grid, const lpm_params *params, int32_t n_nuclides,
-                            uint64_t *bytes_host);
+/* Bytes of device workspace lpm_create needs (particle SoA store, grids, ledger, scan state,
+ * read-out staging and, when meteo->nt > 1, the interleaved snapshot-pair buffer of the current
+ * met interval: 32 bytes per met cell).  Only the grid and nt of `meteo` are read. */
+int32_t lpm_workspace_bytes(const lpm_grid *conc_grid, const lpm_meteo *meteo, const lpm_params *params,
+                            int32_t n_nuclides, uint64_t *bytes_host);
 
 /* R9 release schedule, count mode: how many of the LOCAL particles (global ids pid_offset +
  * l*pid_stride < n_particles) are born at steps <= step, for a release starting at step s_start

@@ -77,7 +77,7 @@ def load():
     L.lpm_version.restype = i32
     L.lpm_status_string.restype = C.c_char_p
     L.lpm_status_string.argtypes = [i32]
-    L.lpm_workspace_bytes.argtypes = [C.POINTER(lpm_grid), C.POINTER(lpm_params), i32, C.POINTER(u64)]
+    L.lpm_workspace_bytes.argtypes = [C.POINTER(lpm_grid), C.POINTER(lpm_meteo), C.POINTER(lpm_params), i32, C.POINTER(u64)]
     L.lpm_schedule_born.argtypes = [u64, u64, u64, i64, i64, i64, C.POINTER(u64)]
     L.lpm_create.argtypes = [C.POINTER(lpm_grid), C.POINTER(lpm_meteo), C.POINTER(lpm_nuclide), i32,
                              C.POINTER(lpm_params), vp, u64, vp, C.POINTER(vp)]
@@ -127,11 +127,12 @@ def _grid(g) -> lpm_grid:
     return lpm_grid(g.nx, g.ny, g.nz, 0, g.x0, g.y0, g.z0, g.dx, g.dy, g.dz)
 
 
-def workspace_bytes(cgrid, capacity: int, n_nuclides: int, compact: bool) -> int:
+def workspace_bytes(cgrid, capacity: int, n_nuclides: int, compact: bool, mgrid=None, nt: int = 1) -> int:
     p = lpm_params(dt=1.0, capacity=capacity, compact=1 if compact else 0, h_dep=1.0)
     out = C.c_uint64()
     g = _grid(cgrid)
-    rc = load().lpm_workspace_bytes(C.byref(g), C.byref(p), n_nuclides, C.byref(out))
+    met = lpm_meteo(grid=_grid(mgrid if mgrid is not None else cgrid), nt=nt)
+    rc = load().lpm_workspace_bytes(C.byref(g), C.byref(met), C.byref(p), n_nuclides, C.byref(out))
     if rc:
         raise LpmError(rc, "lpm_workspace_bytes")
     return out.value
@@ -175,7 +176,7 @@ class Simulation:
             fields_dev = torch.from_numpy(np.ascontiguousarray(f)).to(self.device)
         assert fields_dev.dtype == torch.float32 and fields_dev.is_contiguous()
         self.fields_dev = fields_dev
-        nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact)
+        nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact, w.mgrid, w.nt)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         cg = _grid(w.cgrid)
         met = lpm_meteo(grid=_grid(w.mgrid), nt=w.nt, t0=w.t0, dt_snap=w.dt_snap, fields_dev=fields_dev.data_ptr(),

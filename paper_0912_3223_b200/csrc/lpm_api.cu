@@ -27,12 +27,12 @@ struct Release {
 };
 
 struct Layout {
-    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, total;
+    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, total;
 };
 
 uint64_t up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
-Layout make_layout(const lpm_grid &g, uint64_t cap, int K, bool compact)
+Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K, bool compact)
 {
     Layout L{};
     const uint64_t cells3 = (uint64_t)g.nx * g.ny * g.nz, cells2 = (uint64_t)g.nx * g.ny;
@@ -49,6 +49,7 @@ Layout make_layout(const lpm_grid &g, uint64_t cap, int K, bool compact)
     L.tile = o; o += compact ? up(8 * (cap / kScanTile + 2)) : 0;
     L.injlog = o; o += compact ? up(8 * kInjLog) : 0;
     L.stage = o; o += up(4 * cells3 * K);  // fp32 read-out staging for the *_host entry points
+    L.pair = o; o += met.nt > 1 ? up(32ull * met.grid.nx * met.grid.ny * met.grid.nz) : 0;  // (F_s, F_s+1) per met cell
     L.total = o;
     return L;
 }
@@ -88,6 +89,7 @@ struct lpm_handle {
     std::vector<Release> rel;
     uint64_t next_base;
     uint64_t step, bin_step;
+    int pair_snap;  // snapshot index s whose pair (s, s+1) the pair buffer holds, -1 = none
     bool binned;
     int sms, occ;
     uint64_t launches;
@@ -210,6 +212,7 @@ void base_args(const lpm_handle *h, StepArgs &A)
     A.q1 = h->K > 1 ? (float *)(h->ws + h->L.q1) : nullptr;
     A.pid = h->prm.compact ? (uint32_t *)(h->ws + h->L.pid) : nullptr;
     A.met = (const float4 *)h->met.fields_dev;
+    A.pair = h->met.nt > 1 ? (const void *)(h->ws + h->L.pair) : nullptr;
     const lpm_grid &mg = h->met.grid;
     A.snap_cells = (uint64_t)mg.nx * mg.ny * mg.nz;
     A.mg = gridf(mg);
@@ -302,11 +305,11 @@ const char *lpm_status_string(int32_t s)
     }
 }
 
-int32_t lpm_workspace_bytes(const lpm_grid *g, const lpm_params *p, int32_t K, uint64_t *bytes)
+int32_t lpm_workspace_bytes(const lpm_grid *g, const lpm_meteo *met, const lpm_params *p, int32_t K, uint64_t *bytes)
 {
-    if (!grid_ok(g) || !p || !bytes || K < 1 || K > LPM_MAX_NUCLIDES || p->capacity == 0 || p->capacity >= (1ull << 32))
+    if (!grid_ok(g) || !met || !grid_ok(&met->grid) || met->nt < 1 || !p || !bytes || K < 1 || K > LPM_MAX_NUCLIDES || p->capacity == 0 || p->capacity >= (1ull << 32))
         return LPM_ERR_INVALID_ARG;
-    *bytes = make_layout(*g, p->capacity, K, p->compact != 0).total;
+    *bytes = make_layout(*g, *met, p->capacity, K, p->compact != 0).total;
     return LPM_OK;
 }
 
@@ -338,7 +341,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return LPM_ERR_NO_DEVICE;
     if (prop.major != 10) return LPM_ERR_NO_DEVICE;
 
-    const Layout L = make_layout(*cg, p->capacity, K, p->compact != 0);
+    const Layout L = make_layout(*cg, *met, p->capacity, K, p->compact != 0);
     if (ws_bytes < L.total) return LPM_ERR_WORKSPACE_TOO_SMALL;
 
     lpm_handle *h = new (std::nothrow) lpm_handle();
@@ -350,6 +353,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     h->L = L;
     h->sms = prop.multiProcessorCount;
     h->err[0] = 0;
+    h->pair_snap = -1;
     // R5 / R8 constants: double formula, rounded once to fp32 where the kernels consume fp32
     h->sigma_h = (float)sqrt(2.0 * met->Kh * p->dt);
     const bool uniform = p->h_dep >= met->H_mix;
@@ -445,8 +449,19 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
             if ((uint64_t)m > to_bin) m = (int)to_bin;
         }
         A.step0 = h->step;
+        for (int s = 0; s < m; ++s) {
+            fill_entry(h, h->step + s, A.tab[s]);
+            // a launch stays inside one met interval: the pair buffer holds snapshots (s, s+1)
+            if ((A.tab[s].snap & 0xffff) != (A.tab[0].snap & 0xffff)) { m = s; break; }
+        }
         A.m_steps = m;
-        for (int s = 0; s < m; ++s) fill_entry(h, h->step + s, A.tab[s]);
+        if (h->met.nt > 1 && (A.tab[0].snap & 0xffff) != h->pair_snap) {
+            const int sn = A.tab[0].snap & 0xffff;
+            CK(launch_pair_repack(A.met + (uint64_t)sn * A.snap_cells, A.met + (uint64_t)(sn + 1) * A.snap_cells,
+                                  h->ws + h->L.pair, A.snap_cells, h->st));
+            h->launches++;
+            h->pair_snap = sn;
+        }
         if (compact) {
             InjectArgs I{};
             I.xyzq = A.xyzq; I.q1 = A.q1; I.pid = A.pid; I.ctrl = A.ctrl;
@@ -703,6 +718,7 @@ int32_t lpm_upload_meteo(lpm_handle *h, int32_t first, int32_t n_snap, const voi
     const uint64_t snap_bytes = 16ull * g.nx * g.ny * g.nz;
     CK(cudaMemcpyAsync((char *)h->met.fields_dev + (uint64_t)first * snap_bytes, src, snap_bytes * (uint64_t)n_snap,
                        cudaMemcpyHostToDevice, h->st));
+    if (h->pair_snap >= first - 1 && h->pair_snap < first + n_snap) h->pair_snap = -1;  // the pair buffer is stale
     return LPM_OK;
 }
 
@@ -799,9 +815,26 @@ int32_t lpm_test_sample(const lpm_meteo *met, double t, const void *xyz, uint64_
     tmp.prm.dt = t;
     fill_entry(&tmp, 1, e);
     const lpm_grid &g = met->grid;
-    return launch_test_sample((const float4 *)met->fields_dev, (uint64_t)g.nx * g.ny * g.nz, gridf(g), met->nt > 1, e.snap & 0xffff,
-                              e.a, (float)met->kz_min, (const float4 *)xyz, n, (float4 *)out, (cudaStream_t)st) == cudaSuccess
-               ? LPM_OK : LPM_ERR_CUDA;
+    const uint64_t cells = (uint64_t)g.nx * g.ny * g.nz;
+    const float4 *f = (const float4 *)met->fields_dev;
+    cudaStream_t s = (cudaStream_t)st;
+    const int sn = e.snap & 0xffff;
+    void *pair = nullptr;
+    if (met->nt > 1) {  // same path as lpm_step: interleave snapshots (sn, sn+1), then sample the pair buffer
+        if (cudaMalloc(&pair, 32 * cells) != cudaSuccess) return LPM_ERR_CUDA;
+        if (launch_pair_repack(f + (uint64_t)sn * cells, f + (uint64_t)(sn + 1) * cells, pair, cells, s) != cudaSuccess) {
+            cudaFree(pair);
+            return LPM_ERR_CUDA;
+        }
+    }
+    cudaError_t rc = launch_test_sample(f + (uint64_t)sn * cells, pair, gridf(g), e.a, (float)met->kz_min, (const float4 *)xyz, n,
+                                        (float4 *)out, s);
+    if (pair) {
+        const cudaError_t rs = cudaStreamSynchronize(s);
+        if (rc == cudaSuccess) rc = rs;
+        cudaFree(pair);
+    }
+    return rc == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
 }
 
 }  // extern "C"

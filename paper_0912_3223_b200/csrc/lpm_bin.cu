@@ -202,24 +202,22 @@ cudaError_t launch_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uin
     return cudaGetLastError();
 }
 
-__global__ void test_sample_kernel(const float4 *met, uint64_t snap_cells, GridF mg, int two, int snap, float a, float kz_min,
+__global__ void test_sample_kernel(const float4 *met, const Texel2 *pair, GridF mg, float a, float kz_min,
                                    const float4 *xyz, uint64_t n, float4 *out)
 {
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
         const float4 p = xyz[i];
         const Corner c = corner_of(mg, p.x, p.y, p.z);
-        const float4 *s0 = met + (uint64_t)snap * snap_cells;
-        float4 m = trilinear(s0, c);
-        if (two) m = lerp4(m, trilinear(s0 + snap_cells, c), a);
+        float4 m = pair ? trilinear_pair(pair, c, a) : trilinear(met, c);   // the step kernel's two paths
         m.w = fmaxf(m.w, kz_min);
         out[i] = m;
     }
 }
 
-cudaError_t launch_test_sample(const float4 *met, uint64_t snap_cells, GridF mg, int two, int snap, float a, float kz_min,
+cudaError_t launch_test_sample(const float4 *met, const void *pair, GridF mg, float a, float kz_min,
                                const float4 *xyz, uint64_t n, float4 *out, cudaStream_t st)
 {
-    test_sample_kernel<<<148, 256, 0, st>>>(met, snap_cells, mg, two, snap, a, kz_min, xyz, n, out);
+    test_sample_kernel<<<148, 256, 0, st>>>(met, (const Texel2 *)pair, mg, a, kz_min, xyz, n, out);
     return cudaGetLastError();
 }
 

@@ -32,8 +32,10 @@ struct StepArgs {
     float4 *xyzq;
     float *q1;
     uint32_t *pid;        // compact mode only
-    // meteorology
+    // meteorology: `met` = caller's snapshots [nt][cells] (one-snapshot path); `pair` = the library's
+    // interleaved (F_s, F_s+1) buffer of the current met interval (two-snapshot path, 32 B per cell)
     const float4 *met;
+    const void *pair;
     uint64_t snap_cells;  // cells per snapshot
     GridF mg;
     int32_t nt;
@@ -102,6 +104,7 @@ struct BinArgs {
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int grid_blocks, cudaStream_t st);
 int step_max_blocks_per_sm(int K, bool compact, bool two_snap);
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
+cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, uint64_t cells, cudaStream_t st);
 cudaError_t launch_bin(const BinArgs &a, int blocks, cudaStream_t st);
 cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3, int K, const double *scale, cudaStream_t st);
 cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, double inv_area, cudaStream_t st);
@@ -111,7 +114,7 @@ cudaError_t launch_import(float4 *xyzq, uint64_t n, const uint8_t *status, cudaS
 cudaError_t launch_iota(uint32_t *pid, uint64_t n, cudaStream_t st);
 cudaError_t launch_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st);
 cudaError_t launch_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, float *out, cudaStream_t st);
-cudaError_t launch_test_sample(const float4 *met, uint64_t snap_cells, GridF mg, int two, int snap, float a, float kz_min,
+cudaError_t launch_test_sample(const float4 *met, const void *pair, GridF mg, float a, float kz_min,
                                const float4 *xyz, uint64_t n, float4 *out, cudaStream_t st);
 
 }  // namespace lpm

@@ -60,13 +60,9 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
 
     // a0 + a2: weather at X_old, t_n
     const Corner c = corner_of(A.mg, x, y, z);
-    const int snap = e.snap & 0xffff;
-    const float4 *s0 = A.met + (uint64_t)snap * A.snap_cells;
-    float4 m = trilinear(s0, c);
-    if (TWO) {
-        const float4 m1 = trilinear(s0 + A.snap_cells, c);
-        m = lerp4(m, m1, e.a);
-    }
+    float4 m;
+    if (TWO) m = trilinear_pair((const Texel2 *)A.pair, c, e.a);
+    else m = trilinear(A.met, c);
     const float kz = fmaxf(m.w, A.kz_min);
 
     // a3: Eq.(1) + Eq.(2)
@@ -391,6 +387,25 @@ int step_max_blocks_per_sm(int K, bool compact, bool two)
 {
     if (K == 1) return two ? occ_t<1, true>(compact) : occ_t<1, false>(compact);
     return two ? occ_t<2, true>(compact) : occ_t<2, false>(compact);
+}
+
+// a0: interleave the two snapshots of the current met interval into the pair buffer
+__global__ void __launch_bounds__(256) pair_repack_kernel(const float4 *__restrict__ s0, const float4 *__restrict__ s1,
+                                                          Texel2 *__restrict__ pair, uint64_t cells)
+{
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < cells; i += (uint64_t)gridDim.x * blockDim.x) {
+        Texel2 t;
+        t.a = __ldg(s0 + i);
+        t.b = __ldg(s1 + i);
+        pair[i] = t;
+    }
+}
+
+cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, uint64_t cells, cudaStream_t st)
+{
+    const uint64_t want = (cells + 255) / 256;
+    pair_repack_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(s0, s1, (Texel2 *)pair, cells);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st)
