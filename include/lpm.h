@@ -85,6 +85,10 @@ typedef struct {
     int32_t bin_every;      /* concentration binning cadence in steps ("n"); 0 = never   */
     int32_t steps_per_launch; /* 0 = auto; 1 = one model step per kernel launch; m > 1 fuses up to
                                * m steps per launch with the particle state kept in registers   */
+    int32_t gather_sort;      /* gather-locality pass before a fused launch (slots listed in met-cell
+                               * order): 0 = auto (on from 65536 particles), 1 = always, -1 = never.
+                               * Results per particle do not depend on it.                        */
+    int32_t reserved;
 } lpm_params;
 
 typedef struct {
@@ -214,8 +218,9 @@ int32_t lpm_set_timing(lpm_handle *h, int32_t enable);
 /* Synchronises, then returns out_host[0] = total ms in step kernels, [1] = their launch count,
  * [2] = total ms in binning kernels (memsets of the grids included), [3] = their launch count,
  * [4] = particle-steps executed by the timed step launches (born particles x steps, host count),
- * [5] = particles read by the timed binning launches; accumulated since lpm_set_timing. */
-int32_t lpm_get_timing(lpm_handle *h, double *out_host /* [6] */);
+ * [5] = particles read by the timed binning launches, [6] = total ms in gather-locality sort
+ * passes, [7] = their count; accumulated since lpm_set_timing. */
+int32_t lpm_get_timing(lpm_handle *h, double *out_host /* [8] */);
 
 /* ---- stand-alone kernels for parity tests (device arrays in, device arrays out) ------------ */
 

@@ -55,7 +55,8 @@ class lpm_nuclide(C.Structure):
 
 class lpm_params(C.Structure):
     _fields_ = [("dt", C.c_double), ("seed", C.c_uint64), ("capacity", C.c_uint64), ("boundary_mode", C.c_int32),
-                ("compact", C.c_int32), ("h_dep", C.c_double), ("bin_every", C.c_int32), ("steps_per_launch", C.c_int32)]
+                ("compact", C.c_int32), ("h_dep", C.c_double), ("bin_every", C.c_int32), ("steps_per_launch", C.c_int32),
+                ("gather_sort", C.c_int32), ("reserved", C.c_int32)]
 
 
 class lpm_source(C.Structure):
@@ -162,7 +163,7 @@ class Simulation:
     """
 
     def __init__(self, w, *, steps_per_launch: int = 0, bin_every: Optional[int] = None, fields_dev=None,
-                 stream=None, auto_release: bool = True):
+                 stream=None, auto_release: bool = True, gather_sort: int = 0):
         torch = _require_cuda()
         L = load()
         self._L = L
@@ -185,7 +186,7 @@ class Simulation:
         prm = lpm_params(dt=w.dt, seed=w.seed, capacity=w.capacity,
                          boundary_mode=1 if w.boundary_mode == "absorb" else 0, compact=1 if w.compact else 0,
                          h_dep=w.h_dep, bin_every=w.bin_every if bin_every is None else bin_every,
-                         steps_per_launch=steps_per_launch)
+                         steps_per_launch=steps_per_launch, gather_sort=gather_sort)
         h = C.c_void_p()
         with torch.cuda.stream(self.stream):
             rc = L.lpm_create(C.byref(cg), C.byref(met), nucs, w.K, C.byref(prm), self.workspace.data_ptr(), nbytes,
@@ -269,10 +270,10 @@ class Simulation:
         self._ck(self._L.lpm_set_timing(self._h, 1 if on else 0), "lpm_set_timing")
 
     def get_timing(self):
-        out = (C.c_double * 6)()
+        out = (C.c_double * 8)()
         self._ck(self._L.lpm_get_timing(self._h, out), "lpm_get_timing")
         return dict(step_ms=out[0], step_launches=int(out[1]), bin_ms=out[2], bin_launches=int(out[3]),
-                    particle_steps=out[4], binned_particles=out[5])
+                    particle_steps=out[4], binned_particles=out[5], sort_ms=out[6], sort_launches=int(out[7]))
 
     @property
     def num_active(self) -> int:

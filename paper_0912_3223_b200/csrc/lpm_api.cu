@@ -27,12 +27,12 @@ struct Release {
 };
 
 struct Layout {
-    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, total;
+    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, keys, perm, hist, partial, total;
 };
 
 uint64_t up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
-Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K, bool compact)
+Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K, bool compact, bool sort)
 {
     Layout L{};
     const uint64_t cells3 = (uint64_t)g.nx * g.ny * g.nz, cells2 = (uint64_t)g.nx * g.ny;
@@ -50,6 +50,11 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     L.injlog = o; o += compact ? up(8 * kInjLog) : 0;
     L.stage = o; o += up(4 * cells3 * K);  // fp32 read-out staging for the *_host entry points
     L.pair = o; o += met.nt > 1 ? up(32ull * met.grid.nx * met.grid.ny * met.grid.nz) : 0;  // (F_s, F_s+1) per met cell
+    const uint64_t mcells = (uint64_t)met.grid.nx * met.grid.ny * met.grid.nz;
+    L.keys = o; o += sort ? up(4 * cap) : 0;            // gather-locality pass: met-cell key per slot
+    L.perm = o; o += sort ? up(4 * cap) : 0;            //   slots in met-cell order
+    L.hist = o; o += sort ? up(4 * (mcells + 1)) : 0;   //   per-cell counts / offsets
+    L.partial = o; o += sort ? up(4 * sort_partial_entries(mcells)) : 0;
     L.total = o;
     return L;
 }
@@ -62,6 +67,10 @@ GridF gridf(const lpm_grid &g)
     f.inv_dx = (float)(1.0 / g.dx); f.inv_dy = (float)(1.0 / g.dy); f.inv_dz = (float)(1.0 / g.dz);
     return f;
 }
+
+// the gather-locality pass applies to the slot-addressed store (compact mode keeps id order)
+bool sort_enabled(const lpm_params *p) { return p->gather_sort >= 0 && !p->compact; }
+constexpr uint64_t kSortAutoMin = 65536;
 
 bool grid_ok(const lpm_grid *g)
 {
@@ -98,9 +107,9 @@ struct lpm_handle {
     struct Span { cudaEvent_t a, b; int kind; };
     std::vector<Span> spans;
     std::vector<cudaEvent_t> ev_pool;
-    double t_ms[2], t_units[2];
+    double t_ms[3], t_units[3];
     uint64_t t_base;  // compact mode: device particle-step counter at lpm_set_timing
-    uint64_t t_launches[2];
+    uint64_t t_launches[3];
     int sticky;
     char err[512];
 };
@@ -309,7 +318,7 @@ int32_t lpm_workspace_bytes(const lpm_grid *g, const lpm_meteo *met, const lpm_p
 {
     if (!grid_ok(g) || !met || !grid_ok(&met->grid) || met->nt < 1 || !p || !bytes || K < 1 || K > LPM_MAX_NUCLIDES || p->capacity == 0 || p->capacity >= (1ull << 32))
         return LPM_ERR_INVALID_ARG;
-    *bytes = make_layout(*g, *met, p->capacity, K, p->compact != 0).total;
+    *bytes = make_layout(*g, *met, p->capacity, K, p->compact != 0, sort_enabled(p)).total;
     return LPM_OK;
 }
 
@@ -341,7 +350,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return LPM_ERR_NO_DEVICE;
     if (prop.major != 10) return LPM_ERR_NO_DEVICE;
 
-    const Layout L = make_layout(*cg, *met, p->capacity, K, p->compact != 0);
+    const Layout L = make_layout(*cg, *met, p->capacity, K, p->compact != 0, sort_enabled(p));
     if (ws_bytes < L.total) return LPM_ERR_WORKSPACE_TOO_SMALL;
 
     lpm_handle *h = new (std::nothrow) lpm_handle();
@@ -500,6 +509,16 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                 double units = 0.0;
                 if (h->timing)
                     for (int s = 0; s < m; ++s) units += (double)born_local(r, (int64_t)h->step + s);
+                A.perm = nullptr;
+                if (sort_enabled(&h->prm) && A.n_prev > 0 && (h->prm.gather_sort > 0 || A.n_prev >= kSortAutoMin)) {
+                    uint32_t *perm = (uint32_t *)(h->ws + h->L.perm);
+                    const int sspan = span_open(h, 2, (double)A.n_prev);
+                    CK(launch_sort_by_cell(A.xyzq + r.base, A.n_prev, A.mg, (uint32_t *)(h->ws + h->L.keys),
+                                           (uint32_t *)(h->ws + h->L.hist), (uint32_t *)(h->ws + h->L.partial), perm, h->st));
+                    span_close(h, sspan);
+                    h->launches += 5;
+                    A.perm = perm;
+                }
                 CK(cudaMemsetAsync(A.ctrl + 16, 0, 8, h->st));  // tile ticket of the slot kernel
                 const int span = span_open(h, 0, units);
                 CK(launch_step(A, h->K, false, grid_blocks(h, n), h->st));
@@ -750,7 +769,7 @@ int32_t lpm_set_timing(lpm_handle *h, int32_t enable)
     CK(cudaStreamSynchronize(h->st));
     spans_collect(h);
     h->timing = enable != 0;
-    for (int i = 0; i < 2; ++i) { h->t_ms[i] = 0.0; h->t_units[i] = 0.0; h->t_launches[i] = 0; }
+    for (int i = 0; i < 3; ++i) { h->t_ms[i] = 0.0; h->t_units[i] = 0.0; h->t_launches[i] = 0; }
     if (h->prm.compact) {
         CK(cudaMemcpyAsync(&h->t_base, (uint64_t *)(h->ws + h->L.ctrl) + 3, 8, cudaMemcpyDeviceToHost, h->st));
         CK(cudaStreamSynchronize(h->st));
@@ -766,6 +785,7 @@ int32_t lpm_get_timing(lpm_handle *h, double *out)
     out[0] = h->t_ms[0]; out[1] = (double)h->t_launches[0];
     out[2] = h->t_ms[1]; out[3] = (double)h->t_launches[1];
     out[4] = h->t_units[0]; out[5] = h->t_units[1];
+    out[6] = h->t_ms[2]; out[7] = (double)h->t_launches[2];
     if (h->prm.compact) {  // the live count is device-side: cumulative particle-steps since lpm_set_timing
         uint64_t now = 0;
         CK(cudaMemcpyAsync(&now, (uint64_t *)(h->ws + h->L.ctrl) + 3, 8, cudaMemcpyDeviceToHost, h->st));

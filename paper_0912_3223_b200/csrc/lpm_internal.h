@@ -56,6 +56,7 @@ struct StepArgs {
     double wet_scale[LPM_MAX_NUCLIDES];  // (1 - p_dry if uniform) * p_wet
     // population (slot-addressed mode): slots [0, n) of the release block starting at `base`
     uint64_t base, n, n_prev;  // slots >= n_prev are born inside this launch
+    const uint32_t *perm;      // gather-locality pass: slots [0, n_prev) listed in met-cell order, or null
     uint64_t pid_offset, pid_stride;
     uint64_t rel_N, rel_c;     // count mode: N (global count); rate mode: c slots per step
     int64_t rel_s_start, rel_S;
@@ -104,6 +105,9 @@ struct BinArgs {
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int grid_blocks, cudaStream_t st);
 int step_max_blocks_per_sm(int K, bool compact, bool two_snap);
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
+cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
+                                uint32_t *perm, cudaStream_t st);
+uint64_t sort_partial_entries(uint64_t n_cells);
 cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, uint64_t cells, cudaStream_t st);
 cudaError_t launch_bin(const BinArgs &a, int blocks, cudaStream_t st);
 cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3, int K, const double *scale, cudaStream_t st);

@@ -1,0 +1,139 @@
+// lpm_sort.cu — gather-locality pass of the step (pulled into the hot path).
+//
+// The particle store stays in particle-id order (slot l <-> id, R9), but before a fused launch the
+// slots are listed in order of the MET CELL their particle sits in (counting sort of 4-byte slot
+// indices: histogram -> exclusive scan -> scatter).  The step kernel then walks that list, so the
+// 32 lanes of a warp sample the same or neighbouring texels: one or two L1 wavefronts per gather
+// instead of one per lane, and the texels stay in L1.  Only indices move; the 16-24 B particle
+// records are read and written in place (a scattered 16 B access per particle per launch of up to
+// 96 steps is noise).  The paper relied on the texture cache for locality; this is
+// its sm_100a counterpart.
+#include "lpm_device.cuh"
+
+namespace lpm {
+
+constexpr int kScanItems = 16;                       // items per thread in the scan kernels
+constexpr int kScanBlock = 256 * kScanItems;         // items per block
+
+// pass 1: key = met cell of the particle (edge-clamped; exited slots go to the last bucket)
+__global__ void __launch_bounds__(256) sort_key_kernel(const float4 *__restrict__ xyzq, uint64_t n, GridF g, uint32_t n_cells,
+                                                       uint32_t *__restrict__ keys, uint32_t *__restrict__ hist)
+{
+    for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n; l += (uint64_t)gridDim.x * blockDim.x) {
+        const float4 p = xyzq[l];
+        uint32_t key = n_cells;
+        if (p.z >= 0.0f) {
+            const int i = min(max((int)floorf((p.x - g.x0) * g.inv_dx), 0), g.nx - 1);
+            const int j = min(max((int)floorf((p.y - g.y0) * g.inv_dy), 0), g.ny - 1);
+            const int k = min(max((int)floorf((p.z - g.z0) * g.inv_dz), 0), g.nz - 1);
+            key = (uint32_t)((k * g.ny + j) * g.nx + i);
+        }
+        keys[l] = key;
+        atomicAdd(hist + key, 1u);
+    }
+}
+
+// pass 2: exclusive scan of hist[0..m) in place: block totals -> scan of the totals -> rescan
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t *s_warp, uint32_t &total)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    uint32_t woff = 0, tot = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+        const uint32_t t = s_warp[w];
+        woff += w < warp ? t : 0u;
+        tot += t;
+    }
+    __syncthreads();
+    total = tot;
+    return woff + inc - v;
+}
+
+__global__ void __launch_bounds__(256) scan_totals_kernel(const uint32_t *__restrict__ hist, uint32_t m, uint32_t *__restrict__ partial)
+{
+    __shared__ uint32_t s_warp[8];
+    const uint32_t base = blockIdx.x * kScanBlock + threadIdx.x * kScanItems;
+    uint32_t s = 0;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) s += base + i < m ? hist[base + i] : 0u;
+    uint32_t total;
+    block_exclusive_scan(s, s_warp, total);
+    if (threadIdx.x == 0) partial[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(256) scan_partials_kernel(uint32_t *partial, uint32_t nb)
+{
+    __shared__ uint32_t s_warp[8];
+    uint32_t carry = 0;
+    for (uint32_t b0 = 0; b0 < nb; b0 += 256) {
+        const uint32_t i = b0 + threadIdx.x;
+        const uint32_t v = i < nb ? partial[i] : 0u;
+        uint32_t total;
+        const uint32_t ex = block_exclusive_scan(v, s_warp, total);
+        if (i < nb) partial[i] = carry + ex;
+        carry += total;
+    }
+}
+
+__global__ void __launch_bounds__(256) scan_apply_kernel(uint32_t *__restrict__ hist, uint32_t m, const uint32_t *__restrict__ partial)
+{
+    __shared__ uint32_t s_warp[8];
+    const uint32_t base = blockIdx.x * kScanBlock + threadIdx.x * kScanItems;
+    uint32_t v[kScanItems], s = 0;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) { v[i] = base + i < m ? hist[base + i] : 0u; s += v[i]; }
+    uint32_t total;
+    uint32_t run = partial[blockIdx.x] + block_exclusive_scan(s, s_warp, total);
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        if (base + i < m) hist[base + i] = run;
+        run += v[i];
+    }
+}
+
+// pass 3: scatter slot indices; lanes of a warp that share a key claim their range with one atomic
+__global__ void __launch_bounds__(256) sort_scatter_kernel(const uint32_t *__restrict__ keys, uint64_t n, uint32_t *__restrict__ offs,
+                                                           uint32_t *__restrict__ perm)
+{
+    const uint64_t n_round = (n + 31) & ~(uint64_t)31;
+    const int lane = threadIdx.x & 31;
+    for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n_round; l += (uint64_t)gridDim.x * blockDim.x) {
+        const bool live = l < n;
+        const uint32_t key = live ? keys[l] : 0xffffffffu;
+        const uint32_t peers = __match_any_sync(0xffffffffu, key);
+        const int leader = __ffs(peers) - 1;
+        uint32_t base = 0;
+        if (live && lane == leader) base = atomicAdd(offs + key, (uint32_t)__popc(peers));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (live) perm[base + __popc(peers & ((1u << lane) - 1u))] = (uint32_t)l;
+    }
+}
+
+cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
+                                uint32_t *perm, cudaStream_t st)
+{
+    const uint32_t n_cells = (uint32_t)g.nx * g.ny * g.nz, m = n_cells + 1;
+    cudaError_t e = cudaMemsetAsync(hist, 0, 4ull * m, st);
+    if (e != cudaSuccess) return e;
+    const uint64_t want = (n + 255) / 256;
+    const int blocks = (int)(want < 148 * 8 ? (want ? want : 1) : 148 * 8);
+    sort_key_kernel<<<blocks, 256, 0, st>>>(xyzq, n, g, n_cells, keys, hist);
+    const uint32_t nb = (m + kScanBlock - 1) / kScanBlock;
+    scan_totals_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
+    scan_partials_kernel<<<1, 256, 0, st>>>(partial, nb);
+    scan_apply_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
+    sort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, hist, perm);
+    return cudaGetLastError();
+}
+
+uint64_t sort_partial_entries(uint64_t n_cells) { return (n_cells + 1 + kScanBlock - 1) / kScanBlock + 1; }
+
+}  // namespace lpm

@@ -166,7 +166,11 @@ __global__ void __launch_bounds__(kStepThreads) step_slots_kernel(const __grid_c
     // are resident together work on tiles spread over the whole slot range (= over all particle
     // ages, hence over the whole plume) instead of on ~3e5 neighbouring particles that would all
     // hit the same few deposition-map cells and met lines at the same time.
-    const uint32_t n_tiles = (uint32_t)((A.n + kStepThreads - 1) / kStepThreads);
+    // tiles [0, t_old) walk the sorted slot list (particles that existed before this launch), tiles
+    // [t_old, n_tiles) the slots born inside this launch, in id order (all at the source point)
+    const uint32_t t_old = A.perm ? (uint32_t)((A.n_prev + kStepThreads - 1) / kStepThreads) : 0u;
+    const uint64_t first_new = A.perm ? A.n_prev : 0ull;
+    const uint32_t n_tiles = t_old + (uint32_t)((A.n - first_new + kStepThreads - 1) / kStepThreads);
     const uint32_t G = min(n_tiles, (uint32_t)gridDim.x);
     const uint32_t R = (n_tiles + G - 1) / G;
     const uint32_t n_tickets = G * R;
@@ -177,8 +181,15 @@ __global__ void __launch_bounds__(kStepThreads) step_slots_kernel(const __grid_c
         const uint32_t t = s_ticket;
         if (t >= n_tickets) break;
         const uint32_t tile = (t % G) * R + t / G;
-        const uint64_t l = (uint64_t)tile * kStepThreads + threadIdx.x;
-        if (l >= A.n) continue;
+        uint64_t l;
+        if (tile < t_old) {
+            const uint64_t idx = (uint64_t)tile * kStepThreads + threadIdx.x;
+            if (idx >= A.n_prev) continue;
+            l = A.perm[idx];
+        } else {
+            l = first_new + (uint64_t)(tile - t_old) * kStepThreads + threadIdx.x;
+            if (l >= A.n) continue;
+        }
         const uint64_t slot = A.base + l;
         const uint32_t pid = (uint32_t)(A.pid_offset + l * A.pid_stride);
         float x, y, z, q[K];
