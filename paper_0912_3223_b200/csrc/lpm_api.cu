@@ -59,12 +59,19 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     return L;
 }
 
-GridF gridf(const lpm_grid &g)
+// zfast: the buffer the kernels sample is the z-fastest pair buffer (32-byte texels); otherwise the
+// caller's x-fastest snapshot (16-byte texels)
+GridF gridf(const lpm_grid &g, bool zfast = false)
 {
     GridF f;
     f.nx = g.nx; f.ny = g.ny; f.nz = g.nz;
     f.x0 = (float)g.x0; f.y0 = (float)g.y0; f.z0 = (float)g.z0;
     f.inv_dx = (float)(1.0 / g.dx); f.inv_dy = (float)(1.0 / g.dy); f.inv_dz = (float)(1.0 / g.dz);
+    f.fx1 = (float)(g.nx - 1); f.fy1 = (float)(g.ny - 1); f.fz1 = (float)(g.nz - 1);
+    f.ix2 = g.nx > 2 ? g.nx - 2 : 0; f.iy2 = g.ny > 2 ? g.ny - 2 : 0; f.iz2 = g.nz > 2 ? g.nz - 2 : 0;
+    if (zfast) { f.ez = 1u; f.ex = (uint32_t)g.nz; f.ey = (uint32_t)g.nz * (uint32_t)g.nx; f.line_shift = 2; }
+    else { f.ex = 1u; f.ey = (uint32_t)g.nx; f.ez = (uint32_t)g.nx * (uint32_t)g.ny; f.line_shift = 3; }
+    f.sx = g.nx > 1 ? f.ex : 0u; f.sy = g.ny > 1 ? f.ey : 0u; f.sz = g.nz > 1 ? f.ez : 0u;
     return f;
 }
 
@@ -211,7 +218,11 @@ void fill_entry(const lpm_handle *h, uint64_t n, StepEntry &e)
     const bool raining = h->rain_on && t >= h->rt0 && t < h->rt1;  // G6
     e.a = a;
     e.snap = s | (raining ? 1 << 16 : 0);
-    for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) e.G[k] = k < h->K ? G_of(h, k, n) : 1.0;
+    for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) {
+        e.G[k] = k < h->K ? G_of(h, k, n) : 1.0;
+        e.Gf[k] = (float)e.G[k];
+        e.Gp[k] = k < h->K ? (float)(e.G[k] * (double)h->p_dry[k]) : 0.0f;
+    }
 }
 
 void base_args(const lpm_handle *h, StepArgs &A)
@@ -224,7 +235,7 @@ void base_args(const lpm_handle *h, StepArgs &A)
     A.pair = h->met.nt > 1 ? (const void *)(h->ws + h->L.pair) : nullptr;
     const lpm_grid &mg = h->met.grid;
     A.snap_cells = (uint64_t)mg.nx * mg.ny * mg.nz;
-    A.mg = gridf(mg);
+    A.mg = gridf(mg, h->met.nt > 1);
     A.nt = h->met.nt;
     A.bx0 = (float)mg.x0; A.bx1 = (float)(mg.x0 + mg.nx * mg.dx);
     A.by0 = (float)mg.y0; A.by1 = (float)(mg.y0 + mg.ny * mg.dy);
@@ -241,9 +252,14 @@ void base_args(const lpm_handle *h, StepArgs &A)
     for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) {
         A.p_dry[k] = h->p_dry[k]; A.p_wet[k] = h->p_wet[k];
         A.dec_scale[k] = h->dec_scale[k]; A.wet_scale[k] = h->wet_scale[k];
+        A.wet_scale_f[k] = (float)h->wet_scale[k];
     }
     A.rx0 = (float)h->rx0; A.rx1 = (float)h->rx1; A.ry0 = (float)h->ry0; A.ry1 = (float)h->ry1;
     A.seed_lo = (uint32_t)h->prm.seed; A.seed_hi = (uint32_t)(h->prm.seed >> 32);
+    for (uint32_t r = 0; r < 10; ++r) {  // R1 key schedule: the key is bumped by the Weyl constants between rounds
+        A.rk[2 * r] = A.seed_lo + r * 0x9E3779B9u;
+        A.rk[2 * r + 1] = A.seed_hi + r * 0xBB67AE85u;
+    }
     A.ledger = (double *)(h->ws + h->L.ledger);
     A.ctrl = (uint64_t *)(h->ws + h->L.ctrl);
     A.tile_state = h->prm.compact ? (uint64_t *)(h->ws + h->L.tile) : nullptr;
@@ -379,7 +395,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         h->wet_scale[k] = keep_dry * (double)h->p_wet[k];
     }
     h->dry_mode = !any_dry ? kDryNone : (uniform ? kDryUniform : kDryLayer);
-    h->occ = step_max_blocks_per_sm(K, p->compact != 0, met->nt > 1);
+    h->occ = step_max_blocks_per_sm(K, p->compact != 0, met->nt > 1, h->dry_mode);
     if (cudaMemsetAsync(ws, 0, L.total, h->st) != cudaSuccess) { delete h; return LPM_ERR_CUDA; }
     h->launches++;
     *out = h;
@@ -467,7 +483,7 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
         if (h->met.nt > 1 && (A.tab[0].snap & 0xffff) != h->pair_snap) {
             const int sn = A.tab[0].snap & 0xffff;
             CK(launch_pair_repack(A.met + (uint64_t)sn * A.snap_cells, A.met + (uint64_t)(sn + 1) * A.snap_cells,
-                                  h->ws + h->L.pair, A.snap_cells, h->st));
+                                  h->ws + h->L.pair, h->met.grid.nx, h->met.grid.ny, h->met.grid.nz, h->st));
             h->launches++;
             h->pair_snap = sn;
         }
@@ -842,12 +858,12 @@ int32_t lpm_test_sample(const lpm_meteo *met, double t, const void *xyz, uint64_
     void *pair = nullptr;
     if (met->nt > 1) {  // same path as lpm_step: interleave snapshots (sn, sn+1), then sample the pair buffer
         if (cudaMalloc(&pair, 32 * cells) != cudaSuccess) return LPM_ERR_CUDA;
-        if (launch_pair_repack(f + (uint64_t)sn * cells, f + (uint64_t)(sn + 1) * cells, pair, cells, s) != cudaSuccess) {
+        if (launch_pair_repack(f + (uint64_t)sn * cells, f + (uint64_t)(sn + 1) * cells, pair, g.nx, g.ny, g.nz, s) != cudaSuccess) {
             cudaFree(pair);
             return LPM_ERR_CUDA;
         }
     }
-    cudaError_t rc = launch_test_sample(f + (uint64_t)sn * cells, pair, gridf(g), e.a, (float)met->kz_min, (const float4 *)xyz, n,
+    cudaError_t rc = launch_test_sample(f + (uint64_t)sn * cells, pair, gridf(g, met->nt > 1), e.a, (float)met->kz_min, (const float4 *)xyz, n,
                                         (float4 *)out, s);
     if (pair) {
         const cudaError_t rs = cudaStreamSynchronize(s);

@@ -208,7 +208,7 @@ __global__ void test_sample_kernel(const float4 *met, const Texel2 *pair, GridF 
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
         const float4 p = xyz[i];
         const Corner c = corner_of(mg, p.x, p.y, p.z);
-        float4 m = pair ? trilinear_pair(pair, c, a) : trilinear(met, c);   // the step kernel's two paths
+        float4 m = pair ? trilinear_pair(pair, c, mg, a) : trilinear(met, c, mg);   // the step kernel's two paths
         m.w = fmaxf(m.w, kz_min);
         out[i] = m;
     }

@@ -15,6 +15,8 @@ constexpr int kScanTile = kStepThreads;  // particles per look-back tile (compac
 // Per-step scalars, host-computed in double (DESIGN.md §3 R4, R8).
 struct StepEntry {
     double G[LPM_MAX_NUCLIDES];  // G_k(t_n): activity = q * G (decay and uniform dry loss folded in)
+    float Gf[LPM_MAX_NUCLIDES];  // (float)G_k(t_n), the factor the per-step fp32 arithmetic uses
+    float Gp[LPM_MAX_NUCLIDES];  // (float)(G_k(t_n) * p_dry,k): uniform dry deposit of one step per unit q
     float a;                     // time weight between snapshot `snap` and `snap + 1`
     int32_t snap;                // bits 0..15 snapshot index, bit 16 = raining
 };
@@ -23,6 +25,15 @@ struct GridF {  // fp32 view of a grid, exactly as the kernels use it
     int32_t nx, ny, nz;
     float x0, y0, z0;          // (float) lower corner
     float inv_dx, inv_dy, inv_dz;  // (float)(1.0 / d)
+    // derived, for the met sampling R4: the upper clamp of the grid coordinate, the largest lower
+    // corner index, and the element strides to the upper corner (0 on an axis with a single cell:
+    // i1 = min(i0 + 1, n - 1) = i0 + 1 whenever n >= 2, because i0 <= n - 2)
+    float fx1, fy1, fz1;       // (float)(n - 1)
+    int32_t ix2, iy2, iz2;     // max(n - 2, 0)
+    uint32_t ex, ey, ez;       // element strides of cell (i, j, k) in the sampled buffer: x-fastest (1, nx, nx*ny)
+                               // for the caller's snapshots, z-fastest (nz, nx*nz, 1) for the pair buffer
+    uint32_t sx, sy, sz;       // stride to the upper corner on each axis: n > 1 ? e : 0
+    uint32_t line_shift;       // log2(texels per 128-byte line of the sampled buffer): gather-locality key = offset >> shift
 };
 
 enum DryMode : int32_t { kDryNone = 0, kDryUniform = 1, kDryLayer = 2 };
@@ -50,10 +61,12 @@ struct StepArgs {
     float p_dry[LPM_MAX_NUCLIDES], p_wet[LPM_MAX_NUCLIDES];
     float rx0, rx1, ry0, ry1;
     uint32_t seed_lo, seed_hi;
+    uint32_t rk[20];      // Philox round keys (k0, k1) of rounds 0..9: key + r * Weyl constants (R1)
     // ledger: double [K][8]: 2 dry, 3 wet, 4 decayed, 5 exited, 6 offgrid
     double *ledger;
     double dec_scale[LPM_MAX_NUCLIDES];  // (1 - f_lambda) * (1 - p_dry if uniform)
     double wet_scale[LPM_MAX_NUCLIDES];  // (1 - p_dry if uniform) * p_wet
+    float wet_scale_f[LPM_MAX_NUCLIDES]; // (float)wet_scale
     // population (slot-addressed mode): slots [0, n) of the release block starting at `base`
     uint64_t base, n, n_prev;  // slots >= n_prev are born inside this launch
     const uint32_t *perm;      // gather-locality pass: slots [0, n_prev) listed in met-cell order, or null
@@ -103,12 +116,12 @@ struct BinArgs {
 
 // launchers implemented in the .cu files; all return the cudaError of the launch
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int grid_blocks, cudaStream_t st);
-int step_max_blocks_per_sm(int K, bool compact, bool two_snap);
+int step_max_blocks_per_sm(int K, bool compact, bool two_snap, int dry_mode);
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
                                 uint32_t *perm, cudaStream_t st);
 uint64_t sort_partial_entries(uint64_t n_cells);
-cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, uint64_t cells, cudaStream_t st);
+cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, cudaStream_t st);
 cudaError_t launch_bin(const BinArgs &a, int blocks, cudaStream_t st);
 cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3, int K, const double *scale, cudaStream_t st);
 cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, double inv_area, cudaStream_t st);

@@ -15,18 +15,19 @@ namespace lpm {
 constexpr int kScanItems = 16;                       // items per thread in the scan kernels
 constexpr int kScanBlock = 256 * kScanItems;         // items per block
 
-// pass 1: key = met cell of the particle (edge-clamped; exited slots go to the last bucket)
-__global__ void __launch_bounds__(256) sort_key_kernel(const float4 *__restrict__ xyzq, uint64_t n, GridF g, uint32_t n_cells,
+// pass 1: key = 128-byte line of the sampled met buffer that holds the particle's cell (edge-clamped;
+// exited slots go to the last bucket, n_keys - 1)
+__global__ void __launch_bounds__(256) sort_key_kernel(const float4 *__restrict__ xyzq, uint64_t n, GridF g, uint32_t n_keys,
                                                        uint32_t *__restrict__ keys, uint32_t *__restrict__ hist)
 {
     for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n; l += (uint64_t)gridDim.x * blockDim.x) {
         const float4 p = xyzq[l];
-        uint32_t key = n_cells;
+        uint32_t key = n_keys - 1;
         if (p.z >= 0.0f) {
             const int i = min(max((int)floorf((p.x - g.x0) * g.inv_dx), 0), g.nx - 1);
             const int j = min(max((int)floorf((p.y - g.y0) * g.inv_dy), 0), g.ny - 1);
             const int k = min(max((int)floorf((p.z - g.z0) * g.inv_dz), 0), g.nz - 1);
-            key = (uint32_t)((k * g.ny + j) * g.nx + i);
+            key = ((uint32_t)i * g.ex + (uint32_t)j * g.ey + (uint32_t)k * g.ez) >> g.line_shift;
         }
         keys[l] = key;
         atomicAdd(hist + key, 1u);
@@ -120,12 +121,12 @@ __global__ void __launch_bounds__(256) sort_scatter_kernel(const uint32_t *__res
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
                                 uint32_t *perm, cudaStream_t st)
 {
-    const uint32_t n_cells = (uint32_t)g.nx * g.ny * g.nz, m = n_cells + 1;
+    const uint32_t n_keys = (((uint32_t)g.nx * g.ny * g.nz - 1u) >> g.line_shift) + 2u, m = n_keys;
     cudaError_t e = cudaMemsetAsync(hist, 0, 4ull * m, st);
     if (e != cudaSuccess) return e;
     const uint64_t want = (n + 255) / 256;
     const int blocks = (int)(want < 148 * 8 ? (want ? want : 1) : 148 * 8);
-    sort_key_kernel<<<blocks, 256, 0, st>>>(xyzq, n, g, n_cells, keys, hist);
+    sort_key_kernel<<<blocks, 256, 0, st>>>(xyzq, n, g, n_keys, keys, hist);
     const uint32_t nb = (m + kScanBlock - 1) / kScanBlock;
     scan_totals_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
     scan_partials_kernel<<<1, 256, 0, st>>>(partial, nb);

@@ -19,7 +19,8 @@ namespace lpm {
 template <int K>
 struct Acc {  // per-thread ledger partial sums, in activity units before the per-nuclide scale
     float dry[K], wet[K], dec[K];
-    float off[K];  // deposit that fell off the map (already scaled)
+    float both[K];  // steps where the dry and the decay ledger see the same activity (uniform dry / no sink, no rain)
+    float off[K];   // deposit that fell off the map (already scaled)
 };
 
 // a6 run-length aggregation: a particle stays in one 2-D map cell for several steps, so its
@@ -48,32 +49,47 @@ __device__ __forceinline__ void dep_flush(const StepArgs &A, Dep<K> &d, Acc<K> &
 }
 
 // One model step of one particle.  Returns false when the particle left the domain (ABSORB).
-template <int K, bool TWO>
+// Source order = intended issue order: the eight gathers go out first and the ~150 instructions of
+// Philox + Box-Muller run while they are in flight.
+// a6: make (x, y)'s map cell the current run of the aggregator (flushing the previous run)
+template <int K>
+__device__ __forceinline__ void deposit_at(const StepArgs &A, float x, float y, Acc<K> &acc, Dep<K> &dep)
+{
+    const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
+    const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
+    const int c = (ci | cj) >= 0 ? cj * A.cg.nx + ci : -1;
+    if (c != dep.cell) {
+        dep_flush<K>(A, dep, acc);
+        dep.cell = c;
+    }
+}
+
+template <int K, bool TWO, int DRY>
 __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e, uint32_t step_lo,
                                           uint32_t pid_lo, float &x, float &y, float &z,
                                           float (&q)[K], Acc<K> &acc, Dep<K> &dep)
 {
-    // a1: three N(0,1) from Philox stream 0
-    const uint4 r = philox4x32_10(step_lo, 0u, pid_lo, 0u, A.seed_lo, A.seed_hi);
-    float n0, n1, n2;
-    normals3(r, n0, n1, n2);
-
     // a0 + a2: weather at X_old, t_n
     const Corner c = corner_of(A.mg, x, y, z);
     float4 m;
-    if (TWO) m = trilinear_pair((const Texel2 *)A.pair, c, e.a);
-    else m = trilinear(A.met, c);
+    if (TWO) m = trilinear_pair((const Texel2 *)A.pair, c, A.mg, e.a);
+    else m = trilinear(A.met, c, A.mg);
     const float kz = fmaxf(m.w, A.kz_min);
+
+    // a1: three N(0,1) from Philox stream 0
+    const uint4 r = philox4x32_10_rk(step_lo, pid_lo, A.rk);
+    float n0, n1, n2;
+    normals3(r, n0, n1, n2);
 
     // a3: Eq.(1) + Eq.(2)
     x = fmaf(A.sigma_h, n0, fmaf(m.x, A.dt, x));
     y = fmaf(A.sigma_h, n1, fmaf(m.y, A.dt, y));
-    z = fmaf(sqrtf(2.0f * A.dt * kz), n2, fmaf(m.z, A.dt, z));
+    z = fmaf(sqrt_nr(2.0f * A.dt * kz), n2, fmaf(m.z, A.dt, z));
 
     // a4: reflection (R6), lateral boundary (R7)
-    if (z < 0.0f) z = -z;
+    z = fabsf(z);
     if (z > A.H) z = 2.0f * A.H - z;
-    if (z < 0.0f) z = 0.0f;
+    z = fmaxf(z, 0.0f);
     if (A.absorb) {
         const bool inside = (x >= A.bx0) & (x < A.bx1) & (y >= A.by0) & (y < A.by1);
         if (!inside) {
@@ -84,27 +100,40 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
     }
 
     // a5: deposition then decay at the new position (R8).  Activity = q * G_k(t_n); decay and
-    // uniform dry loss live in G, so q only changes for position-dependent sinks.
+    // uniform dry loss live in G, so q only changes for position-dependent sinks.  DRY is a
+    // template parameter and the rain flag is the same for every thread, so the common cases are
+    // straight-line code: no sink at all (2 FMA), uniform dry deposition without rain (4 FMA + the
+    // scatter).
+    const bool raining = (e.snap >> 16) & 1;
+    if (DRY != kDryLayer && !raining) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) acc.both[k] = fmaf(q[k], e.Gf[k], acc.both[k]);
+        if (DRY == kDryNone) return true;
+        deposit_at<K>(A, x, y, acc, dep);
+#pragma unroll
+        for (int k = 0; k < K; ++k) dep.a[k] = fmaf(q[k], e.Gp[k], dep.a[k]);
+        return true;
+    }
+    const bool dry_here = DRY == kDryUniform || (DRY == kDryLayer && z < A.h_dep);
+    const bool wet_here = raining & (x >= A.rx0) & (x < A.rx1) & (y >= A.ry0) & (y < A.ry1);
     float inc[K];
 #pragma unroll
-    for (int k = 0; k < K; ++k) inc[k] = 0.0f;
-    const bool dry_here = (A.dry_mode == kDryUniform) | ((A.dry_mode == kDryLayer) & (z < A.h_dep));
-    const bool raining = (e.snap >> 16) & 1;
-    const bool wet_here = raining & (x >= A.rx0) & (x < A.rx1) & (y >= A.ry0) & (y < A.ry1);
-#pragma unroll
     for (int k = 0; k < K; ++k) {
-        const float G = (float)e.G[k];
+        const float G = e.Gf[k];
         float act = q[k] * G;
+        inc[k] = 0.0f;
         if (dry_here) {
-            inc[k] = act * A.p_dry[k];
             acc.dry[k] += act;
-            if (A.dry_mode == kDryLayer) {
+            if (DRY == kDryLayer) {
+                inc[k] = act * A.p_dry[k];
                 q[k] = fmaf(-q[k], A.p_dry[k], q[k]);
                 act = q[k] * G;
+            } else {
+                inc[k] = q[k] * e.Gp[k];
             }
         }
         if (wet_here) {
-            inc[k] = fmaf(act, (float)A.wet_scale[k], inc[k]);
+            inc[k] = fmaf(act, A.wet_scale_f[k], inc[k]);
             acc.wet[k] += act;
             q[k] = fmaf(-q[k], A.p_wet[k], q[k]);
             act = q[k] * G;
@@ -114,13 +143,7 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
 
     // a6: deposit at the cell of the NEW (x, y), run-length aggregated in registers
     if (dry_here | wet_here) {
-        const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
-        const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
-        const int c = (ci | cj) >= 0 ? cj * A.cg.nx + ci : -1;
-        if (c != dep.cell) {
-            dep_flush<K>(A, dep, acc);
-            dep.cell = c;
-        }
+        deposit_at<K>(A, x, y, acc, dep);
 #pragma unroll
         for (int k = 0; k < K; ++k) dep.a[k] += inc[k];
     }
@@ -136,7 +159,8 @@ __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &ac
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
     for (int k = 0; k < K; ++k) {
-        const float d = warp_sum(acc.dry[k]), w = warp_sum(acc.wet[k]), c = warp_sum(acc.dec[k]), o = warp_sum(acc.off[k]);
+        const float b = warp_sum(acc.both[k]);
+        const float d = (A.dry_mode == kDryUniform ? b : 0.0f) + warp_sum(acc.dry[k]), w = warp_sum(acc.wet[k]), c = b + warp_sum(acc.dec[k]), o = warp_sum(acc.off[k]);
         if (lane == 0) { s_part[warp][4 * k] = d; s_part[warp][4 * k + 1] = w; s_part[warp][4 * k + 2] = c; s_part[warp][4 * k + 3] = o; }
     }
     __syncthreads();
@@ -154,13 +178,18 @@ __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &ac
 // Particles of one release occupy the slots base + [0, n); slot l carries global particle id
 // pid_offset + l * pid_stride, so ids (and birth steps, R9) are implied by the slot.  Persistent
 // grid-stride loop; up to kMaxFused model steps per launch.
-template <int K, bool TWO>
-__global__ void __launch_bounds__(kStepThreads) step_slots_kernel(const __grid_constant__ StepArgs A)
+#ifndef LPM_STEP_MINB
+#define LPM_STEP_MINB 3
+#endif
+static_assert(sizeof(StepArgs) <= 32764, "StepArgs must fit the kernel-parameter space (32764 B since CUDA 12.1 on sm_70+)");
+
+template <int K, bool TWO, int DRY>
+__global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel(const __grid_constant__ StepArgs A)
 {
     __shared__ uint32_t s_ticket;
     Acc<K> acc;
 #pragma unroll
-    for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = acc.off[k] = 0.0f;
+    for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = acc.both[k] = acc.off[k] = 0.0f;
 
     // Dynamic, DECORRELATED tile schedule: ticket t -> tile (t % G) * R + t / G, so the CTAs that
     // are resident together work on tiles spread over the whole slot range (= over all particle
@@ -213,11 +242,12 @@ __global__ void __launch_bounds__(kStepThreads) step_slots_kernel(const __grid_c
         dep.cell = -2;
 #pragma unroll
         for (int k = 0; k < K; ++k) dep.a[k] = 0.0f;
+        // the trip count is the same for every thread (uniform table index, uniform branches inside
+        // the step); a particle born inside this launch or absorbed at the boundary skips steps
         bool alive = true;
-        for (int s = s_begin; s < A.m_steps; ++s) {
-            alive = step_once<K, TWO>(A, A.tab[s], (uint32_t)(A.step0 + s), pid, x, y, z, q, acc, dep);
-            if (!alive) break;
-        }
+        const uint32_t step0 = (uint32_t)A.step0;
+        for (int s = 0; s < A.m_steps; ++s)
+            if (alive & (s >= s_begin)) alive = step_once<K, TWO, DRY>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, dep);
         dep_flush<K>(A, dep, acc);
         if (!alive) z = -1.0f - z;  // exit position kept, slot marked inactive
         A.xyzq[slot] = make_float4(x, y, z, q[0]);
@@ -244,7 +274,7 @@ __device__ __forceinline__ void st_state(uint64_t *p, uint64_t v)
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-template <int K, bool TWO>
+template <int K, bool TWO, int DRY>
 __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid_constant__ StepArgs A)
 {
     __shared__ uint32_t s_tile;
@@ -252,7 +282,7 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
     __shared__ uint32_t s_excl;
     Acc<K> acc;
 #pragma unroll
-    for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = acc.off[k] = 0.0f;
+    for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = acc.both[k] = acc.off[k] = 0.0f;
 
     const uint64_t n = A.ctrl[0];
     const uint32_t n_tiles = (uint32_t)((n + kScanTile - 1) / kScanTile);
@@ -279,7 +309,7 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
             dep.cell = -2;
 #pragma unroll
             for (int k = 0; k < K; ++k) dep.a[k] = 0.0f;
-            alive = step_once<K, TWO>(A, A.tab[0], (uint32_t)A.step0, pid, x, y, z, q, acc, dep);
+            alive = step_once<K, TWO, DRY>(A, A.tab[0], (uint32_t)A.step0, pid, x, y, z, q, acc, dep);
             dep_flush<K>(A, dep, acc);
         }
         // survivors: rank inside the tile
@@ -370,52 +400,65 @@ __global__ void __launch_bounds__(256) inject_kernel(const __grid_constant__ Inj
 }
 
 // ------------------------------------------------------------------ launchers
+// One instantiation per (nuclide count, one / two met snapshots, dry-deposition mode); `f` receives
+// the kernel function pointer of the variant that matches the handle.
+typedef void (*StepKernel)(const StepArgs);
+
 template <int K, bool TWO>
-static cudaError_t launch_t(const StepArgs &a, bool compact, int blocks, cudaStream_t st)
+static StepKernel pick_dry(bool compact, int dry)
 {
-    if (compact) step_compact_kernel<K, TWO><<<blocks, kStepThreads, 0, st>>>(a);
-    else step_slots_kernel<K, TWO><<<blocks, kStepThreads, 0, st>>>(a);
-    return cudaGetLastError();
+    if (compact) {
+        if (dry == kDryNone) return step_compact_kernel<K, TWO, kDryNone>;
+        return dry == kDryUniform ? step_compact_kernel<K, TWO, kDryUniform> : step_compact_kernel<K, TWO, kDryLayer>;
+    }
+    if (dry == kDryNone) return step_slots_kernel<K, TWO, kDryNone>;
+    return dry == kDryUniform ? step_slots_kernel<K, TWO, kDryUniform> : step_slots_kernel<K, TWO, kDryLayer>;
+}
+
+static StepKernel pick(int K, bool compact, bool two, int dry)
+{
+    if (K == 1) return two ? pick_dry<1, true>(compact, dry) : pick_dry<1, false>(compact, dry);
+    return two ? pick_dry<2, true>(compact, dry) : pick_dry<2, false>(compact, dry);
 }
 
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int blocks, cudaStream_t st)
 {
-    const bool two = a.nt > 1;
-    if (K == 1) return two ? launch_t<1, true>(a, compact, blocks, st) : launch_t<1, false>(a, compact, blocks, st);
-    return two ? launch_t<2, true>(a, compact, blocks, st) : launch_t<2, false>(a, compact, blocks, st);
+    pick(K, compact, a.nt > 1, a.dry_mode)<<<blocks, kStepThreads, 0, st>>>(a);
+    return cudaGetLastError();
 }
 
-template <int K, bool TWO>
-static int occ_t(bool compact)
+int step_max_blocks_per_sm(int K, bool compact, bool two, int dry)
 {
     int nb = 0;
-    if (compact) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_compact_kernel<K, TWO>, kStepThreads, 0);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, step_slots_kernel<K, TWO>, kStepThreads, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick(K, compact, two, dry), kStepThreads, 0);
     return nb;
 }
 
-int step_max_blocks_per_sm(int K, bool compact, bool two)
-{
-    if (K == 1) return two ? occ_t<1, true>(compact) : occ_t<1, false>(compact);
-    return two ? occ_t<2, true>(compact) : occ_t<2, false>(compact);
-}
-
-// a0: interleave the two snapshots of the current met interval into the pair buffer
+// a0: interleave the two snapshots of the current met interval into the pair buffer and turn the
+// layout z-fastest: pair[(j*nx + i)*nz + k] = (F_s, F_s+1)(k, j, i).  A particle's z-cell changes
+// every few steps (sigma_z per step ~ dz/3) while its column changes slowly, so with columns
+// contiguous the 32 lanes of a column-sorted warp touch <= 8 128-byte lines per gather instead of
+// one line per lane.  One thread per output texel: coalesced 32-byte writes, strided 16-byte reads
+// (once per met interval, < 1 ms).
 __global__ void __launch_bounds__(256) pair_repack_kernel(const float4 *__restrict__ s0, const float4 *__restrict__ s1,
-                                                          Texel2 *__restrict__ pair, uint64_t cells)
+                                                          Texel2 *__restrict__ pair, uint32_t nx, uint32_t ny, uint32_t nz)
 {
-    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < cells; i += (uint64_t)gridDim.x * blockDim.x) {
+    const uint64_t cells = (uint64_t)nx * ny * nz, plane = (uint64_t)nx * ny;
+    for (uint64_t o = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; o < cells; o += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t col = o / nz;
+        const uint32_t k = (uint32_t)(o - col * nz);
+        const uint64_t src = (uint64_t)k * plane + col;
         Texel2 t;
-        t.a = __ldg(s0 + i);
-        t.b = __ldg(s1 + i);
-        pair[i] = t;
+        t.a = __ldg(s0 + src);
+        t.b = __ldg(s1 + src);
+        pair[o] = t;
     }
 }
 
-cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, uint64_t cells, cudaStream_t st)
+cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, cudaStream_t st)
 {
-    const uint64_t want = (cells + 255) / 256;
-    pair_repack_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(s0, s1, (Texel2 *)pair, cells);
+    const uint64_t want = ((uint64_t)nx * ny * nz + 255) / 256;
+    pair_repack_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(s0, s1, (Texel2 *)pair, (uint32_t)nx, (uint32_t)ny, (uint32_t)nz);
     return cudaGetLastError();
 }
 
