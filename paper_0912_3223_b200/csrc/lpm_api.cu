@@ -27,7 +27,7 @@ struct Release {
 };
 
 struct Layout {
-    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, keys, perm, hist, partial, total;
+    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, blend, keys, perm, hist, partial, total;
 };
 
 uint64_t up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
@@ -51,6 +51,7 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     L.stage = o; o += up(4 * cells3 * K);  // fp32 read-out staging for the *_host entry points
     L.pair = o; o += met.nt > 1 ? up(32ull * met.grid.nx * met.grid.ny * met.grid.nz) : 0;  // (F_s, F_s+1) per met cell
     const uint64_t mcells = (uint64_t)met.grid.nx * met.grid.ny * met.grid.nz;
+    L.blend = o; o += up(16ull * mcells * (met.nt > 1 ? kBlendDepth : 1));  // z-fastest F(t_n), one buffer per fused step
     L.keys = o; o += sort ? up(4 * cap) : 0;            // gather-locality pass: met-cell key per slot
     L.perm = o; o += sort ? up(4 * cap) : 0;            //   slots in met-cell order
     L.hist = o; o += sort ? up(4 * (mcells + 1)) : 0;   //   per-cell counts / offsets
@@ -59,8 +60,8 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     return L;
 }
 
-// zfast: the buffer the kernels sample is the z-fastest pair buffer (32-byte texels); otherwise the
-// caller's x-fastest snapshot (16-byte texels)
+// zfast: strides of the library's z-fastest met buffers; otherwise x-fastest (only nx, ny, nz, the
+// corner and the inverse spacings matter for the binning grid)
 GridF gridf(const lpm_grid &g, bool zfast = false)
 {
     GridF f;
@@ -69,8 +70,8 @@ GridF gridf(const lpm_grid &g, bool zfast = false)
     f.inv_dx = (float)(1.0 / g.dx); f.inv_dy = (float)(1.0 / g.dy); f.inv_dz = (float)(1.0 / g.dz);
     f.fx1 = (float)(g.nx - 1); f.fy1 = (float)(g.ny - 1); f.fz1 = (float)(g.nz - 1);
     f.ix2 = g.nx > 2 ? g.nx - 2 : 0; f.iy2 = g.ny > 2 ? g.ny - 2 : 0; f.iz2 = g.nz > 2 ? g.nz - 2 : 0;
-    if (zfast) { f.ez = 1u; f.ex = (uint32_t)g.nz; f.ey = (uint32_t)g.nz * (uint32_t)g.nx; f.line_shift = 2; }
-    else { f.ex = 1u; f.ey = (uint32_t)g.nx; f.ez = (uint32_t)g.nx * (uint32_t)g.ny; f.line_shift = 3; }
+    if (zfast) { f.ez = 1u; f.ex = (uint32_t)g.nz; f.ey = (uint32_t)g.nz * (uint32_t)g.nx; }
+    else { f.ex = 1u; f.ey = (uint32_t)g.nx; f.ez = (uint32_t)g.nx * (uint32_t)g.ny; }
     f.sx = g.nx > 1 ? f.ex : 0u; f.sy = g.ny > 1 ? f.ey : 0u; f.sz = g.nz > 1 ? f.ez : 0u;
     return f;
 }
@@ -106,6 +107,13 @@ struct lpm_handle {
     uint64_t next_base;
     uint64_t step, bin_step;
     int pair_snap;  // snapshot index s whose pair (s, s+1) the pair buffer holds, -1 = none
+    // a0: the blend buffers hold F(t_n) for steps [blend_step0, blend_step0 + blend_n) (blend_n = 0: nothing)
+    uint64_t blend_step0;
+    int blend_n;
+    // gather-locality pass: the perm buffer lists slots [0, perm_n) of the (single) release as sorted at step perm_step
+    uint64_t perm_n, perm_step;
+    bool perm_valid;
+    double dep_bound[LPM_MAX_NUCLIDES];  // largest activity a particle can carry (fixed-point scale of the deposit tables)
     bool binned;
     int sms, occ;
     uint64_t launches;
@@ -217,11 +225,14 @@ void fill_entry(const lpm_handle *h, uint64_t n, StepEntry &e)
     }
     const bool raining = h->rain_on && t >= h->rt0 && t < h->rt1;  // G6
     e.a = a;
+    e.buf = 0;
+    e.pad_ = 0;
     e.snap = s | (raining ? 1 << 16 : 0);
     for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) {
         e.G[k] = k < h->K ? G_of(h, k, n) : 1.0;
         e.Gf[k] = (float)e.G[k];
         e.Gp[k] = k < h->K ? (float)(e.G[k] * (double)h->p_dry[k]) : 0.0f;
+        e.Gps[k] = 0.0f;
     }
 }
 
@@ -231,17 +242,30 @@ void base_args(const lpm_handle *h, StepArgs &A)
     A.xyzq = (float4 *)(h->ws + h->L.xyzq);
     A.q1 = h->K > 1 ? (float *)(h->ws + h->L.q1) : nullptr;
     A.pid = h->prm.compact ? (uint32_t *)(h->ws + h->L.pid) : nullptr;
-    A.met = (const float4 *)h->met.fields_dev;
-    A.pair = h->met.nt > 1 ? (const void *)(h->ws + h->L.pair) : nullptr;
+    A.blend = (const float4 *)(h->ws + h->L.blend);
     const lpm_grid &mg = h->met.grid;
     A.snap_cells = (uint64_t)mg.nx * mg.ny * mg.nz;
-    A.mg = gridf(mg, h->met.nt > 1);
-    A.nt = h->met.nt;
+    A.mg = gridf(mg, true);
     A.bx0 = (float)mg.x0; A.bx1 = (float)(mg.x0 + mg.nx * mg.dx);
     A.by0 = (float)mg.y0; A.by1 = (float)(mg.y0 + mg.ny * mg.dy);
     A.cg = gridf(h->cg);
     A.dep = (double *)(h->ws + h->L.dep);
     A.dep_stride = (uint64_t)h->cg.nx * h->cg.ny;
+    A.any_dep = (h->dry_mode != kDryNone || h->rain_on) ? 1 : 0;
+    for (int w = 0; w < 2 * LPM_MAX_NUCLIDES; ++w) {
+        // S = largest power of two <= 2^20 / (largest possible increment): activity <= dep_bound, one step
+        // deposits at most the fraction p_dry (dry) or p_wet (wet) of it.  Only efficiency depends on the
+        // bound: an increment outside [2^17, 2^20) / S takes the direct fp64 RED.
+        const int k = w / 2;
+        const double frac = k < h->K ? (w & 1 ? (double)h->p_wet[k] : (double)h->p_dry[k]) : 0.0;
+        const double inc_max = (k < h->K ? h->dep_bound[k] : 0.0) * frac;
+        int e = 0;
+        if (inc_max > 0.0) { frexp(1048576.0 / inc_max, &e); e -= 1; }
+        if (e > 100) e = 100;
+        if (e < -100) e = -100;
+        A.dep_scale[w] = (float)ldexp(1.0, e);
+        A.dep_inv_scale[w] = ldexp(1.0, -e);
+    }
     A.dt = (float)h->prm.dt;
     A.sigma_h = h->sigma_h;
     A.kz_min = (float)h->met.kz_min;
@@ -307,6 +331,51 @@ int do_bin(lpm_handle *h)
     span_close(h, span);
     h->bin_step = h->step;
     h->binned = true;
+    return LPM_OK;
+}
+
+// a0: make the blend buffers hold F(t_n) for the m steps starting at h->step (entries A.tab[0..m)
+// are filled and lie inside one met interval) and point the entries at them.
+int ensure_blend(lpm_handle *h, StepArgs &A, int m, int m_max)
+{
+    const lpm_grid &g = h->met.grid;
+    const float4 *met = (const float4 *)h->met.fields_dev;
+    float4 *blend = (float4 *)(h->ws + h->L.blend);
+    if (h->met.nt == 1) {
+        if (h->blend_n == 0) {
+            CK(launch_transpose(met, blend, g.nx, g.ny, g.nz, h->st));
+            h->launches++;
+            h->blend_n = 1;
+        }
+        for (int s = 0; s < m; ++s) A.tab[s].buf = 0;
+        return LPM_OK;
+    }
+    const int sn = A.tab[0].snap & 0xffff;
+    if (sn != h->pair_snap) {
+        CK(launch_pair_repack(met + (uint64_t)sn * A.snap_cells, met + (uint64_t)(sn + 1) * A.snap_cells, h->ws + h->L.pair,
+                              g.nx, g.ny, g.nz, h->st));
+        h->launches++;
+        h->pair_snap = sn;
+        h->blend_n = 0;
+    }
+    if (!(h->blend_n > 0 && h->step >= h->blend_step0 && h->step + (uint64_t)m <= h->blend_step0 + (uint64_t)h->blend_n)) {
+        float a[kBlendDepth];
+        int cnt = 0;
+        for (; cnt < m; ++cnt) a[cnt] = A.tab[cnt].a;
+        if (m_max < kBlendDepth) {  // short launches (compact mode, steps_per_launch): blend ahead, reuse over the next launches
+            for (; cnt < kBlendDepth; ++cnt) {
+                StepEntry e;
+                fill_entry(h, h->step + (uint64_t)cnt, e);
+                if ((e.snap & 0xffff) != sn) break;
+                a[cnt] = e.a;
+            }
+        }
+        CK(launch_blend(h->ws + h->L.pair, blend, A.snap_cells, cnt, a, h->st));
+        h->launches++;
+        h->blend_step0 = h->step;
+        h->blend_n = cnt;
+    }
+    for (int s = 0; s < m; ++s) A.tab[s].buf = (uint32_t)(h->step + (uint64_t)s - h->blend_step0);
     return LPM_OK;
 }
 
@@ -395,7 +464,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         h->wet_scale[k] = keep_dry * (double)h->p_wet[k];
     }
     h->dry_mode = !any_dry ? kDryNone : (uniform ? kDryUniform : kDryLayer);
-    h->occ = step_max_blocks_per_sm(K, p->compact != 0, met->nt > 1, h->dry_mode);
+    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode);
     if (cudaMemsetAsync(ws, 0, L.total, h->st) != cudaSuccess) { delete h; return LPM_ERR_CUDA; }
     h->launches++;
     *out = h;
@@ -452,6 +521,7 @@ int32_t lpm_release(lpm_handle *h, const lpm_source *src, const double *act, uin
         r.base = h->next_base;
         h->next_base += (r.n_local + 63) / 64 * 64;  // keep blocks 1 KB aligned for float4 access
     }
+    for (int k = 0; k < h->K; ++k) if (r.emit[k] > h->dep_bound[k]) h->dep_bound[k] = r.emit[k];
     h->rel.push_back(r);
     return LPM_OK;
 }
@@ -464,6 +534,7 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
     int m_max = h->prm.steps_per_launch > 0 ? h->prm.steps_per_launch : kMaxFused;
     if (m_max > kMaxFused) m_max = kMaxFused;
     if (compact) m_max = 1;
+    if (h->met.nt > 1 && m_max > kBlendDepth) m_max = kBlendDepth;  // one time-blended met buffer per fused step
     StepArgs A;
     base_args(h, A);
     int64_t left = n_steps;
@@ -476,16 +547,14 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
         A.step0 = h->step;
         for (int s = 0; s < m; ++s) {
             fill_entry(h, h->step + s, A.tab[s]);
+            for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) A.tab[s].Gps[k] = A.tab[s].Gp[k] * A.dep_scale[2 * k];
             // a launch stays inside one met interval: the pair buffer holds snapshots (s, s+1)
             if ((A.tab[s].snap & 0xffff) != (A.tab[0].snap & 0xffff)) { m = s; break; }
         }
         A.m_steps = m;
-        if (h->met.nt > 1 && (A.tab[0].snap & 0xffff) != h->pair_snap) {
-            const int sn = A.tab[0].snap & 0xffff;
-            CK(launch_pair_repack(A.met + (uint64_t)sn * A.snap_cells, A.met + (uint64_t)(sn + 1) * A.snap_cells,
-                                  h->ws + h->L.pair, h->met.grid.nx, h->met.grid.ny, h->met.grid.nz, h->st));
-            h->launches++;
-            h->pair_snap = sn;
+        {
+            const int rc = ensure_blend(h, A, m, m_max);
+            if (rc) return rc;
         }
         if (compact) {
             InjectArgs I{};
@@ -526,14 +595,25 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                 if (h->timing)
                     for (int s = 0; s < m; ++s) units += (double)born_local(r, (int64_t)h->step + s);
                 A.perm = nullptr;
+                A.n_perm = 0;
                 if (sort_enabled(&h->prm) && A.n_prev > 0 && (h->prm.gather_sort > 0 || A.n_prev >= kSortAutoMin)) {
+                    // the list is kept for `period` model steps (one release: the perm buffer is its own);
+                    // particles born since the last sort are walked in slot order behind it
                     uint32_t *perm = (uint32_t *)(h->ws + h->L.perm);
-                    const int sspan = span_open(h, 2, (double)A.n_prev);
-                    CK(launch_sort_by_cell(A.xyzq + r.base, A.n_prev, A.mg, (uint32_t *)(h->ws + h->L.keys),
-                                           (uint32_t *)(h->ws + h->L.hist), (uint32_t *)(h->ws + h->L.partial), perm, h->st));
-                    span_close(h, sspan);
-                    h->launches += 5;
+                    const bool single = h->rel.size() == 1;
+                    const uint64_t period = h->prm.gather_sort > 0 ? (uint64_t)h->prm.gather_sort : (uint64_t)kSortPeriod;
+                    if (!single || !h->perm_valid || h->step - h->perm_step >= period || h->perm_n > A.n_prev) {
+                        const int sspan = span_open(h, 2, (double)A.n_prev);
+                        CK(launch_sort_by_cell(A.xyzq + r.base, A.n_prev, A.mg, (uint32_t *)(h->ws + h->L.keys),
+                                               (uint32_t *)(h->ws + h->L.hist), (uint32_t *)(h->ws + h->L.partial), perm, h->st));
+                        span_close(h, sspan);
+                        h->launches += 5;
+                        h->perm_n = A.n_prev;
+                        h->perm_step = h->step;
+                        h->perm_valid = single;
+                    }
                     A.perm = perm;
+                    A.n_perm = h->perm_n;
                 }
                 CK(cudaMemsetAsync(A.ctrl + 16, 0, 8, h->st));  // tile ticket of the slot kernel
                 const int span = span_open(h, 0, units);
@@ -685,6 +765,20 @@ int32_t lpm_set_particles(lpm_handle *h, const void *xyzq, const float *q1, cons
     }
     h->step = step_index;
     h->binned = false;
+    h->perm_valid = false;
+    if (n) {  // the installed activities bound the deposit increments from now on
+        float *mx = (float *)(h->ws + h->L.air);
+        float mq[2] = {0.f, 0.f};
+        CK(cudaMemsetAsync(mx, 0, 8, h->st));
+        CK(launch_qmax((const float4 *)(h->ws + h->L.xyzq), h->K > 1 ? (const float *)(h->ws + h->L.q1) : nullptr, n, h->K, mx, h->st));
+        h->launches++;
+        CK(cudaMemcpyAsync(mq, mx, 8, cudaMemcpyDeviceToHost, h->st));
+        CK(cudaStreamSynchronize(h->st));
+        for (int k = 0; k < h->K; ++k) {
+            const double b = (double)mq[k] * G_of(h, k, step_index);
+            if (!h->prm.compact || b > h->dep_bound[k]) h->dep_bound[k] = b;
+        }
+    }
     return LPM_OK;
 }
 
@@ -754,6 +848,7 @@ int32_t lpm_upload_meteo(lpm_handle *h, int32_t first, int32_t n_snap, const voi
     CK(cudaMemcpyAsync((char *)h->met.fields_dev + (uint64_t)first * snap_bytes, src, snap_bytes * (uint64_t)n_snap,
                        cudaMemcpyHostToDevice, h->st));
     if (h->pair_snap >= first - 1 && h->pair_snap < first + n_snap) h->pair_snap = -1;  // the pair buffer is stale
+    h->blend_n = 0;                                                                    // and so are the blended fields
     return LPM_OK;
 }
 
@@ -855,21 +950,23 @@ int32_t lpm_test_sample(const lpm_meteo *met, double t, const void *xyz, uint64_
     const float4 *f = (const float4 *)met->fields_dev;
     cudaStream_t s = (cudaStream_t)st;
     const int sn = e.snap & 0xffff;
+    // the same path as lpm_step: z-fastest (pair ->) blended buffer, then the step kernel's sampling
     void *pair = nullptr;
-    if (met->nt > 1) {  // same path as lpm_step: interleave snapshots (sn, sn+1), then sample the pair buffer
-        if (cudaMalloc(&pair, 32 * cells) != cudaSuccess) return LPM_ERR_CUDA;
-        if (launch_pair_repack(f + (uint64_t)sn * cells, f + (uint64_t)(sn + 1) * cells, pair, g.nx, g.ny, g.nz, s) != cudaSuccess) {
-            cudaFree(pair);
-            return LPM_ERR_CUDA;
-        }
+    float4 *blend = nullptr;
+    if (cudaMalloc((void **)&blend, 16 * cells) != cudaSuccess) return LPM_ERR_CUDA;
+    cudaError_t rc;
+    if (met->nt > 1) {
+        if (cudaMalloc(&pair, 32 * cells) != cudaSuccess) { cudaFree(blend); return LPM_ERR_CUDA; }
+        rc = launch_pair_repack(f + (uint64_t)sn * cells, f + (uint64_t)(sn + 1) * cells, pair, g.nx, g.ny, g.nz, s);
+        if (rc == cudaSuccess) rc = launch_blend(pair, blend, cells, 1, &e.a, s);
+    } else {
+        rc = launch_transpose(f, blend, g.nx, g.ny, g.nz, s);
     }
-    cudaError_t rc = launch_test_sample(f + (uint64_t)sn * cells, pair, gridf(g, met->nt > 1), e.a, (float)met->kz_min, (const float4 *)xyz, n,
-                                        (float4 *)out, s);
-    if (pair) {
-        const cudaError_t rs = cudaStreamSynchronize(s);
-        if (rc == cudaSuccess) rc = rs;
-        cudaFree(pair);
-    }
+    if (rc == cudaSuccess) rc = launch_test_sample(blend, gridf(g, true), (float)met->kz_min, (const float4 *)xyz, n, (float4 *)out, s);
+    const cudaError_t rs = cudaStreamSynchronize(s);
+    if (rc == cudaSuccess) rc = rs;
+    cudaFree(blend);
+    if (pair) cudaFree(pair);
     return rc == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
 }
 

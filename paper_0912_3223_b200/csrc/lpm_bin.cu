@@ -169,6 +169,32 @@ cudaError_t launch_iota(uint32_t *pid, uint64_t n, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// largest stored q per nuclide (lpm_set_particles: bound of the fixed-point deposit scale); q >= 0, so
+// the order of the float bit patterns is the order of the values
+__global__ void qmax_kernel(const float4 *__restrict__ xyzq, const float *__restrict__ q1, uint64_t n, int K, float *out2)
+{
+    float m0 = 0.f, m1 = 0.f;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+        m0 = fmaxf(m0, xyzq[i].w);
+        if (K > 1) m1 = fmaxf(m1, q1[i]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        m0 = fmaxf(m0, __shfl_xor_sync(0xffffffffu, m0, o));
+        m1 = fmaxf(m1, __shfl_xor_sync(0xffffffffu, m1, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax((unsigned int *)out2, __float_as_uint(m0));
+        atomicMax((unsigned int *)out2 + 1, __float_as_uint(m1));
+    }
+}
+
+cudaError_t launch_qmax(const float4 *xyzq, const float *q1, uint64_t n, int K, float *out2, cudaStream_t st)
+{
+    qmax_kernel<<<148 * 4, 256, 0, st>>>(xyzq, q1, n, K, out2);
+    return cudaGetLastError();
+}
+
 // ------------------------------------------------------------------ stand-alone parity kernels
 __global__ void test_philox_kernel(uint32_t seed_lo, uint32_t seed_hi, uint32_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out)
 {
@@ -202,22 +228,21 @@ cudaError_t launch_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uin
     return cudaGetLastError();
 }
 
-__global__ void test_sample_kernel(const float4 *met, const Texel2 *pair, GridF mg, float a, float kz_min,
-                                   const float4 *xyz, uint64_t n, float4 *out)
+__global__ void test_sample_kernel(const float4 *blend, GridF mg, float kz_min, const float4 *xyz, uint64_t n, float4 *out)
 {
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
         const float4 p = xyz[i];
         const Corner c = corner_of(mg, p.x, p.y, p.z);
-        float4 m = pair ? trilinear_pair(pair, c, mg, a) : trilinear(met, c, mg);   // the step kernel's two paths
+        float4 m = trilinear(blend, c, mg);   // the step kernel's sampling of a blended buffer
         m.w = fmaxf(m.w, kz_min);
         out[i] = m;
     }
 }
 
-cudaError_t launch_test_sample(const float4 *met, const void *pair, GridF mg, float a, float kz_min,
-                               const float4 *xyz, uint64_t n, float4 *out, cudaStream_t st)
+cudaError_t launch_test_sample(const float4 *blend, GridF mg, float kz_min, const float4 *xyz, uint64_t n, float4 *out,
+                               cudaStream_t st)
 {
-    test_sample_kernel<<<148, 256, 0, st>>>(met, (const Texel2 *)pair, mg, a, kz_min, xyz, n, out);
+    test_sample_kernel<<<148, 256, 0, st>>>(blend, mg, kz_min, xyz, n, out);
     return cudaGetLastError();
 }
 

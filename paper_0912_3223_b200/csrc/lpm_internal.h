@@ -8,7 +8,9 @@
 
 namespace lpm {
 
-constexpr int kMaxFused = 96;        // model steps fused into one launch (table lives in kernel params)
+constexpr int kMaxFused = 16;        // model steps fused into one launch (table lives in kernel params)
+constexpr int kBlendDepth = kMaxFused;  // time-blended met buffers kept: one per fused step
+constexpr int kSortPeriod = 96;      // model steps between two gather-locality sorts of a release
 constexpr int kStepThreads = 256;    // CTA size of the step kernel
 constexpr int kScanTile = kStepThreads;  // particles per look-back tile (compaction)
 
@@ -17,8 +19,11 @@ struct StepEntry {
     double G[LPM_MAX_NUCLIDES];  // G_k(t_n): activity = q * G (decay and uniform dry loss folded in)
     float Gf[LPM_MAX_NUCLIDES];  // (float)G_k(t_n), the factor the per-step fp32 arithmetic uses
     float Gp[LPM_MAX_NUCLIDES];  // (float)(G_k(t_n) * p_dry,k): uniform dry deposit of one step per unit q
+    float Gps[LPM_MAX_NUCLIDES]; // Gp * S_dry,k: the same in the fixed-point units of the deposit tables
     float a;                     // time weight between snapshot `snap` and `snap + 1`
     int32_t snap;                // bits 0..15 snapshot index, bit 16 = raining
+    uint32_t buf;                // which time-blended met buffer holds F(t_n) (a0)
+    uint32_t pad_;
 };
 
 struct GridF {  // fp32 view of a grid, exactly as the kernels use it
@@ -30,10 +35,9 @@ struct GridF {  // fp32 view of a grid, exactly as the kernels use it
     // i1 = min(i0 + 1, n - 1) = i0 + 1 whenever n >= 2, because i0 <= n - 2)
     float fx1, fy1, fz1;       // (float)(n - 1)
     int32_t ix2, iy2, iz2;     // max(n - 2, 0)
-    uint32_t ex, ey, ez;       // element strides of cell (i, j, k) in the sampled buffer: x-fastest (1, nx, nx*ny)
-                               // for the caller's snapshots, z-fastest (nz, nx*nz, 1) for the pair buffer
+    uint32_t ex, ey, ez;       // element strides of cell (i, j, k) in the sampled buffer: z-fastest (nz, nx*nz, 1)
+                               // for the library's met buffers (x-fastest (1, nx, nx*ny) is the caller's layout)
     uint32_t sx, sy, sz;       // stride to the upper corner on each axis: n > 1 ? e : 0
-    uint32_t line_shift;       // log2(texels per 128-byte line of the sampled buffer): gather-locality key = offset >> shift
 };
 
 enum DryMode : int32_t { kDryNone = 0, kDryUniform = 1, kDryLayer = 2 };
@@ -43,18 +47,19 @@ struct StepArgs {
     float4 *xyzq;
     float *q1;
     uint32_t *pid;        // compact mode only
-    // meteorology: `met` = caller's snapshots [nt][cells] (one-snapshot path); `pair` = the library's
-    // interleaved (F_s, F_s+1) buffer of the current met interval (two-snapshot path, 32 B per cell)
-    const float4 *met;
-    const void *pair;
+    // meteorology (a0): `blend` = the library's z-fastest float4 buffers [n_buf][cells]; buffer
+    // tab[s].buf holds the field at the time of fused step s, F(t_n) = F_s + a (F_s+1 - F_s)
+    const float4 *blend;
     uint64_t snap_cells;  // cells per snapshot
     GridF mg;
-    int32_t nt;
     float bx0, bx1, by0, by1;  // lateral boundary (met box), fp32
     // deposition map
     GridF cg;
     double *dep;          // [K][ny][nx]
     uint64_t dep_stride;
+    float dep_scale[2 * LPM_MAX_NUCLIDES];       // fixed-point scales of the CTA-private deposit sums (powers of two): [2k] dry, [2k+1] wet
+    double dep_inv_scale[2 * LPM_MAX_NUCLIDES];  // their inverses
+    int32_t any_dep, pad0_;                  // some sink can deposit (dry deposition or a rain box)
     // physics
     float dt, sigma_h, kz_min, H, h_dep;
     int32_t dry_mode, absorb;
@@ -69,7 +74,8 @@ struct StepArgs {
     float wet_scale_f[LPM_MAX_NUCLIDES]; // (float)wet_scale
     // population (slot-addressed mode): slots [0, n) of the release block starting at `base`
     uint64_t base, n, n_prev;  // slots >= n_prev are born inside this launch
-    const uint32_t *perm;      // gather-locality pass: slots [0, n_prev) listed in met-cell order, or null
+    const uint32_t *perm;      // gather-locality pass: slots [0, n_perm) listed in dual-cell order, or null
+    uint64_t n_perm;           // slots [n_perm, n) are walked in slot order
     uint64_t pid_offset, pid_stride;
     uint64_t rel_N, rel_c;     // count mode: N (global count); rate mode: c slots per step
     int64_t rel_s_start, rel_S;
@@ -116,12 +122,14 @@ struct BinArgs {
 
 // launchers implemented in the .cu files; all return the cudaError of the launch
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int grid_blocks, cudaStream_t st);
-int step_max_blocks_per_sm(int K, bool compact, bool two_snap, int dry_mode);
+int step_max_blocks_per_sm(int K, bool compact, int dry_mode);
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
                                 uint32_t *perm, cudaStream_t st);
 uint64_t sort_partial_entries(uint64_t n_cells);
 cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, cudaStream_t st);
+cudaError_t launch_transpose(const float4 *s0, float4 *out, int nx, int ny, int nz, cudaStream_t st);
+cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, cudaStream_t st);
 cudaError_t launch_bin(const BinArgs &a, int blocks, cudaStream_t st);
 cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3, int K, const double *scale, cudaStream_t st);
 cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, double inv_area, cudaStream_t st);
@@ -129,9 +137,10 @@ cudaError_t launch_airborne(const float4 *xyzq, const float *q1, uint64_t n, con
 cudaError_t launch_export(const float4 *xyzq, uint64_t n, const uint64_t *n_dev, float4 *out, uint8_t *status, cudaStream_t st);
 cudaError_t launch_import(float4 *xyzq, uint64_t n, const uint8_t *status, cudaStream_t st);
 cudaError_t launch_iota(uint32_t *pid, uint64_t n, cudaStream_t st);
+cudaError_t launch_qmax(const float4 *xyzq, const float *q1, uint64_t n, int K, float *out2, cudaStream_t st);
 cudaError_t launch_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st);
 cudaError_t launch_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, float *out, cudaStream_t st);
-cudaError_t launch_test_sample(const float4 *met, const void *pair, GridF mg, float a, float kz_min,
-                               const float4 *xyz, uint64_t n, float4 *out, cudaStream_t st);
+cudaError_t launch_test_sample(const float4 *blend, GridF mg, float kz_min, const float4 *xyz, uint64_t n, float4 *out,
+                               cudaStream_t st);
 
 }  // namespace lpm

@@ -15,20 +15,19 @@ namespace lpm {
 constexpr int kScanItems = 16;                       // items per thread in the scan kernels
 constexpr int kScanBlock = 256 * kScanItems;         // items per block
 
-// pass 1: key = 128-byte line of the sampled met buffer that holds the particle's cell (edge-clamped;
-// exited slots go to the last bucket, n_keys - 1)
+// pass 1: key = offset of the LOWER CORNER texel (i0, j0, k0) of the particle's trilinear stencil in
+// the sampled met buffer (the "dual cell"), computed by the same corner_of() the gather uses:
+// particles with equal keys read exactly the same eight texels, so a warp of equal keys costs one
+// L1 sector per gather instruction instead of one per lane (the L1 data pipe delivers one 32-byte
+// sector per cycle; with keys by containing cell a warp still spans the 8 octants = up to 8 lower
+// corners).  Exited slots go to the last bucket, n_keys - 1.
 __global__ void __launch_bounds__(256) sort_key_kernel(const float4 *__restrict__ xyzq, uint64_t n, GridF g, uint32_t n_keys,
                                                        uint32_t *__restrict__ keys, uint32_t *__restrict__ hist)
 {
     for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n; l += (uint64_t)gridDim.x * blockDim.x) {
         const float4 p = xyzq[l];
         uint32_t key = n_keys - 1;
-        if (p.z >= 0.0f) {
-            const int i = min(max((int)floorf((p.x - g.x0) * g.inv_dx), 0), g.nx - 1);
-            const int j = min(max((int)floorf((p.y - g.y0) * g.inv_dy), 0), g.ny - 1);
-            const int k = min(max((int)floorf((p.z - g.z0) * g.inv_dz), 0), g.nz - 1);
-            key = ((uint32_t)i * g.ex + (uint32_t)j * g.ey + (uint32_t)k * g.ez) >> g.line_shift;
-        }
+        if (p.z >= 0.0f) key = corner_of(g, p.x, p.y, p.z).o;
         keys[l] = key;
         atomicAdd(hist + key, 1u);
     }
@@ -121,7 +120,7 @@ __global__ void __launch_bounds__(256) sort_scatter_kernel(const uint32_t *__res
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
                                 uint32_t *perm, cudaStream_t st)
 {
-    const uint32_t n_keys = (((uint32_t)g.nx * g.ny * g.nz - 1u) >> g.line_shift) + 2u, m = n_keys;
+    const uint32_t n_keys = (uint32_t)g.nx * g.ny * g.nz + 1u, m = n_keys;
     cudaError_t e = cudaMemsetAsync(hist, 0, 4ull * m, st);
     if (e != cudaSuccess) return e;
     const uint64_t want = (n + 255) / 256;

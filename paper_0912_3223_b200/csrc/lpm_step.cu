@@ -2,12 +2,12 @@
 //
 // One thread carries one particle through m >= 1 model steps with its state in registers:
 //   a1 Philox4x32-10 + Box-Muller      (R1-R3)
-//   a0/a2 trilinear gathers of float4 (u,v,w,Kz) from one or two L2-resident snapshots and the
-//         linear blend in time           (R4)
+//   a0 the met field of every fused step is blended in time once per launch (blend_kernel below)
+//   a2 trilinear gathers of float4 (u,v,w,Kz) from that step's z-fastest buffer (R4)
 //   a3 advection + random walk          (R5; Eq.(1)(2))
 //   a4 reflection, lateral boundary     (R6, R7)
 //   a5 decay / dry / wet deposition     (R8)
-//   a6 deposit scatter into the 2-D map (fp64 RED; the map stays in L2)
+//   a6 deposit scatter into the 2-D map (CTA-private fixed-point table in shared memory, then fp64 RED)
 //   a7 stable in-place compaction by a single-pass decoupled look-back scan (compact mode)
 // The paper's kernel staged particle state in shared memory and sampled hardware textures
 // (P:L110-114); neither survives on B200: there is no reuse to stage, and texture filtering's
@@ -20,60 +20,115 @@ template <int K>
 struct Acc {  // per-thread ledger partial sums, in activity units before the per-nuclide scale
     float dry[K], wet[K], dec[K];
     float both[K];  // steps where the dry and the decay ledger see the same activity (uniform dry / no sink, no rain)
-    float off[K];   // deposit that fell off the map (already scaled)
+    float off[K];   // deposit that fell off the map (activity)
 };
 
-// a6 run-length aggregation: a particle stays in one 2-D map cell for several steps, so its
-// deposit increments are summed in registers and sent to the map (one fp64 RED per nuclide) only
-// when the cell changes or the launch ends.  cell: >= 0 map cell, -1 off the map, -2 empty.
+// a6 deposit scatter, CTA-privatised (S§8(a) a6 "privatised reduce"): the particles of a tile are
+// spatial neighbours (gather-locality order), so over the fused steps of a launch their deposits
+// fall into a few hundred map cells.  Each CTA sums them in a 1024-slot open-addressing table in
+// shared memory keyed by the map cell and sends ONE fp64 RED per touched cell and nuclide to the
+// L2-resident map when the tile is done, instead of one per particle-step.
+// The sums are FIXED-POINT integers: increment -> rint(inc * S_k), S_k = 2^20 / (largest possible
+// increment) rounded down to a power of two, added with the native 32-bit shared atomic (ATOMS.ADD;
+// fp32 and 64-bit shared atomics are CAS loops on sm_100).  At most kStepThreads * kMaxFused = 2^12
+// increments < 2^20 meet in a slot per tile, so a slot cannot overflow; integer addition is
+// associative, so a tile's sums do not depend on the order of the atomics.  Increments in
+// [2^17, 2^20) take this path (>= 18 significant bits, round to nearest: relative error <= 1.9e-6
+// per increment, unbiased; B4); smaller ones (a particle that carries < 1/8 of the
+// largest activity), increments that do not fit and a full table take the direct fp64 RED.
+constexpr int kDepSlots = 1024, kDepSlotBits = 10, kDepProbes = 8;
+static_assert(kStepThreads * kMaxFused <= 4096, "fixed-point deposit sums: 20 bits + 12 bits of count");
+
+// Dry and wet increments differ by orders of magnitude (p_dry ~ 5e-6, p_wet ~ 5e-4 per step), so each
+// has its own scale and its own sum: slot word 2k = dry, 2k + 1 = wet deposit of nuclide k.
 template <int K>
-struct Dep {
-    int cell;
-    float a[K];
+struct DepTab {
+    uint32_t tag[kDepSlots];           // map cell + 1, 0 = empty
+    uint32_t sum[2 * K][kDepSlots];
 };
 
 template <int K>
-__device__ __forceinline__ void dep_flush(const StepArgs &A, Dep<K> &d, Acc<K> &acc)
+__device__ __forceinline__ void dep_clear(DepTab<K> &T)
 {
-    if (d.cell >= 0) {
-        double *p = A.dep + (uint32_t)d.cell;
+    for (int i = threadIdx.x; i < kDepSlots; i += kStepThreads) {
+        T.tag[i] = 0u;
 #pragma unroll
-        for (int k = 0; k < K; ++k) atomicAdd(p + k * A.dep_stride, (double)d.a[k]);
-    } else if (d.cell == -1) {
-#pragma unroll
-        for (int k = 0; k < K; ++k) acc.off[k] += d.a[k];
+        for (int k = 0; k < 2 * K; ++k) T.sum[k][i] = 0u;
     }
-    d.cell = -2;
+}
+
+// all threads of the CTA; barriers on both sides belong to the caller
+template <int K>
+__device__ __forceinline__ void dep_flush(const StepArgs &A, DepTab<K> &T)
+{
+    for (int i = threadIdx.x; i < kDepSlots; i += kStepThreads) {
+        const uint32_t key = T.tag[i];
+        if (key == 0u) continue;
+        T.tag[i] = 0u;
 #pragma unroll
-    for (int k = 0; k < K; ++k) d.a[k] = 0.0f;
+        for (int k = 0; k < K; ++k) {
+            const uint32_t vd = T.sum[2 * k][i], vw = T.sum[2 * k + 1][i];
+            T.sum[2 * k][i] = 0u; T.sum[2 * k + 1][i] = 0u;
+            if (vd | vw) atomicAdd(A.dep + (key - 1u) + k * A.dep_stride, (double)vd * A.dep_inv_scale[2 * k] + (double)vw * A.dep_inv_scale[2 * k + 1]);
+        }
+    }
+}
+
+// one increment v (already scaled) into word w of the slot, or straight to the map
+template <int K>
+__device__ __forceinline__ void dep_add(const StepArgs &A, DepTab<K> &T, int slot, uint32_t cell, int k, int w, float v)
+{
+    if (slot >= 0 && v >= 131072.0f && v < 1048575.5f) atomicAdd(&T.sum[w][slot], __float2uint_rn(v));
+    else if (v != 0.0f) atomicAdd(A.dep + cell + k * A.dep_stride, (double)v * A.dep_inv_scale[w]);
+}
+
+// add one particle-step's deposit to the map cell of the NEW (x, y); vd[k], vw[k] = dry and wet
+// increment of nuclide k in the fixed-point units of their sums
+template <int K, bool WET>
+__device__ __forceinline__ void deposit_at(const StepArgs &A, float x, float y, const float (&vd)[K], const float (&vw)[K], Acc<K> &acc,
+                                           DepTab<K> &T)
+{
+    const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
+    const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
+    if ((ci | cj) < 0) {  // off the map: ledger only
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            acc.off[k] += vd[k] * (float)A.dep_inv_scale[2 * k];
+            if (WET) acc.off[k] += vw[k] * (float)A.dep_inv_scale[2 * k + 1];
+        }
+        return;
+    }
+    const uint32_t cell = (uint32_t)(cj * A.cg.nx + ci), key = cell + 1u;
+    uint32_t h = (key * 0x9E3779B1u) >> (32 - kDepSlotBits);
+    int slot = -1;
+#pragma unroll 1
+    for (int p = 0; p < kDepProbes; ++p) {
+        const uint32_t t = *(volatile uint32_t *)&T.tag[h];
+        if (t == key) { slot = (int)h; break; }
+        if (t == 0u) {
+            const uint32_t old = atomicCAS(&T.tag[h], 0u, key);
+            if (old == 0u || old == key) { slot = (int)h; break; }
+        }
+        h = (h + 1u) & (kDepSlots - 1);
+    }
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        dep_add<K>(A, T, slot, cell, k, 2 * k, vd[k]);
+        if (WET) dep_add<K>(A, T, slot, cell, k, 2 * k + 1, vw[k]);
+    }
 }
 
 // One model step of one particle.  Returns false when the particle left the domain (ABSORB).
 // Source order = intended issue order: the eight gathers go out first and the ~150 instructions of
 // Philox + Box-Muller run while they are in flight.
-// a6: make (x, y)'s map cell the current run of the aggregator (flushing the previous run)
-template <int K>
-__device__ __forceinline__ void deposit_at(const StepArgs &A, float x, float y, Acc<K> &acc, Dep<K> &dep)
-{
-    const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
-    const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
-    const int c = (ci | cj) >= 0 ? cj * A.cg.nx + ci : -1;
-    if (c != dep.cell) {
-        dep_flush<K>(A, dep, acc);
-        dep.cell = c;
-    }
-}
-
-template <int K, bool TWO, int DRY>
+template <int K, int DRY>
 __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e, uint32_t step_lo,
                                           uint32_t pid_lo, float &x, float &y, float &z,
-                                          float (&q)[K], Acc<K> &acc, Dep<K> &dep)
+                                          float (&q)[K], Acc<K> &acc, DepTab<K> &dep)
 {
     // a0 + a2: weather at X_old, t_n
     const Corner c = corner_of(A.mg, x, y, z);
-    float4 m;
-    if (TWO) m = trilinear_pair((const Texel2 *)A.pair, c, A.mg, e.a);
-    else m = trilinear(A.met, c, A.mg);
+    const float4 m = trilinear(A.blend + (uint64_t)e.buf * A.snap_cells, c, A.mg);
     const float kz = fmaxf(m.w, A.kz_min);
 
     // a1: three N(0,1) from Philox stream 0
@@ -109,31 +164,33 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
 #pragma unroll
         for (int k = 0; k < K; ++k) acc.both[k] = fmaf(q[k], e.Gf[k], acc.both[k]);
         if (DRY == kDryNone) return true;
-        deposit_at<K>(A, x, y, acc, dep);
+        float vd[K];
 #pragma unroll
-        for (int k = 0; k < K; ++k) dep.a[k] = fmaf(q[k], e.Gp[k], dep.a[k]);
+        for (int k = 0; k < K; ++k) vd[k] = q[k] * e.Gps[k];
+        deposit_at<K, false>(A, x, y, vd, vd, acc, dep);
         return true;
     }
     const bool dry_here = DRY == kDryUniform || (DRY == kDryLayer && z < A.h_dep);
     const bool wet_here = raining & (x >= A.rx0) & (x < A.rx1) & (y >= A.ry0) & (y < A.ry1);
-    float inc[K];
+    float vd[K], vw[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const float G = e.Gf[k];
         float act = q[k] * G;
-        inc[k] = 0.0f;
+        vd[k] = 0.0f;
+        vw[k] = 0.0f;
         if (dry_here) {
             acc.dry[k] += act;
             if (DRY == kDryLayer) {
-                inc[k] = act * A.p_dry[k];
+                vd[k] = act * A.p_dry[k] * A.dep_scale[2 * k];
                 q[k] = fmaf(-q[k], A.p_dry[k], q[k]);
                 act = q[k] * G;
             } else {
-                inc[k] = q[k] * e.Gp[k];
+                vd[k] = q[k] * e.Gps[k];
             }
         }
         if (wet_here) {
-            inc[k] = fmaf(act, A.wet_scale_f[k], inc[k]);
+            vw[k] = act * A.wet_scale_f[k] * A.dep_scale[2 * k + 1];
             acc.wet[k] += act;
             q[k] = fmaf(-q[k], A.p_wet[k], q[k]);
             act = q[k] * G;
@@ -141,12 +198,8 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
         acc.dec[k] += act;
     }
 
-    // a6: deposit at the cell of the NEW (x, y), run-length aggregated in registers
-    if (dry_here | wet_here) {
-        deposit_at<K>(A, x, y, acc, dep);
-#pragma unroll
-        for (int k = 0; k < K; ++k) dep.a[k] += inc[k];
-    }
+    // a6: deposit at the cell of the NEW (x, y)
+    if (dry_here | wet_here) deposit_at<K, true>(A, x, y, vd, vw, acc, dep);
     return true;
 }
 
@@ -183,7 +236,7 @@ __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &ac
 #endif
 static_assert(sizeof(StepArgs) <= 32764, "StepArgs must fit the kernel-parameter space (32764 B since CUDA 12.1 on sm_70+)");
 
-template <int K, bool TWO, int DRY>
+template <int K, int DRY>
 __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel(const __grid_constant__ StepArgs A)
 {
     __shared__ uint32_t s_ticket;
@@ -191,67 +244,70 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
 #pragma unroll
     for (int k = 0; k < K; ++k) acc.dry[k] = acc.wet[k] = acc.dec[k] = acc.both[k] = acc.off[k] = 0.0f;
 
-    // Dynamic, DECORRELATED tile schedule: ticket t -> tile (t % G) * R + t / G, so the CTAs that
-    // are resident together work on tiles spread over the whole slot range (= over all particle
-    // ages, hence over the whole plume) instead of on ~3e5 neighbouring particles that would all
-    // hit the same few deposition-map cells and met lines at the same time.
-    // tiles [0, t_old) walk the sorted slot list (particles that existed before this launch), tiles
-    // [t_old, n_tiles) the slots born inside this launch, in id order (all at the source point)
-    const uint32_t t_old = A.perm ? (uint32_t)((A.n_prev + kStepThreads - 1) / kStepThreads) : 0u;
-    const uint64_t first_new = A.perm ? A.n_prev : 0ull;
+    // Dynamic tile schedule in list order: tiles [0, t_old) walk the sorted slot list (particles that
+    // existed at the last gather-locality sort, in dual-cell order), tiles [t_old, n_tiles) the
+    // younger slots in id order (still close to the source).  The CTAs resident together therefore
+    // work on one small region of the plume: their met gathers hit L1/L2, and their deposits meet
+    // in the CTA-private tables below instead of in the global map.
+    __shared__ DepTab<K> T;
+    dep_clear<K>(T);
+    const uint32_t t_old = A.perm ? (uint32_t)((A.n_perm + kStepThreads - 1) / kStepThreads) : 0u;
+    const uint64_t first_new = A.perm ? A.n_perm : 0ull;
     const uint32_t n_tiles = t_old + (uint32_t)((A.n - first_new + kStepThreads - 1) / kStepThreads);
-    const uint32_t G = min(n_tiles, (uint32_t)gridDim.x);
-    const uint32_t R = (n_tiles + G - 1) / G;
-    const uint32_t n_tickets = G * R;
     for (;;) {
         __syncthreads();
         if (threadIdx.x == 0) s_ticket = (uint32_t)atomicAdd((unsigned long long *)(A.ctrl + 16), 1ull);
         __syncthreads();
-        const uint32_t t = s_ticket;
-        if (t >= n_tickets) break;
-        const uint32_t tile = (t % G) * R + t / G;
+        const uint32_t tile = s_ticket;
+        if (tile >= n_tiles) break;
         uint64_t l;
+        bool valid;
         if (tile < t_old) {
             const uint64_t idx = (uint64_t)tile * kStepThreads + threadIdx.x;
-            if (idx >= A.n_prev) continue;
-            l = A.perm[idx];
+            valid = idx < A.n_perm;
+            l = valid ? A.perm[idx] : 0ull;
         } else {
             l = first_new + (uint64_t)(tile - t_old) * kStepThreads + threadIdx.x;
-            if (l >= A.n) continue;
+            valid = l < A.n;
         }
         const uint64_t slot = A.base + l;
         const uint32_t pid = (uint32_t)(A.pid_offset + l * A.pid_stride);
-        float x, y, z, q[K];
+        float x = 0.f, y = 0.f, z = 0.f, q[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k) q[k] = 0.f;
         int s_begin = 0;
-        if (l >= A.n_prev) {
-            // born inside this launch (R9): count mode b = s_start + floor(j*S/N), rate mode
-            // b = s_start + l / c
-            const int64_t b = A.rel_N ? A.rel_s_start + (int64_t)(((uint64_t)pid * (uint64_t)A.rel_S) / A.rel_N)
-                                      : A.rel_s_start + (int64_t)(l / A.rel_c);
-            s_begin = (int)(b - (int64_t)A.step0);
-            x = A.sx; y = A.sy; z = A.sz;
+        if (valid) {
+            if (l >= A.n_prev) {
+                // born inside this launch (R9): count mode b = s_start + floor(j*S/N), rate mode
+                // b = s_start + l / c
+                const int64_t b = A.rel_N ? A.rel_s_start + (int64_t)(((uint64_t)pid * (uint64_t)A.rel_S) / A.rel_N)
+                                          : A.rel_s_start + (int64_t)(l / A.rel_c);
+                s_begin = (int)(b - (int64_t)A.step0);
+                x = A.sx; y = A.sy; z = A.sz;
 #pragma unroll
-            for (int k = 0; k < K; ++k) q[k] = (float)(A.emit[k] / A.tab[s_begin].G[k]);
-        } else {
-            const float4 p = A.xyzq[slot];
-            x = p.x; y = p.y; z = p.z; q[0] = p.w;
-            if (K > 1) q[1] = A.q1[slot];
-            if (z < 0.0f) continue;  // exited earlier (ABSORB without compaction)
+                for (int k = 0; k < K; ++k) q[k] = (float)(A.emit[k] / A.tab[s_begin].G[k]);
+            } else {
+                const float4 p = A.xyzq[slot];
+                x = p.x; y = p.y; z = p.z; q[0] = p.w;
+                if (K > 1) q[1] = A.q1[slot];
+                valid = z >= 0.0f;  // z < 0: exited earlier (ABSORB without compaction)
+            }
         }
-        Dep<K> dep;
-        dep.cell = -2;
-#pragma unroll
-        for (int k = 0; k < K; ++k) dep.a[k] = 0.0f;
-        // the trip count is the same for every thread (uniform table index, uniform branches inside
-        // the step); a particle born inside this launch or absorbed at the boundary skips steps
-        bool alive = true;
-        const uint32_t step0 = (uint32_t)A.step0;
-        for (int s = 0; s < A.m_steps; ++s)
-            if (alive & (s >= s_begin)) alive = step_once<K, TWO, DRY>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, dep);
-        dep_flush<K>(A, dep, acc);
-        if (!alive) z = -1.0f - z;  // exit position kept, slot marked inactive
-        A.xyzq[slot] = make_float4(x, y, z, q[0]);
-        if (K > 1) A.q1[slot] = q[1];
+        if (valid) {
+            // the trip count is the same for every thread (uniform table index, uniform branches inside
+            // the step); a particle born inside this launch or absorbed at the boundary skips steps
+            bool alive = true;
+            const uint32_t step0 = (uint32_t)A.step0;
+            for (int s = 0; s < A.m_steps; ++s)
+                if (alive & (s >= s_begin)) alive = step_once<K, DRY>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, T);
+            if (!alive) z = -1.0f - z;  // exit position kept, slot marked inactive
+            A.xyzq[slot] = make_float4(x, y, z, q[0]);
+            if (K > 1) A.q1[slot] = q[1];
+        }
+        if (A.any_dep) {
+            __syncthreads();
+            dep_flush<K>(A, T);
+        }
     }
     flush_ledger<K>(A, acc);
 }
@@ -274,7 +330,7 @@ __device__ __forceinline__ void st_state(uint64_t *p, uint64_t v)
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-template <int K, bool TWO, int DRY>
+template <int K, int DRY>
 __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid_constant__ StepArgs A)
 {
     __shared__ uint32_t s_tile;
@@ -289,6 +345,9 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
     const uint32_t epoch = ((uint32_t)(A.step0 + 1) & 0x3fffffffu) << 2;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     constexpr uint32_t FLAG_A = 1u, FLAG_P = 2u;
+    __shared__ DepTab<K> T;
+    dep_clear<K>(T);
+    __syncthreads();
 
     for (;;) {
         if (threadIdx.x == 0) s_tile = (uint32_t)atomicAdd((unsigned long long *)(A.ctrl + 1), 1ull);
@@ -305,12 +364,7 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
             x = p.x; y = p.y; z = p.z; q[0] = p.w;
             if (K > 1) q[1] = A.q1[i];
             pid = A.pid[i];
-            Dep<K> dep;
-            dep.cell = -2;
-#pragma unroll
-            for (int k = 0; k < K; ++k) dep.a[k] = 0.0f;
-            alive = step_once<K, TWO, DRY>(A, A.tab[0], (uint32_t)A.step0, pid, x, y, z, q, acc, dep);
-            dep_flush<K>(A, dep, acc);
+            alive = step_once<K, DRY>(A, A.tab[0], (uint32_t)A.step0, pid, x, y, z, q, acc, T);
         }
         // survivors: rank inside the tile
         const uint32_t ball = __ballot_sync(0xffffffffu, alive);
@@ -366,7 +420,8 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
             if (K > 1) A.q1[dst] = q[1];
             A.pid[dst] = pid;
         }
-        __syncthreads();  // s_tile / s_wtot / s_excl are reused by the next tile
+        if (A.any_dep) dep_flush<K>(A, T);  // every thread's step is behind the barrier above
+        __syncthreads();  // s_tile / s_wtot / s_excl and the deposit table are reused by the next tile
     }
     flush_ledger<K>(A, acc);
 }
@@ -400,37 +455,32 @@ __global__ void __launch_bounds__(256) inject_kernel(const __grid_constant__ Inj
 }
 
 // ------------------------------------------------------------------ launchers
-// One instantiation per (nuclide count, one / two met snapshots, dry-deposition mode); `f` receives
-// the kernel function pointer of the variant that matches the handle.
+// One instantiation per (nuclide count, dry-deposition mode).
 typedef void (*StepKernel)(const StepArgs);
 
-template <int K, bool TWO>
+template <int K>
 static StepKernel pick_dry(bool compact, int dry)
 {
     if (compact) {
-        if (dry == kDryNone) return step_compact_kernel<K, TWO, kDryNone>;
-        return dry == kDryUniform ? step_compact_kernel<K, TWO, kDryUniform> : step_compact_kernel<K, TWO, kDryLayer>;
+        if (dry == kDryNone) return step_compact_kernel<K, kDryNone>;
+        return dry == kDryUniform ? step_compact_kernel<K, kDryUniform> : step_compact_kernel<K, kDryLayer>;
     }
-    if (dry == kDryNone) return step_slots_kernel<K, TWO, kDryNone>;
-    return dry == kDryUniform ? step_slots_kernel<K, TWO, kDryUniform> : step_slots_kernel<K, TWO, kDryLayer>;
+    if (dry == kDryNone) return step_slots_kernel<K, kDryNone>;
+    return dry == kDryUniform ? step_slots_kernel<K, kDryUniform> : step_slots_kernel<K, kDryLayer>;
 }
 
-static StepKernel pick(int K, bool compact, bool two, int dry)
-{
-    if (K == 1) return two ? pick_dry<1, true>(compact, dry) : pick_dry<1, false>(compact, dry);
-    return two ? pick_dry<2, true>(compact, dry) : pick_dry<2, false>(compact, dry);
-}
+static StepKernel pick(int K, bool compact, int dry) { return K == 1 ? pick_dry<1>(compact, dry) : pick_dry<2>(compact, dry); }
 
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int blocks, cudaStream_t st)
 {
-    pick(K, compact, a.nt > 1, a.dry_mode)<<<blocks, kStepThreads, 0, st>>>(a);
+    pick(K, compact, a.dry_mode)<<<blocks, kStepThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 
-int step_max_blocks_per_sm(int K, bool compact, bool two, int dry)
+int step_max_blocks_per_sm(int K, bool compact, int dry)
 {
     int nb = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick(K, compact, two, dry), kStepThreads, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick(K, compact, dry), kStepThreads, 0);
     return nb;
 }
 
@@ -459,6 +509,60 @@ cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, i
 {
     const uint64_t want = ((uint64_t)nx * ny * nz + 255) / 256;
     pair_repack_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(s0, s1, (Texel2 *)pair, (uint32_t)nx, (uint32_t)ny, (uint32_t)nz);
+    return cudaGetLastError();
+}
+
+// a0, one snapshot (nt = 1): z-fastest copy of the caller's x-fastest snapshot
+__global__ void __launch_bounds__(256) transpose_kernel(const float4 *__restrict__ s0, float4 *__restrict__ out, uint32_t nx, uint32_t ny,
+                                                        uint32_t nz)
+{
+    const uint64_t cells = (uint64_t)nx * ny * nz, plane = (uint64_t)nx * ny;
+    for (uint64_t o = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; o < cells; o += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t col = o / nz;
+        out[o] = __ldg(s0 + (uint64_t)(uint32_t)(o - col * nz) * plane + col);
+    }
+}
+
+cudaError_t launch_transpose(const float4 *s0, float4 *out, int nx, int ny, int nz, cudaStream_t st)
+{
+    const uint64_t want = ((uint64_t)nx * ny * nz + 255) / 256;
+    transpose_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(s0, out, (uint32_t)nx, (uint32_t)ny, (uint32_t)nz);
+    return cudaGetLastError();
+}
+
+// a0, time weighting (R4; "interpolating ... in ... time"): for each of the m fused steps of
+// the coming launch, out[s][o] = F_s + a_s (F_s+1 - F_s), texel by texel.  Interpolation in space and
+// in time are both linear, so blending the texels first and sampling the blended field is the same
+// function as sampling both snapshots and blending the samples; it halves the bytes the step kernel
+// gathers (the L1 data pipe, not HBM or the ALUs, is what bounds that kernel) and its FMA count.
+// Streaming: reads the pair buffer once, writes m x 16 bytes per cell.
+struct BlendArgs {
+    const Texel2 *pair;
+    float4 *out;
+    uint64_t cells;
+    int32_t m;
+    float a[kBlendDepth];
+};
+
+__global__ void __launch_bounds__(256) blend_kernel(const __grid_constant__ BlendArgs B)
+{
+    for (uint64_t o = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; o < B.cells; o += (uint64_t)gridDim.x * blockDim.x) {
+        Texel2 t;
+        asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+            : "=f"(t.a.x), "=f"(t.a.y), "=f"(t.a.z), "=f"(t.a.w), "=f"(t.b.x), "=f"(t.b.y), "=f"(t.b.z), "=f"(t.b.w)
+            : "l"(B.pair + o));
+#pragma unroll 4
+        for (int s = 0; s < B.m; ++s) B.out[(uint64_t)s * B.cells + o] = lerp4(t.a, t.b, B.a[s]);
+    }
+}
+
+cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, cudaStream_t st)
+{
+    BlendArgs B;
+    B.pair = (const Texel2 *)pair; B.out = out; B.cells = cells; B.m = m;
+    for (int s = 0; s < kBlendDepth; ++s) B.a[s] = s < m ? a[s] : 0.0f;
+    const uint64_t want = (cells + 255) / 256;
+    blend_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(B);
     return cudaGetLastError();
 }
 

@@ -237,7 +237,7 @@ def test_T3_n_steps(lpm, orc, name, scale, stride, steps, nt, req):
 
 
 def test_fused_equals_unfused_bitwise(lpm):
-    """P14 determinism: the particle state is bit-identical for 1, 7 and 96 steps per launch."""
+    """P14 determinism: the particle state is bit-identical for 1, 7 and the default (16) steps per launch."""
     w = make("c3", scale=2e-3, n_steps=700).replace(nt=3)
     res = []
     for spl in (1, 7, 0):
@@ -248,7 +248,7 @@ def test_fused_equals_unfused_bitwise(lpm):
     for r in res[1:]:
         np.testing.assert_array_equal(res[0][0], r[0])
         np.testing.assert_array_equal(res[0][1], r[1])
-    assert res[0][2] > res[2][2] * 20
+    assert res[0][2] > res[2][2] * 5
 
 
 # ------------------------------------------------------------------ a8: binning fed identical positions
