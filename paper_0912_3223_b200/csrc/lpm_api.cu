@@ -113,6 +113,9 @@ struct lpm_handle {
     // gather-locality pass: the perm buffer lists slots [0, perm_n) of the (single) release as sorted at step perm_step
     uint64_t perm_n, perm_step;
     bool perm_valid;
+    // keys + histogram of slots [0, keys_n) left by the step launch that ended at step keys_step
+    uint64_t keys_n, keys_step;
+    bool keys_ready;
     double dep_bound[LPM_MAX_NUCLIDES];  // largest activity a particle can carry (fixed-point scale of the deposit tables)
     bool binned;
     int sms, occ;
@@ -596,24 +599,40 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                     for (int s = 0; s < m; ++s) units += (double)born_local(r, (int64_t)h->step + s);
                 A.perm = nullptr;
                 A.n_perm = 0;
+                A.keys_out = nullptr; A.hist_out = nullptr; A.n_keys = 0;
                 if (sort_enabled(&h->prm) && A.n_prev > 0 && (h->prm.gather_sort > 0 || A.n_prev >= kSortAutoMin)) {
                     // the list is kept for `period` model steps (one release: the perm buffer is its own);
                     // particles born since the last sort are walked in slot order behind it
                     uint32_t *perm = (uint32_t *)(h->ws + h->L.perm);
                     const bool single = h->rel.size() == 1;
                     const uint64_t period = h->prm.gather_sort > 0 ? (uint64_t)h->prm.gather_sort : (uint64_t)kSortPeriod;
+                    const uint32_t n_keys = (uint32_t)A.snap_cells + 1u;
+                    uint32_t *keys = (uint32_t *)(h->ws + h->L.keys), *hist = (uint32_t *)(h->ws + h->L.hist);
                     if (!single || !h->perm_valid || h->step - h->perm_step >= period || h->perm_n > A.n_prev) {
                         const int sspan = span_open(h, 2, (double)A.n_prev);
-                        CK(launch_sort_by_cell(A.xyzq + r.base, A.n_prev, A.mg, (uint32_t *)(h->ws + h->L.keys),
-                                               (uint32_t *)(h->ws + h->L.hist), (uint32_t *)(h->ws + h->L.partial), perm, h->st));
+                        if (single && h->keys_ready && h->keys_n == A.n_prev && h->keys_step == h->step) {
+                            CK(launch_sort_finish(keys, A.n_prev, n_keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->st));
+                            h->launches += 4;
+                        } else {
+                            CK(launch_sort_by_cell(A.xyzq + r.base, A.n_prev, A.mg, keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->st));
+                            h->launches += 5;
+                        }
                         span_close(h, sspan);
-                        h->launches += 5;
                         h->perm_n = A.n_prev;
                         h->perm_step = h->step;
                         h->perm_valid = single;
                     }
                     A.perm = perm;
                     A.n_perm = h->perm_n;
+                    // will the next launch sort?  then this one leaves the keys and the histogram
+                    h->keys_ready = false;
+                    if (single && h->step + (uint64_t)m - h->perm_step >= period) {
+                        CK(cudaMemsetAsync(hist, 0, 4ull * n_keys, h->st));
+                        A.keys_out = keys; A.hist_out = hist; A.n_keys = n_keys;
+                        h->keys_ready = true;
+                        h->keys_n = n;
+                        h->keys_step = h->step + (uint64_t)m;
+                    }
                 }
                 CK(cudaMemsetAsync(A.ctrl + 16, 0, 8, h->st));  // tile ticket of the slot kernel
                 const int span = span_open(h, 0, units);
@@ -766,6 +785,7 @@ int32_t lpm_set_particles(lpm_handle *h, const void *xyzq, const float *q1, cons
     h->step = step_index;
     h->binned = false;
     h->perm_valid = false;
+    h->keys_ready = false;
     if (n) {  // the installed activities bound the deposit increments from now on
         float *mx = (float *)(h->ws + h->L.air);
         float mq[2] = {0.f, 0.f};

@@ -10,7 +10,7 @@ namespace lpm {
 
 constexpr int kMaxFused = 16;        // model steps fused into one launch (table lives in kernel params)
 constexpr int kBlendDepth = kMaxFused;  // time-blended met buffers kept: one per fused step
-constexpr int kSortPeriod = 96;      // model steps between two gather-locality sorts of a release
+constexpr int kSortPeriod = 32;      // model steps between two gather-locality sorts of a release
 constexpr int kStepThreads = 256;    // CTA size of the step kernel
 constexpr int kScanTile = kStepThreads;  // particles per look-back tile (compaction)
 
@@ -76,6 +76,8 @@ struct StepArgs {
     uint64_t base, n, n_prev;  // slots >= n_prev are born inside this launch
     const uint32_t *perm;      // gather-locality pass: slots [0, n_perm) listed in dual-cell order, or null
     uint64_t n_perm;           // slots [n_perm, n) are walked in slot order
+    uint32_t *keys_out, *hist_out;  // non-null: the launch before a sort leaves each slot's dual-cell key and the histogram
+    uint32_t n_keys, pad1_;
     uint64_t pid_offset, pid_stride;
     uint64_t rel_N, rel_c;     // count mode: N (global count); rate mode: c slots per step
     int64_t rel_s_start, rel_S;
@@ -126,6 +128,8 @@ int step_max_blocks_per_sm(int K, bool compact, int dry_mode);
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
                                 uint32_t *perm, cudaStream_t st);
+cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, uint32_t *perm,
+                               cudaStream_t st);
 uint64_t sort_partial_entries(uint64_t n_cells);
 cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, cudaStream_t st);
 cudaError_t launch_transpose(const float4 *s0, float4 *out, int nx, int ny, int nz, cudaStream_t st);

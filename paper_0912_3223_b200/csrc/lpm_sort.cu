@@ -117,21 +117,32 @@ __global__ void __launch_bounds__(256) sort_scatter_kernel(const uint32_t *__res
     }
 }
 
-cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
-                                uint32_t *perm, cudaStream_t st)
+// passes 2 + 3 on keys and a histogram that are already there (written by sort_key_kernel, or by the
+// step kernel itself at the end of the launch that precedes a sort)
+cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, uint32_t *perm,
+                               cudaStream_t st)
 {
-    const uint32_t n_keys = (uint32_t)g.nx * g.ny * g.nz + 1u, m = n_keys;
-    cudaError_t e = cudaMemsetAsync(hist, 0, 4ull * m, st);
-    if (e != cudaSuccess) return e;
+    const uint32_t m = n_keys;
     const uint64_t want = (n + 255) / 256;
     const int blocks = (int)(want < 148 * 8 ? (want ? want : 1) : 148 * 8);
-    sort_key_kernel<<<blocks, 256, 0, st>>>(xyzq, n, g, n_keys, keys, hist);
     const uint32_t nb = (m + kScanBlock - 1) / kScanBlock;
     scan_totals_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
     scan_partials_kernel<<<1, 256, 0, st>>>(partial, nb);
     scan_apply_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
     sort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, hist, perm);
     return cudaGetLastError();
+}
+
+cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
+                                uint32_t *perm, cudaStream_t st)
+{
+    const uint32_t n_keys = (uint32_t)g.nx * g.ny * g.nz + 1u;
+    cudaError_t e = cudaMemsetAsync(hist, 0, 4ull * n_keys, st);
+    if (e != cudaSuccess) return e;
+    const uint64_t want = (n + 255) / 256;
+    const int blocks = (int)(want < 148 * 8 ? (want ? want : 1) : 148 * 8);
+    sort_key_kernel<<<blocks, 256, 0, st>>>(xyzq, n, g, n_keys, keys, hist);
+    return launch_sort_finish(keys, n, n_keys, hist, partial, perm, st);
 }
 
 uint64_t sort_partial_entries(uint64_t n_cells) { return (n_cells + 1 + kScanBlock - 1) / kScanBlock + 1; }

@@ -232,7 +232,7 @@ __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &ac
 // pid_offset + l * pid_stride, so ids (and birth steps, R9) are implied by the slot.  Persistent
 // grid-stride loop; up to kMaxFused model steps per launch.
 #ifndef LPM_STEP_MINB
-#define LPM_STEP_MINB 3
+#define LPM_STEP_MINB 4
 #endif
 static_assert(sizeof(StepArgs) <= 32764, "StepArgs must fit the kernel-parameter space (32764 B since CUDA 12.1 on sm_70+)");
 
@@ -270,6 +270,7 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             l = first_new + (uint64_t)(tile - t_old) * kStepThreads + threadIdx.x;
             valid = l < A.n;
         }
+        const bool in_range = valid;
         const uint64_t slot = A.base + l;
         const uint32_t pid = (uint32_t)(A.pid_offset + l * A.pid_stride);
         float x = 0.f, y = 0.f, z = 0.f, q[K];
@@ -303,6 +304,12 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             if (!alive) z = -1.0f - z;  // exit position kept, slot marked inactive
             A.xyzq[slot] = make_float4(x, y, z, q[0]);
             if (K > 1) A.q1[slot] = q[1];
+        }
+        if (A.keys_out && in_range) {
+            // pass 1 of the coming gather-locality sort, for free: the new position is in registers
+            const uint32_t key = (valid && z >= 0.0f) ? corner_of(A.mg, x, y, z).o : A.n_keys - 1u;
+            A.keys_out[l] = key;
+            atomicAdd(A.hist_out + key, 1u);
         }
         if (A.any_dep) {
             __syncthreads();
