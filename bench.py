@@ -43,9 +43,13 @@ if ROOT not in sys.path:
 METRIC = "particle_steps_per_s"
 UNIT = "particle-steps/s"
 # SURVEY.md §8(d) / DESIGN.md §6: algorithmic lane-operations per particle-step (FMA = 1), frozen
-# before any tuning: 250 with one met snapshot, 310 with on-the-fly time interpolation.
+# before any tuning: 250 with one met snapshot, 310 with time interpolation (the figure stays 310
+# although the kernel now samples a time-blended buffer: the budget is implementation-independent).
 LANE_OPS_STATIC, LANE_OPS_TIME = 250.0, 310.0
 SMS, LANES_PER_SM = 148, 128          # 4 SMSP x 32 lanes: one warp instruction per clock per SMSP
+LAUNCH_STEPS = 16                     # model steps fused per step-kernel launch (csrc kMaxFused)
+# dram__bytes_read.sum + dram__bytes_write.sum of one captured step-kernel launch, bytes (profiles/r01c_c4_step_kernel_ncu.md)
+NCU_TRAFFIC = {}
 ORACLE_STRIDE = {"c1": 1, "c2": 40, "c3": 400, "c3_hdep80": 400, "c4": 4000, "c5": 1}
 ORACLE_SCALE_C5 = 1.0e-3              # c5 cannot be pid-strided (capacity couples particles): 1/1000 scale
 
@@ -204,6 +208,16 @@ def run_ours(args):
     build()
     import paper_0912_3223_b200 as lpm
 
+    # measured denominators (lpm_probe micro-benchmarks, outside every timed region)
+    probes = {}
+    if rank == 0 and not args.no_probes:
+        for key, kind, fp in (("ffma_lane_ops_per_s", "ffma", 0), ("imad_lop_lane_ops_per_s", "imad_lop", 0),
+                              ("l1_gather_sectors_per_s", "gather", 64 << 10), ("l2_gather_sectors_per_s", "gather", 64 << 20),
+                              ("red_f64_l2_resident_per_s", "red_f64", 16 << 20), ("red_f64_600MB_per_s", "red_f64", 600 << 20),
+                              ("red_same_address_per_s", "red_same", 0), ("shared_atomic_per_s", "atoms", 0)):
+            probes[key] = lpm.probe(kind, fp, scratch_bytes=1 << 30 if fp > (1 << 28) else 1 << 28)
+        torch.cuda.empty_cache()
+
     w = make_workload(args.workload, args.scale, world, rank)
     interval = w.bin_every
     W, K = args.warmup, args.steps
@@ -338,19 +352,48 @@ def run_ours(args):
     achieved = lane_ops * (k_units / world) / n_launch / (avg_ms * 1e-3) / 1e12 if avg_ms > 0 else 0.0
     peak = SMS * LANES_PER_SM * pk["sm_max_mhz"] * 1e6 / 1e12
     state_bytes = 16 + 4 * (w.K - 1) + (4 if w.compact else 0)
+    k_rate = (k_units / world) / (step_ms * 1e-3) if step_ms > 0 else 0.0      # particle-steps/s inside the step kernel
+    fused = 1 if w.compact else LAUNCH_STEPS
+    hbm_per_ps = 2.0 * (state_bytes + (0 if w.compact else 4)) / fused          # state read + written once per launch (+ list entry)
     roofline = {
         "kernel": "step_compact_kernel" if w.compact else "step_slots_kernel", "bound": "alu",
         "achieved": achieved, "peak": peak, "unit": "Tlane-op/s", "frac": achieved / peak if peak else None,
-        "traffic": None,
+        # dram__bytes_read + dram__bytes_write of ONE captured launch (profiles/r01c_*): not per average launch
+        "traffic": NCU_TRAFFIC.get(args.workload),
         "lane_ops_per_particle_step": lane_ops, "avg_launch_ms": avg_ms, "launches": tim["step_launches"],
+        "kernel_particle_steps_per_s": k_rate,
         "share_of_step": step_ms / ms if ms else None,
-        "peak_source": f"{SMS} SMs x {LANES_PER_SM} lanes x {pk['sm_max_mhz']:.0f} MHz (clocks.max.sm, {pk['source']})",
-        "hbm_side": {"bytes_per_launch_per_particle": 2 * state_bytes, "hbm_peak_gbs": pk["hbm_gbs"], "peak_source": pk["source"]},
+        "peak_source": f"{SMS} SMs x {LANES_PER_SM} lanes x {pk['sm_max_mhz']:.0f} MHz (clocks.max.sm, {pk['source']}): one warp "
+                       "instruction per clock per SM sub-partition (DESIGN.md 6)",
+        "frac_of_measured_ffma": achieved * 1e12 / probes["ffma_lane_ops_per_s"] if probes.get("ffma_lane_ops_per_s") else None,
+        "hbm_side": {"bytes_per_particle_step": hbm_per_ps, "fused_steps_per_launch": fused, "hbm_peak_gbs": pk["hbm_gbs"],
+                     "peak_source": pk["source"], "frac": k_rate * hbm_per_ps / (pk["hbm_gbs"] * 1e9)},
+        # what ncu shows to be the binding unit (profiles/r01c_*): the L1 data pipe, one 32-byte sector per gathered
+        # texel; achieved = gathers issued per second against the probe's L1-resident gather rate
+        "l1_gather_side": {"gathers_per_particle_step": 8, "achieved_per_s": 8.0 * k_rate,
+                           "peak_per_s": probes.get("l1_gather_sectors_per_s"),
+                           "frac": 8.0 * k_rate / probes["l1_gather_sectors_per_s"] if probes.get("l1_gather_sectors_per_s") else None,
+                           "note": "upper bound of the sector count: lanes that share a texel share a sector"},
     }
-    bin_bytes = (12 + 4 * w.K) * (b_units / world)
+    bpp = 12 + 4 * w.K
+    n_bin = b_units / world
+    bin_bytes = bpp * n_bin
+    grid_bytes = (4 + 8 * w.K) * g.nx * g.ny * g.nz
+    red_rate = probes.get("red_f64_l2_resident_per_s")
+    t_hbm = (bin_bytes + tim["bin_launches"] * grid_bytes) / (pk["hbm_gbs"] * 1e9)      # particles read + grids zeroed
+    t_atom = (1 + w.K) * n_bin / red_rate if red_rate else None                          # one count + K sums per particle
+    t_roof = max(t_hbm, t_atom) if t_atom else t_hbm
     binning = {"kernel": "bin_kernel", "gbs": bin_bytes / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else None,
                "avg_ms": bin_ms / max(tim["bin_launches"], 1), "launches": tim["bin_launches"],
-               "bytes_per_particle": 12 + 4 * w.K, "note": "span includes the memsets of the count and sum grids"}
+               "bytes_per_particle": bpp, "particles": n_bin,
+               "roofline": {"bound": "atomic" if t_atom and t_atom >= t_hbm else "hbm", "roof_ms": t_roof * 1e3, "measured_ms": bin_ms,
+                            "frac": t_roof * 1e3 / bin_ms if bin_ms > 0 else None,
+                            "hbm_ms": t_hbm * 1e3, "atomic_ms": t_atom * 1e3 if t_atom else None,
+                            "atomics_per_particle": 1 + w.K,
+                            "atomic_peak_per_s": red_rate, "atomic_peak_source": "lpm_probe red.global.add.f64, random addresses, "
+                            "L2-resident 16 MB footprint (the plume's cells are L2-resident; over the full grid footprint the "
+                            "random-address rate is red_f64_600MB_per_s)"},
+               "note": "span = memsets of the count and sum grids + bin kernel"}
 
     # ---------------- cpu baseline (oracle, bounded sample) ----------------
     cpu = None
@@ -372,7 +415,7 @@ def run_ours(args):
         "e2e": {"value": units / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                 "ms_per_step": ms_e2e / K, "sim_hours_per_s": sim_hours / (ms_e2e * 1e-3)},
         "gpu_launches": launches,
-        "roofline": roofline, "binning": binning, "cpu_baseline": cpu, "clocks": clocks,
+        "roofline": roofline, "binning": binning, "measured_peaks": probes, "cpu_baseline": cpu, "clocks": clocks,
         "check": {"conc_sum_resident": total_mass, "conc_sum_e2e": e2e_mass},
     }
     print(json.dumps(line))
@@ -411,6 +454,7 @@ def main():
     ap.add_argument("--workload", default="c4", choices=("c1", "c2", "c3", "c3_hdep80", "c4", "c5"))
     ap.add_argument("--scale", type=float, default=1.0, help="particle-count scale of the workload (1.0 = BASELINE size)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-probes", action="store_true", help="skip the lpm_probe micro-benchmarks (measured peaks)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print(f"note: --warmup {args.warmup} < 3; timing rules ask for at least 3", file=sys.stderr)

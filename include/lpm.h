@@ -16,9 +16,9 @@
  *    pointers; small structs are host structs copied at the call.
  *  - OWNERSHIP: the caller owns every device buffer (workspace, met snapshots, outputs).  The
  *    library borrows `workspace_dev` and `meteo.fields_dev` for the life of the handle and never
- *    frees caller memory.  The library keeps a re-packed copy of the two snapshots of the current
- *    met interval: snapshot data must be in place before the first step of the interval that uses
- *    it, and later changes must go through lpm_upload_meteo (which invalidates the copy).
+ *    frees caller memory.  The library keeps re-packed, time-blended copies of the two snapshots of
+ *    the current met interval: snapshot data must be in place before the first step of the interval
+ *    that uses it, and later changes must go through lpm_upload_meteo (which invalidates the copies).
  *  - One handle = one GPU = one CUDA stream.  Calls enqueue work on that stream and return; calls
  *    that return host scalars (lpm_num_active, lpm_ledger, lpm_get_particles' count) synchronise
  *    the stream first.  A handle is not thread-safe.
@@ -83,11 +83,12 @@ typedef struct {
     int32_t compact;        /* 1: stable stream compaction of exited particles after every step */
     double h_dep;           /* dry deposition acts where z' < h_dep; h_dep >= H_mix: everywhere */
     int32_t bin_every;      /* concentration binning cadence in steps ("n"); 0 = never   */
-    int32_t steps_per_launch; /* 0 = auto; 1 = one model step per kernel launch; m > 1 fuses up to
-                               * m steps per launch with the particle state kept in registers   */
-    int32_t gather_sort;      /* gather-locality pass before a fused launch (slots listed in met-cell
-                               * order): 0 = auto (on from 65536 particles), 1 = always, -1 = never.
-                               * Results per particle do not depend on it.                        */
+    int32_t steps_per_launch; /* 0 = auto (16); 1 = one model step per kernel launch; m > 1 fuses up to
+                               * min(m, 16) steps per launch with the particle state in registers */
+    int32_t gather_sort;      /* gather-locality pass (slots listed in the order of the lower-corner met
+                               * cell of their trilinear stencil): 0 = auto (from 65536 particles, every
+                               * 32 steps), p > 0 = always, every p model steps (1 = before every launch),
+                               * -1 = never.  Results per particle do not depend on it.            */
     int32_t reserved;
 } lpm_params;
 
@@ -108,8 +109,9 @@ int32_t lpm_version(void);
 const char *lpm_status_string(int32_t status);
 
 /* Bytes of device workspace lpm_create needs (particle SoA store, grids, ledger, scan state,
- * read-out staging and, when meteo->nt > 1, the interleaved snapshot-pair buffer of the current
- * met interval: 32 bytes per met cell).  Only the grid and nt of `meteo` are read. */
+ * read-out staging, the z-fastest time-blended met buffers (16 bytes per met cell and fused step) and,
+ * when meteo->nt > 1, the interleaved snapshot-pair buffer of the current met interval: 32 bytes per
+ * met cell).  Only the grid and nt of `meteo` are read. */
 int32_t lpm_workspace_bytes(const lpm_grid *conc_grid, const lpm_meteo *meteo, const lpm_params *params,
                             int32_t n_nuclides, uint64_t *bytes_host);
 
@@ -222,6 +224,28 @@ int32_t lpm_set_timing(lpm_handle *h, int32_t enable);
  * passes, [7] = their count; accumulated since lpm_set_timing. */
 int32_t lpm_get_timing(lpm_handle *h, double *out_host /* [8] */);
 
+/* ---- micro-benchmarks: measured denominators of the rooflines ------------------ */
+
+/* Time one micro-benchmark with CUDA events on `cuda_stream` (after two warm-up launches, `reps`
+ * timed launches) and return operations per second in *ops_per_s_host.  `scratch_dev` is a caller
+ * buffer of scratch_bytes (contents are overwritten); footprint_bytes <= scratch_bytes is the
+ * address range the memory probes spread over.  kind:
+ *   LPM_PROBE_FFMA      fp32 FMA lane-operations / s (8 independent chains per thread)
+ *   LPM_PROBE_IMAD_LOP  Philox round mix, IMAD.WIDE.U32 + LOP3, lane-operations / s
+ *   LPM_PROBE_RED_F64   random-address red.global.add.f64 over the footprint, atomics / s
+ *   LPM_PROBE_RED_U32   random-address red.global.add.u32 over the footprint, atomics / s
+ *   LPM_PROBE_RED_SAME  every thread adds to ONE double (hottest-cell service rate), atomics / s
+ *   LPM_PROBE_ATOMS     conflict-free shared-memory atomicAdd (u32), atomics / s
+ *   LPM_PROBE_GATHER    16-byte loads, each lane its own 32-byte sector of an L1-resident window of
+ *                       footprint_bytes: L1 sectors / s (the met gather of a decorrelated warp)
+ * Errors: INVALID_ARG (null, unknown kind, scratch < 1 MiB), NO_DEVICE, CUDA. */
+typedef enum {
+    LPM_PROBE_FFMA = 0, LPM_PROBE_IMAD_LOP = 1, LPM_PROBE_RED_F64 = 2, LPM_PROBE_RED_U32 = 3,
+    LPM_PROBE_RED_SAME = 4, LPM_PROBE_ATOMS = 5, LPM_PROBE_GATHER = 6
+} lpm_probe_kind;
+int32_t lpm_probe(int32_t kind, uint64_t footprint_bytes, void *scratch_dev, uint64_t scratch_bytes, int32_t reps,
+                  double *ops_per_s_host, void *cuda_stream);
+
 /* ---- stand-alone kernels for parity tests (device arrays in, device arrays out) ------------ */
 
 /* Philox4x32-10 (R1): out_dev[4*i..] = philox(key = seed, ctr = (step, stream, pid_lo, pid_hi))
@@ -231,6 +255,9 @@ int32_t lpm_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t 
 /* The three N(0,1) of R3 for the same counters: out_dev[3*i..]. */
 int32_t lpm_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, float *out_dev,
                          void *cuda_stream);
+/* R2 + R3 on given raw words: out_dev[3*i..] = the three N(0,1) Box-Muller makes of the four 32-bit
+ * words r_dev[4*i..] (so a test can sweep all 2^24 uniforms the step can ever see). */
+int32_t lpm_test_box_muller(const uint32_t *r_dev, uint64_t n, float *out_dev, void *cuda_stream);
 /* Met sampling R4 at n points: xyz_dev float4 (w ignored), out_dev float4 (u, v, w, Kz). */
 int32_t lpm_test_sample(const lpm_meteo *meteo, double t, const void *xyz_dev, uint64_t n,
                         void *out_dev, void *cuda_stream);

@@ -27,7 +27,7 @@ SYMBOLS = (
     "lpm_deposition_f64", "lpm_bin_now", "lpm_num_active", "lpm_step_index", "lpm_mass_scale", "lpm_get_particles",
     "lpm_set_particles", "lpm_ledger", "lpm_injected", "lpm_last_error", "lpm_launch_count", "lpm_test_philox",
     "lpm_test_normals", "lpm_test_sample", "lpm_upload_meteo", "lpm_concentration_host", "lpm_deposition_host",
-    "lpm_set_timing", "lpm_get_timing",
+    "lpm_set_timing", "lpm_get_timing", "lpm_probe", "lpm_test_box_muller",
 )
 
 
@@ -106,6 +106,8 @@ def load():
     L.lpm_deposition_host.argtypes = [vp, vp]
     L.lpm_set_timing.argtypes = [vp, i32]
     L.lpm_get_timing.argtypes = [vp, C.POINTER(dbl)]
+    L.lpm_probe.argtypes = [i32, u64, vp, u64, i32, C.POINTER(dbl), vp]
+    L.lpm_test_box_muller.argtypes = [vp, u64, vp, vp]
     L.lpm_test_philox.argtypes = [u64, u64, C.c_uint32, u64, u64, vp, vp]
     L.lpm_test_normals.argtypes = [u64, u64, u64, u64, vp, vp]
     L.lpm_test_sample.argtypes = [C.POINTER(lpm_meteo), dbl, vp, u64, vp, vp]
@@ -348,6 +350,22 @@ class Simulation:
         self.torch.cuda.current_stream().synchronize()
 
 
+# ---------------------------------------------------------------- micro-benchmarks
+PROBE_KINDS = {"ffma": 0, "imad_lop": 1, "red_f64": 2, "red_u32": 3, "red_same": 4, "atoms": 5, "gather": 6}
+
+
+def probe(kind: str, footprint_bytes: int = 0, scratch_bytes: int = 1 << 28, reps: int = 5) -> float:
+    """lpm_probe: operations per second of one micro-benchmark (see include/lpm.h)."""
+    torch = _require_cuda()
+    scratch = torch.zeros(scratch_bytes // 4, dtype=torch.float32, device="cuda")
+    out = C.c_double()
+    rc = load().lpm_probe(PROBE_KINDS[kind], footprint_bytes, scratch.data_ptr(), scratch_bytes, reps, C.byref(out),
+                          torch.cuda.current_stream().cuda_stream)
+    if rc:
+        raise LpmError(rc, "lpm_probe")
+    return out.value
+
+
 # ---------------------------------------------------------------- stand-alone parity kernels
 def philox_kernel(seed, step, stream_id, pid0, n):
     torch = _require_cuda()
@@ -356,6 +374,17 @@ def philox_kernel(seed, step, stream_id, pid0, n):
     if rc:
         raise LpmError(rc, "lpm_test_philox")
     return out.cpu().numpy().view(np.uint32)
+
+
+def box_muller_kernel(words):
+    """normals of raw Philox words: words uint32 [n][4] (numpy) -> float32 [n][3]."""
+    torch = _require_cuda()
+    r = torch.from_numpy(np.ascontiguousarray(words, dtype=np.uint32).view(np.int32)).cuda()
+    out = torch.empty((r.shape[0], 3), dtype=torch.float32, device="cuda")
+    rc = load().lpm_test_box_muller(r.data_ptr(), r.shape[0], out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    if rc:
+        raise LpmError(rc, "lpm_test_box_muller")
+    return out.cpu().numpy()
 
 
 def normals_kernel(seed, step, pid0, n):

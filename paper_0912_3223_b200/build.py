@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblpm_b200.so")
-SOURCES = ("lpm_api.cu", "lpm_step.cu", "lpm_bin.cu", "lpm_sort.cu")
+SOURCES = ("lpm_api.cu", "lpm_step.cu", "lpm_bin.cu", "lpm_sort.cu", "lpm_probe.cu")
 HEADERS = ("lpm_internal.h", "lpm_device.cuh", os.path.join("..", "..", "include", "lpm.h"))
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]

@@ -939,6 +939,16 @@ static int dev_ok()
     return cudaGetDeviceCount(&ndev) == cudaSuccess && ndev > 0;
 }
 
+int32_t lpm_probe(int32_t kind, uint64_t footprint, void *scratch, uint64_t scratch_bytes, int32_t reps, double *ops, void *st)
+{
+    if (!scratch || !ops || kind < 0 || kind > LPM_PROBE_GATHER || scratch_bytes < (1u << 20) || reps < 1 || ((uintptr_t)scratch & 15))
+        return LPM_ERR_INVALID_ARG;
+    if (!dev_ok()) return LPM_ERR_NO_DEVICE;
+    if (footprint == 0 || footprint > scratch_bytes) footprint = scratch_bytes;
+    if (kind == LPM_PROBE_GATHER && footprint > scratch_bytes - 64) footprint = scratch_bytes - 64;
+    return run_probe(kind, footprint, scratch, scratch_bytes, reps, ops, (cudaStream_t)st) == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
+}
+
 int32_t lpm_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out, void *st)
 {
     if (!out) return LPM_ERR_INVALID_ARG;
@@ -951,6 +961,13 @@ int32_t lpm_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n
     if (!out) return LPM_ERR_INVALID_ARG;
     if (!dev_ok()) return LPM_ERR_NO_DEVICE;
     return launch_test_normals(seed, step, pid0, n, out, (cudaStream_t)st) == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
+}
+
+int32_t lpm_test_box_muller(const uint32_t *r, uint64_t n, float *out, void *st)
+{
+    if (!r || !out || ((uintptr_t)r & 15)) return LPM_ERR_INVALID_ARG;
+    if (!dev_ok()) return LPM_ERR_NO_DEVICE;
+    return launch_test_box_muller(r, n, out, (cudaStream_t)st) == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
 }
 
 int32_t lpm_test_sample(const lpm_meteo *met, double t, const void *xyz, uint64_t n, void *out, void *st)

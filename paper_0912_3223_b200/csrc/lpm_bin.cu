@@ -228,6 +228,21 @@ cudaError_t launch_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uin
     return cudaGetLastError();
 }
 
+__global__ void test_box_muller_kernel(const uint4 *__restrict__ r, uint64_t n, float *out)
+{
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+        float n0, n1, n2;
+        normals3(r[i], n0, n1, n2);
+        out[3 * i] = n0; out[3 * i + 1] = n1; out[3 * i + 2] = n2;
+    }
+}
+
+cudaError_t launch_test_box_muller(const uint32_t *r, uint64_t n, float *out, cudaStream_t st)
+{
+    test_box_muller_kernel<<<148 * 8, 256, 0, st>>>((const uint4 *)r, n, out);
+    return cudaGetLastError();
+}
+
 __global__ void test_sample_kernel(const float4 *blend, GridF mg, float kz_min, const float4 *xyz, uint64_t n, float4 *out)
 {
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {

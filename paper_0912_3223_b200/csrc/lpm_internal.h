@@ -131,6 +131,8 @@ cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_
 cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, uint32_t *perm,
                                cudaStream_t st);
 uint64_t sort_partial_entries(uint64_t n_cells);
+cudaError_t run_probe(int kind, uint64_t footprint_bytes, void *scratch_dev, uint64_t scratch_bytes, int reps, double *ops,
+                      cudaStream_t st);
 cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, cudaStream_t st);
 cudaError_t launch_transpose(const float4 *s0, float4 *out, int nx, int ny, int nz, cudaStream_t st);
 cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, cudaStream_t st);
@@ -143,6 +145,7 @@ cudaError_t launch_import(float4 *xyzq, uint64_t n, const uint8_t *status, cudaS
 cudaError_t launch_iota(uint32_t *pid, uint64_t n, cudaStream_t st);
 cudaError_t launch_qmax(const float4 *xyzq, const float *q1, uint64_t n, int K, float *out2, cudaStream_t st);
 cudaError_t launch_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st);
+cudaError_t launch_test_box_muller(const uint32_t *r, uint64_t n, float *out, cudaStream_t st);
 cudaError_t launch_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, float *out, cudaStream_t st);
 cudaError_t launch_test_sample(const float4 *blend, GridF mg, float kz_min, const float4 *xyz, uint64_t n, float4 *out,
                                cudaStream_t st);

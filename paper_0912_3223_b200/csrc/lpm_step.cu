@@ -163,11 +163,12 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
     if (DRY != kDryLayer && !raining) {
 #pragma unroll
         for (int k = 0; k < K; ++k) acc.both[k] = fmaf(q[k], e.Gf[k], acc.both[k]);
-        if (DRY == kDryNone) return true;
-        float vd[K];
+        if constexpr (DRY != kDryNone) {
+            float vd[K];
 #pragma unroll
-        for (int k = 0; k < K; ++k) vd[k] = q[k] * e.Gps[k];
-        deposit_at<K, false>(A, x, y, vd, vd, acc, dep);
+            for (int k = 0; k < K; ++k) vd[k] = q[k] * e.Gps[k];
+            deposit_at<K, false>(A, x, y, vd, vd, acc, dep);
+        }
         return true;
     }
     const bool dry_here = DRY == kDryUniform || (DRY == kDryLayer && z < A.h_dep);

@@ -54,6 +54,36 @@ def test_normals_match_oracle(lpm, orc):
     assert np.abs(got).max() <= math.sqrt(48 * math.log(2)) * (1 + 1e-6)
 
 
+def test_box_muller_exhaustive(lpm):
+    """R2 + R3 over ALL 2^24 uniforms the step can see, against the definition in fp64: the kernel's own
+    log / sqrt / sincospi (csrc/lpm_device.cuh) must hold |err| <= 3e-7 |n| + 1.5e-7 everywhere."""
+    k = np.arange(1 << 24, dtype=np.uint64)
+    two_pi = 2.0 * np.pi
+    # sweep 1: every u1 = (k+1) 2^-24 with u2 = 0 (n0 = R1, n1 = 0); every u3 with u4 = 0 (n2 = R2)
+    w = np.zeros((1 << 24, 4), dtype=np.uint32)
+    w[:, 0] = (k << 8).astype(np.uint32)
+    w[:, 2] = ((k[::-1]) << 8).astype(np.uint32)
+    got = lpm.box_muller_kernel(w).astype(np.float64)
+    R = np.sqrt(-2.0 * np.log((k + 1.0) * 2.0 ** -24))
+    for col, want in ((0, R), (2, R[::-1])):
+        err = np.abs(got[:, col] - want)
+        assert np.all(err <= 3e-7 * want + 1.5e-7), (col, err.max(), int(np.argmax(err - 3e-7 * want)))
+    assert np.all(got[:, 1] == 0.0) and got[-1, 0] == 0.0          # u1 = 1 -> R = 0 exactly
+    # sweep 2: every u2 = k 2^-24 (and u4) at R close to 1: r0 chosen so that u1 ~ exp(-1/2)
+    u1k = int(round(np.exp(-0.5) * 2 ** 24)) - 1
+    w = np.zeros((1 << 24, 4), dtype=np.uint32)
+    w[:, 0] = np.uint32(u1k << 8)
+    w[:, 2] = np.uint32(u1k << 8)
+    w[:, 1] = (k << 8).astype(np.uint32)
+    w[:, 3] = (k << 8).astype(np.uint32)
+    got = lpm.box_muller_kernel(w).astype(np.float64)
+    R1 = np.sqrt(-2.0 * np.log((u1k + 1.0) * 2.0 ** -24))
+    th = two_pi * k * 2.0 ** -24
+    for col, want in ((0, R1 * np.cos(th)), (1, R1 * np.sin(th)), (2, R1 * np.cos(th))):
+        err = np.abs(got[:, col] - want)
+        assert np.all(err <= 3e-7 * np.abs(want) + 1.5e-7), (col, err.max())
+
+
 # ------------------------------------------------------------------ a0 + a2: met sampling
 @pytest.mark.parametrize("name,t", [("c2", 0.0), ("c2", 4321.0), ("c3", 5 * 3600.0 + 1234.0), ("c1", 10.0)])
 def test_met_sampling(lpm, orc, name, t):
