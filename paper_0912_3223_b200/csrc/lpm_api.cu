@@ -51,7 +51,7 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     L.stage = o; o += up(4 * cells3 * K);  // fp32 read-out staging for the *_host entry points
     L.pair = o; o += met.nt > 1 ? up(32ull * met.grid.nx * met.grid.ny * met.grid.nz) : 0;  // (F_s, F_s+1) per met cell
     const uint64_t mcells = (uint64_t)met.grid.nx * met.grid.ny * met.grid.nz;
-    L.blend = o; o += up(16ull * mcells * (met.nt > 1 ? kBlendDepth : 1));  // z-fastest F(t_n), one buffer per fused step
+    L.blend = o; o += up(16ull * mcells * (met.nt > 1 ? kBlendDepth : 1) + 16);  // z-fastest F(t_n), one buffer per fused step (+ 1 pad texel)
     L.keys = o; o += sort ? up(4 * cap) : 0;            // gather-locality pass: met-cell key per slot
     L.perm = o; o += sort ? up(4 * cap) : 0;            //   slots in met-cell order
     L.hist = o; o += sort ? up(4 * (mcells + 1)) : 0;   //   per-cell counts / offsets
@@ -990,7 +990,8 @@ int32_t lpm_test_sample(const lpm_meteo *met, double t, const void *xyz, uint64_
     // the same path as lpm_step: z-fastest (pair ->) blended buffer, then the step kernel's sampling
     void *pair = nullptr;
     float4 *blend = nullptr;
-    if (cudaMalloc((void **)&blend, 16 * cells) != cudaSuccess) return LPM_ERR_CUDA;
+    if (cudaMalloc((void **)&blend, 16 * cells + 16) != cudaSuccess) return LPM_ERR_CUDA;
+    cudaMemsetAsync(blend + cells, 0, 16, s);  // pad texel (read with weight 0 when nz = 1)
     cudaError_t rc;
     if (met->nt > 1) {
         if (cudaMalloc(&pair, 32 * cells) != cudaSuccess) { cudaFree(blend); return LPM_ERR_CUDA; }
