@@ -80,7 +80,8 @@ typedef struct {
     uint64_t seed;          /* Philox key (R1)                                                  */
     uint64_t capacity;      /* maximum number of particle slots                        */
     int32_t boundary_mode;  /* lpm_boundary_mode; the boundary is the met-grid box (R7)         */
-    int32_t compact;        /* 1: stable stream compaction of exited particles after every step */
+    int32_t compact;        /* 1: stream compaction of exited particles after every step, stable with
+                             * respect to the storage order (= id order unless gather_sort reorders) */
     double h_dep;           /* dry deposition acts where z' < h_dep; h_dep >= H_mix: everywhere */
     int32_t bin_every;      /* concentration binning cadence in steps ("n"); 0 = never   */
     int32_t steps_per_launch; /* 0 = auto (16); 1 = one model step per kernel launch; m > 1 fuses up to
@@ -88,7 +89,9 @@ typedef struct {
     int32_t gather_sort;      /* gather-locality pass (slots listed in the order of the lower-corner met
                                * cell of their trilinear stencil): 0 = auto (from 65536 particles, every
                                * 32 steps), p > 0 = always, every p model steps (1 = before every launch),
-                               * -1 = never.  Results per particle do not depend on it.            */
+                               * -1 = never.  Results per particle do not depend on it.  With compact = 1
+                               * the records themselves are sorted (the id travels with the particle), so
+                               * the store is then in met-cell order, not in id order.             */
     int32_t reserved;
 } lpm_params;
 

@@ -130,8 +130,8 @@ def _grid(g) -> lpm_grid:
     return lpm_grid(g.nx, g.ny, g.nz, 0, g.x0, g.y0, g.z0, g.dx, g.dy, g.dz)
 
 
-def workspace_bytes(cgrid, capacity: int, n_nuclides: int, compact: bool, mgrid=None, nt: int = 1) -> int:
-    p = lpm_params(dt=1.0, capacity=capacity, compact=1 if compact else 0, h_dep=1.0)
+def workspace_bytes(cgrid, capacity: int, n_nuclides: int, compact: bool, mgrid=None, nt: int = 1, gather_sort: int = 0) -> int:
+    p = lpm_params(dt=1.0, capacity=capacity, compact=1 if compact else 0, h_dep=1.0, gather_sort=gather_sort)
     out = C.c_uint64()
     g = _grid(cgrid)
     met = lpm_meteo(grid=_grid(mgrid if mgrid is not None else cgrid), nt=nt)
@@ -179,7 +179,7 @@ class Simulation:
             fields_dev = torch.from_numpy(np.ascontiguousarray(f)).to(self.device)
         assert fields_dev.dtype == torch.float32 and fields_dev.is_contiguous()
         self.fields_dev = fields_dev
-        nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact, w.mgrid, w.nt)
+        nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact, w.mgrid, w.nt, gather_sort)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         cg = _grid(w.cgrid)
         met = lpm_meteo(grid=_grid(w.mgrid), nt=w.nt, t0=w.t0, dt_snap=w.dt_snap, fields_dev=fields_dev.data_ptr(),

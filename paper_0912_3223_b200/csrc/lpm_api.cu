@@ -27,7 +27,7 @@ struct Release {
 };
 
 struct Layout {
-    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, blend, keys, perm, hist, partial, total;
+    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, blend, keys, perm, hist, partial, alt_xyzq, alt_q1, alt_pid, total;
 };
 
 uint64_t up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
@@ -53,9 +53,12 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     const uint64_t mcells = (uint64_t)met.grid.nx * met.grid.ny * met.grid.nz;
     L.blend = o; o += up(16ull * mcells * (met.nt > 1 ? kBlendDepth : 1) + 16);  // z-fastest F(t_n), one buffer per fused step (+ 1 pad texel)
     L.keys = o; o += sort ? up(4 * cap) : 0;            // gather-locality pass: met-cell key per slot
-    L.perm = o; o += sort ? up(4 * cap) : 0;            //   slots in met-cell order
+    L.perm = o; o += sort && !compact ? up(4 * cap) : 0;  //   slots in met-cell order (slot-addressed store)
     L.hist = o; o += sort ? up(4 * (mcells + 1)) : 0;   //   per-cell counts / offsets
     L.partial = o; o += sort ? up(4 * sort_partial_entries(mcells)) : 0;
+    L.alt_xyzq = o; o += sort && compact ? up(16 * cap) : 0;           //   compact store: the records themselves are sorted,
+    L.alt_q1 = o; o += sort && compact && K > 1 ? up(4 * cap) : 0;     //   through these alternate buffers
+    L.alt_pid = o; o += sort && compact ? up(4 * cap) : 0;
     L.total = o;
     return L;
 }
@@ -76,9 +79,14 @@ GridF gridf(const lpm_grid &g, bool zfast = false)
     return f;
 }
 
-// the gather-locality pass applies to the slot-addressed store (compact mode keeps id order)
-bool sort_enabled(const lpm_params *p) { return p->gather_sort >= 0 && !p->compact; }
+// the gather-locality pass: a list of slot indices for the slot-addressed store, a physical sort of the
+// records for the compact store (from 65536 slots of capacity, or when asked for)
 constexpr uint64_t kSortAutoMin = 65536;
+bool sort_enabled(const lpm_params *p)
+{
+    if (p->compact) return p->gather_sort > 0 || (p->gather_sort == 0 && p->capacity >= kSortAutoMin);
+    return p->gather_sort >= 0;
+}
 
 bool grid_ok(const lpm_grid *g)
 {
@@ -116,6 +124,7 @@ struct lpm_handle {
     // keys + histogram of slots [0, keys_n) left by the step launch that ended at step keys_step
     uint64_t keys_n, keys_step;
     bool keys_ready;
+    uint64_t csort_step;  // compact store: step of the last physical sort
     double dep_bound[LPM_MAX_NUCLIDES];  // largest activity a particle can carry (fixed-point scale of the deposit tables)
     bool binned;
     int sms, occ;
@@ -577,6 +586,19 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                 sp.sx = (float)r.src.x; sp.sy = (float)r.src.y; sp.sz = (float)r.src.z;
                 for (int k = 0; k < h->K; ++k) sp.q[k] = (float)(r.emit[k] / A.tab[0].G[k]);
             }
+            if (sort_enabled(&h->prm)) {
+                const uint64_t period = h->prm.gather_sort > 0 ? (uint64_t)h->prm.gather_sort : (uint64_t)kSortPeriod;
+                if (h->step - h->csort_step >= period) {
+                    const int sspan = span_open(h, 2, 0.0);
+                    CK(launch_sort_records(A.xyzq, A.q1, A.pid, A.ctrl + 2, h->prm.capacity, A.mg, (uint32_t *)(h->ws + h->L.keys),
+                                           (uint32_t *)(h->ws + h->L.hist), (uint32_t *)(h->ws + h->L.partial),
+                                           (float4 *)(h->ws + h->L.alt_xyzq), h->K > 1 ? (float *)(h->ws + h->L.alt_q1) : nullptr,
+                                           (uint32_t *)(h->ws + h->L.alt_pid), h->st));
+                    span_close(h, sspan);
+                    h->launches += 6;
+                    h->csort_step = h->step;
+                }
+            }
             CK(launch_inject(I, h->st));
             const int span = span_open(h, 0, 0.0);
             CK(launch_step(A, h->K, true, h->sms * (h->occ > 0 ? h->occ : 1), h->st));
@@ -786,6 +808,7 @@ int32_t lpm_set_particles(lpm_handle *h, const void *xyzq, const float *q1, cons
     h->binned = false;
     h->perm_valid = false;
     h->keys_ready = false;
+    h->csort_step = step_index;
     if (n) {  // the installed activities bound the deposit increments from now on
         float *mx = (float *)(h->ws + h->L.air);
         float mq[2] = {0.f, 0.f};

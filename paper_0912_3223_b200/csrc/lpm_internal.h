@@ -130,6 +130,8 @@ cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_
                                 uint32_t *perm, cudaStream_t st);
 cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, uint32_t *perm,
                                cudaStream_t st);
+cudaError_t launch_sort_records(float4 *xyzq, float *q1, uint32_t *pid, const uint64_t *n_dev, uint64_t capacity, GridF g, uint32_t *keys,
+                                uint32_t *hist, uint32_t *partial, float4 *xyzq_alt, float *q1_alt, uint32_t *pid_alt, cudaStream_t st);
 uint64_t sort_partial_entries(uint64_t n_cells);
 cudaError_t run_probe(int kind, uint64_t footprint_bytes, void *scratch_dev, uint64_t scratch_bytes, int reps, double *ops,
                       cudaStream_t st);

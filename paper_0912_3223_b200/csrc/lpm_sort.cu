@@ -22,8 +22,10 @@ constexpr int kScanBlock = 256 * kScanItems;         // items per block
 // sector per cycle; with keys by containing cell a warp still spans the 8 octants = up to 8 lower
 // corners).  Exited slots go to the last bucket, n_keys - 1.
 __global__ void __launch_bounds__(256) sort_key_kernel(const float4 *__restrict__ xyzq, uint64_t n, GridF g, uint32_t n_keys,
-                                                       uint32_t *__restrict__ keys, uint32_t *__restrict__ hist)
+                                                       uint32_t *__restrict__ keys, uint32_t *__restrict__ hist,
+                                                       const uint64_t *__restrict__ n_dev = nullptr)
 {
+    if (n_dev) n = *n_dev;
     for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n; l += (uint64_t)gridDim.x * blockDim.x) {
         const float4 p = xyzq[l];
         uint32_t key = n_keys - 1;
@@ -115,6 +117,69 @@ __global__ void __launch_bounds__(256) sort_scatter_kernel(const uint32_t *__res
         base = __shfl_sync(0xffffffffu, base, leader);
         if (live) perm[base + __popc(peers & ((1u << lane) - 1u))] = (uint32_t)l;
     }
+}
+
+// pass 3, compact mode: move the RECORDS (position, activities, id) instead of listing indices: the
+// store itself ends up in dual-cell order (the id travels with the particle there), so the step
+// kernel streams it coalesced and consecutive tiles are spatial neighbours.  Order inside a key is
+// whatever the atomics give; per-particle results do not depend on storage order (Philox is keyed
+// by the id).
+__global__ void __launch_bounds__(256) sort_scatter_records_kernel(const uint32_t *__restrict__ keys, const uint64_t *__restrict__ n_dev,
+                                                                   uint32_t *__restrict__ offs, const float4 *__restrict__ xyzq,
+                                                                   const float *__restrict__ q1, const uint32_t *__restrict__ pid,
+                                                                   float4 *__restrict__ xyzq_o, float *__restrict__ q1_o,
+                                                                   uint32_t *__restrict__ pid_o)
+{
+    const uint64_t n = *n_dev;
+    const uint64_t n_round = (n + 31) & ~(uint64_t)31;
+    const int lane = threadIdx.x & 31;
+    for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n_round; l += (uint64_t)gridDim.x * blockDim.x) {
+        const bool live = l < n;
+        const uint32_t key = live ? keys[l] : 0xffffffffu;
+        const uint32_t peers = __match_any_sync(0xffffffffu, key);
+        const int leader = __ffs(peers) - 1;
+        uint32_t base = 0;
+        if (live && lane == leader) base = atomicAdd(offs + key, (uint32_t)__popc(peers));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (live) {
+            const uint32_t d = base + __popc(peers & ((1u << lane) - 1u));
+            xyzq_o[d] = xyzq[l];
+            if (q1) q1_o[d] = q1[l];
+            pid_o[d] = pid[l];
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) copy_records_kernel(const uint64_t *__restrict__ n_dev, const float4 *__restrict__ xyzq,
+                                                           const float *__restrict__ q1, const uint32_t *__restrict__ pid,
+                                                           float4 *__restrict__ xyzq_o, float *__restrict__ q1_o, uint32_t *__restrict__ pid_o)
+{
+    const uint64_t n = *n_dev;
+    for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n; l += (uint64_t)gridDim.x * blockDim.x) {
+        xyzq_o[l] = xyzq[l];
+        if (q1) q1_o[l] = q1[l];
+        pid_o[l] = pid[l];
+    }
+}
+
+// compact mode: physical sort of the live records [0, *n_dev) by dual cell, through the alternate
+// buffers and back
+cudaError_t launch_sort_records(float4 *xyzq, float *q1, uint32_t *pid, const uint64_t *n_dev, uint64_t capacity, GridF g, uint32_t *keys,
+                                uint32_t *hist, uint32_t *partial, float4 *xyzq_alt, float *q1_alt, uint32_t *pid_alt, cudaStream_t st)
+{
+    const uint32_t n_keys = (uint32_t)g.nx * g.ny * g.nz + 1u, m = n_keys;
+    cudaError_t e = cudaMemsetAsync(hist, 0, 4ull * n_keys, st);
+    if (e != cudaSuccess) return e;
+    const uint64_t want = (capacity + 255) / 256;
+    const int blocks = (int)(want < 148 * 8 ? (want ? want : 1) : 148 * 8);
+    sort_key_kernel<<<blocks, 256, 0, st>>>(xyzq, 0, g, n_keys, keys, hist, n_dev);
+    const uint32_t nb = (m + kScanBlock - 1) / kScanBlock;
+    scan_totals_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
+    scan_partials_kernel<<<1, 256, 0, st>>>(partial, nb);
+    scan_apply_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
+    sort_scatter_records_kernel<<<blocks, 256, 0, st>>>(keys, n_dev, hist, xyzq, q1, pid, xyzq_alt, q1_alt, pid_alt);
+    copy_records_kernel<<<blocks, 256, 0, st>>>(n_dev, xyzq_alt, q1_alt, pid_alt, xyzq, q1, pid);
+    return cudaGetLastError();
 }
 
 // passes 2 + 3 on keys and a histogram that are already there (written by sort_key_kernel, or by the

@@ -407,6 +407,35 @@ def test_c5_compaction_small(lpm, orc):
     assert abs((lg[0][1] + lg[0][4] + lg[0][5]) / lg[0][0] - 1) < 1e-5
 
 
+def test_c5_compaction_with_record_sort(lpm, orc):
+    """a7 + gather-locality sort of the compact store (records reordered by met cell every 8 steps):
+    the SET of survivors, their states by id, the injected log and the ledger equal the oracle's."""
+    w = make("c5", scale=2e-3, n_steps=600).replace(nt=3, capacity=60_000)
+    small = Grid(60, 60, 25, -4.6e4, -6.0e3, 0.0, 200.0, 200.0, 50.0)
+    w = w.replace(mgrid=small, cgrid=small)
+    sim = lpm.Simulation(w, gather_sort=8)
+    o = orc.OracleSim(w)
+    for chunk in (7, 33, 560):
+        sim.step(chunk)
+        o.step(chunk)
+        gp, p = sim.get_particles_host(), o.particles()
+        frag = o.fragile_pids()
+        assert len(np.unique(gp["pid"])) == len(gp["pid"]) == sim.num_active
+        assert np.isin(np.setxor1d(gp["pid"], p["pid"]), frag).all()
+        common, gi, pi = np.intersect1d(gp["pid"], p["pid"], return_indices=True)
+        gg = {k: gp[k][gi] for k in ("x", "y", "z")}
+        gg["m"] = gp["m"][:, gi]
+        pp = {k: p[k][pi] for k in ("x", "y", "z")}
+        pp["m"] = p["m"][:, pi]
+        _n_step_compare(gg, pp, w, np.isin(common, frag), 0.999, f"c5 sorted step {sim.step_index}")
+    assert not np.all(np.diff(gp["pid"].astype(np.int64)) > 0)              # the store really was reordered
+    assert [sim.injected(s) for s in (0, 300, 599)] == [o.injected(s) for s in (0, 300, 599)]
+    lg, lo = sim.ledger(), o.ledger()
+    assert abs(lg[0][0] / lo[0][0] - 1) < 1e-12 and abs((lg[0][1] + lg[0][4] + lg[0][5]) / lg[0][0] - 1) < 1e-5
+    cg, co = sim.counts().cpu().numpy().astype(np.int64), o.counts().astype(np.int64)
+    assert abs(int(cg.sum()) - int(co.sum())) <= 3
+
+
 def test_c5_capacity_throttle(lpm, orc):
     w = make("c5", scale=1e-3, n_steps=40).replace(nt=2, capacity=1000)     # 40 / step, full after 25 steps
     sim = lpm.Simulation(w)
