@@ -12,7 +12,7 @@ constexpr int kMaxFused = 16;        // model steps fused into one launch (table
 constexpr int kBlendDepth = kMaxFused;  // time-blended met buffers kept: one per fused step
 constexpr int kSortPeriod = 32;      // model steps between two gather-locality sorts of a release
 constexpr int kStepThreads = 256;    // CTA size of the step kernel
-constexpr int kScanTile = kStepThreads;  // particles per look-back tile (compaction)
+constexpr int kScanTile = 4 * kStepThreads;  // particles per look-back tile (compaction): 4 per thread
 
 // Per-step scalars, host-computed in double (DESIGN.md §3 R4, R8).
 struct StepEntry {

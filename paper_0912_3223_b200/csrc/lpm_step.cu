@@ -322,7 +322,7 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
 
 // ------------------------------------------------------------------ compacting kernel (a7)
 // One model step with stable in-place stream compaction of the particles that left the domain,
-// fused into the store: each 256-particle tile steps its particles, counts survivors, obtains its
+// fused into the store: each 1024-particle tile (4 per thread) steps its particles, counts survivors, obtains its
 // exclusive output offset from a single-pass decoupled look-back over the tile states, and
 // writes its survivors at [offset, offset + count).  In place is safe: a tile publishes only
 // after it has loaded its inputs, and the destination range of tile t lies inside the source
@@ -341,8 +341,10 @@ __device__ __forceinline__ void st_state(uint64_t *p, uint64_t v)
 template <int K, int DRY>
 __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid_constant__ StepArgs A)
 {
+    constexpr int kItems = kScanTile / kStepThreads;  // particles per thread and tile: amortises the tile's barriers and look-back
+    constexpr int kParts = kItems * (kStepThreads / 32);
     __shared__ uint32_t s_tile;
-    __shared__ uint32_t s_wtot[kStepThreads / 32];
+    __shared__ uint32_t s_woff[kParts];  // survivors per (item, warp), then their exclusive offsets in index order
     __shared__ uint32_t s_excl;
     Acc<K> acc;
 #pragma unroll
@@ -353,6 +355,7 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
     const uint32_t epoch = ((uint32_t)(A.step0 + 1) & 0x3fffffffu) << 2;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     constexpr uint32_t FLAG_A = 1u, FLAG_P = 2u;
+    static_assert(kParts == 32, "the per-tile offsets are scanned by one warp");
     __shared__ DepTab<K> T;
     dep_clear<K>(T);
     __syncthreads();
@@ -363,30 +366,45 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
         const uint32_t tile = s_tile;
         if (tile >= n_tiles) break;
 
-        const uint64_t i = (uint64_t)tile * kScanTile + threadIdx.x;
-        bool alive = false;
-        float x = 0.f, y = 0.f, z = 0.f, q[K];
-        uint32_t pid = 0;
-        if (i < n) {
-            const float4 p = A.xyzq[i];
-            x = p.x; y = p.y; z = p.z; q[0] = p.w;
-            if (K > 1) q[1] = A.q1[i];
-            pid = A.pid[i];
-            alive = step_once<K, DRY>(A, A.tab[0], (uint32_t)A.step0, pid, x, y, z, q, acc, T);
-        }
-        // survivors: rank inside the tile
-        const uint32_t ball = __ballot_sync(0xffffffffu, alive);
-        const uint32_t rank = __popc(ball & ((1u << lane) - 1u));
-        if (lane == 0) s_wtot[warp] = __popc(ball);
-        __syncthreads();  // also orders every thread's input loads before the publication below
-        uint32_t woff = 0, total = 0;
+        float x[kItems], y[kItems], z[kItems], q[kItems][K];
+        uint32_t pid[kItems], rank[kItems];
+        bool alive[kItems];
 #pragma unroll
-        for (int w = 0; w < kStepThreads / 32; ++w) {
-            const uint32_t t = s_wtot[w];
-            woff += (w < warp) ? t : 0u;
-            total += t;
+        for (int j = 0; j < kItems; ++j) {
+            const uint64_t i = (uint64_t)tile * kScanTile + (uint32_t)j * kStepThreads + threadIdx.x;
+            alive[j] = false;
+            x[j] = y[j] = z[j] = 0.f;
+            pid[j] = 0;
+#pragma unroll
+            for (int k = 0; k < K; ++k) q[j][k] = 0.f;
+            if (i < n) {
+                const float4 p = A.xyzq[i];
+                x[j] = p.x; y[j] = p.y; z[j] = p.z; q[j][0] = p.w;
+                if (K > 1) q[j][1] = A.q1[i];
+                pid[j] = A.pid[i];
+            }
         }
+#pragma unroll
+        for (int j = 0; j < kItems; ++j) {
+            const uint64_t i = (uint64_t)tile * kScanTile + (uint32_t)j * kStepThreads + threadIdx.x;
+            if (i < n) alive[j] = step_once<K, DRY>(A, A.tab[0], (uint32_t)A.step0, pid[j], x[j], y[j], z[j], q[j], acc, T);
+            // survivors: rank inside the (item, warp) part
+            const uint32_t ball = __ballot_sync(0xffffffffu, alive[j]);
+            rank[j] = __popc(ball & ((1u << lane) - 1u));
+            if (lane == 0) s_woff[j * (kStepThreads / 32) + warp] = __popc(ball);
+        }
+        __syncthreads();  // also orders every thread's input loads before the publication below
         if (warp == 0) {
+            // exclusive scan of the 32 part counts (index order = item-major), tile total
+            const uint32_t cnt = s_woff[lane];
+            uint32_t inc = cnt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += t;
+            }
+            s_woff[lane] = inc - cnt;
+            const uint32_t total = __shfl_sync(0xffffffffu, inc, 31);
             uint32_t excl = 0;
             if (lane == 0) {
                 __threadfence();
@@ -422,14 +440,17 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
             }
         }
         __syncthreads();
-        if (alive) {
-            const uint64_t dst = (uint64_t)s_excl + woff + rank;
-            A.xyzq[dst] = make_float4(x, y, z, q[0]);
-            if (K > 1) A.q1[dst] = q[1];
-            A.pid[dst] = pid;
+#pragma unroll
+        for (int j = 0; j < kItems; ++j) {
+            if (alive[j]) {
+                const uint64_t dst = (uint64_t)s_excl + s_woff[j * (kStepThreads / 32) + warp] + rank[j];
+                A.xyzq[dst] = make_float4(x[j], y[j], z[j], q[j][0]);
+                if (K > 1) A.q1[dst] = q[j][1];
+                A.pid[dst] = pid[j];
+            }
         }
         if (A.any_dep) dep_flush<K>(A, T);  // every thread's step is behind the barrier above
-        __syncthreads();  // s_tile / s_wtot / s_excl and the deposit table are reused by the next tile
+        __syncthreads();  // s_tile / s_woff / s_excl and the deposit table are reused by the next tile
     }
     flush_ledger<K>(A, acc);
 }
