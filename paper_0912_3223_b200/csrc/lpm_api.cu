@@ -125,6 +125,7 @@ struct lpm_handle {
     uint64_t keys_n, keys_step;
     bool keys_ready;
     uint64_t csort_step;  // compact store: step of the last physical sort
+    bool bbox_valid;      // ctrl[20..21] holds the met-column box of the particles as the last step launch left them
     double dep_bound[LPM_MAX_NUCLIDES];  // largest activity a particle can carry (fixed-point scale of the deposit tables)
     bool binned;
     int sms, occ;
@@ -365,7 +366,7 @@ int ensure_blend(lpm_handle *h, StepArgs &A, int m, int m_max)
     const int sn = A.tab[0].snap & 0xffff;
     if (sn != h->pair_snap) {
         CK(launch_pair_repack(met + (uint64_t)sn * A.snap_cells, met + (uint64_t)(sn + 1) * A.snap_cells, h->ws + h->L.pair,
-                              g.nx, g.ny, g.nz, h->st));
+                              g.nx, g.ny, g.nz, (uint32_t *)(A.ctrl + 20) + 4, h->st));
         h->launches++;
         h->pair_snap = sn;
         h->blend_n = 0;
@@ -382,7 +383,21 @@ int ensure_blend(lpm_handle *h, StepArgs &A, int m, int m_max)
                 a[cnt] = e.a;
             }
         }
-        CK(launch_blend(h->ws + h->L.pair, blend, A.snap_cells, cnt, a, h->st));
+        // plume box: columns reachable within the cnt steps these buffers serve (B6)
+        BlendBox box{};
+        box.bb = h->bbox_valid ? (const uint32_t *)(A.ctrl + 20) : nullptr;
+        box.nx = g.nx; box.ny = g.ny; box.nz = g.nz;
+        const double walk = 5.768 * (double)h->sigma_h * 1.0001;
+        box.reach_x = (float)((double)cnt * h->prm.dt / g.dx * 1.0001); box.reach_y = (float)((double)cnt * h->prm.dt / g.dy * 1.0001);
+        box.walk_x = (float)((double)cnt * walk / g.dx); box.walk_y = (float)((double)cnt * walk / g.dy);
+        for (const Release &r : h->rel) {
+            if (r.fixed || box.n_src >= LPM_MAX_RELEASES) continue;
+            int si = (int)floor((r.src.x - g.x0) / g.dx), sj = (int)floor((r.src.y - g.y0) / g.dy);
+            box.src_i[box.n_src] = si < 0 ? 0 : (si > g.nx - 1 ? g.nx - 1 : si);
+            box.src_j[box.n_src] = sj < 0 ? 0 : (sj > g.ny - 1 ? g.ny - 1 : sj);
+            box.n_src++;
+        }
+        CK(launch_blend(h->ws + h->L.pair, blend, A.snap_cells, cnt, a, &box, h->st));
         h->launches++;
         h->blend_step0 = h->step;
         h->blend_n = cnt;
@@ -567,6 +582,16 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
         {
             const int rc = ensure_blend(h, A, m, m_max);
             if (rc) return rc;
+        }
+        A.bbox = nullptr;
+        if (h->met.nt > 1 && h->step + (uint64_t)m >= h->blend_step0 + (uint64_t)h->blend_n) {
+            // the next launch blends again: the step launches below leave the met-column box of their particles
+            CK(cudaMemsetAsync(A.ctrl + 20, 0xff, 8, h->st));  // {i_min, j_min} = 0xffffffff
+            CK(cudaMemsetAsync(A.ctrl + 21, 0, 8, h->st));     // {i_max, j_max} = 0
+            A.bbox = (uint32_t *)(A.ctrl + 20);
+            h->bbox_valid = true;
+        } else if (h->met.nt > 1) {
+            h->bbox_valid = false;  // (cannot happen before a blend: kept for safety when the coverage logic changes)
         }
         if (compact) {
             InjectArgs I{};
@@ -808,6 +833,8 @@ int32_t lpm_set_particles(lpm_handle *h, const void *xyzq, const float *q1, cons
     h->binned = false;
     h->perm_valid = false;
     h->keys_ready = false;
+    h->bbox_valid = false;
+    h->blend_n = 0;
     h->csort_step = step_index;
     if (n) {  // the installed activities bound the deposit increments from now on
         float *mx = (float *)(h->ws + h->L.air);
@@ -1018,8 +1045,10 @@ int32_t lpm_test_sample(const lpm_meteo *met, double t, const void *xyz, uint64_
     cudaError_t rc;
     if (met->nt > 1) {
         if (cudaMalloc(&pair, 32 * cells) != cudaSuccess) { cudaFree(blend); return LPM_ERR_CUDA; }
-        rc = launch_pair_repack(f + (uint64_t)sn * cells, f + (uint64_t)(sn + 1) * cells, pair, g.nx, g.ny, g.nz, s);
-        if (rc == cudaSuccess) rc = launch_blend(pair, blend, cells, 1, &e.a, s);
+        BlendBox box{};
+        box.nx = g.nx; box.ny = g.ny; box.nz = g.nz;
+        rc = launch_pair_repack(f + (uint64_t)sn * cells, f + (uint64_t)(sn + 1) * cells, pair, g.nx, g.ny, g.nz, nullptr, s);
+        if (rc == cudaSuccess) rc = launch_blend(pair, blend, cells, 1, &e.a, &box, s);
     } else {
         rc = launch_transpose(f, blend, g.nx, g.ny, g.nz, s);
     }

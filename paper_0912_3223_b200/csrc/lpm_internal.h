@@ -76,6 +76,7 @@ struct StepArgs {
     uint64_t base, n, n_prev;  // slots >= n_prev are born inside this launch
     const uint32_t *perm;      // gather-locality pass: slots [0, n_perm) listed in dual-cell order, or null
     uint64_t n_perm;           // slots [n_perm, n) are walked in slot order
+    uint32_t *bbox;            // {i_min, j_min, i_max, j_max} of the met columns of the particles at the end of the launch (atomics)
     uint32_t *keys_out, *hist_out;  // non-null: the launch before a sort leaves each slot's dual-cell key and the histogram
     uint32_t n_keys, pad1_;
     uint64_t pid_offset, pid_stride;
@@ -135,9 +136,18 @@ cudaError_t launch_sort_records(float4 *xyzq, float *q1, uint32_t *pid, const ui
 uint64_t sort_partial_entries(uint64_t n_cells);
 cudaError_t run_probe(int kind, uint64_t footprint_bytes, void *scratch_dev, uint64_t scratch_bytes, int reps, double *ops,
                       cudaStream_t st);
-cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, cudaStream_t st);
+cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, uint32_t *uvmax, cudaStream_t st);
 cudaError_t launch_transpose(const float4 *s0, float4 *out, int nx, int ny, int nz, cudaStream_t st);
-cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, cudaStream_t st);
+// plume bounding box (a0): blend only the met columns a particle can reach during the coming launch
+struct BlendBox {
+    const uint32_t *bb;   // device: {i_min, j_min, i_max, j_max} of the particles' met columns, {|u|max, |v|max} float bits; null = whole field
+    int32_t nx, ny, nz;
+    float reach_x, reach_y;    // cells per (m/s) of wind:  steps * dt / dx
+    float walk_x, walk_y;      // cells of random walk: steps * 5.768 sigma_h / dx  (|N(0,1)| <= sqrt(48 ln 2) by construction, R3)
+    int32_t n_src;
+    int32_t src_i[LPM_MAX_RELEASES], src_j[LPM_MAX_RELEASES];   // source columns (newborn particles)
+};
+cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, const BlendBox *box, cudaStream_t st);
 cudaError_t launch_bin(const BinArgs &a, int blocks, cudaStream_t st);
 cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3, int K, const double *scale, cudaStream_t st);
 cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, double inv_area, cudaStream_t st);

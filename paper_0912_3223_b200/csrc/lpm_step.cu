@@ -306,6 +306,19 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             A.xyzq[slot] = make_float4(x, y, z, q[0]);
             if (K > 1) A.q1[slot] = q[1];
         }
+        if (A.bbox) {
+            // met columns of the particles at the end of the launch -> plume box of the next blend
+            const bool live = valid && z >= 0.0f;
+            const int ci = min(max(__float2int_rd((x - A.mg.x0) * A.mg.inv_dx), 0), A.mg.nx - 1);
+            const int cj = min(max(__float2int_rd((y - A.mg.y0) * A.mg.inv_dy), 0), A.mg.ny - 1);
+            const uint32_t i0 = __reduce_min_sync(0xffffffffu, live ? (uint32_t)ci : 0xffffffffu);
+            const uint32_t i1 = __reduce_max_sync(0xffffffffu, live ? (uint32_t)ci : 0u);
+            const uint32_t j0 = __reduce_min_sync(0xffffffffu, live ? (uint32_t)cj : 0xffffffffu);
+            const uint32_t j1 = __reduce_max_sync(0xffffffffu, live ? (uint32_t)cj : 0u);
+            if ((threadIdx.x & 31) == 0 && i0 != 0xffffffffu) {
+                atomicMin(A.bbox, i0); atomicMin(A.bbox + 1, j0); atomicMax(A.bbox + 2, i1); atomicMax(A.bbox + 3, j1);
+            }
+        }
         if (A.keys_out && in_range) {
             // pass 1 of the coming gather-locality sort, for free: the new position is in registers
             const uint32_t key = (valid && z >= 0.0f) ? corner_of(A.mg, x, y, z).o : A.n_keys - 1u;
@@ -449,6 +462,23 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
                 A.pid[dst] = pid[j];
             }
         }
+        if (A.bbox) {
+            // met columns of the survivors -> plume box of the next blend
+            uint32_t i0 = 0xffffffffu, i1 = 0u, j0 = 0xffffffffu, j1 = 0u;
+#pragma unroll
+            for (int j = 0; j < kItems; ++j) {
+                if (alive[j]) {
+                    const uint32_t ci = (uint32_t)min(max(__float2int_rd((x[j] - A.mg.x0) * A.mg.inv_dx), 0), A.mg.nx - 1);
+                    const uint32_t cj = (uint32_t)min(max(__float2int_rd((y[j] - A.mg.y0) * A.mg.inv_dy), 0), A.mg.ny - 1);
+                    i0 = min(i0, ci); i1 = max(i1, ci); j0 = min(j0, cj); j1 = max(j1, cj);
+                }
+            }
+            i0 = __reduce_min_sync(0xffffffffu, i0); i1 = __reduce_max_sync(0xffffffffu, i1);
+            j0 = __reduce_min_sync(0xffffffffu, j0); j1 = __reduce_max_sync(0xffffffffu, j1);
+            if (lane == 0 && i0 != 0xffffffffu) {
+                atomicMin(A.bbox, i0); atomicMin(A.bbox + 1, j0); atomicMax(A.bbox + 2, i1); atomicMax(A.bbox + 3, j1);
+            }
+        }
         if (A.any_dep) dep_flush<K>(A, T);  // every thread's step is behind the barrier above
         __syncthreads();  // s_tile / s_woff / s_excl and the deposit table are reused by the next tile
     }
@@ -520,9 +550,11 @@ int step_max_blocks_per_sm(int K, bool compact, int dry)
 // one line per lane.  One thread per output texel: coalesced 32-byte writes, strided 16-byte reads
 // (once per met interval, < 1 ms).
 __global__ void __launch_bounds__(256) pair_repack_kernel(const float4 *__restrict__ s0, const float4 *__restrict__ s1,
-                                                          Texel2 *__restrict__ pair, uint32_t nx, uint32_t ny, uint32_t nz)
+                                                          Texel2 *__restrict__ pair, uint32_t nx, uint32_t ny, uint32_t nz,
+                                                          uint32_t *__restrict__ uvmax)
 {
     const uint64_t cells = (uint64_t)nx * ny * nz, plane = (uint64_t)nx * ny;
+    float um = 0.f, vm = 0.f;  // largest |u|, |v| of the interval: bounds the advection of the plume box
     for (uint64_t o = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; o < cells; o += (uint64_t)gridDim.x * blockDim.x) {
         const uint64_t col = o / nz;
         const uint32_t k = (uint32_t)(o - col * nz);
@@ -531,13 +563,31 @@ __global__ void __launch_bounds__(256) pair_repack_kernel(const float4 *__restri
         t.a = __ldg(s0 + src);
         t.b = __ldg(s1 + src);
         pair[o] = t;
+        um = fmaxf(um, fmaxf(fabsf(t.a.x), fabsf(t.b.x)));
+        vm = fmaxf(vm, fmaxf(fabsf(t.a.y), fabsf(t.b.y)));
+    }
+    if (uvmax) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            um = fmaxf(um, __shfl_xor_sync(0xffffffffu, um, o));
+            vm = fmaxf(vm, __shfl_xor_sync(0xffffffffu, vm, o));
+        }
+        if ((threadIdx.x & 31) == 0) {
+            atomicMax(uvmax, __float_as_uint(um));   // non-negative floats order like their bit patterns
+            atomicMax(uvmax + 1, __float_as_uint(vm));
+        }
     }
 }
 
-cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, cudaStream_t st)
+cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, uint32_t *uvmax, cudaStream_t st)
 {
+    if (uvmax) {
+        const cudaError_t e = cudaMemsetAsync(uvmax, 0, 8, st);
+        if (e != cudaSuccess) return e;
+    }
     const uint64_t want = ((uint64_t)nx * ny * nz + 255) / 256;
-    pair_repack_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(s0, s1, (Texel2 *)pair, (uint32_t)nx, (uint32_t)ny, (uint32_t)nz);
+    pair_repack_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(s0, s1, (Texel2 *)pair, (uint32_t)nx, (uint32_t)ny, (uint32_t)nz,
+                                                                                uvmax);
     return cudaGetLastError();
 }
 
@@ -571,25 +621,51 @@ struct BlendArgs {
     uint64_t cells;
     int32_t m;
     float a[kBlendDepth];
+    BlendBox box;
 };
 
+// Only the columns a particle can reach are blended: the box of the particles' columns at the end of
+// the previous launch (accumulated by the step kernel), widened by the largest possible displacement
+// of the coming steps, (|u|max dt + 5.768 sigma_h) per step (trilinear values are convex combinations
+// of texels, |N(0,1)| <= 5.768 by R3), + 2 columns for the stencil, united with the source columns.
 __global__ void __launch_bounds__(256) blend_kernel(const __grid_constant__ BlendArgs B)
 {
-    for (uint64_t o = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; o < B.cells; o += (uint64_t)gridDim.x * blockDim.x) {
-        Texel2 t;
+    int i_lo = 0, i_hi = B.box.nx - 1, j_lo = 0, j_hi = B.box.ny - 1;
+    if (B.box.bb) {
+        const float um = __uint_as_float(B.box.bb[4]), vm = __uint_as_float(B.box.bb[5]);
+        const int mx = (int)ceilf(um * B.box.reach_x + B.box.walk_x) + 2, my = (int)ceilf(vm * B.box.reach_y + B.box.walk_y) + 2;
+        int a0 = (int)min(B.box.bb[0], 0x3fffffffu), b0 = (int)min(B.box.bb[1], 0x3fffffffu), a1 = (int)B.box.bb[2], b1 = (int)B.box.bb[3];
+        if (a0 > a1) { a0 = 0x3fffffff; a1 = -1; b0 = 0x3fffffff; b1 = -1; }   // no particle yet
+        for (int r = 0; r < B.box.n_src; ++r) {
+            a0 = min(a0, B.box.src_i[r]); a1 = max(a1, B.box.src_i[r]);
+            b0 = min(b0, B.box.src_j[r]); b1 = max(b1, B.box.src_j[r]);
+        }
+        if (a0 > a1) return;   // nothing can be sampled
+        i_lo = max(a0 - mx, 0); i_hi = min(a1 + mx, B.box.nx - 1);
+        j_lo = max(b0 - my, 0); j_hi = min(b1 + my, B.box.ny - 1);
+    }
+    const uint32_t W = (uint32_t)(i_hi - i_lo + 1), nz = (uint32_t)B.box.nz;
+    const uint64_t total = (uint64_t)W * (uint32_t)(j_hi - j_lo + 1) * nz;
+    for (uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t c = t / nz;
+        const uint32_t k = (uint32_t)(t - c * nz);
+        const uint32_t jj = (uint32_t)(c / W), ii = (uint32_t)(c - (uint64_t)jj * W);
+        const uint64_t o = ((uint64_t)(j_lo + jj) * (uint32_t)B.box.nx + (uint32_t)(i_lo + ii)) * nz + k;
+        Texel2 tx;
         asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-            : "=f"(t.a.x), "=f"(t.a.y), "=f"(t.a.z), "=f"(t.a.w), "=f"(t.b.x), "=f"(t.b.y), "=f"(t.b.z), "=f"(t.b.w)
+            : "=f"(tx.a.x), "=f"(tx.a.y), "=f"(tx.a.z), "=f"(tx.a.w), "=f"(tx.b.x), "=f"(tx.b.y), "=f"(tx.b.z), "=f"(tx.b.w)
             : "l"(B.pair + o));
 #pragma unroll 4
-        for (int s = 0; s < B.m; ++s) B.out[(uint64_t)s * B.cells + o] = lerp4(t.a, t.b, B.a[s]);
+        for (int s = 0; s < B.m; ++s) B.out[(uint64_t)s * B.cells + o] = lerp4(tx.a, tx.b, B.a[s]);
     }
 }
 
-cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, cudaStream_t st)
+cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, const BlendBox *box, cudaStream_t st)
 {
     BlendArgs B;
     B.pair = (const Texel2 *)pair; B.out = out; B.cells = cells; B.m = m;
     for (int s = 0; s < kBlendDepth; ++s) B.a[s] = s < m ? a[s] : 0.0f;
+    B.box = *box;
     const uint64_t want = (cells + 255) / 256;
     blend_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(B);
     return cudaGetLastError();
