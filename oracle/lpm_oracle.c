@@ -15,7 +15,7 @@
  * the exact Gaussian puff / folded normal (P4), 2^(-t/T) decay (P5), mass ledger (P6), affine
  * reproduction of the interpolation (P7), well-mixed reflection (P8), brute-force binning (P9),
  * closed-form deposition (P10, P11), compaction (P12), schedule (P13), independent numpy trace
- * (P14).  PARITY UNPINNED (no printed value or implementation exists to compare against): the
+ * (P14), geometric-series dose of a resting decaying cloud (P15).  PARITY UNPINNED (no printed value or implementation exists to compare against): the
  * dry-deposition rate law p_dry = 1-exp(-vd dt/h_dep) and h_dep, and the treatment of ground,
  * top and lateral boundaries (the paper gives none: L84-86 "out of scope of this paper").
  *
@@ -101,6 +101,7 @@ typedef struct orc_sim {
     uint64_t *inj_log; uint64_t inj_cap;
     uint64_t *frag_pids; uint64_t n_frag, frag_cap; /* pids ever flagged fragile (T3) */
     uint64_t bin_step;
+    double *dose;     /* [K][nz][ny][nx] time-integrated concentration, Bq s m^-3; NULL = not accumulated */
 } orc_sim;
 
 /* ------------------------------------------------------------------ R1: Philox4x32-10
@@ -295,7 +296,7 @@ void orc_destroy(orc_sim *s)
     free(s->x); free(s->y); free(s->z); free(s->pid); free(s->status); free(s->fragile);
     free(s->dcell); free(s->nearface); free(s->moved);
     for (int k = 0; k < ORC_MAXK; ++k) { free(s->m[k]); free(s->inc_dry[k]); free(s->inc_wet[k]); free(s->inc_dec[k]); }
-    free(s->conc_sum); free(s->cnt); free(s->dep); free(s->dep_slack); free(s->inj_log); free(s->frag_pids);
+    free(s->conc_sum); free(s->cnt); free(s->dep); free(s->dep_slack); free(s->inj_log); free(s->frag_pids); free(s->dose);
     free(s);
 }
 
@@ -565,9 +566,33 @@ int32_t orc_step(orc_sim *s, int32_t n_steps)
             s->n = o;
         }
         s->step = n + 1;
-        if (c->bin_every > 0 && s->step % (uint64_t)c->bin_every == 0) orc_bin_now(s);
+        if (c->bin_every > 0 && s->step % (uint64_t)c->bin_every == 0) {
+            orc_bin_now(s);
+            /* PAPER.md L108 / Fig. 2b (L218) "time integrated dosage": the gridded activity concentration of every
+             * n-th step times the interval it stands for, summed (rectangle rule at the binning cadence) */
+            if (s->dose) {
+                size_t nc = (size_t)cg->nx * cg->ny * cg->nz * c->K;
+                double V = cg->dx * cg->dy * cg->dz, T = (double)c->bin_every * c->dt;
+                for (size_t i = 0; i < nc; ++i) s->dose[i] += s->conc_sum[i] / V * T;
+            }
+        }
     }
     return 0;
+}
+
+/* start accumulating the time-integrated concentration at every cadence binning from now on */
+void orc_enable_dose(orc_sim *s)
+{
+    const orc_grid *g = &s->cfg.cgrid;
+    if (!s->dose) s->dose = calloc((size_t)g->nx * g->ny * g->nz * s->cfg.K, sizeof(double));
+    if (!s->dose) abort();
+}
+
+void orc_dose(const orc_sim *s, double *out)
+{
+    const orc_grid *g = &s->cfg.cgrid;
+    size_t n = (size_t)g->nx * g->ny * g->nz * s->cfg.K;
+    for (size_t i = 0; i < n; ++i) out[i] = s->dose ? s->dose[i] : 0.0;
 }
 
 /* ------------------------------------------------------------------ accessors (test hooks) */

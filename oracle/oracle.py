@@ -85,6 +85,8 @@ def lib():
         L.orc_ledger.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_concentration.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_counts.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_enable_dose.argtypes = [C.c_void_p]
+        L.orc_dose.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_deposition.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_injected.argtypes = [C.c_void_p, C.c_uint64]
         L.orc_injected.restype = C.c_uint64
@@ -268,6 +270,16 @@ class OracleSim:
         g = self.w.cgrid
         out = np.zeros((self.K, g.nz, g.ny, g.nx))
         lib().orc_concentration(self._h, _p(out))
+        return out
+
+    def enable_dose(self):
+        lib().orc_enable_dose(self._h)
+
+    def dose(self):
+        """time-integrated concentration [K][nz][ny][nx], Bq s m^-3 (S§8(f)3)"""
+        g = self.w.cgrid
+        out = np.zeros((self.K, g.nz, g.ny, g.nx), dtype=np.float64)
+        lib().orc_dose(self._h, _p(out))
         return out
 
     def counts(self):

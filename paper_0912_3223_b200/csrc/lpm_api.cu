@@ -71,6 +71,7 @@ GridF gridf(const lpm_grid &g, bool zfast = false)
     f.nx = g.nx; f.ny = g.ny; f.nz = g.nz;
     f.x0 = (float)g.x0; f.y0 = (float)g.y0; f.z0 = (float)g.z0;
     f.inv_dx = (float)(1.0 / g.dx); f.inv_dy = (float)(1.0 / g.dy); f.inv_dz = (float)(1.0 / g.dz);
+    f.cx = (float)(-g.x0 / g.dx - 0.5); f.cy = (float)(-g.y0 / g.dy - 0.5); f.cz = (float)(-g.z0 / g.dz - 0.5);
     f.fx1 = (float)(g.nx - 1); f.fy1 = (float)(g.ny - 1); f.fz1 = (float)(g.nz - 1);
     f.ix2 = g.nx > 2 ? g.nx - 2 : 0; f.iy2 = g.ny > 2 ? g.ny - 2 : 0; f.iz2 = g.nz > 2 ? g.nz - 2 : 0;
     if (zfast) { f.ez = 1u; f.ex = (uint32_t)g.nz; f.ey = (uint32_t)g.nz * (uint32_t)g.nx; }

@@ -33,6 +33,7 @@ struct GridF {  // fp32 view of a grid, exactly as the kernels use it
     // derived, for the met sampling R4: the upper clamp of the grid coordinate, the largest lower
     // corner index, and the element strides to the upper corner (0 on an axis with a single cell:
     // i1 = min(i0 + 1, n - 1) = i0 + 1 whenever n >= 2, because i0 <= n - 2)
+    float cx, cy, cz;          // (float)(-p0/d - 1/2): grid coordinate of the stencil g = p * inv_d + c
     float fx1, fy1, fz1;       // (float)(n - 1)
     int32_t ix2, iy2, iz2;     // max(n - 2, 0)
     uint32_t ex, ey, ez;       // element strides of cell (i, j, k) in the sampled buffer: z-fastest (nz, nx*nz, 1)

@@ -323,3 +323,32 @@ def test_oracle_deterministic_across_thread_counts():
         np.testing.assert_array_equal(res[0][0][key], res[1][0][key])
     np.testing.assert_array_equal(res[0][1], res[1][1])
     np.testing.assert_array_equal(res[0][2], res[1][2])
+
+
+# ------------------------------------------------------------------ P15: time-integrated concentration (S§8(f)3)
+def test_dose_of_a_resting_decaying_cloud_is_a_geometric_series():
+    """No wind, no diffusion: the particles rest, the cell concentration decays as 2^(-t/T), and the dose
+    after n binnings is the rectangle-rule sum  C0 T_bin sum_{b=1..n} 2^(-b T_bin / T)  (closed form)."""
+    T_half = 3600.0
+    n, be, dt, nb = 50, 20, 10.0, 7
+    w = custom(uniform_met(), n=n, nuclides=[Nuclide("X", T_half)], dt=dt, bin_every=be, src=(30.0, -20.0, 150.0),
+               activity=[2.0e6], H=1000.0, n_steps=be * nb)
+    o = orc.OracleSim(w)
+    o.enable_dose()
+    o.step(be * nb)
+    g = w.cgrid
+    V = g.dx * g.dy * g.dz
+    Tb = be * dt
+    r = 2.0 ** (-Tb / T_half)
+    want = 2.0e6 / V * Tb * r * (1 - r ** nb) / (1 - r)
+    d = o.dose()
+    i, j, k = int((30.0 - g.x0) // g.dx), int((-20.0 - g.y0) // g.dy), int(150.0 // g.dz)
+    assert abs(d[0, k, j, i] / want - 1) < 1e-12
+    assert d.sum() == pytest.approx(d[0, k, j, i], rel=1e-15)
+    # dose = sum over binnings of the concentration field times the interval (definition, re-run step by step)
+    o2 = orc.OracleSim(w)
+    acc = np.zeros_like(d)
+    for _ in range(nb):
+        o2.step(be)
+        acc += o2.concentration() * Tb
+    np.testing.assert_allclose(d, acc, rtol=1e-13, atol=0)
