@@ -92,7 +92,8 @@ typedef struct {
                                * -1 = never.  Results per particle do not depend on it.  With compact = 1
                                * the records themselves are sorted (the id travels with the particle), so
                                * the store is then in met-cell order, not in id order.             */
-    int32_t reserved;
+    int32_t dose;             /* 1: accumulate the time-integrated concentration (Fig. 2b "time
+                               * integrated dosage") at every cadence binning; read with lpm_dose        */
 } lpm_params;
 
 typedef struct {
@@ -162,6 +163,9 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps);
 /* Concentration in Bq m^-3, float [K][nz][ny][nx], of the particle state at the current step
  * (re-bins first if the internal grid is stale). */
 int32_t lpm_concentration(lpm_handle *h, float *out_dev);
+/* Time-integrated concentration in Bq s m^-3, float [K][nz][ny][nx]: sum over the cadence binnings so far
+ * of (concentration at that binning) x (bin_every * dt) (rectangle rule; needs params.dose = 1, else STATE). */
+int32_t lpm_dose(lpm_handle *h, float *out_dev);
 /* Particle counts per cell, uint32 [nz][ny][nx], same snapshot rule. */
 int32_t lpm_counts(lpm_handle *h, uint32_t *out_dev);
 /* Cumulative deposited activity in Bq m^-2, float [K][ny][nx] (not decayed on the ground). */

@@ -27,7 +27,7 @@ SYMBOLS = (
     "lpm_deposition_f64", "lpm_bin_now", "lpm_num_active", "lpm_step_index", "lpm_mass_scale", "lpm_get_particles",
     "lpm_set_particles", "lpm_ledger", "lpm_injected", "lpm_last_error", "lpm_launch_count", "lpm_test_philox",
     "lpm_test_normals", "lpm_test_sample", "lpm_upload_meteo", "lpm_concentration_host", "lpm_deposition_host",
-    "lpm_set_timing", "lpm_get_timing", "lpm_probe", "lpm_test_box_muller",
+    "lpm_set_timing", "lpm_get_timing", "lpm_probe", "lpm_test_box_muller", "lpm_dose",
 )
 
 
@@ -56,7 +56,7 @@ class lpm_nuclide(C.Structure):
 class lpm_params(C.Structure):
     _fields_ = [("dt", C.c_double), ("seed", C.c_uint64), ("capacity", C.c_uint64), ("boundary_mode", C.c_int32),
                 ("compact", C.c_int32), ("h_dep", C.c_double), ("bin_every", C.c_int32), ("steps_per_launch", C.c_int32),
-                ("gather_sort", C.c_int32), ("reserved", C.c_int32)]
+                ("gather_sort", C.c_int32), ("dose", C.c_int32)]
 
 
 class lpm_source(C.Structure):
@@ -88,6 +88,7 @@ def load():
     L.lpm_step.argtypes = [vp, i32]
     L.lpm_concentration.argtypes = [vp, vp]
     L.lpm_counts.argtypes = [vp, vp]
+    L.lpm_dose.argtypes = [vp, vp]
     L.lpm_deposition.argtypes = [vp, vp]
     L.lpm_deposition_f64.argtypes = [vp, vp]
     L.lpm_bin_now.argtypes = [vp]
@@ -130,8 +131,9 @@ def _grid(g) -> lpm_grid:
     return lpm_grid(g.nx, g.ny, g.nz, 0, g.x0, g.y0, g.z0, g.dx, g.dy, g.dz)
 
 
-def workspace_bytes(cgrid, capacity: int, n_nuclides: int, compact: bool, mgrid=None, nt: int = 1, gather_sort: int = 0) -> int:
-    p = lpm_params(dt=1.0, capacity=capacity, compact=1 if compact else 0, h_dep=1.0, gather_sort=gather_sort)
+def workspace_bytes(cgrid, capacity: int, n_nuclides: int, compact: bool, mgrid=None, nt: int = 1, gather_sort: int = 0,
+                    dose: bool = False) -> int:
+    p = lpm_params(dt=1.0, capacity=capacity, compact=1 if compact else 0, h_dep=1.0, gather_sort=gather_sort, dose=1 if dose else 0)
     out = C.c_uint64()
     g = _grid(cgrid)
     met = lpm_meteo(grid=_grid(mgrid if mgrid is not None else cgrid), nt=nt)
@@ -165,7 +167,7 @@ class Simulation:
     """
 
     def __init__(self, w, *, steps_per_launch: int = 0, bin_every: Optional[int] = None, fields_dev=None,
-                 stream=None, auto_release: bool = True, gather_sort: int = 0):
+                 stream=None, auto_release: bool = True, gather_sort: int = 0, dose: bool = False):
         torch = _require_cuda()
         L = load()
         self._L = L
@@ -179,7 +181,7 @@ class Simulation:
             fields_dev = torch.from_numpy(np.ascontiguousarray(f)).to(self.device)
         assert fields_dev.dtype == torch.float32 and fields_dev.is_contiguous()
         self.fields_dev = fields_dev
-        nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact, w.mgrid, w.nt, gather_sort)
+        nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact, w.mgrid, w.nt, gather_sort, dose)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         cg = _grid(w.cgrid)
         met = lpm_meteo(grid=_grid(w.mgrid), nt=w.nt, t0=w.t0, dt_snap=w.dt_snap, fields_dev=fields_dev.data_ptr(),
@@ -188,7 +190,7 @@ class Simulation:
         prm = lpm_params(dt=w.dt, seed=w.seed, capacity=w.capacity,
                          boundary_mode=1 if w.boundary_mode == "absorb" else 0, compact=1 if w.compact else 0,
                          h_dep=w.h_dep, bin_every=w.bin_every if bin_every is None else bin_every,
-                         steps_per_launch=steps_per_launch, gather_sort=gather_sort)
+                         steps_per_launch=steps_per_launch, gather_sort=gather_sort, dose=1 if dose else 0)
         h = C.c_void_p()
         with torch.cuda.stream(self.stream):
             rc = L.lpm_create(C.byref(cg), C.byref(met), nucs, w.K, C.byref(prm), self.workspace.data_ptr(), nbytes,
@@ -234,6 +236,13 @@ class Simulation:
         if out is None:
             out = self.torch.empty((self.K, g.nz, g.ny, g.nx), dtype=self.torch.float32, device=self.device)
         self._ck(self._L.lpm_concentration(self._h, out.data_ptr()), "lpm_concentration")
+        return out
+
+    def dose(self, out=None):
+        g = self.w.cgrid
+        if out is None:
+            out = self.torch.empty((self.K, g.nz, g.ny, g.nx), dtype=self.torch.float32, device=self.device)
+        self._ck(self._L.lpm_dose(self._h, out.data_ptr()), "lpm_dose")
         return out
 
     def counts(self, out=None):

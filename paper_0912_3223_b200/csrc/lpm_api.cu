@@ -27,12 +27,12 @@ struct Release {
 };
 
 struct Layout {
-    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, blend, keys, perm, hist, partial, alt_xyzq, alt_q1, alt_pid, total;
+    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, blend, keys, perm, hist, partial, alt_xyzq, alt_q1, alt_pid, dose, total;
 };
 
 uint64_t up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
-Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K, bool compact, bool sort)
+Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K, bool compact, bool sort, bool dose)
 {
     Layout L{};
     const uint64_t cells3 = (uint64_t)g.nx * g.ny * g.nz, cells2 = (uint64_t)g.nx * g.ny;
@@ -59,6 +59,7 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     L.alt_xyzq = o; o += sort && compact ? up(16 * cap) : 0;           //   compact store: the records themselves are sorted,
     L.alt_q1 = o; o += sort && compact && K > 1 ? up(4 * cap) : 0;     //   through these alternate buffers
     L.alt_pid = o; o += sort && compact ? up(4 * cap) : 0;
+    L.dose = o; o += dose ? up(8 * cells3 * K) : 0;                    // time-integrated concentration (S 8(f)3)
     L.total = o;
     return L;
 }
@@ -431,7 +432,7 @@ int32_t lpm_workspace_bytes(const lpm_grid *g, const lpm_meteo *met, const lpm_p
 {
     if (!grid_ok(g) || !met || !grid_ok(&met->grid) || met->nt < 1 || !p || !bytes || K < 1 || K > LPM_MAX_NUCLIDES || p->capacity == 0 || p->capacity >= (1ull << 32))
         return LPM_ERR_INVALID_ARG;
-    *bytes = make_layout(*g, *met, p->capacity, K, p->compact != 0, sort_enabled(p)).total;
+    *bytes = make_layout(*g, *met, p->capacity, K, p->compact != 0, sort_enabled(p), p->dose != 0).total;
     return LPM_OK;
 }
 
@@ -463,7 +464,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return LPM_ERR_NO_DEVICE;
     if (prop.major != 10) return LPM_ERR_NO_DEVICE;
 
-    const Layout L = make_layout(*cg, *met, p->capacity, K, p->compact != 0, sort_enabled(p));
+    const Layout L = make_layout(*cg, *met, p->capacity, K, p->compact != 0, sort_enabled(p), p->dose != 0);
     if (ws_bytes < L.total) return LPM_ERR_WORKSPACE_TOO_SMALL;
 
     lpm_handle *h = new (std::nothrow) lpm_handle();
@@ -694,6 +695,15 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
         if (h->prm.bin_every > 0 && h->step % (uint64_t)h->prm.bin_every == 0) {
             const int rc = do_bin(h);
             if (rc) return rc;
+            if (h->prm.dose) {
+                // P:L108 / Fig. 2b "time integrated dosage": concentration of this binning x the interval it stands for
+                const double T = (double)h->prm.bin_every * h->prm.dt, V = h->cg.dx * h->cg.dy * h->cg.dz;
+                double sc[LPM_MAX_NUCLIDES] = {0, 0};
+                for (int k = 0; k < h->K; ++k) sc[k] = G_of(h, k, h->step) / V * T;
+                CK(launch_dose_accum((const double *)(h->ws + h->L.conc), (double *)(h->ws + h->L.dose),
+                                     (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz, h->K, sc, h->st));
+                h->launches++;
+            }
         }
     }
     return LPM_OK;
@@ -715,6 +725,17 @@ int32_t lpm_concentration(lpm_handle *h, float *out)
     double scale[LPM_MAX_NUCLIDES] = {0, 0};
     for (int k = 0; k < h->K; ++k) scale[k] = G_of(h, k, h->bin_step) / V;
     CK(launch_conc_readout((const double *)(h->ws + h->L.conc), out, (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz, h->K, scale, h->st));
+    h->launches++;
+    return LPM_OK;
+}
+
+int32_t lpm_dose(lpm_handle *h, float *out)
+{
+    if (!h || !out) return fail(h, LPM_ERR_INVALID_ARG, "lpm_dose: null");
+    if (!h->prm.dose) return fail(h, LPM_ERR_STATE, "lpm_dose: params.dose was 0 at lpm_create");
+    if (h->sticky) return h->sticky;
+    const double one[LPM_MAX_NUCLIDES] = {1.0, 1.0};
+    CK(launch_conc_readout((const double *)(h->ws + h->L.dose), out, (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz, h->K, one, h->st));
     h->launches++;
     return LPM_OK;
 }

@@ -75,6 +75,24 @@ cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3,
     return cudaGetLastError();
 }
 
+// S 8(f)3 dose grid: dose[k][cell] += sum_q[k][cell] * G_k(t_b) / V * T_bin at every cadence binning
+__global__ void dose_accum_kernel(const double *__restrict__ conc, double *__restrict__ dose, uint64_t cells3, int K, double s0, double s1)
+{
+    const uint64_t total = cells3 * (uint64_t)K;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
+        const double c = conc[i];
+        if (c != 0.0) dose[i] += c * (i < cells3 ? s0 : s1);
+    }
+}
+
+cudaError_t launch_dose_accum(const double *conc, double *dose, uint64_t cells3, int K, const double *scale, cudaStream_t st)
+{
+    const uint64_t total = cells3 * K;
+    int blocks = (int)((total + 255) / 256 < 148 * 8 ? (total + 255) / 256 : 148 * 8);
+    dose_accum_kernel<<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(conc, dose, cells3, K, scale[0], K > 1 ? scale[1] : 0.0);
+    return cudaGetLastError();
+}
+
 __global__ void dep_readout_kernel(const double *__restrict__ dep, float *out32, double *out64, uint64_t total, double inv_area)
 {
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {

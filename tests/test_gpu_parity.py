@@ -373,6 +373,43 @@ def test_deposition_map_end_to_end_with_slack(lpm, orc):
         assert abs(dg[k].sum() / do[k].sum() - 1) < 1e-5
 
 
+# ------------------------------------------------------------------ S§8(f)3: time-integrated concentration
+def test_dose_grid(lpm, orc):
+    """(f)3: resting decaying cloud (no wind, no diffusion): the dose grid equals the oracle's cell by cell to
+    fp32 mass precision; then a moving two-nuclide plume: integrated dose (sum over cells x V) within 1e-5 and
+    cell by cell on well-populated cells."""
+    w = custom(uniform_met(), n=5000, nuclides=[Nuclide("X", 3600.0)], dt=10.0, bin_every=20, src=(30.0, -20.0, 150.0),
+               activity=[2.0e6], H=1000.0, n_steps=140)
+    sim, o = lpm.Simulation(w, dose=True), orc.OracleSim(w)
+    o.enable_dose()
+    sim.step(140)
+    o.step(140)
+    dg, do = sim.dose().cpu().numpy().astype(np.float64), o.dose()
+    assert (do > 0).sum() == 1 and np.array_equal(dg > 0, do > 0)
+    assert abs(dg[do > 0][0] / do[do > 0][0] - 1) < 1e-6
+    with pytest.raises(lpm.LpmError):
+        lpm.Simulation(w).dose()                        # params.dose = 0: call-order error, not zeros
+
+    w = make("c3", scale=1.0, n_steps=1440)
+    w.release.pid_stride = 250                           # 40000 of the 1e7 particles
+    w = w.replace(nt=6, capacity=40_000, bin_every=120)
+    sim, o = lpm.Simulation(w, dose=True), orc.OracleSim(w)
+    o.enable_dose()
+    sim.step(1440)
+    o.step(1440)
+    dg, do = sim.dose().cpu().numpy().astype(np.float64), o.dose()
+    for k in range(2):
+        assert abs(dg[k].sum() / do[k].sum() - 1) < 1e-5
+    # cell by cell: a particle within the position tolerance of a face may sit in the neighbour cell on one side,
+    # so compare the 2 x 2 x 2 coarsened field where the cloud is dense
+    def coarse(a):
+        K, nz, ny, nx = a.shape
+        return a[:, :nz // 2 * 2, :ny // 2 * 2, :nx // 2 * 2].reshape(K, nz // 2, 2, ny // 2, 2, nx // 2, 2).sum(axis=(2, 4, 6))
+    cg, co = coarse(dg), coarse(do)
+    dense = co > 0.02 * co.max()
+    assert dense.sum() > 20 and np.abs(cg[dense] / co[dense] - 1).max() < 5e-3
+
+
 # ------------------------------------------------------------------ a7: compaction (config 5 shape)
 def test_c5_compaction_small(lpm, orc):
     """1/100-scale-class C5: ABSORB + stable compaction each step, rate-mode injection with a
