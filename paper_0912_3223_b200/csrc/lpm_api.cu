@@ -27,7 +27,7 @@ struct Release {
 };
 
 struct Layout {
-    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, blend, keys, perm, hist, partial, alt_xyzq, alt_q1, alt_pid, dose, total;
+    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, blend, keys, perm, hist, partial, alt_xyzq, alt_q1, alt_pid, dose, mask, total;
 };
 
 uint64_t up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
@@ -59,6 +59,7 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     L.alt_xyzq = o; o += sort && compact ? up(16 * cap) : 0;           //   compact store: the records themselves are sorted,
     L.alt_q1 = o; o += sort && compact && K > 1 ? up(4 * cap) : 0;     //   through these alternate buffers
     L.alt_pid = o; o += sort && compact ? up(4 * cap) : 0;
+    L.mask = o; o += up((uint64_t)((met.grid.nx + kMaskTile - 1) / kMaskTile) * ((met.grid.ny + kMaskTile - 1) / kMaskTile));  // plume mask tiles
     L.dose = o; o += dose ? up(8 * cells3 * K) : 0;                    // time-integrated concentration (S 8(f)3)
     L.total = o;
     return L;
@@ -127,7 +128,7 @@ struct lpm_handle {
     uint64_t keys_n, keys_step;
     bool keys_ready;
     uint64_t csort_step;  // compact store: step of the last physical sort
-    bool bbox_valid;      // ctrl[20..21] holds the met-column box of the particles as the last step launch left them
+    bool bbox_valid;      // the mask tiles hold the met columns of the particles as the last step launch left them
     double dep_bound[LPM_MAX_NUCLIDES];  // largest activity a particle can carry (fixed-point scale of the deposit tables)
     bool binned;
     int sms, occ;
@@ -368,7 +369,7 @@ int ensure_blend(lpm_handle *h, StepArgs &A, int m, int m_max)
     const int sn = A.tab[0].snap & 0xffff;
     if (sn != h->pair_snap) {
         CK(launch_pair_repack(met + (uint64_t)sn * A.snap_cells, met + (uint64_t)(sn + 1) * A.snap_cells, h->ws + h->L.pair,
-                              g.nx, g.ny, g.nz, (uint32_t *)(A.ctrl + 20) + 4, h->st));
+                              g.nx, g.ny, g.nz, (uint32_t *)(A.ctrl + 22), h->st));
         h->launches++;
         h->pair_snap = sn;
         h->blend_n = 0;
@@ -387,7 +388,8 @@ int ensure_blend(lpm_handle *h, StepArgs &A, int m, int m_max)
         }
         // plume box: columns reachable within the cnt steps these buffers serve (B6)
         BlendBox box{};
-        box.bb = h->bbox_valid ? (const uint32_t *)(A.ctrl + 20) : nullptr;
+        box.flags = h->bbox_valid ? (const uint8_t *)(h->ws + h->L.mask) : nullptr;
+        box.uvmax = (const uint32_t *)(A.ctrl + 22);
         box.nx = g.nx; box.ny = g.ny; box.nz = g.nz;
         const double walk = 5.768 * (double)h->sigma_h * 1.0001;
         box.reach_x = (float)((double)cnt * h->prm.dt / g.dx * 1.0001); box.reach_y = (float)((double)cnt * h->prm.dt / g.dy * 1.0001);
@@ -585,12 +587,13 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
             const int rc = ensure_blend(h, A, m, m_max);
             if (rc) return rc;
         }
-        A.bbox = nullptr;
+        A.mask = nullptr;
         if (h->met.nt > 1 && h->step + (uint64_t)m >= h->blend_step0 + (uint64_t)h->blend_n) {
-            // the next launch blends again: the step launches below leave the met-column box of their particles
-            CK(cudaMemsetAsync(A.ctrl + 20, 0xff, 8, h->st));  // {i_min, j_min} = 0xffffffff
-            CK(cudaMemsetAsync(A.ctrl + 21, 0, 8, h->st));     // {i_max, j_max} = 0
-            A.bbox = (uint32_t *)(A.ctrl + 20);
+            // the next launch blends again: the step launches below flag the mask tiles that hold their particles
+            const int ntx = (h->met.grid.nx + kMaskTile - 1) / kMaskTile, nty = (h->met.grid.ny + kMaskTile - 1) / kMaskTile;
+            CK(cudaMemsetAsync(h->ws + h->L.mask, 0, (size_t)ntx * nty, h->st));
+            A.mask = (uint8_t *)(h->ws + h->L.mask);
+            A.mask_ntx = ntx;
             h->bbox_valid = true;
         } else if (h->met.nt > 1) {
             h->bbox_valid = false;  // (cannot happen before a blend: kept for safety when the coverage logic changes)

@@ -77,7 +77,8 @@ struct StepArgs {
     uint64_t base, n, n_prev;  // slots >= n_prev are born inside this launch
     const uint32_t *perm;      // gather-locality pass: slots [0, n_perm) listed in dual-cell order, or null
     uint64_t n_perm;           // slots [n_perm, n) are walked in slot order
-    uint32_t *bbox;            // {i_min, j_min, i_max, j_max} of the met columns of the particles at the end of the launch (atomics)
+    uint8_t *mask;             // non-null: flag the mask tile of each particle's met column at the end of the launch
+    int32_t mask_ntx, pad2_;
     uint32_t *keys_out, *hist_out;  // non-null: the launch before a sort leaves each slot's dual-cell key and the histogram
     uint32_t n_keys, pad1_;
     uint64_t pid_offset, pid_stride;
@@ -139,12 +140,16 @@ cudaError_t run_probe(int kind, uint64_t footprint_bytes, void *scratch_dev, uin
                       cudaStream_t st);
 cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, uint32_t *uvmax, cudaStream_t st);
 cudaError_t launch_transpose(const float4 *s0, float4 *out, int nx, int ny, int nz, cudaStream_t st);
-// plume bounding box (a0): blend only the met columns a particle can reach during the coming launch
+// plume mask (a0): blend only the met columns a particle can reach during the coming launch.  The met
+// columns are grouped in tiles of kMaskTile x kMaskTile; the step kernel flags the tiles that hold a
+// particle, the blend kernel processes a tile if a flagged tile (or a source) lies within reach.
+constexpr int kMaskTile = 8;
 struct BlendBox {
-    const uint32_t *bb;   // device: {i_min, j_min, i_max, j_max} of the particles' met columns, {|u|max, |v|max} float bits; null = whole field
+    const uint8_t *flags;   // device: one byte per tile [nty][ntx], != 0 = holds a particle; null = whole field
+    const uint32_t *uvmax;  // device: {|u|max, |v|max} of the current met interval, float bits
     int32_t nx, ny, nz;
-    float reach_x, reach_y;    // cells per (m/s) of wind:  steps * dt / dx
-    float walk_x, walk_y;      // cells of random walk: steps * 5.768 sigma_h / dx  (|N(0,1)| <= sqrt(48 ln 2) by construction, R3)
+    float reach_x, reach_y;    // columns per (m/s) of wind:  steps * dt / dx
+    float walk_x, walk_y;      // columns of random walk: steps * 5.768 sigma_h / dx  (|N(0,1)| <= sqrt(48 ln 2) by construction, R3)
     int32_t n_src;
     int32_t src_i[LPM_MAX_RELEASES], src_j[LPM_MAX_RELEASES];   // source columns (newborn particles)
 };

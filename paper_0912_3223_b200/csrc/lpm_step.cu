@@ -306,18 +306,11 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             A.xyzq[slot] = make_float4(x, y, z, q[0]);
             if (K > 1) A.q1[slot] = q[1];
         }
-        if (A.bbox) {
-            // met columns of the particles at the end of the launch -> plume box of the next blend
-            const bool live = valid && z >= 0.0f;
+        if (A.mask && valid && z >= 0.0f) {
+            // tile of the particle's met column at the end of the launch -> plume mask of the next blend
             const int ci = min(max(__float2int_rd((x - A.mg.x0) * A.mg.inv_dx), 0), A.mg.nx - 1);
             const int cj = min(max(__float2int_rd((y - A.mg.y0) * A.mg.inv_dy), 0), A.mg.ny - 1);
-            const uint32_t i0 = __reduce_min_sync(0xffffffffu, live ? (uint32_t)ci : 0xffffffffu);
-            const uint32_t i1 = __reduce_max_sync(0xffffffffu, live ? (uint32_t)ci : 0u);
-            const uint32_t j0 = __reduce_min_sync(0xffffffffu, live ? (uint32_t)cj : 0xffffffffu);
-            const uint32_t j1 = __reduce_max_sync(0xffffffffu, live ? (uint32_t)cj : 0u);
-            if ((threadIdx.x & 31) == 0 && i0 != 0xffffffffu) {
-                atomicMin(A.bbox, i0); atomicMin(A.bbox + 1, j0); atomicMax(A.bbox + 2, i1); atomicMax(A.bbox + 3, j1);
-            }
+            A.mask[(cj / kMaskTile) * A.mask_ntx + ci / kMaskTile] = 1;
         }
         if (A.keys_out && in_range) {
             // pass 1 of the coming gather-locality sort, for free: the new position is in registers
@@ -462,21 +455,15 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
                 A.pid[dst] = pid[j];
             }
         }
-        if (A.bbox) {
-            // met columns of the survivors -> plume box of the next blend
-            uint32_t i0 = 0xffffffffu, i1 = 0u, j0 = 0xffffffffu, j1 = 0u;
+        if (A.mask) {
+            // tiles of the survivors' met columns -> plume mask of the next blend
 #pragma unroll
             for (int j = 0; j < kItems; ++j) {
                 if (alive[j]) {
-                    const uint32_t ci = (uint32_t)min(max(__float2int_rd((x[j] - A.mg.x0) * A.mg.inv_dx), 0), A.mg.nx - 1);
-                    const uint32_t cj = (uint32_t)min(max(__float2int_rd((y[j] - A.mg.y0) * A.mg.inv_dy), 0), A.mg.ny - 1);
-                    i0 = min(i0, ci); i1 = max(i1, ci); j0 = min(j0, cj); j1 = max(j1, cj);
+                    const int ci = min(max(__float2int_rd((x[j] - A.mg.x0) * A.mg.inv_dx), 0), A.mg.nx - 1);
+                    const int cj = min(max(__float2int_rd((y[j] - A.mg.y0) * A.mg.inv_dy), 0), A.mg.ny - 1);
+                    A.mask[(cj / kMaskTile) * A.mask_ntx + ci / kMaskTile] = 1;
                 }
-            }
-            i0 = __reduce_min_sync(0xffffffffu, i0); i1 = __reduce_max_sync(0xffffffffu, i1);
-            j0 = __reduce_min_sync(0xffffffffu, j0); j1 = __reduce_max_sync(0xffffffffu, j1);
-            if (lane == 0 && i0 != 0xffffffffu) {
-                atomicMin(A.bbox, i0); atomicMin(A.bbox + 1, j0); atomicMax(A.bbox + 2, i1); atomicMax(A.bbox + 3, j1);
             }
         }
         if (A.any_dep) dep_flush<K>(A, T);  // every thread's step is behind the barrier above
@@ -624,39 +611,54 @@ struct BlendArgs {
     BlendBox box;
 };
 
-// Only the columns a particle can reach are blended: the box of the particles' columns at the end of
-// the previous launch (accumulated by the step kernel), widened by the largest possible displacement
-// of the coming steps, (|u|max dt + 5.768 sigma_h) per step (trilinear values are convex combinations
-// of texels, |N(0,1)| <= 5.768 by R3), + 2 columns for the stencil, united with the source columns.
+// Only the columns a particle can reach are blended: a tile of 8 x 8 met columns is processed if a
+// tile flagged by the step kernel (a particle sat there at the end of the previous launch) or a
+// source column lies within the largest possible displacement of the coming steps,
+// (|u|max dt + 5.768 sigma_h) per step (trilinear values are convex combinations of texels,
+// |N(0,1)| <= 5.768 by R3), + 2 columns for the stencil, measured in whole tiles (rounded up).
 __global__ void __launch_bounds__(256) blend_kernel(const __grid_constant__ BlendArgs B)
 {
-    int i_lo = 0, i_hi = B.box.nx - 1, j_lo = 0, j_hi = B.box.ny - 1;
-    if (B.box.bb) {
-        const float um = __uint_as_float(B.box.bb[4]), vm = __uint_as_float(B.box.bb[5]);
+    const int nx = B.box.nx, ny = B.box.ny, ntx = (nx + kMaskTile - 1) / kMaskTile, nty = (ny + kMaskTile - 1) / kMaskTile;
+    int mtx = 0, mty = 0;
+    bool all = B.box.flags == nullptr;
+    if (!all) {
+        const float um = __uint_as_float(B.box.uvmax[0]), vm = __uint_as_float(B.box.uvmax[1]);
         const int mx = (int)ceilf(um * B.box.reach_x + B.box.walk_x) + 2, my = (int)ceilf(vm * B.box.reach_y + B.box.walk_y) + 2;
-        int a0 = (int)min(B.box.bb[0], 0x3fffffffu), b0 = (int)min(B.box.bb[1], 0x3fffffffu), a1 = (int)B.box.bb[2], b1 = (int)B.box.bb[3];
-        if (a0 > a1) { a0 = 0x3fffffff; a1 = -1; b0 = 0x3fffffff; b1 = -1; }   // no particle yet
-        for (int r = 0; r < B.box.n_src; ++r) {
-            a0 = min(a0, B.box.src_i[r]); a1 = max(a1, B.box.src_i[r]);
-            b0 = min(b0, B.box.src_j[r]); b1 = max(b1, B.box.src_j[r]);
-        }
-        if (a0 > a1) return;   // nothing can be sampled
-        i_lo = max(a0 - mx, 0); i_hi = min(a1 + mx, B.box.nx - 1);
-        j_lo = max(b0 - my, 0); j_hi = min(b1 + my, B.box.ny - 1);
+        mtx = (mx + kMaskTile - 1) / kMaskTile;
+        mty = (my + kMaskTile - 1) / kMaskTile;
+        if ((2 * mtx + 1) * (2 * mty + 1) > 1024) all = true;   // reach of the order of the domain: no point in masking
     }
-    const uint32_t W = (uint32_t)(i_hi - i_lo + 1), nz = (uint32_t)B.box.nz;
-    const uint64_t total = (uint64_t)W * (uint32_t)(j_hi - j_lo + 1) * nz;
-    for (uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (uint64_t)gridDim.x * blockDim.x) {
-        const uint64_t c = t / nz;
-        const uint32_t k = (uint32_t)(t - c * nz);
-        const uint32_t jj = (uint32_t)(c / W), ii = (uint32_t)(c - (uint64_t)jj * W);
-        const uint64_t o = ((uint64_t)(j_lo + jj) * (uint32_t)B.box.nx + (uint32_t)(i_lo + ii)) * nz + k;
-        Texel2 tx;
-        asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-            : "=f"(tx.a.x), "=f"(tx.a.y), "=f"(tx.a.z), "=f"(tx.a.w), "=f"(tx.b.x), "=f"(tx.b.y), "=f"(tx.b.z), "=f"(tx.b.w)
-            : "l"(B.pair + o));
+    const uint32_t nz = (uint32_t)B.box.nz;
+    constexpr int kParts = 4;   // blocks per tile (rows jj = part, part + kParts, ...): enough CTAs on small grids
+    for (int item = blockIdx.x; item < ntx * nty * kParts; item += gridDim.x) {
+        const int tile = item / kParts, part = item % kParts;
+        const int ti = tile % ntx, tj = tile / ntx;
+        if (!all) {
+            int hit = 0;
+            const int w = 2 * mtx + 1, nn = w * (2 * mty + 1);
+            for (int t = threadIdx.x; t < nn; t += blockDim.x) {
+                const int a = ti + t % w - mtx, b = tj + t / w - mty;
+                if (a >= 0 && a < ntx && b >= 0 && b < nty && B.box.flags[b * ntx + a]) hit = 1;
+            }
+            if (threadIdx.x < B.box.n_src) {
+                const int a = B.box.src_i[threadIdx.x] / kMaskTile, b = B.box.src_j[threadIdx.x] / kMaskTile;
+                if (abs(a - ti) <= mtx && abs(b - tj) <= mty) hit = 1;
+            }
+            if (!__syncthreads_or(hit)) continue;
+        }
+        const uint32_t i0 = (uint32_t)(ti * kMaskTile), j0 = (uint32_t)(tj * kMaskTile);
+        const uint32_t w = min((uint32_t)kMaskTile, (uint32_t)nx - i0), h = min((uint32_t)kMaskTile, (uint32_t)ny - j0);
+        const uint32_t row = w * nz;   // the w columns of a tile row are contiguous (z fastest, then x)
+        for (uint32_t jj = (uint32_t)part; jj < h; jj += kParts)
+        for (uint32_t r = threadIdx.x; r < row; r += blockDim.x) {
+            const uint64_t o = ((uint64_t)(j0 + jj) * (uint32_t)nx + i0) * nz + r;
+            Texel2 tx;
+            asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                : "=f"(tx.a.x), "=f"(tx.a.y), "=f"(tx.a.z), "=f"(tx.a.w), "=f"(tx.b.x), "=f"(tx.b.y), "=f"(tx.b.z), "=f"(tx.b.w)
+                : "l"(B.pair + o));
 #pragma unroll 4
-        for (int s = 0; s < B.m; ++s) B.out[(uint64_t)s * B.cells + o] = lerp4(tx.a, tx.b, B.a[s]);
+            for (int s = 0; s < B.m; ++s) B.out[(uint64_t)s * B.cells + o] = lerp4(tx.a, tx.b, B.a[s]);
+        }
     }
 }
 
@@ -666,8 +668,8 @@ cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, c
     B.pair = (const Texel2 *)pair; B.out = out; B.cells = cells; B.m = m;
     for (int s = 0; s < kBlendDepth; ++s) B.a[s] = s < m ? a[s] : 0.0f;
     B.box = *box;
-    const uint64_t want = (cells + 255) / 256;
-    blend_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(B);
+    const int tiles = ((box->nx + kMaskTile - 1) / kMaskTile) * ((box->ny + kMaskTile - 1) / kMaskTile);
+    blend_kernel<<<tiles * 4 < 148 * 8 ? tiles * 4 : 148 * 8, 256, 0, st>>>(B);
     return cudaGetLastError();
 }
 
