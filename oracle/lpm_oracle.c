@@ -55,6 +55,8 @@ typedef struct {
     double rx0, rx1, ry0, ry1, rt0, rt1; /* rain box (R8/G6)                                  */
     double frag_delta;     /* metres: distance to a discontinuity that flags a particle fragile */
     double face_delta;     /* metres: distance to a deposition-map cell face counted as slack   */
+    int32_t dep_mode;      /* 0: expected-mass deposition (R8); 1: paper-literal Bernoulli deposition (R11) */
+    int32_t pad2_;
 } orc_config;
 
 typedef struct {
@@ -433,6 +435,32 @@ static void step_particle(orc_sim *s, uint64_t i, uint64_t n, double t_n, int ra
         if (near_x || near_y) s->fragile[i] = 1;
     }
     int any = 0;
+    if (c->dep_mode == 1) {
+        /* R11, the paper's own form ("deposition ... considered stochastic", L114 "testing for
+         * dry and wet depositions", L108 a deposited particle becomes inactive): one Bernoulli trial per
+         * nuclide and sink per step, from Philox stream 1 of the same (seed, id, step): word k decides dry,
+         * word 2 + k decides wet deposition of nuclide k; u = (word >> 8) 2^-24 in [0, 1), event iff u < p
+         * (p the fp32 parameter of R8; the comparison is exact on both sides).  The event deposits the
+         * nuclide's WHOLE activity at the new (x, y); dry is tried first, wet only if dry did not fire. */
+        uint32_t r1[4];
+        orc_philox_draw(c->seed, s->pid[i], n, 1u, r1);
+        const double sc = 1.0 / 16777216.0;
+        for (int k = 0; k < c->K; ++k) {
+            double m = s->m[k][i], dd = 0.0, dw = 0.0;
+            if (m > 0.0) {
+                double ud = (double)(r1[k] >> 8) * sc, uw = (double)(r1[2 + k] >> 8) * sc;
+                if (eligible && ud < (double)s->p_dry[k]) { dd = m; m = 0.0; }
+                else if (wet && uw < (double)s->p_wet[k]) { dw = m; m = 0.0; }
+            }
+            double mn = m * s->f_decay[k];
+            s->inc_dry[k][i] = dd; s->inc_wet[k][i] = dw; s->inc_dec[k][i] = m - mn;
+            s->m[k][i] = mn;
+            if (dd != 0.0 || dw != 0.0) any = 1;
+        }
+        int empty = 1;
+        for (int k = 0; k < c->K; ++k) if (s->m[k][i] > 0.0) empty = 0;
+        if (empty) s->status[i] = 2; /* deposited: inactive from now on (L108) */
+    } else
     for (int k = 0; k < c->K; ++k) {
         double m = s->m[k][i];
         double dd = eligible ? m * (double)s->p_dry[k] : 0.0;
@@ -519,6 +547,7 @@ int32_t orc_step(orc_sim *s, int32_t n_steps)
                 for (int k = 0; k < c->K; ++k) { s->ledger[k][5] += s->m[k][i]; s->m[k][i] = 0.0; }
                 continue;
             }
+            /* status 2 (deposited in this step, R11) falls through: its increments are booked below */
             for (int k = 0; k < c->K; ++k) {
                 double d = s->inc_dry[k][i] + s->inc_wet[k][i];
                 s->ledger[k][2] += s->inc_dry[k][i];

@@ -44,7 +44,8 @@ class Config(C.Structure):
                 ("bin_every", C.c_int32), ("rain_on", C.c_int32),
                 ("rx0", C.c_double), ("rx1", C.c_double), ("ry0", C.c_double), ("ry1", C.c_double),
                 ("rt0", C.c_double), ("rt1", C.c_double),
-                ("frag_delta", C.c_double), ("face_delta", C.c_double)]
+                ("frag_delta", C.c_double), ("face_delta", C.c_double),
+                ("dep_mode", C.c_int32), ("pad2_", C.c_int32)]
 
 
 class Source(C.Structure):
@@ -164,7 +165,8 @@ def cell_index(p, p0, dp, n):
 class OracleSim:
     """The fp64 oracle run of a `workloads.Workload`."""
 
-    def __init__(self, w, frag_delta: float = 0.05, face_delta: float = 0.0, bin_every: Optional[int] = None):
+    def __init__(self, w, frag_delta: float = 0.05, face_delta: float = 0.0, bin_every: Optional[int] = None,
+                 dep_mode: int = 0):
         self.w = w
         self.K = w.K
         self._fields = np.ascontiguousarray(w.fields(), dtype=np.float32)
@@ -186,6 +188,7 @@ class OracleSim:
             cfg.rx0, cfg.rx1, cfg.ry0, cfg.ry1 = w.rain.x0, w.rain.x1, w.rain.y0, w.rain.y1
             cfg.rt0, cfg.rt1 = w.rain.t_start, w.rain.t_end
         cfg.frag_delta, cfg.face_delta = frag_delta, face_delta
+        cfg.dep_mode = dep_mode
         self._cfg = cfg
         self._h = lib().orc_create(C.byref(cfg))
         if not self._h:

@@ -352,3 +352,67 @@ def test_dose_of_a_resting_decaying_cloud_is_a_geometric_series():
         o2.step(be)
         acc += o2.concentration() * Tb
     np.testing.assert_allclose(d, acc, rtol=1e-13, atol=0)
+
+
+# ------------------------------------------------------------------ P16: Bernoulli deposition (S§8(f)1, R11)
+def test_bernoulli_deposition_survival_law_and_ledger():
+    """Uniform dry deposition as a per-step Bernoulli trial: survivors ~ Binomial(N, (1-p)^n); a deposited
+    particle drops its whole (decayed) activity once; emitted = airborne + dry + decayed exactly."""
+    N, n, dt, H = 20000, 12, 10.0, 100.0
+    w = custom(uniform_met(u=1.0, kz=1.0), n=N, nuclides=[Nuclide("X", 5000.0, vd=1.0)], dt=dt, Kh=10.0, H=H, h_dep=H,
+               activity=[float(N)], n_steps=n, src=(0.0, 0.0, 50.0))
+    o = orc.OracleSim(w, dep_mode=1)
+    o.step(n)
+    p = float(o.p_dry(0))
+    assert abs(p - (1 - math.exp(-1.0 * dt / H))) < 1e-7
+    st = o.particles()["status"]
+    surv = int((st == 0).sum())
+    q = (1 - p) ** n
+    assert abs(surv - N * q) < 4 * math.sqrt(N * q * (1 - q))
+    assert set(np.unique(st)) <= {0, 2}
+    led = o.ledger()[0]
+    assert abs((led[1] + led[2] + led[4]) / led[0] - 1) < 1e-12 and led[3] == 0 and led[5] == 0
+    # every deposit is one whole particle: dry ledger = sum over deposited particles of 2^(-t_dep/T)
+    assert led[2] < (N - surv) * 1.0 and led[2] > (N - surv) * 2.0 ** (-n * dt / 5000.0)
+    dep = o.deposition()
+    g = w.cgrid
+    assert abs(dep.sum() * g.dx * g.dy + led[6] - led[2]) < 1e-9 * led[2]
+
+
+def test_bernoulli_deposition_replays_from_the_draws():
+    """Independent replay: the step at which nuclide k of particle j deposits follows from Philox stream 1
+    alone when every particle is eligible (uniform dry, rain everywhere): first step with u_dry < p_dry, else
+    u_wet < p_wet."""
+    n, steps = 60, 30
+    nuc = [Nuclide("A", 0.0, vd=0.5, lambda_wet=2.0e-3), Nuclide("B", 0.0, vd=0.2, lambda_wet=8.0e-3)]
+    w = custom(uniform_met(), n=n, nuclides=nuc, dt=10.0, H=100.0, h_dep=100.0, activity=[float(n), 2.0 * n], n_steps=steps,
+               rain=RainBox(-1e9, 1e9, -1e9, 1e9, 0.0, 1e9), seed=77)
+    o = orc.OracleSim(w, dep_mode=1)
+    o.step(steps)
+    m = o.particles()["m"]
+    pd = [float(o.p_dry(k)) for k in range(2)]
+    pw = [float(o.p_wet(k)) for k in range(2)]
+    dry = np.zeros(2)
+    wet = np.zeros(2)
+    for j in range(n):
+        for k in range(2):
+            gone = None
+            for s in range(steps):
+                r = orc.philox_draw(77, j, s, 1)
+                ud, uw = (int(r[k]) >> 8) / 2.0 ** 24, (int(r[2 + k]) >> 8) / 2.0 ** 24
+                if ud < pd[k]:
+                    gone = "d"
+                    break
+                if uw < pw[k]:
+                    gone = "w"
+                    break
+            a = 1.0 if k == 0 else 2.0
+            if gone is None:
+                assert m[k][j] == a
+            else:
+                assert m[k][j] == 0.0
+                (dry if gone == "d" else wet)[k] += a
+    led = o.ledger()
+    for k in range(2):
+        assert led[k][2] == pytest.approx(dry[k], rel=1e-14) and led[k][3] == pytest.approx(wet[k], rel=1e-14)
+    assert dry.sum() > 0 and wet.sum() > 0
