@@ -245,7 +245,7 @@ def run_ours(args):
 
     # ---------------- leg 1: inputs resident in HBM ----------------
     fields_dev = fields_host.to("cuda", non_blocking=True)
-    sim = lpm.Simulation(w, fields_dev=fields_dev)
+    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode)
     conc_dev = torch.empty((w.K, g.nz, g.ny, g.nx), dtype=torch.float32, device="cuda")
     dep_dev = torch.empty((w.K, g.ny, g.nx), dtype=torch.float32, device="cuda")
     for _ in range(W):
@@ -286,7 +286,7 @@ def run_ours(args):
 
     # ---------------- leg 2: end to end through the host-buffer C-ABI calls ----------------
     fields_dev.zero_()
-    sim = lpm.Simulation(w, fields_dev=fields_dev)
+    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode)
     sim.upload_meteo(0, fields_host[0:1])
     uploaded = 0
     h2d = d2h = 0
@@ -409,7 +409,7 @@ def run_ours(args):
         "config": {"workload": f"{args.workload} (BASELINE.json configs[{ {'c1': 0, 'c2': 1, 'c3': 2, 'c3_hdep80': 2, 'c4': 3, 'c5': 4}[args.workload] }])",
                    "particles_per_gpu": w.capacity, "nuclides": w.K, "model_steps_per_bench_step": interval, "dt_s": w.dt,
                    "conc_grid": [g.nx, g.ny, g.nz], "met_grid": [w.mgrid.nx, w.mgrid.ny, w.mgrid.nz], "met_snapshots": w.nt,
-                   "scale": args.scale, "l2": "particle store larger than L2, no flush" if w.capacity * state_bytes > 126e6 else "inputs fit L2 (small config)",
+                   "scale": args.scale, "dep_mode": args.dep_mode, "l2": "particle store larger than L2, no flush" if w.capacity * state_bytes > 126e6 else "inputs fit L2 (small config)",
                    "parallelism": f"pid-strided ensemble x{world}, grids all-reduced per output" if world > 1 else "single GPU"},
         "sim_hours_per_s": sim_hours / (ms * 1e-3),
         "e2e": {"value": units / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
@@ -453,6 +453,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--workload", default="c4", choices=("c1", "c2", "c3", "c3_hdep80", "c4", "c5"))
     ap.add_argument("--scale", type=float, default=1.0, help="particle-count scale of the workload (1.0 = BASELINE size)")
+    ap.add_argument("--dep-mode", type=int, default=0, choices=(0, 1), help="0 expected-mass deposition (default), 1 Bernoulli deposition (S 8(f)1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probes", action="store_true", help="skip the lpm_probe micro-benchmarks (measured peaks)")
     args = ap.parse_args()

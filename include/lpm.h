@@ -49,6 +49,7 @@ typedef enum {
 } lpm_status;
 
 typedef enum { LPM_BOUNDARY_OPEN = 0, LPM_BOUNDARY_ABSORB = 1 } lpm_boundary_mode;
+typedef enum { LPM_DEP_EXPECTED = 0, LPM_DEP_BERNOULLI = 1 } lpm_dep_mode;
 
 /* Regular grid of nx*ny*nz cells of size dx*dy*dz with lower corner (x0, y0, z0). */
 typedef struct {
@@ -94,6 +95,12 @@ typedef struct {
                                * the store is then in met-cell order, not in id order.             */
     int32_t dose;             /* 1: accumulate the time-integrated concentration (Fig. 2b "time
                                * integrated dosage") at every cadence binning; read with lpm_dose        */
+    int32_t dep_mode;         /* lpm_dep_mode: 0 expected-mass deposition (every step removes the fraction p
+                               * of the activity), 1 the paper's stochastic form: one
+                               * Bernoulli trial per nuclide and sink per step from Philox stream 1, an
+                               * event deposits the nuclide's whole activity once; a particle that
+                               * carries nothing any more becomes inactive (status 2)                */
+    int32_t reserved;
 } lpm_params;
 
 typedef struct {
@@ -184,7 +191,8 @@ int32_t lpm_step_index(lpm_handle *h, uint64_t *step_host);
  * G_k(t) the host-side fp64 decay (and uniform dry-deposition) factor at the current step (R8). */
 int32_t lpm_mass_scale(lpm_handle *h, double *scale_host /* [K] */);
 /* Copy out the particle state: xyzq_dev float4 (x, y, z, q0) per slot, q1_dev (K = 2, may be
- * NULL), pid_dev uint32 (may be NULL), status_dev uint8 0 = active, 1 = exited (may be NULL).
+ * NULL), pid_dev uint32 (may be NULL), status_dev uint8 0 = active, 1 = exited, 2 = deposited all it carried
+ * (dep_mode 1) (may be NULL).
  * Buffers must hold capacity entries; *n_host receives the slot count.  Exited particles report
  * their exit position. */
 int32_t lpm_get_particles(lpm_handle *h, void *xyzq_dev, float *q1_dev, uint32_t *pid_dev,

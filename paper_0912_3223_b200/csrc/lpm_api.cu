@@ -267,7 +267,8 @@ void base_args(const lpm_handle *h, StepArgs &A)
     A.cg = gridf(h->cg);
     A.dep = (double *)(h->ws + h->L.dep);
     A.dep_stride = (uint64_t)h->cg.nx * h->cg.ny;
-    A.any_dep = (h->dry_mode != kDryNone || h->rain_on) ? 1 : 0;
+    A.bern = h->prm.dep_mode == 1 ? 1 : 0;
+    A.any_dep = (!A.bern && (h->dry_mode != kDryNone || h->rain_on)) ? 1 : 0;
     for (int w = 0; w < 2 * LPM_MAX_NUCLIDES; ++w) {
         // S = largest power of two <= 2^20 / (largest possible increment): activity <= dep_bound, one step
         // deposits at most the fraction p_dry (dry) or p_wet (wet) of it.  Only efficiency depends on the
@@ -458,7 +459,8 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     if (met->nt < 1 || met->nt > 32767 || !met->fields_dev || ((uintptr_t)met->fields_dev & 15) || ((uintptr_t)ws & 255))
         return LPM_ERR_INVALID_ARG;
     if (!(p->dt > 0) || p->capacity == 0 || p->capacity >= (1ull << 32) || !(met->H_mix > 0) || met->Kh < 0 ||
-        (met->nt > 1 && !(met->dt_snap > 0)) || p->bin_every < 0 || p->steps_per_launch < 0 || !(p->h_dep > 0))
+        (met->nt > 1 && !(met->dt_snap > 0)) || p->bin_every < 0 || p->steps_per_launch < 0 || !(p->h_dep > 0) || p->dep_mode < 0 ||
+        p->dep_mode > 1)
         return LPM_ERR_INVALID_ARG;
     int ndev = 0, dev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return LPM_ERR_NO_DEVICE;
@@ -481,7 +483,9 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     h->pair_snap = -1;
     // R5 / R8 constants: double formula, rounded once to fp32 where the kernels consume fp32
     h->sigma_h = (float)sqrt(2.0 * met->Kh * p->dt);
-    const bool uniform = p->h_dep >= met->H_mix;
+    // uniform dry deposition folds into the scalar G only in the expected-mass form; Bernoulli trials (R11) are per particle
+    const bool eligible_everywhere = p->h_dep >= met->H_mix;
+    const bool uniform = eligible_everywhere && p->dep_mode != 1;
     bool any_dry = false;
     for (int k = 0; k < K; ++k) {
         h->p_dry[k] = nuc[k].vd > 0 ? (float)(-expm1(-nuc[k].vd * p->dt / p->h_dep)) : 0.0f;
@@ -494,8 +498,8 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         h->dec_scale[k] = -expm1(-lam_dt) * keep_dry;
         h->wet_scale[k] = keep_dry * (double)h->p_wet[k];
     }
-    h->dry_mode = !any_dry ? kDryNone : (uniform ? kDryUniform : kDryLayer);
-    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode);
+    h->dry_mode = !any_dry ? kDryNone : (eligible_everywhere ? kDryUniform : kDryLayer);
+    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode, p->dep_mode == 1);
     if (cudaMemsetAsync(ws, 0, L.total, h->st) != cudaSuccess) { delete h; return LPM_ERR_CUDA; }
     h->launches++;
     *out = h;
@@ -812,7 +816,7 @@ int32_t lpm_get_particles(lpm_handle *h, void *xyzq, float *q1, uint32_t *pid, u
     *n_host = n;
     if (!n) return LPM_OK;
     if (xyzq || status) {
-        CK(launch_export((const float4 *)(h->ws + h->L.xyzq), n, nullptr, (float4 *)xyzq, status, h->st));
+        CK(launch_export((const float4 *)(h->ws + h->L.xyzq), h->K > 1 ? (const float *)(h->ws + h->L.q1) : nullptr, n, nullptr, (float4 *)xyzq, status, h->st));
         h->launches++;
     }
     if (q1 && h->K > 1) CK(cudaMemcpyAsync(q1, h->ws + h->L.q1, 4 * n, cudaMemcpyDeviceToDevice, h->st));

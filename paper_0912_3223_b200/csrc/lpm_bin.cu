@@ -145,21 +145,23 @@ cudaError_t launch_airborne(const float4 *xyzq, const float *q1, uint64_t n, con
 }
 
 // export: decode the in-band exit marker (z' = -1 - z) into a status byte
-__global__ void export_kernel(const float4 *__restrict__ xyzq, uint64_t n_host, const uint64_t *n_dev, float4 *out, uint8_t *status)
+// status 1 = left the domain (ABSORB), 2 = deposited everything it carried (Bernoulli deposition, R11)
+__global__ void export_kernel(const float4 *__restrict__ xyzq, const float *__restrict__ q1, uint64_t n_host, const uint64_t *n_dev, float4 *out,
+                              uint8_t *status)
 {
     const uint64_t n = n_dev ? *n_dev : n_host;
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
         float4 p = xyzq[i];
         uint8_t s = 0;
-        if (p.z < 0.0f) { p.z = -1.0f - p.z; s = 1; }
+        if (p.z < 0.0f) { p.z = -1.0f - p.z; s = (p.w == 0.0f && (!q1 || q1[i] == 0.0f)) ? 2 : 1; }
         if (out) out[i] = p;
         if (status) status[i] = s;
     }
 }
 
-cudaError_t launch_export(const float4 *xyzq, uint64_t n, const uint64_t *n_dev, float4 *out, uint8_t *status, cudaStream_t st)
+cudaError_t launch_export(const float4 *xyzq, const float *q1, uint64_t n, const uint64_t *n_dev, float4 *out, uint8_t *status, cudaStream_t st)
 {
-    export_kernel<<<148 * 4, 256, 0, st>>>(xyzq, n, n_dev, out, status);
+    export_kernel<<<148 * 4, 256, 0, st>>>(xyzq, q1, n, n_dev, out, status);
     return cudaGetLastError();
 }
 

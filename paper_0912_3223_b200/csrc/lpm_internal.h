@@ -60,7 +60,7 @@ struct StepArgs {
     uint64_t dep_stride;
     float dep_scale[2 * LPM_MAX_NUCLIDES];       // fixed-point scales of the CTA-private deposit sums (powers of two): [2k] dry, [2k+1] wet
     double dep_inv_scale[2 * LPM_MAX_NUCLIDES];  // their inverses
-    int32_t any_dep, pad0_;                  // some sink can deposit (dry deposition or a rain box)
+    int32_t any_dep, bern;                   // some sink deposits through the tables; dep_mode 1: Bernoulli deposition (R11)
     // physics
     float dt, sigma_h, kz_min, H, h_dep;
     int32_t dry_mode, absorb;
@@ -127,7 +127,7 @@ struct BinArgs {
 
 // launchers implemented in the .cu files; all return the cudaError of the launch
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int grid_blocks, cudaStream_t st);
-int step_max_blocks_per_sm(int K, bool compact, int dry_mode);
+int step_max_blocks_per_sm(int K, bool compact, int dry_mode, bool bern);
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
                                 uint32_t *perm, cudaStream_t st);
@@ -159,7 +159,7 @@ cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3,
 cudaError_t launch_dose_accum(const double *conc, double *dose, uint64_t cells3, int K, const double *scale, cudaStream_t st);
 cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, double inv_area, cudaStream_t st);
 cudaError_t launch_airborne(const float4 *xyzq, const float *q1, uint64_t n, const uint64_t *n_dev, int K, double *out2, cudaStream_t st);
-cudaError_t launch_export(const float4 *xyzq, uint64_t n, const uint64_t *n_dev, float4 *out, uint8_t *status, cudaStream_t st);
+cudaError_t launch_export(const float4 *xyzq, const float *q1, uint64_t n, const uint64_t *n_dev, float4 *out, uint8_t *status, cudaStream_t st);
 cudaError_t launch_import(float4 *xyzq, uint64_t n, const uint8_t *status, cudaStream_t st);
 cudaError_t launch_iota(uint32_t *pid, uint64_t n, cudaStream_t st);
 cudaError_t launch_qmax(const float4 *xyzq, const float *q1, uint64_t n, int K, float *out2, cudaStream_t st);

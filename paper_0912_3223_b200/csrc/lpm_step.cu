@@ -121,7 +121,7 @@ __device__ __forceinline__ void deposit_at(const StepArgs &A, float x, float y, 
 // One model step of one particle.  Returns false when the particle left the domain (ABSORB).
 // Source order = intended issue order: the eight gathers go out first and the ~150 instructions of
 // Philox + Box-Muller run while they are in flight.
-template <int K, int DRY>
+template <int K, int DRY, bool BERN>
 __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e, uint32_t step_lo,
                                           uint32_t pid_lo, float &x, float &y, float &z,
                                           float (&q)[K], Acc<K> &acc, DepTab<K> &dep)
@@ -132,7 +132,7 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
     const float kz = fmaxf(m.w, A.kz_min);
 
     // a1: three N(0,1) from Philox stream 0
-    const uint4 r = philox4x32_10_rk(step_lo, pid_lo, A.rk);
+    const uint4 r = philox4x32_10_rk<0u>(step_lo, pid_lo, A.rk);
     float n0, n1, n2;
     normals3(r, n0, n1, n2);
 
@@ -160,6 +160,42 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
     // straight-line code: no sink at all (2 FMA), uniform dry deposition without rain (4 FMA + the
     // scatter).
     const bool raining = (e.snap >> 16) & 1;
+    if constexpr (BERN) {
+        // R11, the paper's own form: one Bernoulli trial per nuclide and sink per step from
+        // Philox stream 1; u = (word >> 8) 2^-24 < p decides (exact on both sides); an event deposits the
+        // nuclide's whole activity at the new (x, y) - a rare event, so straight to the map with an fp64 RED;
+        // a particle that carries nothing any more becomes inactive.
+        const bool dry_here = DRY == kDryUniform || (DRY == kDryLayer && z < A.h_dep);
+        const bool wet_here = raining & (x >= A.rx0) & (x < A.rx1) & (y >= A.ry0) & (y < A.ry1);
+        if (dry_here | wet_here) {
+            const uint4 r1 = philox4x32_10_rk<1u>(step_lo, pid_lo, A.rk);
+            const uint32_t wd[2] = {r1.x, r1.y}, ww[2] = {r1.z, r1.w};
+            constexpr float s24 = 5.9604644775390625e-08f;
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                if (q[k] > 0.0f) {
+                    const bool d = dry_here && __uint2float_rn(wd[k] >> 8) * s24 < A.p_dry[k];
+                    const bool w = !d && wet_here && __uint2float_rn(ww[k] >> 8) * s24 < A.p_wet[k];
+                    if (d | w) {
+                        const double act = (double)q[k] * e.G[k];
+                        const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
+                        const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
+                        if ((ci | cj) >= 0) atomicAdd(A.dep + (uint32_t)(cj * A.cg.nx + ci) + k * A.dep_stride, act);
+                        else atomicAdd(A.ledger + k * 8 + 6, act);
+                        atomicAdd(A.ledger + k * 8 + (d ? 2 : 3), act);
+                        q[k] = 0.0f;
+                    }
+                }
+            }
+        }
+        bool empty = true;
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            acc.both[k] = fmaf(q[k], e.Gf[k], acc.both[k]);
+            empty &= !(q[k] > 0.0f);
+        }
+        return !empty;
+    }
     if (DRY != kDryLayer && !raining) {
 #pragma unroll
         for (int k = 0; k < K; ++k) acc.both[k] = fmaf(q[k], e.Gf[k], acc.both[k]);
@@ -214,7 +250,7 @@ __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &ac
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const float b = warp_sum(acc.both[k]);
-        const float d = (A.dry_mode == kDryUniform ? b : 0.0f) + warp_sum(acc.dry[k]), w = warp_sum(acc.wet[k]), c = b + warp_sum(acc.dec[k]), o = warp_sum(acc.off[k]);
+        const float d = (A.dry_mode == kDryUniform && !A.bern ? b : 0.0f) + warp_sum(acc.dry[k]), w = warp_sum(acc.wet[k]), c = b + warp_sum(acc.dec[k]), o = warp_sum(acc.off[k]);
         if (lane == 0) { s_part[warp][4 * k] = d; s_part[warp][4 * k + 1] = w; s_part[warp][4 * k + 2] = c; s_part[warp][4 * k + 3] = o; }
     }
     __syncthreads();
@@ -237,7 +273,7 @@ __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &ac
 #endif
 static_assert(sizeof(StepArgs) <= 32764, "StepArgs must fit the kernel-parameter space (32764 B since CUDA 12.1 on sm_70+)");
 
-template <int K, int DRY>
+template <int K, int DRY, bool BERN>
 __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel(const __grid_constant__ StepArgs A)
 {
     __shared__ uint32_t s_ticket;
@@ -301,7 +337,7 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             bool alive = true;
             const uint32_t step0 = (uint32_t)A.step0;
             for (int s = 0; s < A.m_steps; ++s)
-                if (alive & (s >= s_begin)) alive = step_once<K, DRY>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, T);
+                if (alive & (s >= s_begin)) alive = step_once<K, DRY, BERN>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, T);
             if (!alive) z = -1.0f - z;  // exit position kept, slot marked inactive
             A.xyzq[slot] = make_float4(x, y, z, q[0]);
             if (K > 1) A.q1[slot] = q[1];
@@ -344,7 +380,7 @@ __device__ __forceinline__ void st_state(uint64_t *p, uint64_t v)
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-template <int K, int DRY>
+template <int K, int DRY, bool BERN>
 __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid_constant__ StepArgs A)
 {
     constexpr int kItems = kScanTile / kStepThreads;  // particles per thread and tile: amortises the tile's barriers and look-back
@@ -393,7 +429,7 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
 #pragma unroll
         for (int j = 0; j < kItems; ++j) {
             const uint64_t i = (uint64_t)tile * kScanTile + (uint32_t)j * kStepThreads + threadIdx.x;
-            if (i < n) alive[j] = step_once<K, DRY>(A, A.tab[0], (uint32_t)A.step0, pid[j], x[j], y[j], z[j], q[j], acc, T);
+            if (i < n) alive[j] = step_once<K, DRY, BERN>(A, A.tab[0], (uint32_t)A.step0, pid[j], x[j], y[j], z[j], q[j], acc, T);
             // survivors: rank inside the (item, warp) part
             const uint32_t ball = __ballot_sync(0xffffffffu, alive[j]);
             rank[j] = __popc(ball & ((1u << lane) - 1u));
@@ -501,32 +537,36 @@ __global__ void __launch_bounds__(256) inject_kernel(const __grid_constant__ Inj
 }
 
 // ------------------------------------------------------------------ launchers
-// One instantiation per (nuclide count, dry-deposition mode).
 typedef void (*StepKernel)(const StepArgs);
 
-template <int K>
+// One instantiation per (nuclide count, dry-deposition mode, expected-mass / Bernoulli deposition).
+template <int K, bool BERN>
 static StepKernel pick_dry(bool compact, int dry)
 {
     if (compact) {
-        if (dry == kDryNone) return step_compact_kernel<K, kDryNone>;
-        return dry == kDryUniform ? step_compact_kernel<K, kDryUniform> : step_compact_kernel<K, kDryLayer>;
+        if (dry == kDryNone) return step_compact_kernel<K, kDryNone, BERN>;
+        return dry == kDryUniform ? step_compact_kernel<K, kDryUniform, BERN> : step_compact_kernel<K, kDryLayer, BERN>;
     }
-    if (dry == kDryNone) return step_slots_kernel<K, kDryNone>;
-    return dry == kDryUniform ? step_slots_kernel<K, kDryUniform> : step_slots_kernel<K, kDryLayer>;
+    if (dry == kDryNone) return step_slots_kernel<K, kDryNone, BERN>;
+    return dry == kDryUniform ? step_slots_kernel<K, kDryUniform, BERN> : step_slots_kernel<K, kDryLayer, BERN>;
 }
 
-static StepKernel pick(int K, bool compact, int dry) { return K == 1 ? pick_dry<1>(compact, dry) : pick_dry<2>(compact, dry); }
+static StepKernel pick(int K, bool compact, int dry, bool bern)
+{
+    if (bern) return K == 1 ? pick_dry<1, true>(compact, dry) : pick_dry<2, true>(compact, dry);
+    return K == 1 ? pick_dry<1, false>(compact, dry) : pick_dry<2, false>(compact, dry);
+}
 
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int blocks, cudaStream_t st)
 {
-    pick(K, compact, a.dry_mode)<<<blocks, kStepThreads, 0, st>>>(a);
+    pick(K, compact, a.dry_mode, a.bern != 0)<<<blocks, kStepThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 
-int step_max_blocks_per_sm(int K, bool compact, int dry)
+int step_max_blocks_per_sm(int K, bool compact, int dry, bool bern)
 {
     int nb = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick(K, compact, dry), kStepThreads, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick(K, compact, dry, bern), kStepThreads, 0);
     return nb;
 }
 

@@ -410,6 +410,58 @@ def test_dose_grid(lpm, orc):
     assert dense.sum() > 20 and np.abs(cg[dense] / co[dense] - 1).max() < 5e-3
 
 
+# ------------------------------------------------------------------ S§8(f)1: Bernoulli deposition (R11)
+@pytest.mark.parametrize("h_dep", [1000.0, 80.0])
+def test_bernoulli_deposition(lpm, orc, h_dep):
+    """(f)1: the paper's stochastic deposition.  The trials use exact 24-bit uniforms against fp32 parameters,
+    so the decisions are identical on both sides: the same particles deposit at the same steps (except fragile
+    ones), the deposit map matches up to face slack, and the ledger closes."""
+    w = make("c3", scale=1.0, n_steps=900)
+    w.release.pid_stride = 500                          # 20000 of the 1e7 particles
+    # large deposition velocities / scavenging so that a few thousand events happen in 900 steps
+    nuc = [Nuclide("I-131", w.nuclides[0].half_life_s, 0.05, 3.0e-4), Nuclide("Cs-137", w.nuclides[1].half_life_s, 0.1, 1.0e-4)]
+    w = w.replace(nt=4, capacity=20_000, h_dep=h_dep, nuclides=nuc, bin_every=300,
+                  rain=RainBox(-4.2e4, -3.0e4, -2.0e3, 2.0e3, 2000.0, 8000.0))
+    sim = lpm.Simulation(w, dep_mode=1)
+    o = orc.OracleSim(w, dep_mode=1, face_delta=1.5)
+    sim.step(900)
+    o.step(900)
+    g, p = sim.get_particles_host(), o.particles()
+    assert g["x"].shape[0] == p["x"].shape[0] > 1500
+    frag = np.isin(p["pid"], o.fragile_pids())
+    ok = ~frag
+    assert frag.mean() < (0.02 if h_dep >= 1000.0 else 0.15)     # the z = h_dep surface sits 30 m above the source
+    np.testing.assert_array_equal(g["status"][ok], p["status"][ok])
+    assert (p["status"] == 2).sum() > 50
+    for k in range(2):                                    # the same nuclides are gone from the same particles
+        np.testing.assert_array_equal((g["m"][k] == 0)[ok], (p["m"][k] == 0)[ok])
+        assert ((p["m"][k] == 0) & (p["status"] == 0)).sum() > 20   # one nuclide gone, the other still airborne
+    act = ok & (p["status"] == 0)
+    sub = {kk: g[kk][act] for kk in ("x", "y", "z")}
+    sub["m"] = g["m"][:, act]
+    ref = {kk: p[kk][act] for kk in ("x", "y", "z")}
+    ref["m"] = p["m"][:, act]
+    keep = (ref["m"] > 0).all(axis=0)
+    _n_step_compare({kk: (v[:, keep] if kk == "m" else v[keep]) for kk, v in sub.items()},
+                    {kk: (v[:, keep] if kk == "m" else v[keep]) for kk, v in ref.items()}, w, np.zeros(keep.sum(), dtype=bool), 0.999,
+                    f"bernoulli h_dep={h_dep}")
+    lg, lo = sim.ledger(), o.ledger()
+    for k in range(2):
+        assert lo[k][2] > 0 and lo[k][3] > 0
+        for f in (0, 1, 4):
+            assert abs(lg[k][f] / lo[k][f] - 1) < 2e-5, (k, f)
+        assert abs((lg[k][1] + lg[k][2] + lg[k][3] + lg[k][4]) / lg[k][0] - 1) < 1e-5
+        # dry / wet totals: whole particles; they can differ only by the fragile particles' events
+        fr_mass = lo[k][0] / 20_000 * max(frag.sum(), 1)
+        assert abs(lg[k][2] - lo[k][2]) <= 1.001 * fr_mass + 1e-5 * lo[k][2]
+        assert abs(lg[k][3] - lo[k][3]) <= 1.001 * fr_mass + 1e-5 * lo[k][3]
+    dg = sim.deposition(f64=True).cpu().numpy()
+    do, slack = o.deposition(with_slack=True)
+    area = w.cgrid.dx * w.cgrid.dy
+    excess = np.maximum(np.abs(dg - do) - (1e-5 * do + 1.0001 * slack + 1e-30), 0.0)
+    assert excess.sum() * area <= 1.001 * (lo[0][0] + lo[1][0]) / 20_000 * max(frag.sum(), 1) + 1e-4 * do.sum() * area
+
+
 # ------------------------------------------------------------------ a7: compaction (config 5 shape)
 def test_c5_compaction_small(lpm, orc):
     """1/100-scale-class C5: ABSORB + stable compaction each step, rate-mode injection with a
