@@ -56,7 +56,8 @@ typedef struct {
     double frag_delta;     /* metres: distance to a discontinuity that flags a particle fragile */
     double face_delta;     /* metres: distance to a deposition-map cell face counted as slack   */
     int32_t dep_mode;      /* 0: expected-mass deposition (R8); 1: paper-literal Bernoulli deposition (R11) */
-    int32_t pad2_;
+    int32_t kz_mode;       /* 0: Kz is the interpolated gridded field (R4); 1: Eq.(3) per particle (R12)    */
+    const float *surface;  /* kz_mode 1: borrowed, [nt][ny][nx][4] = (u*, 1/L, Hz, unused), x fastest         */
 } orc_config;
 
 typedef struct {
@@ -224,6 +225,43 @@ void orc_sample_met(const orc_grid *g, int32_t nt, double t0, double dt_snap, co
     } else {
         for (int c = 0; c < 4; ++c) out[c] = A[c];
     }
+}
+
+/* ------------------------------------------------------------------ R12: Eq.(3) per particle
+ * PAPER.md L79-82 Eq.(3): Kz(z) = k u* z / Phi(z/L) * (1 - z/Hz)^2, "where k, u*, z, Phi, L and Hz are the von
+ * Karman constant, friction velocity, height, stability function, Monin-Obukhov length and mixing layer
+ * height".  The paper defines no Phi (G2); reading R12 takes the Businger-Dyer forms
+ * Phi = 1 + 5 zeta (zeta = z/L >= 0), Phi = (1 - 16 zeta)^(-1/2) (zeta < 0), k = 0.4, Kz = 0 at and above Hz.
+ * u*, 1/L and Hz are 2-D fields sampled like the weather (L106: linear in x, y and time; cell-centred,
+ * edge-clamped as R4); 1/L, not L, is the stored and interpolated quantity (neutral = 0). */
+void orc_sample_surface(const orc_grid *g, int32_t nt, double t0, double dt_snap, const float *surface, double t, double x,
+                        double y, double out[3])
+{
+    int32_t s, i0, i1, j0, j1;
+    float a;
+    double fx, fy;
+    orc_time_weight(nt, t0, dt_snap, t, &s, &a);
+    axis_weights(x, g->x0, g->dx, g->nx, &i0, &i1, &fx);
+    axis_weights(y, g->y0, g->dy, g->ny, &j0, &j1, &fy);
+    const size_t plane = (size_t)g->nx * g->ny * 4;
+    for (int c = 0; c < 3; ++c) {
+        double v[2] = {0.0, 0.0};
+        for (int tt = 0; tt < (nt > 1 ? 2 : 1); ++tt) {
+            const float *f = surface + (size_t)(s + tt) * plane;
+            v[tt] = (1.0 - fy) * ((1.0 - fx) * (double)f[4 * ((size_t)j0 * g->nx + i0) + c] + fx * (double)f[4 * ((size_t)j0 * g->nx + i1) + c]) +
+                    fy * ((1.0 - fx) * (double)f[4 * ((size_t)j1 * g->nx + i0) + c] + fx * (double)f[4 * ((size_t)j1 * g->nx + i1) + c]);
+        }
+        out[c] = nt > 1 ? (1.0 - (double)a) * v[0] + (double)a * v[1] : v[0];
+    }
+}
+
+double orc_kz_eq3(double ustar, double inv_L, double Hz, double z)
+{
+    if (!(z < Hz) || !(z > 0.0)) return 0.0;
+    double zeta = z * inv_L;
+    double phi = zeta >= 0.0 ? 1.0 + 5.0 * zeta : 1.0 / sqrt(1.0 - 16.0 * zeta);
+    double t = 1.0 - z / Hz;
+    return 0.4 * ustar * z / phi * t * t;
 }
 
 /* ------------------------------------------------------------------ R10: cell index
@@ -395,6 +433,11 @@ static void step_particle(orc_sim *s, uint64_t i, uint64_t n, double t_n, int ra
     /* R4: weather at X_old, t_n (forward Euler; Eq.(1) uses the wind at the old position) */
     orc_sample_met(&c->mgrid, c->nt, c->t0, c->dt_snap, c->fields, t_n, s->x[i], s->y[i], s->z[i], met);
     double u = met[0], v = met[1], w = met[2], Kz = met[3];
+    if (c->kz_mode == 1) { /* R12: "computing the turbulent diffusion coefficient" per particle (L106, L112-113) */
+        double sf[3];
+        orc_sample_surface(&c->mgrid, c->nt, c->t0, c->dt_snap, c->surface, t_n, s->x[i], s->y[i], sf);
+        Kz = orc_kz_eq3(sf[0], sf[1], sf[2], s->z[i]);
+    }
     if (Kz < c->kz_min) Kz = c->kz_min;
 
     /* R5: Eq.(1) + Eq.(2) */

@@ -45,7 +45,7 @@ class Config(C.Structure):
                 ("rx0", C.c_double), ("rx1", C.c_double), ("ry0", C.c_double), ("ry1", C.c_double),
                 ("rt0", C.c_double), ("rt1", C.c_double),
                 ("frag_delta", C.c_double), ("face_delta", C.c_double),
-                ("dep_mode", C.c_int32), ("pad2_", C.c_int32)]
+                ("dep_mode", C.c_int32), ("kz_mode", C.c_int32), ("surface", C.c_void_p)]
 
 
 class Source(C.Structure):
@@ -100,6 +100,10 @@ def lib():
         L.orc_time_weight.argtypes = [C.c_int32, C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
         L.orc_sample_met.argtypes = [C.POINTER(Grid), C.c_int32, C.c_double, C.c_double, C.c_void_p,
                                      C.c_double, C.c_double, C.c_double, C.c_double, C.c_void_p]
+        L.orc_kz_eq3.argtypes = [C.c_double] * 4
+        L.orc_kz_eq3.restype = C.c_double
+        L.orc_sample_surface.argtypes = [C.POINTER(Grid), C.c_int32, C.c_double, C.c_double, C.c_void_p,
+                                         C.c_double, C.c_double, C.c_double, C.c_void_p]
         L.orc_cell_index.argtypes = [C.c_float, C.c_double, C.c_double, C.c_int32]
         L.orc_cell_index.restype = C.c_int32
         _lib = L
@@ -157,6 +161,17 @@ def sample_met(grid, nt, t0, dt_snap, fields, t, x, y, z):
     return out
 
 
+def kz_eq3(ustar, inv_L, Hz, z):
+    return lib().orc_kz_eq3(ustar, inv_L, Hz, z)
+
+
+def sample_surface(grid, nt, t0, dt_snap, surface, t, x, y):
+    out = np.zeros(3)
+    sf = np.ascontiguousarray(surface, dtype=np.float32)
+    lib().orc_sample_surface(C.byref(_grid(grid)), nt, t0, dt_snap, sf.ctypes.data, t, x, y, _p(out))
+    return out
+
+
 def cell_index(p, p0, dp, n):
     return lib().orc_cell_index(float(np.float32(p)), p0, dp, n)
 
@@ -189,6 +204,11 @@ class OracleSim:
             cfg.rt0, cfg.rt1 = w.rain.t_start, w.rain.t_end
         cfg.frag_delta, cfg.face_delta = frag_delta, face_delta
         cfg.dep_mode = dep_mode
+        self._surface = None
+        if getattr(w, "kz_mode", 0) == 1:
+            self._surface = np.ascontiguousarray(w.surface(), dtype=np.float32)
+            cfg.kz_mode = 1
+            cfg.surface = self._surface.ctypes.data
         self._cfg = cfg
         self._h = lib().orc_create(C.byref(cfg))
         if not self._h:

@@ -8,6 +8,8 @@ from scipy import stats
 
 from helpers import T_I131, custom, uniform_met
 from oracle import oracle as orc
+from dataclasses import replace as dataclasses_replace
+
 from workloads import Grid, Nuclide, RainBox, Release, make
 
 
@@ -416,3 +418,59 @@ def test_bernoulli_deposition_replays_from_the_draws():
     for k in range(2):
         assert led[k][2] == pytest.approx(dry[k], rel=1e-14) and led[k][3] == pytest.approx(wet[k], rel=1e-14)
     assert dry.sum() > 0 and wet.sum() > 0
+
+
+# ------------------------------------------------------------------ P17: Eq.(3) per particle (S§8(f)2, R12)
+def test_eq3_profile_values():
+    """Kz = k u* z / Phi(z/L) (1 - z/Hz)^2 with Businger-Dyer Phi: hand-computed values and the neutral closed form."""
+    for z in (0.5, 25.0, 333.3, 975.0):
+        assert orc.kz_eq3(0.4, 0.0, 1000.0, z) == pytest.approx(0.16 * z * (1 - z / 1000.0) ** 2, rel=1e-15)
+    assert orc.kz_eq3(0.5, 0.002, 1000.0, 100.0) == pytest.approx(8.1, rel=1e-14)                       # zeta = 0.2: Phi = 2
+    assert orc.kz_eq3(0.5, -0.01, 1000.0, 100.0) == pytest.approx(16.2 * math.sqrt(17.0), rel=1e-14)    # zeta = -1: Phi = 17^-1/2
+    assert orc.kz_eq3(0.5, 0.0, 1000.0, 1000.0) == 0.0 and orc.kz_eq3(0.5, 0.0, 1000.0, 1200.0) == 0.0
+    assert orc.kz_eq3(0.5, 0.0, 1000.0, 0.0) == 0.0
+
+
+def test_surface_sampling_reproduces_affine_fields():
+    g = Grid(12, 9, 4, -600.0, 100.0, 0.0, 100.0, 50.0, 25.0)
+    xc = g.x0 + (np.arange(g.nx) + 0.5) * g.dx
+    yc = g.y0 + (np.arange(g.ny) + 0.5) * g.dy
+    Y, X = np.meshgrid(yc, xc, indexing="ij")
+    sf = np.zeros((2, g.ny, g.nx, 4), dtype=np.float32)
+    for s, t in enumerate((0.0, 3600.0)):
+        sf[s, ..., 0] = 0.25 + X / 4096.0 + t / 8192.0
+        sf[s, ..., 1] = Y / 65536.0 - 1.0 / 1024.0          # exactly representable in fp32
+        sf[s, ..., 2] = 1000.0 + 0.5 * X - 0.25 * Y
+    rng = np.random.default_rng(4)
+    for _ in range(200):
+        x, y, t = rng.uniform(xc[0], xc[-1]), rng.uniform(yc[0], yc[-1]), rng.uniform(0, 3600.0)
+        got = orc.sample_surface(g, 2, 0.0, 3600.0, sf, t, x, y)
+        a = float(np.float32(t / 3600.0))                  # the time weight is an fp32 parameter (R4)
+        assert got[0] == pytest.approx(0.25 + x / 4096.0 + a * 3600.0 / 8192.0, rel=1e-12)
+        assert got[1] == pytest.approx(y / 65536.0 - 1.0 / 1024.0, rel=1e-9, abs=1e-15)
+        assert got[2] == pytest.approx(1000.0 + 0.5 * x - 0.25 * y, rel=1e-12)
+    lo = orc.sample_surface(g, 2, 0.0, 3600.0, sf, 0.0, -1e9, -1e9)       # edge-clamped
+    assert lo[2] == pytest.approx(float(sf[0, 0, 0, 2]))
+
+
+def test_eq3_mode_equals_gridded_mode_at_cell_centre_heights():
+    """With uniform neutral surface fields Eq.(3) IS c2's Kz recipe, and the gridded field interpolates it exactly at
+    the cell-centre heights: one step from there gives the same positions in both modes."""
+    w0 = make("c2", scale=1e-3).replace(nt=2)
+    w1 = dataclasses_replace(w0, kz_mode=1, surface_fn=lambda t, Y, X: (0.4, 0.0, 1000.0))
+    g = w0.mgrid
+    rng = np.random.default_rng(9)
+    n = 500
+    x = rng.uniform(-2e4, 2e4, n)
+    y = rng.uniform(-2e4, 2e4, n)
+    z = g.z0 + (rng.integers(1, g.nz - 1, n) + 0.5) * g.dz
+    res = []
+    for w in (w0, w1):
+        o = orc.OracleSim(w.replace(release=None, capacity=n), bin_every=0)
+        o.set_particles(x, y, z, np.ones((1, n)), pid=np.arange(n))
+        o.set_step_index(100)
+        o.step(1)
+        res.append(o.particles())
+    for k in ("x", "y", "z"):
+        np.testing.assert_allclose(res[0][k], res[1][k], rtol=0, atol=2e-5)   # fp32 field values vs fp64 formula
+    assert np.abs(res[0]["z"] - z).max() > 1.0

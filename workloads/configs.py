@@ -19,7 +19,7 @@ from typing import List, Optional
 
 import numpy as np
 
-NAMES = ("c1", "c2", "c3", "c3_hdep80", "c4", "c5")
+NAMES = ("c1", "c2", "c2_eq3", "c3", "c3_hdep80", "c4", "c5")
 
 HOUR = 3600.0
 DAY = 86400.0
@@ -99,6 +99,8 @@ class Workload:
     release: Optional[Release]
     rain: Optional[RainBox] = None
     met_fn: object = field(default=None, repr=False)   # (t, Z, Y, X) -> u, v, w, kz  in float64
+    kz_mode: int = 0                                   # 1: Kz from Eq.(3) per particle (R12) with the 2-D fields below
+    surface_fn: object = field(default=None, repr=False)   # (t, Y, X) -> ustar, 1/L, Hz  in float64 (cell centres)
     _fields: object = field(default=None, repr=False)
 
     @property
@@ -130,6 +132,20 @@ class Workload:
                     _SNAP_CACHE[key] = out[s].copy()
             self._fields = out
         return self._fields
+
+    def surface(self) -> np.ndarray:
+        """float32 array [nt][ny][nx][4] = (u*, 1/L, Hz, 0) at the met grid's column centres, x fastest."""
+        g = self.mgrid
+        xc = g.x0 + (np.arange(g.nx, dtype=np.float64) + 0.5) * g.dx
+        yc = g.y0 + (np.arange(g.ny, dtype=np.float64) + 0.5) * g.dy
+        Y, X = np.meshgrid(yc, xc, indexing="ij")
+        out = np.zeros((self.nt, g.ny, g.nx, 4), dtype=np.float32)
+        for s in range(self.nt):
+            us, il, hz = self.surface_fn(self.t0 + s * self.dt_snap, Y, X)
+            out[s, ..., 0] = np.broadcast_to(us, Y.shape)
+            out[s, ..., 1] = np.broadcast_to(il, Y.shape)
+            out[s, ..., 2] = np.broadcast_to(hz, Y.shape)
+        return out
 
     def replace(self, **kw) -> "Workload":
         w = dataclasses.replace(self, **kw)
@@ -167,6 +183,15 @@ def _met_c2(t, Z, Y, X):
     theta = np.deg2rad(30.0 * Z / 1000.0 + 10.0 * (t / HOUR))
     kz = np.maximum(0.1, k * ustar * Z * (1.0 - Z / H) ** 2)
     return speed * np.cos(theta), speed * np.sin(theta), 0.0, kz
+
+
+def _surface_c2(t, Y, X):
+    """c2_eq3 (S§8(f)2): friction velocity, inverse Obukhov length and mixing height as smooth 2-D fields that
+    change over the two hours: near-neutral with a stable (1/L > 0) half and an unstable half of the domain."""
+    ustar = 0.4 * (1.0 + 0.2 * np.sin(2.0 * np.pi * X / 40.0e3)) * (1.0 + 0.1 * t / HOUR)
+    inv_L = 0.004 * np.sin(2.0 * np.pi * Y / 60.0e3) - 0.002 * t / HOUR
+    Hz = 1000.0 * (1.0 - 0.2 * np.cos(2.0 * np.pi * (X + Y) / 80.0e3)) - 50.0 * t / HOUR
+    return ustar, inv_L, Hz
 
 
 def _wind_c3(t, Z, Y, X):
@@ -267,6 +292,8 @@ def make(name: str, scale: float = 1.0, n_steps: Optional[int] = None) -> Worklo
         w = _c1(scale)
     elif name == "c2":
         w = _c2(scale)
+    elif name == "c2_eq3":
+        w = dataclasses.replace(_c2(scale), name="c2_eq3", kz_mode=1, surface_fn=_surface_c2)
     elif name == "c3":
         w = _c3(scale)
     elif name == "c3_hdep80":
