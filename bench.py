@@ -50,7 +50,7 @@ SMS, LANES_PER_SM = 148, 128          # 4 SMSP x 32 lanes: one warp instruction 
 LAUNCH_STEPS = 16                     # model steps fused per step-kernel launch (csrc kMaxFused)
 # dram__bytes_read.sum + dram__bytes_write.sum of one captured step-kernel launch, bytes (profiles/r01c_c4_step_kernel_ncu.md)
 NCU_TRAFFIC = {"c4": 3.586e9 + 1.934e9}   # launch 171 of `bench.py --steps 1 --warmup 3`: 16 steps x 3.16e7 particles
-ORACLE_STRIDE = {"c1": 1, "c2": 40, "c3": 400, "c3_hdep80": 400, "c4": 4000, "c5": 1}
+ORACLE_STRIDE = {"c1": 1, "c2": 40, "c2_eq3": 40, "c3": 400, "c3_hdep80": 400, "c4": 4000, "c5": 1}
 ORACLE_SCALE_C5 = 1.0e-3              # c5 cannot be pid-strided (capacity couples particles): 1/1000 scale
 
 
@@ -406,7 +406,7 @@ def run_ours(args):
         "metric": METRIC, "value": units / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{args.workload} (BASELINE.json configs[{ {'c1': 0, 'c2': 1, 'c3': 2, 'c3_hdep80': 2, 'c4': 3, 'c5': 4}[args.workload] }])",
+        "config": {"workload": f"{args.workload} (BASELINE.json configs[{ {'c1': 0, 'c2': 1, 'c2_eq3': 1, 'c3': 2, 'c3_hdep80': 2, 'c4': 3, 'c5': 4}[args.workload] }])",
                    "particles_per_gpu": w.capacity, "nuclides": w.K, "model_steps_per_bench_step": interval, "dt_s": w.dt,
                    "conc_grid": [g.nx, g.ny, g.nz], "met_grid": [w.mgrid.nx, w.mgrid.ny, w.mgrid.nz], "met_snapshots": w.nt,
                    "scale": args.scale, "dep_mode": args.dep_mode, "l2": "particle store larger than L2, no flush" if w.capacity * state_bytes > 126e6 else "inputs fit L2 (small config)",
@@ -451,7 +451,7 @@ def main():
     ap.add_argument("--steps", type=int, default=9)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
-    ap.add_argument("--workload", default="c4", choices=("c1", "c2", "c3", "c3_hdep80", "c4", "c5"))
+    ap.add_argument("--workload", default="c4", choices=("c1", "c2", "c2_eq3", "c3", "c3_hdep80", "c4", "c5"))
     ap.add_argument("--scale", type=float, default=1.0, help="particle-count scale of the workload (1.0 = BASELINE size)")
     ap.add_argument("--dep-mode", type=int, default=0, choices=(0, 1), help="0 expected-mass deposition (default), 1 Bernoulli deposition (S 8(f)1)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -63,10 +63,14 @@ typedef struct {
  * horizontal diffusivity.  H_mix: reflecting lid (R6).  kz_min: floor on the sampled Kz. */
 typedef struct {
     lpm_grid grid;
-    int32_t nt, reserved;
+    int32_t nt;
+    int32_t kz_mode;          /* 0: Kz is the w component of the texels (sampled like the wind); 1: Kz from Eq.(3)
+                               * per particle with the 2-D fields of surface_dev (R12)       */
     double t0, dt_snap;
     const void *fields_dev;
     double Kh, H_mix, kz_min;
+    const void *surface_dev;  /* kz_mode 1: float4 (u* [m/s], 1/L [1/m], Hz [m], unused) [nt][ny][nx], x fastest,
+                               * 16-byte aligned, borrowed like fields_dev; else ignored (may be NULL)             */
 } lpm_meteo;
 
 /* Isotope constants. half_life_s <= 0 means stable. */

@@ -44,9 +44,9 @@ class lpm_grid(C.Structure):
 
 
 class lpm_meteo(C.Structure):
-    _fields_ = [("grid", lpm_grid), ("nt", C.c_int32), ("reserved", C.c_int32), ("t0", C.c_double),
+    _fields_ = [("grid", lpm_grid), ("nt", C.c_int32), ("kz_mode", C.c_int32), ("t0", C.c_double),
                 ("dt_snap", C.c_double), ("fields_dev", C.c_void_p), ("Kh", C.c_double), ("H_mix", C.c_double),
-                ("kz_min", C.c_double)]
+                ("kz_min", C.c_double), ("surface_dev", C.c_void_p)]
 
 
 class lpm_nuclide(C.Structure):
@@ -132,11 +132,11 @@ def _grid(g) -> lpm_grid:
 
 
 def workspace_bytes(cgrid, capacity: int, n_nuclides: int, compact: bool, mgrid=None, nt: int = 1, gather_sort: int = 0,
-                    dose: bool = False) -> int:
+                    dose: bool = False, kz_mode: int = 0) -> int:
     p = lpm_params(dt=1.0, capacity=capacity, compact=1 if compact else 0, h_dep=1.0, gather_sort=gather_sort, dose=1 if dose else 0)
     out = C.c_uint64()
     g = _grid(cgrid)
-    met = lpm_meteo(grid=_grid(mgrid if mgrid is not None else cgrid), nt=nt)
+    met = lpm_meteo(grid=_grid(mgrid if mgrid is not None else cgrid), nt=nt, kz_mode=kz_mode)
     rc = load().lpm_workspace_bytes(C.byref(g), C.byref(met), C.byref(p), n_nuclides, C.byref(out))
     if rc:
         raise LpmError(rc, "lpm_workspace_bytes")
@@ -181,11 +181,16 @@ class Simulation:
             fields_dev = torch.from_numpy(np.ascontiguousarray(f)).to(self.device)
         assert fields_dev.dtype == torch.float32 and fields_dev.is_contiguous()
         self.fields_dev = fields_dev
-        nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact, w.mgrid, w.nt, gather_sort, dose)
+        kz_mode = int(getattr(w, "kz_mode", 0))
+        self.surface_dev = None
+        if kz_mode == 1:
+            self.surface_dev = torch.from_numpy(np.ascontiguousarray(w.surface(), dtype=np.float32)).to(self.device)
+        nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact, w.mgrid, w.nt, gather_sort, dose, kz_mode)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         cg = _grid(w.cgrid)
         met = lpm_meteo(grid=_grid(w.mgrid), nt=w.nt, t0=w.t0, dt_snap=w.dt_snap, fields_dev=fields_dev.data_ptr(),
-                        Kh=w.Kh, H_mix=w.H_mix, kz_min=w.kz_min)
+                        Kh=w.Kh, H_mix=w.H_mix, kz_min=w.kz_min, kz_mode=kz_mode,
+                        surface_dev=self.surface_dev.data_ptr() if self.surface_dev is not None else None)
         nucs = (lpm_nuclide * w.K)(*[lpm_nuclide(n.half_life_s, n.vd, n.lambda_wet) for n in w.nuclides])
         prm = lpm_params(dt=w.dt, seed=w.seed, capacity=w.capacity,
                          boundary_mode=1 if w.boundary_mode == "absorb" else 0, compact=1 if w.compact else 0,

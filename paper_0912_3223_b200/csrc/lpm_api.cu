@@ -27,7 +27,7 @@ struct Release {
 };
 
 struct Layout {
-    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, blend, keys, perm, hist, partial, alt_xyzq, alt_q1, alt_pid, dose, mask, total;
+    uint64_t xyzq, q1, pid, cnt, conc, dep, ledger, air, ctrl, tile, injlog, stage, pair, blend, keys, perm, hist, partial, alt_xyzq, alt_q1, alt_pid, dose, mask, surf, total;
 };
 
 uint64_t up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
@@ -60,6 +60,7 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     L.alt_q1 = o; o += sort && compact && K > 1 ? up(4 * cap) : 0;     //   through these alternate buffers
     L.alt_pid = o; o += sort && compact ? up(4 * cap) : 0;
     L.mask = o; o += up((uint64_t)((met.grid.nx + kMaskTile - 1) / kMaskTile) * ((met.grid.ny + kMaskTile - 1) / kMaskTile));  // plume mask tiles
+    L.surf = o; o += met.kz_mode == 1 ? up(16ull * met.grid.nx * met.grid.ny * (met.nt > 1 ? kBlendDepth : 1)) : 0;  // R12 2-D fields per fused step
     L.dose = o; o += dose ? up(8 * cells3 * K) : 0;                    // time-integrated concentration (S 8(f)3)
     L.total = o;
     return L;
@@ -268,6 +269,8 @@ void base_args(const lpm_handle *h, StepArgs &A)
     A.dep = (double *)(h->ws + h->L.dep);
     A.dep_stride = (uint64_t)h->cg.nx * h->cg.ny;
     A.bern = h->prm.dep_mode == 1 ? 1 : 0;
+    A.eq3 = h->met.kz_mode == 1 ? 1 : 0;
+    A.surf = A.eq3 ? (const float4 *)(h->ws + h->L.surf) : nullptr;
     A.any_dep = (!A.bern && (h->dry_mode != kDryNone || h->rain_on)) ? 1 : 0;
     for (int w = 0; w < 2 * LPM_MAX_NUCLIDES; ++w) {
         // S = largest power of two <= 2^20 / (largest possible increment): activity <= dep_bound, one step
@@ -362,6 +365,12 @@ int ensure_blend(lpm_handle *h, StepArgs &A, int m, int m_max)
         if (h->blend_n == 0) {
             CK(launch_transpose(met, blend, g.nx, g.ny, g.nz, h->st));
             h->launches++;
+            if (h->met.kz_mode == 1) {  // R12: the single snapshot of the 2-D fields, as it is
+                const float a0 = 0.0f;
+                CK(launch_blend_surface((const float4 *)h->met.surface_dev, (const float4 *)h->met.surface_dev, (float4 *)(h->ws + h->L.surf),
+                                        (uint64_t)g.nx * g.ny, 1, &a0, h->st));
+                h->launches++;
+            }
             h->blend_n = 1;
         }
         for (int s = 0; s < m; ++s) A.tab[s].buf = 0;
@@ -404,6 +413,12 @@ int ensure_blend(lpm_handle *h, StepArgs &A, int m, int m_max)
         }
         CK(launch_blend(h->ws + h->L.pair, blend, A.snap_cells, cnt, a, &box, h->st));
         h->launches++;
+        if (h->met.kz_mode == 1) {  // R12: the 2-D fields (u*, 1/L, Hz) of the same steps
+            const uint64_t c2 = (uint64_t)g.nx * g.ny;
+            const float4 *sf = (const float4 *)h->met.surface_dev;
+            CK(launch_blend_surface(sf + (uint64_t)sn * c2, sf + (uint64_t)(sn + 1) * c2, (float4 *)(h->ws + h->L.surf), c2, cnt, a, h->st));
+            h->launches++;
+        }
         h->blend_step0 = h->step;
         h->blend_n = cnt;
     }
@@ -456,6 +471,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     *out = nullptr;
     if (!grid_ok(cg) || !met || !grid_ok(&met->grid) || !nuc || !p || !ws || K < 1 || K > LPM_MAX_NUCLIDES)
         return LPM_ERR_INVALID_ARG;
+    if (met->kz_mode < 0 || met->kz_mode > 1 || (met->kz_mode == 1 && (!met->surface_dev || ((uintptr_t)met->surface_dev & 15)))) return LPM_ERR_INVALID_ARG;
     if (met->nt < 1 || met->nt > 32767 || !met->fields_dev || ((uintptr_t)met->fields_dev & 15) || ((uintptr_t)ws & 255))
         return LPM_ERR_INVALID_ARG;
     if (!(p->dt > 0) || p->capacity == 0 || p->capacity >= (1ull << 32) || !(met->H_mix > 0) || met->Kh < 0 ||
@@ -499,7 +515,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         h->wet_scale[k] = keep_dry * (double)h->p_wet[k];
     }
     h->dry_mode = !any_dry ? kDryNone : (eligible_everywhere ? kDryUniform : kDryLayer);
-    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode, p->dep_mode == 1);
+    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode, p->dep_mode == 1, met->kz_mode == 1);
     if (cudaMemsetAsync(ws, 0, L.total, h->st) != cudaSuccess) { delete h; return LPM_ERR_CUDA; }
     h->launches++;
     *out = h;

@@ -51,6 +51,7 @@ struct StepArgs {
     // meteorology (a0): `blend` = the library's z-fastest float4 buffers [n_buf][cells]; buffer
     // tab[s].buf holds the field at the time of fused step s, F(t_n) = F_s + a (F_s+1 - F_s)
     const float4 *blend;
+    const float4 *surf;   // kz_mode 1 (R12): time-blended 2-D fields (u*, 1/L, Hz, -) [n_buf][ny][nx], x fastest; else null
     uint64_t snap_cells;  // cells per snapshot
     GridF mg;
     float bx0, bx1, by0, by1;  // lateral boundary (met box), fp32
@@ -60,6 +61,7 @@ struct StepArgs {
     uint64_t dep_stride;
     float dep_scale[2 * LPM_MAX_NUCLIDES];       // fixed-point scales of the CTA-private deposit sums (powers of two): [2k] dry, [2k+1] wet
     double dep_inv_scale[2 * LPM_MAX_NUCLIDES];  // their inverses
+    int32_t eq3, pad3_;                      // kz_mode 1: Kz from Eq.(3) per particle
     int32_t any_dep, bern;                   // some sink deposits through the tables; dep_mode 1: Bernoulli deposition (R11)
     // physics
     float dt, sigma_h, kz_min, H, h_dep;
@@ -127,7 +129,7 @@ struct BinArgs {
 
 // launchers implemented in the .cu files; all return the cudaError of the launch
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int grid_blocks, cudaStream_t st);
-int step_max_blocks_per_sm(int K, bool compact, int dry_mode, bool bern);
+int step_max_blocks_per_sm(int K, bool compact, int dry_mode, bool bern, bool eq3);
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
                                 uint32_t *perm, cudaStream_t st);
@@ -139,6 +141,7 @@ uint64_t sort_partial_entries(uint64_t n_cells);
 cudaError_t run_probe(int kind, uint64_t footprint_bytes, void *scratch_dev, uint64_t scratch_bytes, int reps, double *ops,
                       cudaStream_t st);
 cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, int nx, int ny, int nz, uint32_t *uvmax, cudaStream_t st);
+cudaError_t launch_blend_surface(const float4 *s0, const float4 *s1, float4 *out, uint64_t cells2, int m, const float *a, cudaStream_t st);
 cudaError_t launch_transpose(const float4 *s0, float4 *out, int nx, int ny, int nz, cudaStream_t st);
 // plume mask (a0): blend only the met columns a particle can reach during the coming launch.  The met
 // columns are grouped in tiles of kMaskTile x kMaskTile; the step kernel flags the tiles that hold a
