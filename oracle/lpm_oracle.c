@@ -58,6 +58,8 @@ typedef struct {
     int32_t dep_mode;      /* 0: expected-mass deposition (R8); 1: paper-literal Bernoulli deposition (R11) */
     int32_t kz_mode;       /* 0: Kz is the interpolated gridded field (R4); 1: Eq.(3) per particle (R12)    */
     const float *surface;  /* kz_mode 1: borrowed, [nt][ny][nx][4] = (u*, 1/L, Hz, unused), x fastest         */
+    const double *z_levels; /* NULL: uniform levels z0 + (k + 1/2) dz; else borrowed, mgrid.nz ascending heights of
+                             * the met levels ("vertical weather information is nonlinear")     */
 } orc_config;
 
 typedef struct {
@@ -176,13 +178,27 @@ static void axis_weights(double p, double p0, double dp, int32_t n, int32_t *i0,
     *f = g - (double)lo;
 }
 
-static void sample_snapshot(const orc_grid *g, const float *snap, double x, double y, double z, double out[4])
+/* non-uniform levels (L110): linear between the two levels that bracket z, clamped below the first and above
+ * the last level; k0 = the last level at or below z, at most n - 2 */
+static void level_weights(double z, const double *zl, int32_t n, int32_t *k0, int32_t *k1, double *f)
+{
+    if (n < 2) { *k0 = *k1 = 0; *f = 0.0; return; }
+    int32_t k = 0;
+    while (k < n - 2 && zl[k + 1] <= z) ++k;
+    double w = (z - zl[k]) / (zl[k + 1] - zl[k]);
+    if (w < 0.0) w = 0.0;
+    if (w > 1.0) w = 1.0;
+    *k0 = k; *k1 = k + 1; *f = w;
+}
+
+static void sample_snapshot(const orc_grid *g, const double *levels, const float *snap, double x, double y, double z, double out[4])
 {
     int32_t i0, i1, j0, j1, k0, k1;
     double fx, fy, fz;
     axis_weights(x, g->x0, g->dx, g->nx, &i0, &i1, &fx);
     axis_weights(y, g->y0, g->dy, g->ny, &j0, &j1, &fy);
-    axis_weights(z, g->z0, g->dz, g->nz, &k0, &k1, &fz);
+    if (levels) level_weights(z, levels, g->nz, &k0, &k1, &fz);
+    else axis_weights(z, g->z0, g->dz, g->nz, &k0, &k1, &fz);
     const int32_t I[2] = {i0, i1}, J[2] = {j0, j1}, Kk[2] = {k0, k1};
     const double wx[2] = {1.0 - fx, fx}, wy[2] = {1.0 - fy, fy}, wz[2] = {1.0 - fz, fz};
     for (int c = 0; c < 4; ++c) out[c] = 0.0;
@@ -211,20 +227,27 @@ void orc_time_weight(int32_t nt, double t0, double dt_snap, double t, int32_t *s
     *a_out = (float)a;
 }
 
-void orc_sample_met(const orc_grid *g, int32_t nt, double t0, double dt_snap, const float *fields,
-                    double t, double x, double y, double z, double out[4])
+/* levels == NULL: uniform vertical levels (R4); else the nz ascending level heights (L110) */
+void orc_sample_met_levels(const orc_grid *g, const double *levels, int32_t nt, double t0, double dt_snap, const float *fields,
+                           double t, double x, double y, double z, double out[4])
 {
     int32_t s; float a;
     size_t snap_elems = (size_t)g->nx * g->ny * g->nz * 4;
     orc_time_weight(nt, t0, dt_snap, t, &s, &a);
     double A[4], B[4];
-    sample_snapshot(g, fields + (size_t)s * snap_elems, x, y, z, A);
+    sample_snapshot(g, levels, fields + (size_t)s * snap_elems, x, y, z, A);
     if (nt > 1) {
-        sample_snapshot(g, fields + (size_t)(s + 1) * snap_elems, x, y, z, B);
+        sample_snapshot(g, levels, fields + (size_t)(s + 1) * snap_elems, x, y, z, B);
         for (int c = 0; c < 4; ++c) out[c] = (1.0 - (double)a) * A[c] + (double)a * B[c];
     } else {
         for (int c = 0; c < 4; ++c) out[c] = A[c];
     }
+}
+
+void orc_sample_met(const orc_grid *g, int32_t nt, double t0, double dt_snap, const float *fields,
+                    double t, double x, double y, double z, double out[4])
+{
+    orc_sample_met_levels(g, NULL, nt, t0, dt_snap, fields, t, x, y, z, out);
 }
 
 /* ------------------------------------------------------------------ R12: Eq.(3) per particle
@@ -431,7 +454,7 @@ static void step_particle(orc_sim *s, uint64_t i, uint64_t n, double t_n, int ra
     orc_normals(c->seed, s->pid[i], n, nrm);
 
     /* R4: weather at X_old, t_n (forward Euler; Eq.(1) uses the wind at the old position) */
-    orc_sample_met(&c->mgrid, c->nt, c->t0, c->dt_snap, c->fields, t_n, s->x[i], s->y[i], s->z[i], met);
+    orc_sample_met_levels(&c->mgrid, c->z_levels, c->nt, c->t0, c->dt_snap, c->fields, t_n, s->x[i], s->y[i], s->z[i], met);
     double u = met[0], v = met[1], w = met[2], Kz = met[3];
     if (c->kz_mode == 1) { /* R12: "computing the turbulent diffusion coefficient" per particle (L106, L112-113) */
         double sf[3];

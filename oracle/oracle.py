@@ -45,7 +45,7 @@ class Config(C.Structure):
                 ("rx0", C.c_double), ("rx1", C.c_double), ("ry0", C.c_double), ("ry1", C.c_double),
                 ("rt0", C.c_double), ("rt1", C.c_double),
                 ("frag_delta", C.c_double), ("face_delta", C.c_double),
-                ("dep_mode", C.c_int32), ("kz_mode", C.c_int32), ("surface", C.c_void_p)]
+                ("dep_mode", C.c_int32), ("kz_mode", C.c_int32), ("surface", C.c_void_p), ("z_levels", C.c_void_p)]
 
 
 class Source(C.Structure):
@@ -100,6 +100,8 @@ def lib():
         L.orc_time_weight.argtypes = [C.c_int32, C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
         L.orc_sample_met.argtypes = [C.POINTER(Grid), C.c_int32, C.c_double, C.c_double, C.c_void_p,
                                      C.c_double, C.c_double, C.c_double, C.c_double, C.c_void_p]
+        L.orc_sample_met_levels.argtypes = [C.POINTER(Grid), C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_void_p,
+                                            C.c_double, C.c_double, C.c_double, C.c_double, C.c_void_p]
         L.orc_kz_eq3.argtypes = [C.c_double] * 4
         L.orc_kz_eq3.restype = C.c_double
         L.orc_sample_surface.argtypes = [C.POINTER(Grid), C.c_int32, C.c_double, C.c_double, C.c_void_p,
@@ -153,11 +155,12 @@ def time_weight(nt, t0, dt_snap, t):
     return s.value, a.value
 
 
-def sample_met(grid, nt, t0, dt_snap, fields, t, x, y, z):
+def sample_met(grid, nt, t0, dt_snap, fields, t, x, y, z, z_levels=None):
     f = np.ascontiguousarray(fields, dtype=np.float32)
     out = np.zeros(4, dtype=np.float64)
     g = _grid(grid)
-    lib().orc_sample_met(C.byref(g), nt, t0, dt_snap, _p(f), t, x, y, z, _p(out))
+    lv = None if z_levels is None else np.ascontiguousarray(z_levels, dtype=np.float64)
+    lib().orc_sample_met_levels(C.byref(g), None if lv is None else lv.ctypes.data, nt, t0, dt_snap, _p(f), t, x, y, z, _p(out))
     return out
 
 
@@ -204,6 +207,11 @@ class OracleSim:
             cfg.rt0, cfg.rt1 = w.rain.t_start, w.rain.t_end
         cfg.frag_delta, cfg.face_delta = frag_delta, face_delta
         cfg.dep_mode = dep_mode
+        self._levels = None
+        if getattr(w, "z_levels", None) is not None:
+            self._levels = np.ascontiguousarray(w.z_levels, dtype=np.float64)
+            assert self._levels.shape == (w.mgrid.nz,)
+            cfg.z_levels = self._levels.ctypes.data
         self._surface = None
         if getattr(w, "kz_mode", 0) == 1:
             self._surface = np.ascontiguousarray(w.surface(), dtype=np.float32)

@@ -474,3 +474,25 @@ def test_eq3_mode_equals_gridded_mode_at_cell_centre_heights():
     for k in ("x", "y", "z"):
         np.testing.assert_allclose(res[0][k], res[1][k], rtol=0, atol=2e-5)   # fp32 field values vs fp64 formula
     assert np.abs(res[0]["z"] - z).max() > 1.0
+
+
+# ------------------------------------------------------------------ P18: non-uniform vertical levels
+def test_nonuniform_levels_reproduce_piecewise_linear_profiles():
+    """Values given on non-uniform levels: the sample is the linear interpolant between the bracketing levels
+    (numpy.interp is the textbook definition), clamped outside; uniform levels given explicitly change nothing."""
+    g = Grid(6, 5, 7, 0.0, 0.0, 0.0, 100.0, 100.0, 40.0)
+    zl = np.array([5.0, 20.0, 50.0, 110.0, 230.0, 470.0, 950.0])
+    prof = np.array([1.0, 2.5, 3.0, 4.75, 4.0, 6.5, 7.0])
+    f = np.zeros((1, g.nz, g.ny, g.nx, 4), dtype=np.float32)
+    f[0, :, :, :, 0] = prof[:, None, None]
+    f[0, :, :, :, 3] = (2.0 * prof)[:, None, None]
+    rng = np.random.default_rng(2)
+    for z in list(rng.uniform(-20.0, 1100.0, 300)) + list(zl) + [0.0, 5.0, 950.0, 2000.0]:
+        got = orc.sample_met(g, 1, 0.0, 3600.0, f, 0.0, 250.0, 250.0, float(z), z_levels=zl)
+        want = np.interp(z, zl, prof)
+        assert got[0] == pytest.approx(want, rel=1e-12) and got[3] == pytest.approx(2 * want, rel=1e-12)
+    zu = g.z0 + (np.arange(g.nz) + 0.5) * g.dz
+    for z in rng.uniform(-20.0, 320.0, 100):
+        a = orc.sample_met(g, 1, 0.0, 3600.0, f, 0.0, 130.0, 310.0, float(z), z_levels=zu)
+        b = orc.sample_met(g, 1, 0.0, 3600.0, f, 0.0, 130.0, 310.0, float(z))
+        np.testing.assert_allclose(a, b, rtol=1e-13, atol=1e-15)

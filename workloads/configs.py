@@ -101,6 +101,7 @@ class Workload:
     met_fn: object = field(default=None, repr=False)   # (t, Z, Y, X) -> u, v, w, kz  in float64
     kz_mode: int = 0                                   # 1: Kz from Eq.(3) per particle (R12) with the 2-D fields below
     surface_fn: object = field(default=None, repr=False)   # (t, Y, X) -> ustar, 1/L, Hz  in float64 (cell centres)
+    z_levels: object = None                            # None: uniform levels; else mgrid.nz ascending level heights, m
     _fields: object = field(default=None, repr=False)
 
     @property
@@ -114,12 +115,14 @@ class Workload:
             xc = g.x0 + (np.arange(g.nx, dtype=np.float64) + 0.5) * g.dx
             yc = g.y0 + (np.arange(g.ny, dtype=np.float64) + 0.5) * g.dy
             zc = g.z0 + (np.arange(g.nz, dtype=np.float64) + 0.5) * g.dz
+            if self.z_levels is not None:
+                zc = np.asarray(self.z_levels, dtype=np.float64)
             Z, Y, X = np.meshgrid(zc, yc, xc, indexing="ij")
             out = np.empty((self.nt, g.nz, g.ny, g.nx, 4), dtype=np.float32)
             recipe = getattr(self.met_fn, "__name__", "") if self.met_fn in _RECIPES else None
             for s in range(self.nt):
                 t = self.t0 + s * self.dt_snap
-                key = (recipe, dataclasses.astuple(g), t)
+                key = (recipe, dataclasses.astuple(g), t, None if self.z_levels is None else tuple(np.asarray(self.z_levels).tolist()))
                 if recipe is not None and key in _SNAP_CACHE:
                     out[s] = _SNAP_CACHE[key]
                     continue
@@ -149,7 +152,7 @@ class Workload:
 
     def replace(self, **kw) -> "Workload":
         w = dataclasses.replace(self, **kw)
-        if "mgrid" in kw or "nt" in kw or "met_fn" in kw or "t0" in kw or "dt_snap" in kw:
+        if "mgrid" in kw or "nt" in kw or "met_fn" in kw or "t0" in kw or "dt_snap" in kw or "z_levels" in kw:
             w._fields = None
         return w
 
