@@ -71,6 +71,10 @@ typedef struct {
     double Kh, H_mix, kz_min;
     const void *surface_dev;  /* kz_mode 1: float4 (u* [m/s], 1/L [1/m], Hz [m], unused) [nt][ny][nx], x fastest,
                                * 16-byte aligned, borrowed like fields_dev; else ignored (may be NULL)             */
+    const double *z_levels_host; /* NULL: uniform vertical levels z0 + (k + 1/2) dz.  Else HOST array of grid.nz
+                               * strictly ascending level heights [m] ("vertical weather information is
+                               * nonlinear"; nz <= 64): linear between the bracketing levels, clamped outside;
+                               * copied (as fp32) by lpm_create                                                    */
 } lpm_meteo;
 
 /* Isotope constants. half_life_s <= 0 means stable. */

@@ -46,7 +46,7 @@ class lpm_grid(C.Structure):
 class lpm_meteo(C.Structure):
     _fields_ = [("grid", lpm_grid), ("nt", C.c_int32), ("kz_mode", C.c_int32), ("t0", C.c_double),
                 ("dt_snap", C.c_double), ("fields_dev", C.c_void_p), ("Kh", C.c_double), ("H_mix", C.c_double),
-                ("kz_min", C.c_double), ("surface_dev", C.c_void_p)]
+                ("kz_min", C.c_double), ("surface_dev", C.c_void_p), ("z_levels_host", C.c_void_p)]
 
 
 class lpm_nuclide(C.Structure):
@@ -191,6 +191,10 @@ class Simulation:
         met = lpm_meteo(grid=_grid(w.mgrid), nt=w.nt, t0=w.t0, dt_snap=w.dt_snap, fields_dev=fields_dev.data_ptr(),
                         Kh=w.Kh, H_mix=w.H_mix, kz_min=w.kz_min, kz_mode=kz_mode,
                         surface_dev=self.surface_dev.data_ptr() if self.surface_dev is not None else None)
+        self._levels = None
+        if getattr(w, "z_levels", None) is not None:
+            self._levels = np.ascontiguousarray(w.z_levels, dtype=np.float64)
+            met.z_levels_host = self._levels.ctypes.data
         nucs = (lpm_nuclide * w.K)(*[lpm_nuclide(n.half_life_s, n.vd, n.lambda_wet) for n in w.nuclides])
         prm = lpm_params(dt=w.dt, seed=w.seed, capacity=w.capacity,
                          boundary_mode=1 if w.boundary_mode == "absorb" else 0, compact=1 if w.compact else 0,
@@ -420,6 +424,10 @@ def sample_kernel(w, t, xyz):
     out = torch.empty_like(p)
     met = lpm_meteo(grid=_grid(w.mgrid), nt=w.nt, t0=w.t0, dt_snap=w.dt_snap, fields_dev=f.data_ptr(), Kh=w.Kh,
                     H_mix=w.H_mix, kz_min=w.kz_min)
+    levels = None
+    if getattr(w, "z_levels", None) is not None:
+        levels = np.ascontiguousarray(w.z_levels, dtype=np.float64)
+        met.z_levels_host = levels.ctypes.data
     rc = load().lpm_test_sample(C.byref(met), t, p.data_ptr(), p.shape[0], out.data_ptr(), torch.cuda.current_stream().cuda_stream)
     if rc:
         raise LpmError(rc, "lpm_test_sample")

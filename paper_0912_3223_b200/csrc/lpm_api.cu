@@ -68,9 +68,14 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
 
 // zfast: strides of the library's z-fastest met buffers; otherwise x-fastest (only nx, ny, nz, the
 // corner and the inverse spacings matter for the binning grid)
-GridF gridf(const lpm_grid &g, bool zfast = false)
+GridF gridf(const lpm_grid &g, bool zfast = false, const float *levels = nullptr)
 {
     GridF f;
+    memset(&f, 0, sizeof(f));
+    if (levels) {
+        f.nlev = g.nz;
+        for (int k = 0; k < g.nz && k < kMaxLevels; ++k) f.zlev[k] = levels[k];
+    }
     f.nx = g.nx; f.ny = g.ny; f.nz = g.nz;
     f.x0 = (float)g.x0; f.y0 = (float)g.y0; f.z0 = (float)g.z0;
     f.inv_dx = (float)(1.0 / g.dx); f.inv_dy = (float)(1.0 / g.dy); f.inv_dz = (float)(1.0 / g.dz);
@@ -105,6 +110,8 @@ struct lpm_handle {
     lpm_meteo met;
     lpm_nuclide nuc[LPM_MAX_NUCLIDES];
     lpm_params prm;
+    bool has_levels;
+    float zlev[kMaxLevels];   // non-uniform level heights (fp32 parameters), copied from meteo.z_levels_host
     int K;
     cudaStream_t st;
     char *ws;
@@ -262,7 +269,7 @@ void base_args(const lpm_handle *h, StepArgs &A)
     A.blend = (const float4 *)(h->ws + h->L.blend);
     const lpm_grid &mg = h->met.grid;
     A.snap_cells = (uint64_t)mg.nx * mg.ny * mg.nz;
-    A.mg = gridf(mg, true);
+    A.mg = gridf(mg, true, h->has_levels ? h->zlev : nullptr);
     A.bx0 = (float)mg.x0; A.bx1 = (float)(mg.x0 + mg.nx * mg.dx);
     A.by0 = (float)mg.y0; A.by1 = (float)(mg.y0 + mg.ny * mg.dy);
     A.cg = gridf(h->cg);
@@ -472,6 +479,10 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     if (!grid_ok(cg) || !met || !grid_ok(&met->grid) || !nuc || !p || !ws || K < 1 || K > LPM_MAX_NUCLIDES)
         return LPM_ERR_INVALID_ARG;
     if (met->kz_mode < 0 || met->kz_mode > 1 || (met->kz_mode == 1 && (!met->surface_dev || ((uintptr_t)met->surface_dev & 15)))) return LPM_ERR_INVALID_ARG;
+    if (met->z_levels_host) {
+        if (met->grid.nz > kMaxLevels) return LPM_ERR_INVALID_ARG;
+        for (int k = 1; k < met->grid.nz; ++k) if (!(met->z_levels_host[k] > met->z_levels_host[k - 1])) return LPM_ERR_INVALID_ARG;
+    }
     if (met->nt < 1 || met->nt > 32767 || !met->fields_dev || ((uintptr_t)met->fields_dev & 15) || ((uintptr_t)ws & 255))
         return LPM_ERR_INVALID_ARG;
     if (!(p->dt > 0) || p->capacity == 0 || p->capacity >= (1ull << 32) || !(met->H_mix > 0) || met->Kh < 0 ||
@@ -490,6 +501,9 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     lpm_handle *h = new (std::nothrow) lpm_handle();
     if (!h) return LPM_ERR_INVALID_ARG;
     h->cg = *cg; h->met = *met; h->prm = *p; h->K = K;
+    h->has_levels = met->z_levels_host != nullptr;
+    if (h->has_levels) for (int k = 0; k < met->grid.nz; ++k) h->zlev[k] = (float)met->z_levels_host[k];
+    h->met.z_levels_host = nullptr;  // copied: the caller's array is not needed after lpm_create
     for (int k = 0; k < K; ++k) h->nuc[k] = nuc[k];
     h->st = (cudaStream_t)stream;
     h->ws = (char *)ws;
@@ -515,7 +529,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         h->wet_scale[k] = keep_dry * (double)h->p_wet[k];
     }
     h->dry_mode = !any_dry ? kDryNone : (eligible_everywhere ? kDryUniform : kDryLayer);
-    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode, p->dep_mode == 1, met->kz_mode == 1);
+    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode, p->dep_mode == 1, met->kz_mode == 1, met->z_levels_host != nullptr);
     if (cudaMemsetAsync(ws, 0, L.total, h->st) != cudaSuccess) { delete h; return LPM_ERR_CUDA; }
     h->launches++;
     *out = h;
@@ -1097,7 +1111,12 @@ int32_t lpm_test_sample(const lpm_meteo *met, double t, const void *xyz, uint64_
     } else {
         rc = launch_transpose(f, blend, g.nx, g.ny, g.nz, s);
     }
-    if (rc == cudaSuccess) rc = launch_test_sample(blend, gridf(g, true), (float)met->kz_min, (const float4 *)xyz, n, (float4 *)out, s);
+    float lev[kMaxLevels];
+    if (met->z_levels_host) {
+        if (g.nz > kMaxLevels) { cudaFree(blend); if (pair) cudaFree(pair); return LPM_ERR_INVALID_ARG; }
+        for (int k = 0; k < g.nz; ++k) lev[k] = (float)met->z_levels_host[k];
+    }
+    if (rc == cudaSuccess) rc = launch_test_sample(blend, gridf(g, true, met->z_levels_host ? lev : nullptr), (float)met->kz_min, (const float4 *)xyz, n, (float4 *)out, s);
     const cudaError_t rs = cudaStreamSynchronize(s);
     if (rc == cudaSuccess) rc = rs;
     cudaFree(blend);

@@ -263,11 +263,11 @@ cudaError_t launch_test_box_muller(const uint32_t *r, uint64_t n, float *out, cu
     return cudaGetLastError();
 }
 
-__global__ void test_sample_kernel(const float4 *blend, GridF mg, float kz_min, const float4 *xyz, uint64_t n, float4 *out)
+__global__ void test_sample_kernel(const float4 *blend, const __grid_constant__ GridF mg, float kz_min, const float4 *xyz, uint64_t n, float4 *out)
 {
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
         const float4 p = xyz[i];
-        const Corner c = corner_of(mg, p.x, p.y, p.z);
+        const Corner c = mg.nlev ? corner_of<true>(mg, p.x, p.y, p.z) : corner_of<false>(mg, p.x, p.y, p.z);
         float4 m = trilinear(blend, c, mg);   // the step kernel's sampling of a blended buffer
         m.w = fmaxf(m.w, kz_min);
         out[i] = m;

@@ -10,6 +10,7 @@ namespace lpm {
 
 constexpr int kMaxFused = 16;        // model steps fused into one launch (table lives in kernel params)
 constexpr int kBlendDepth = kMaxFused;  // time-blended met buffers kept: one per fused step
+constexpr int kMaxLevels = 64;       // non-uniform vertical met levels held in the kernel parameters
 constexpr int kSortPeriod = 32;      // model steps between two gather-locality sorts of a release
 constexpr int kStepThreads = 256;    // CTA size of the step kernel
 constexpr int kScanTile = 4 * kStepThreads;  // particles per look-back tile (compaction): 4 per thread
@@ -39,6 +40,8 @@ struct GridF {  // fp32 view of a grid, exactly as the kernels use it
     uint32_t ex, ey, ez;       // element strides of cell (i, j, k) in the sampled buffer: z-fastest (nz, nx*nz, 1)
                                // for the library's met buffers (x-fastest (1, nx, nx*ny) is the caller's layout)
     uint32_t sx, sy, sz;       // stride to the upper corner on each axis: n > 1 ? e : 0
+    int32_t nlev;              // 0: uniform vertical levels; else nz non-uniform level heights, ascending
+    float zlev[kMaxLevels];
 };
 
 enum DryMode : int32_t { kDryNone = 0, kDryUniform = 1, kDryLayer = 2 };
@@ -129,7 +132,7 @@ struct BinArgs {
 
 // launchers implemented in the .cu files; all return the cudaError of the launch
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int grid_blocks, cudaStream_t st);
-int step_max_blocks_per_sm(int K, bool compact, int dry_mode, bool bern, bool eq3);
+int step_max_blocks_per_sm(int K, bool compact, int dry_mode, bool bern, bool eq3, bool zlev);
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
                                 uint32_t *perm, cudaStream_t st);

@@ -21,15 +21,15 @@ constexpr int kScanBlock = 256 * kScanItems;         // items per block
 // L1 sector per gather instruction instead of one per lane (the L1 data pipe delivers one 32-byte
 // sector per cycle; with keys by containing cell a warp still spans the 8 octants = up to 8 lower
 // corners).  Exited slots go to the last bucket, n_keys - 1.
-__global__ void __launch_bounds__(256) sort_key_kernel(const float4 *__restrict__ xyzq, uint64_t n, GridF g, uint32_t n_keys,
+__global__ void __launch_bounds__(256) sort_key_kernel(const float4 *__restrict__ xyzq, uint64_t n, const __grid_constant__ GridF g, uint32_t n_keys,
                                                        uint32_t *__restrict__ keys, uint32_t *__restrict__ hist,
                                                        const uint64_t *__restrict__ n_dev = nullptr)
 {
-    if (n_dev) n = *n_dev;
+    if (n_dev) n = *n_dev;  // (n is a by-value parameter: a local copy)
     for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n; l += (uint64_t)gridDim.x * blockDim.x) {
         const float4 p = xyzq[l];
         uint32_t key = n_keys - 1;
-        if (p.z >= 0.0f) key = corner_of(g, p.x, p.y, p.z).o;
+        if (p.z >= 0.0f) key = g.nlev ? corner_of<true>(g, p.x, p.y, p.z).o : corner_of<false>(g, p.x, p.y, p.z).o;
         keys[l] = key;
         atomicAdd(hist + key, 1u);
     }

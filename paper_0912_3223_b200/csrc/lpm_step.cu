@@ -121,13 +121,13 @@ __device__ __forceinline__ void deposit_at(const StepArgs &A, float x, float y, 
 // One model step of one particle.  Returns false when the particle left the domain (ABSORB).
 // Source order = intended issue order: the eight gathers go out first and the ~150 instructions of
 // Philox + Box-Muller run while they are in flight.
-template <int K, int DRY, bool BERN, bool EQ3>
+template <int K, int DRY, bool BERN, bool EQ3, bool ZLEV>
 __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e, uint32_t step_lo,
                                           uint32_t pid_lo, float &x, float &y, float &z,
                                           float (&q)[K], Acc<K> &acc, DepTab<K> &dep)
 {
     // a0 + a2: weather at X_old, t_n
-    const Corner c = corner_of(A.mg, x, y, z);
+    const Corner c = corner_of<ZLEV>(A.mg, x, y, z);
     const float4 m = trilinear(A.blend + (uint64_t)e.buf * A.snap_cells, c, A.mg);
     // Kz: the interpolated gridded field (R4), or Eq.(3) per particle from the 2-D fields of this step (R12)
     const float kz = fmaxf(EQ3 ? kz_eq3(A.surf + (uint64_t)e.buf * (uint32_t)(A.mg.nx * A.mg.ny), c, A.mg, z) : m.w, A.kz_min);
@@ -274,7 +274,7 @@ __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &ac
 #endif
 static_assert(sizeof(StepArgs) <= 32764, "StepArgs must fit the kernel-parameter space (32764 B since CUDA 12.1 on sm_70+)");
 
-template <int K, int DRY, bool BERN, bool EQ3>
+template <int K, int DRY, bool BERN, bool EQ3, bool ZLEV>
 __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel(const __grid_constant__ StepArgs A)
 {
     __shared__ uint32_t s_ticket;
@@ -338,7 +338,7 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             bool alive = true;
             const uint32_t step0 = (uint32_t)A.step0;
             for (int s = 0; s < A.m_steps; ++s)
-                if (alive & (s >= s_begin)) alive = step_once<K, DRY, BERN, EQ3>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, T);
+                if (alive & (s >= s_begin)) alive = step_once<K, DRY, BERN, EQ3, ZLEV>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, T);
             if (!alive) z = -1.0f - z;  // exit position kept, slot marked inactive
             A.xyzq[slot] = make_float4(x, y, z, q[0]);
             if (K > 1) A.q1[slot] = q[1];
@@ -351,7 +351,7 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
         }
         if (A.keys_out && in_range) {
             // pass 1 of the coming gather-locality sort, for free: the new position is in registers
-            const uint32_t key = (valid && z >= 0.0f) ? corner_of(A.mg, x, y, z).o : A.n_keys - 1u;
+            const uint32_t key = (valid && z >= 0.0f) ? corner_of<ZLEV>(A.mg, x, y, z).o : A.n_keys - 1u;
             A.keys_out[l] = key;
             atomicAdd(A.hist_out + key, 1u);
         }
@@ -381,7 +381,7 @@ __device__ __forceinline__ void st_state(uint64_t *p, uint64_t v)
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-template <int K, int DRY, bool BERN, bool EQ3>
+template <int K, int DRY, bool BERN, bool EQ3, bool ZLEV>
 __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid_constant__ StepArgs A)
 {
     constexpr int kItems = kScanTile / kStepThreads;  // particles per thread and tile: amortises the tile's barriers and look-back
@@ -430,7 +430,7 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
 #pragma unroll
         for (int j = 0; j < kItems; ++j) {
             const uint64_t i = (uint64_t)tile * kScanTile + (uint32_t)j * kStepThreads + threadIdx.x;
-            if (i < n) alive[j] = step_once<K, DRY, BERN, EQ3>(A, A.tab[0], (uint32_t)A.step0, pid[j], x[j], y[j], z[j], q[j], acc, T);
+            if (i < n) alive[j] = step_once<K, DRY, BERN, EQ3, ZLEV>(A, A.tab[0], (uint32_t)A.step0, pid[j], x[j], y[j], z[j], q[j], acc, T);
             // survivors: rank inside the (item, warp) part
             const uint32_t ball = __ballot_sync(0xffffffffu, alive[j]);
             rank[j] = __popc(ball & ((1u << lane) - 1u));
@@ -540,40 +540,41 @@ __global__ void __launch_bounds__(256) inject_kernel(const __grid_constant__ Inj
 // ------------------------------------------------------------------ launchers
 typedef void (*StepKernel)(const StepArgs);
 
-// One instantiation per (nuclide count, dry-deposition mode, expected-mass / Bernoulli deposition, gridded / Eq.(3) Kz).
-template <int K, bool BERN, bool EQ3>
+// One instantiation per (nuclide count, dry-deposition mode, expected-mass / Bernoulli deposition, gridded / Eq.(3) Kz, uniform / non-uniform levels).
+template <int K, bool BERN, bool EQ3, bool ZLEV>
 static StepKernel pick_dry(bool compact, int dry)
 {
     if (compact) {
-        if (dry == kDryNone) return step_compact_kernel<K, kDryNone, BERN, EQ3>;
-        return dry == kDryUniform ? step_compact_kernel<K, kDryUniform, BERN, EQ3> : step_compact_kernel<K, kDryLayer, BERN, EQ3>;
+        if (dry == kDryNone) return step_compact_kernel<K, kDryNone, BERN, EQ3, ZLEV>;
+        return dry == kDryUniform ? step_compact_kernel<K, kDryUniform, BERN, EQ3, ZLEV> : step_compact_kernel<K, kDryLayer, BERN, EQ3, ZLEV>;
     }
-    if (dry == kDryNone) return step_slots_kernel<K, kDryNone, BERN, EQ3>;
-    return dry == kDryUniform ? step_slots_kernel<K, kDryUniform, BERN, EQ3> : step_slots_kernel<K, kDryLayer, BERN, EQ3>;
+    if (dry == kDryNone) return step_slots_kernel<K, kDryNone, BERN, EQ3, ZLEV>;
+    return dry == kDryUniform ? step_slots_kernel<K, kDryUniform, BERN, EQ3, ZLEV> : step_slots_kernel<K, kDryLayer, BERN, EQ3, ZLEV>;
 }
 
-template <int K>
-static StepKernel pick_k(bool compact, int dry, bool bern, bool eq3)
+template <int K, bool BERN>
+static StepKernel pick_kb(bool compact, int dry, bool eq3, bool zlev)
 {
-    if (bern) return eq3 ? pick_dry<K, true, true>(compact, dry) : pick_dry<K, true, false>(compact, dry);
-    return eq3 ? pick_dry<K, false, true>(compact, dry) : pick_dry<K, false, false>(compact, dry);
+    if (eq3) return zlev ? pick_dry<K, BERN, true, true>(compact, dry) : pick_dry<K, BERN, true, false>(compact, dry);
+    return zlev ? pick_dry<K, BERN, false, true>(compact, dry) : pick_dry<K, BERN, false, false>(compact, dry);
 }
 
-static StepKernel pick(int K, bool compact, int dry, bool bern, bool eq3)
+static StepKernel pick(int K, bool compact, int dry, bool bern, bool eq3, bool zlev)
 {
-    return K == 1 ? pick_k<1>(compact, dry, bern, eq3) : pick_k<2>(compact, dry, bern, eq3);
+    if (K == 1) return bern ? pick_kb<1, true>(compact, dry, eq3, zlev) : pick_kb<1, false>(compact, dry, eq3, zlev);
+    return bern ? pick_kb<2, true>(compact, dry, eq3, zlev) : pick_kb<2, false>(compact, dry, eq3, zlev);
 }
 
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int blocks, cudaStream_t st)
 {
-    pick(K, compact, a.dry_mode, a.bern != 0, a.eq3 != 0)<<<blocks, kStepThreads, 0, st>>>(a);
+    pick(K, compact, a.dry_mode, a.bern != 0, a.eq3 != 0, a.mg.nlev != 0)<<<blocks, kStepThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 
-int step_max_blocks_per_sm(int K, bool compact, int dry, bool bern, bool eq3)
+int step_max_blocks_per_sm(int K, bool compact, int dry, bool bern, bool eq3, bool zlev)
 {
     int nb = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick(K, compact, dry, bern, eq3), kStepThreads, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick(K, compact, dry, bern, eq3, zlev), kStepThreads, 0);
     return nb;
 }
 

@@ -108,6 +108,35 @@ def test_met_sampling(lpm, orc, name, t):
     assert np.all(np.abs(got - want) <= 2e-5 * scale + 1e-6), np.abs(got - want).max(axis=0)
 
 
+def test_met_sampling_nonuniform_levels(lpm, orc):
+    """S§8(f)2: non-uniform vertical levels (fp32-representable heights), sampled points below, between
+    and above the levels; then an N-step run on the same levels against the oracle."""
+    zl = np.array([10.0, 30.0, 60.0, 100.0, 150.0, 210.0, 280.0, 360.0, 450.0, 550.0, 660.0, 780.0, 910.0, 1050.0, 1200.0])
+    w = make("c2", scale=0.01, n_steps=600)
+    g = w.mgrid
+    w = w.replace(mgrid=Grid(g.nx, g.ny, len(zl), g.x0, g.y0, g.z0, g.dx, g.dy, g.dz), z_levels=zl, nt=3)
+    g = w.mgrid
+    rng = np.random.default_rng(13)
+    n = 5000
+    xyz = np.stack([rng.uniform(g.x0, g.x0 + g.nx * g.dx, n), rng.uniform(g.y0, g.y0 + g.ny * g.dy, n),
+                    rng.uniform(-50.0, 1400.0, n)], axis=1).astype(np.float32)
+    xyz[:len(zl), 2] = zl
+    xyz[len(zl), 2] = 0.0
+    t = 2345.0
+    got = lpm.sample_kernel(w, t, xyz).astype(np.float64)
+    f = w.fields()
+    want = np.array([orc.sample_met(g, w.nt, w.t0, w.dt_snap, f, t, *map(float, p), z_levels=zl) for p in xyz])
+    want[:, 3] = np.maximum(want[:, 3], w.kz_min)
+    scale = np.abs(f).reshape(-1, 4).max(axis=0)
+    assert np.all(np.abs(got - want) <= 2e-5 * scale + 1e-6), np.abs(got - want).max(axis=0)
+    sim, o = lpm.Simulation(w), orc.OracleSim(w)
+    sim.step(600)
+    o.step(600)
+    gp, p = sim.get_particles_host(), o.particles()
+    assert gp["x"].shape[0] == p["x"].shape[0] > 5000
+    _n_step_compare(gp, p, w, np.zeros(len(p["x"]), dtype=bool), 0.999, "non-uniform levels")
+
+
 # ------------------------------------------------------------------ helpers for state parity
 def _random_state(w, n, rng, K):
     g = w.mgrid
