@@ -78,7 +78,8 @@ __device__ __forceinline__ void dep_flush(const StepArgs &A, DepTab<K> &T)
 template <int K>
 __device__ __forceinline__ void dep_add(const StepArgs &A, DepTab<K> &T, int slot, uint32_t cell, int k, int w, float v)
 {
-    if (slot >= 0 && v >= 131072.0f && v < 1048575.5f) atomicAdd(&T.sum[w][slot], __float2uint_rn(v));
+    const uint32_t iv = __float2uint_rn(v);  // saturating; v >= 0
+    if (slot >= 0 && iv - 131072u < 1048576u - 131072u) atomicAdd(&T.sum[w][slot], iv);   // 2^17 <= iv < 2^20: one unsigned compare
     else if (v != 0.0f) atomicAdd(A.dep + cell + k * A.dep_stride, (double)v * A.dep_inv_scale[w]);
 }
 
