@@ -275,6 +275,10 @@ int32_t lpm_probe(int32_t kind, uint64_t footprint_bytes, void *scratch_dev, uin
  * for pid = pid0 + i. */
 int32_t lpm_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n,
                         uint32_t *out_dev, void *cuda_stream);
+/* The same four words from NVIDIA's cuRAND device Philox4x32-10 (stream 0): curand_init(seed, subsequence = pid,
+ * offset = 4 * step) + curand4() - an implementation independent of both this library and the oracle
+ * (SURVEY.md 8(c) P1).  Test only. */
+int32_t lpm_test_curand_philox(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, uint32_t *out_dev, void *cuda_stream);
 /* The three N(0,1) of R3 for the same counters: out_dev[3*i..]. */
 int32_t lpm_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, float *out_dev,
                          void *cuda_stream);

@@ -27,7 +27,7 @@ SYMBOLS = (
     "lpm_deposition_f64", "lpm_bin_now", "lpm_num_active", "lpm_step_index", "lpm_mass_scale", "lpm_get_particles",
     "lpm_set_particles", "lpm_ledger", "lpm_injected", "lpm_last_error", "lpm_launch_count", "lpm_test_philox",
     "lpm_test_normals", "lpm_test_sample", "lpm_upload_meteo", "lpm_concentration_host", "lpm_deposition_host",
-    "lpm_set_timing", "lpm_get_timing", "lpm_probe", "lpm_test_box_muller", "lpm_dose",
+    "lpm_set_timing", "lpm_get_timing", "lpm_probe", "lpm_test_box_muller", "lpm_dose", "lpm_test_curand_philox",
 )
 
 
@@ -109,6 +109,7 @@ def load():
     L.lpm_get_timing.argtypes = [vp, C.POINTER(dbl)]
     L.lpm_probe.argtypes = [i32, u64, vp, u64, i32, C.POINTER(dbl), vp]
     L.lpm_test_box_muller.argtypes = [vp, u64, vp, vp]
+    L.lpm_test_curand_philox.argtypes = [u64, u64, u64, u64, vp, vp]
     L.lpm_test_philox.argtypes = [u64, u64, C.c_uint32, u64, u64, vp, vp]
     L.lpm_test_normals.argtypes = [u64, u64, u64, u64, vp, vp]
     L.lpm_test_sample.argtypes = [C.POINTER(lpm_meteo), dbl, vp, u64, vp, vp]
@@ -391,6 +392,15 @@ def philox_kernel(seed, step, stream_id, pid0, n):
     rc = load().lpm_test_philox(seed, step, stream_id, pid0, n, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
     if rc:
         raise LpmError(rc, "lpm_test_philox")
+    return out.cpu().numpy().view(np.uint32)
+
+
+def curand_philox_kernel(seed, step, pid0, n):
+    torch = _require_cuda()
+    out = torch.empty((n, 4), dtype=torch.int32, device="cuda")
+    rc = load().lpm_test_curand_philox(seed, step, pid0, n, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    if rc:
+        raise LpmError(rc, "lpm_test_curand_philox")
     return out.cpu().numpy().view(np.uint32)
 
 

@@ -1072,6 +1072,13 @@ int32_t lpm_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n
     return launch_test_normals(seed, step, pid0, n, out, (cudaStream_t)st) == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
 }
 
+int32_t lpm_test_curand_philox(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, uint32_t *out, void *st)
+{
+    if (!out) return LPM_ERR_INVALID_ARG;
+    if (!dev_ok()) return LPM_ERR_NO_DEVICE;
+    return launch_test_curand_philox(seed, step, pid0, n, out, (cudaStream_t)st) == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
+}
+
 int32_t lpm_test_box_muller(const uint32_t *r, uint64_t n, float *out, void *st)
 {
     if (!r || !out || ((uintptr_t)r & 15)) return LPM_ERR_INVALID_ARG;

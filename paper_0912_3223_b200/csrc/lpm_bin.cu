@@ -4,6 +4,8 @@
 // this on the CPU after a D2H copy and suggests a separate GPU kernel.  Here the
 // particles never leave HBM.  Cell rule R10 (exact fp32 index), counts in u32 (exact), sums of the
 // stored q in fp64 so that the result does not depend on the order of the atomics beyond 1e-16.
+#include <curand_kernel.h>
+
 #include "lpm_device.cuh"
 
 namespace lpm {
@@ -228,6 +230,24 @@ __global__ void test_philox_kernel(uint32_t seed_lo, uint32_t seed_hi, uint32_t 
 cudaError_t launch_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st)
 {
     test_philox_kernel<<<148, 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step, stream, pid0, n, out);
+    return cudaGetLastError();
+}
+
+// SURVEY.md 8(c) P1, independent cross-check: NVIDIA's own device Philox4x32-10 (cuRAND, header-only device API)
+// with seed -> key, subsequence -> (ctr.z, ctr.w) = particle id, offset / 4 -> (ctr.x, ctr.y) = step.  Test only.
+__global__ void test_curand_philox_kernel(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, uint32_t *out)
+{
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+        curandStatePhilox4_32_10_t st;
+        curand_init((unsigned long long)seed, (unsigned long long)(pid0 + i), (unsigned long long)(4 * step), &st);
+        const uint4 r = curand4(&st);
+        out[4 * i] = r.x; out[4 * i + 1] = r.y; out[4 * i + 2] = r.z; out[4 * i + 3] = r.w;
+    }
+}
+
+cudaError_t launch_test_curand_philox(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st)
+{
+    test_curand_philox_kernel<<<148, 256, 0, st>>>(seed, step, pid0, n, out);
     return cudaGetLastError();
 }
 

@@ -170,6 +170,7 @@ cudaError_t launch_import(float4 *xyzq, uint64_t n, const uint8_t *status, cudaS
 cudaError_t launch_iota(uint32_t *pid, uint64_t n, cudaStream_t st);
 cudaError_t launch_qmax(const float4 *xyzq, const float *q1, uint64_t n, int K, float *out2, cudaStream_t st);
 cudaError_t launch_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st);
+cudaError_t launch_test_curand_philox(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st);
 cudaError_t launch_test_box_muller(const uint32_t *r, uint64_t n, float *out, cudaStream_t st);
 cudaError_t launch_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, float *out, cudaStream_t st);
 cudaError_t launch_test_sample(const float4 *blend, GridF mg, float kz_min, const float4 *xyz, uint64_t n, float4 *out,

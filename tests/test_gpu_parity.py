@@ -44,6 +44,17 @@ def test_philox_bit_exact(lpm, orc):
         assert list(got[i]) == list(orc.philox_draw(1, int(i), 3, 0))
 
 
+def test_philox_equals_curand_device_philox(lpm, orc):
+    """SURVEY §8(c) P1, independent pin: NVIDIA's cuRAND device Philox4x32-10 with (seed, subsequence = id,
+    offset = 4 step) gives the same words as the library's kernel AND as the oracle."""
+    for seed, step, pid0 in ((1, 0, 0), (1, 3, 7), (4, 8639, 99_999_000), (0xDEADBEEFCAFEF00D, 21599, (1 << 32) - 300)):
+        ours = lpm.philox_kernel(seed, step, 0, pid0, 257)
+        theirs = lpm.curand_philox_kernel(seed, step, pid0, 257)
+        np.testing.assert_array_equal(ours, theirs)
+        for i in (0, 1, 31, 256):
+            assert list(theirs[i]) == list(orc.philox_draw(seed, pid0 + i, step, 0))
+
+
 def test_normals_match_oracle(lpm, orc):
     n = 50_000
     got = lpm.normals_kernel(12345, 17, 100, n).astype(np.float64)
