@@ -202,7 +202,8 @@ int32_t lpm_mass_scale(lpm_handle *h, double *scale_host /* [K] */);
  * NULL), pid_dev uint32 (may be NULL), status_dev uint8 0 = active, 1 = exited, 2 = deposited all it carried
  * (dep_mode 1) (may be NULL).
  * Buffers must hold capacity entries; *n_host receives the slot count.  Exited particles report
- * their exit position. */
+ * their exit position.  With several releases each release owns a block of slots that starts at a multiple of
+ * 64; the unused slots between two blocks read as zeros (binning, ledger and deposition skip them). */
 int32_t lpm_get_particles(lpm_handle *h, void *xyzq_dev, float *q1_dev, uint32_t *pid_dev,
                           uint8_t *status_dev, uint64_t *n_host);
 /* Replace the particle state by n slots (all treated as already born; pid_dev NULL = 0..n-1;

@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 from helpers import T_I131, custom, uniform_met
-from workloads import Grid, Nuclide, RainBox, make
+from workloads import Grid, Nuclide, RainBox, Release, make
 
 pytestmark = pytest.mark.gpu
 
@@ -577,6 +577,36 @@ def test_c5_capacity_throttle(lpm, orc):
     assert sim.num_active == o.n == 1000
     gp, p = sim.get_particles_host(), o.particles()
     np.testing.assert_array_equal(gp["pid"], p["pid"])
+
+
+def test_two_releases(lpm, orc):
+    """Two sources with different positions and release windows in one simulation (slot-addressed store, one block per
+    release, gather-locality sort forced on): ledger, counts and deposition map against the oracle."""
+    w = make("c3", scale=1.0, n_steps=1200)
+    w.release.pid_stride = 1000                          # 10000 of the 1e7 particles from the config's source
+    w = w.replace(nt=5, capacity=30_000, bin_every=400)
+    second = Release(-2.0e4, 1.0e4, 120.0, 2000.0, 9000.0, [3.0e14, 2.0e13], n_particles=12_000)
+    sim = lpm.Simulation(w, gather_sort=16)
+    o = orc.OracleSim(w, face_delta=1.5)
+    sim.release(second)
+    o.release(second)
+    sim.step(1200)
+    o.step(1200)
+    lg, lo = sim.ledger(), o.ledger()
+    for k in range(2):
+        for f in range(5):
+            if lo[k][f] > 0:                                  # (no rain before hour 6: the wet ledger is 0 on both sides)
+                assert abs(lg[k][f] / lo[k][f] - 1) < 2e-5, (k, f, lg[k][f], lo[k][f])
+            else:
+                assert lg[k][f] == 0
+    cg, co = sim.counts().cpu().numpy().astype(np.int64), o.counts().astype(np.int64)
+    assert co.sum() > 10_000 and abs(int(cg.sum()) - int(co.sum())) <= 3 and np.abs(cg - co).sum() <= 0.01 * co.sum()
+    dg = sim.deposition(f64=True).cpu().numpy()
+    do, slack = o.deposition(with_slack=True)
+    excess = np.maximum(np.abs(dg - do) - (1e-5 * do + 1.0001 * slack + 1e-30), 0.0)
+    assert excess.sum() <= 2e-3 * do.sum()
+    for k in range(2):
+        assert abs(dg[k].sum() / do[k].sum() - 1) < 1e-5
 
 
 # ------------------------------------------------------------------ edge cases
