@@ -579,6 +579,49 @@ def test_c5_capacity_throttle(lpm, orc):
     np.testing.assert_array_equal(gp["pid"], p["pid"])
 
 
+@pytest.mark.parametrize("name,stride,steps,nt", [("c4", 4000, 1440, 4), ("c3", 400, 1080, 5)])
+def test_full_size_sampled_against_oracle(lpm, orc, name, stride, steps, nt):
+    """BASELINE.json's FULL particle count in the launch configuration bench.py times (1e8 / 1e7 particles, 148 x 4
+    CTAs, gather sort, plume mask, CTA-private deposit tables): every `stride`-th particle id is an exact subset of
+    the run, so the oracle computes those trajectories one by one; plus properties that hold at any size."""
+    w = make(name, scale=1.0, n_steps=steps).replace(nt=nt)
+    sim = lpm.Simulation(w)
+    sim.step(steps)
+    p = sim.get_particles()
+    n = p["n"]
+    born = lpm.schedule_born(w.release.n_particles, 0, 1, 0, int(math.ceil((w.release.t_end - w.release.t_start) / w.dt)), steps - 1)
+    assert n == born > 1_000_000
+    idx = np.arange(0, n, stride)
+    import torch
+    sel = torch.from_numpy(idx).to(p["xyzq"].device)
+    xyzq = p["xyzq"][sel].cpu().numpy()
+    q1 = p["q1"][sel].cpu().numpy()
+    G = sim.mass_scale()
+    g = dict(x=xyzq[:, 0], y=xyzq[:, 1], z=xyzq[:, 2], m=np.stack([xyzq[:, 3].astype(np.float64) * G[0], q1.astype(np.float64) * G[1]]))
+    ws = make(name, scale=1.0, n_steps=steps)
+    ws.release.pid_stride = stride
+    ws = ws.replace(nt=nt, capacity=len(range(0, ws.release.n_particles, stride)))
+    o = orc.OracleSim(ws)
+    o.step(steps)
+    ref = o.particles()
+    assert len(ref["x"]) == len(idx) and np.array_equal(ref["pid"], idx.astype(np.uint64))
+    frag = np.isin(ref["pid"], o.fragile_pids())
+    _n_step_compare(g, ref, w, frag, 0.999, f"full-size {name}")
+    # properties at full size: the ledger closes, every born in-grid particle is counted exactly once
+    lg = sim.ledger()
+    for k in range(2):
+        assert abs((lg[k][1] + lg[k][2] + lg[k][3] + lg[k][4] + lg[k][5]) / lg[k][0] - 1) < 1e-5
+        assert abs(lg[k][0] / (w.release.total_activity[k] * born / w.release.n_particles) - 1) < 1e-12
+    cnt = sim.counts()
+    cg = w.cgrid
+    xyz = p["xyzq"]
+    inside = ((xyz[:, 0] >= cg.x0) & (xyz[:, 0] < cg.x0 + cg.nx * cg.dx) & (xyz[:, 1] >= cg.y0) & (xyz[:, 1] < cg.y0 + cg.ny * cg.dy) &
+              (xyz[:, 2] >= cg.z0) & (xyz[:, 2] < cg.z0 + cg.nz * cg.dz)).sum().item()
+    assert abs(int(cnt.sum().item()) - inside) <= 8        # fp32 face rounding of the comparison above vs R10's index rule
+    dep = sim.deposition(f64=True)
+    assert abs(float(dep.sum().item()) * cg.dx * cg.dy / (lg[0][2] + lg[0][3] + lg[1][2] + lg[1][3] - lg[0][6] - lg[1][6]) - 1) < 1e-6
+
+
 def test_two_releases(lpm, orc):
     """Two sources with different positions and release windows in one simulation (slot-addressed store, one block per
     release, gather-locality sort forced on): ledger, counts and deposition map against the oracle."""
