@@ -622,6 +622,36 @@ def test_full_size_sampled_against_oracle(lpm, orc, name, stride, steps, nt):
     assert abs(float(dep.sum().item()) * cg.dx * cg.dy / (lg[0][2] + lg[0][3] + lg[1][2] + lg[1][3] - lg[0][6] - lg[1][6]) - 1) < 1e-6
 
 
+def test_full_rate_c5_properties(lpm):
+    """C5 at BASELINE's full injection rate (4e4 particles per step, record sort on): properties that hold at any
+    size - survivors have unique ids and lie inside the domain, the ledger closes, counts = live in-grid particles."""
+    import torch
+    steps = 400
+    w = make("c5", scale=1.0, n_steps=steps).replace(nt=2)
+    sim = lpm.Simulation(w)
+    sim.step(steps)
+    p = sim.get_particles()
+    n = p["n"]
+    assert n == sim.num_active and 0.9 * 40_000 * steps < n <= 40_000 * steps
+    assert sum(sim.injected(s) for s in (0, 1, 200, 399)) == 4 * 40_000
+    pid = p["pid"]
+    assert torch.unique(pid).numel() == n and int(pid.max().item()) < 40_000 * steps
+    assert not bool((pid[1:] > pid[:-1]).all().item())          # the store was re-sorted by met cell (B7)
+    g = w.mgrid
+    xyz = p["xyzq"]
+    assert bool(((xyz[:, 0] >= g.x0) & (xyz[:, 0] < g.x0 + g.nx * g.dx) & (xyz[:, 1] >= g.y0) & (xyz[:, 1] < g.y0 + g.ny * g.dy) &
+                 (xyz[:, 2] >= 0) & (xyz[:, 2] <= w.H_mix)).all().item())
+    assert int(p["status"].max().item()) == 0
+    lg = sim.ledger()[0]
+    assert abs(lg[0] / (40_000 * steps) - 1) < 1e-12             # c5 assigns one unit of activity to every particle
+    assert abs((lg[1] + lg[4] + lg[5]) / lg[0] - 1) < 1e-5
+    cnt = sim.counts()
+    cg = w.cgrid
+    inside = ((xyz[:, 0] >= cg.x0) & (xyz[:, 0] < cg.x0 + cg.nx * cg.dx) & (xyz[:, 1] >= cg.y0) & (xyz[:, 1] < cg.y0 + cg.ny * cg.dy) &
+              (xyz[:, 2] >= cg.z0) & (xyz[:, 2] < cg.z0 + cg.nz * cg.dz)).sum().item()
+    assert abs(int(cnt.sum().item()) - inside) <= 8
+
+
 def test_two_releases(lpm, orc):
     """Two sources with different positions and release windows in one simulation (slot-addressed store, one block per
     release, gather-locality sort forced on): ledger, counts and deposition map against the oracle."""
