@@ -89,8 +89,9 @@ typedef struct {
     uint64_t seed;          /* Philox key (R1)                                                  */
     uint64_t capacity;      /* maximum number of particle slots                        */
     int32_t boundary_mode;  /* lpm_boundary_mode; the boundary is the met-grid box (R7)         */
-    int32_t compact;        /* 1: stream compaction of exited particles after every step, stable with
-                             * respect to the storage order (= id order unless gather_sort reorders) */
+    int32_t compact;        /* 1: stream compaction of exited particles after every step.  Stable (survivors keep
+                             * their order = id order) when gather_sort is off; with gather_sort on the store
+                             * is unordered (re-sorted by met cell) and holes are filled from the tail */
     double h_dep;           /* dry deposition acts where z' < h_dep; h_dep >= H_mix: everywhere */
     int32_t bin_every;      /* concentration binning cadence in steps ("n"); 0 = never   */
     int32_t steps_per_launch; /* 0 = auto (16); 1 = one model step per kernel launch; m > 1 fuses up to

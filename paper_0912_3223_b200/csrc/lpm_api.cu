@@ -664,8 +664,14 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                 }
             }
             CK(launch_inject(I, h->st));
+            // unordered store (the records are re-sorted by met cell anyway, B7): hole list + fill instead of the scan
+            A.holes = sort_enabled(&h->prm) ? (uint32_t *)(h->ws + h->L.keys) : nullptr;
             const int span = span_open(h, 0, 0.0);
             CK(launch_step(A, h->K, true, h->sms * (h->occ > 0 ? h->occ : 1), h->st));
+            if (A.holes) {
+                CK(launch_fill_holes(A.xyzq, A.q1, A.pid, A.ctrl, A.holes, (uint32_t *)(h->ws + h->L.alt_pid), (uint32_t *)(h->ws + h->L.alt_xyzq), h->st));
+                h->launches += 2;
+            }
             span_close(h, span);
             h->launches += 2;
         } else {

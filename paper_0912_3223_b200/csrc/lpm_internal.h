@@ -94,6 +94,7 @@ struct StepArgs {
     // compact mode: device-side control block
     uint64_t *ctrl;      // [0] n_active, [1] ticket, [2] n_out
     uint64_t *tile_state;
+    uint32_t *holes;     // compact + unordered store: slots of the particles that left in this step (count in ctrl[4]); null = stable scan
     // time
     uint64_t step0;
     int32_t m_steps;
@@ -138,6 +139,8 @@ cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_
                                 uint32_t *perm, cudaStream_t st);
 cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, uint32_t *perm,
                                cudaStream_t st);
+cudaError_t launch_fill_holes(float4 *xyzq, float *q1, uint32_t *pid, uint64_t *ctrl, const uint32_t *holes, uint32_t *src, uint32_t *dst,
+                              cudaStream_t st);
 cudaError_t launch_sort_records(float4 *xyzq, float *q1, uint32_t *pid, const uint64_t *n_dev, uint64_t capacity, GridF g, uint32_t *keys,
                                 uint32_t *hist, uint32_t *partial, float4 *xyzq_alt, float *q1_alt, uint32_t *pid_alt, cudaStream_t st);
 uint64_t sort_partial_entries(uint64_t n_cells);

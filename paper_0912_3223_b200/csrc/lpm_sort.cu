@@ -162,6 +162,45 @@ __global__ void __launch_bounds__(256) copy_records_kernel(const uint64_t *__res
     }
 }
 
+// ------------------------------------------------------------------ unordered compaction (B7)
+// After a step in hole-list mode: n = ctrl[0] slots, h = ctrl[4] of them listed in holes[] (their particles
+// left the domain).  The new count is n - h; every listed hole below it receives a live record from the tail
+// [n - h, n) - there are exactly as many of the one as of the other.  Work is proportional to h.
+__global__ void __launch_bounds__(256) fill_collect_kernel(const float4 *__restrict__ xyzq, uint64_t *ctrl, const uint32_t *__restrict__ holes,
+                                                           uint32_t *__restrict__ src, uint32_t *__restrict__ dst)
+{
+    const uint64_t n = ctrl[0], h = ctrl[4], new_n = n - h;
+    const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x, gstride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t j = gtid; j < h; j += gstride) {
+        const uint32_t idx = holes[j];
+        if (idx < new_n) dst[atomicAdd((unsigned long long *)(ctrl + 6), 1ull)] = idx;   // a hole that must be filled
+        const uint64_t i = new_n + j;                                                     // the j-th slot of the tail
+        if (xyzq[i].z >= 0.0f) src[atomicAdd((unsigned long long *)(ctrl + 5), 1ull)] = (uint32_t)i;   // a live record that must move
+    }
+    if (gtid == 0) ctrl[2] = new_n;
+}
+
+__global__ void __launch_bounds__(256) fill_move_kernel(float4 *__restrict__ xyzq, float *__restrict__ q1, uint32_t *__restrict__ pid,
+                                                        const uint64_t *__restrict__ ctrl, const uint32_t *__restrict__ src,
+                                                        const uint32_t *__restrict__ dst)
+{
+    const uint64_t cnt = ctrl[5];   // == ctrl[6]
+    for (uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; j < cnt; j += (uint64_t)gridDim.x * blockDim.x) {
+        const uint32_t s = src[j], d = dst[j];
+        xyzq[d] = xyzq[s];
+        if (q1) q1[d] = q1[s];
+        pid[d] = pid[s];
+    }
+}
+
+cudaError_t launch_fill_holes(float4 *xyzq, float *q1, uint32_t *pid, uint64_t *ctrl, const uint32_t *holes, uint32_t *src, uint32_t *dst,
+                              cudaStream_t st)
+{
+    fill_collect_kernel<<<148, 256, 0, st>>>(xyzq, ctrl, holes, src, dst);
+    fill_move_kernel<<<148, 256, 0, st>>>(xyzq, q1, pid, ctrl, src, dst);
+    return cudaGetLastError();
+}
+
 // compact mode: physical sort of the live records [0, *n_dev) by dual cell, through the alternate
 // buffers and back
 cudaError_t launch_sort_records(float4 *xyzq, float *q1, uint32_t *pid, const uint64_t *n_dev, uint64_t capacity, GridF g, uint32_t *keys,

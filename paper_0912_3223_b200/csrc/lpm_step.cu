@@ -437,60 +437,82 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
             rank[j] = __popc(ball & ((1u << lane) - 1u));
             if (lane == 0) s_woff[j * (kStepThreads / 32) + warp] = __popc(ball);
         }
-        __syncthreads();  // also orders every thread's input loads before the publication below
-        if (warp == 0) {
-            // exclusive scan of the 32 part counts (index order = item-major), tile total
-            const uint32_t cnt = s_woff[lane];
-            uint32_t inc = cnt;
+        if (A.holes) {
+            // Unordered store (gather_sort on, B7): no scan at all.  Survivors are written back where they
+            // are; the slots of the particles that left are listed, and fill_holes_* moves the live records of the
+            // tail into the listed holes below the new count (work proportional to the number of exits).
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-                if (lane >= o) inc += t;
-            }
-            s_woff[lane] = inc - cnt;
-            const uint32_t total = __shfl_sync(0xffffffffu, inc, 31);
-            uint32_t excl = 0;
-            if (lane == 0) {
-                __threadfence();
-                st_state(A.tile_state + tile, ((uint64_t)(epoch | (tile == 0 ? FLAG_P : FLAG_A)) << 32) | total);
-            }
-            if (tile > 0) {
-                // warp-wide look-back: lane l inspects tile (look - l)
-                int look = (int)tile - 1;
-                for (;;) {
-                    const int t = look - lane;
-                    uint64_t st = 0;
-                    uint32_t flag = FLAG_P, val = 0;
-                    if (t >= 0) {
-                        do { st = ld_state(A.tile_state + t); } while (((uint32_t)(st >> 32) & ~3u) != epoch);
-                        flag = (uint32_t)(st >> 32) & 3u;
-                        val = (uint32_t)st;
-                    }
-                    const uint32_t pmask = __ballot_sync(0xffffffffu, flag == FLAG_P);
-                    const int first_p = pmask ? __ffs(pmask) - 1 : 31;  // t < 0 lanes count as P with value 0; no P: all 32 aggregates count
-                    uint32_t contrib = (lane <= first_p) ? val : 0u;
-#pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
-                    excl += contrib;
-                    if (pmask) break;
-                    look -= 32;
+            for (int j = 0; j < kItems; ++j) {
+                const uint64_t i = (uint64_t)tile * kScanTile + (uint32_t)j * kStepThreads + threadIdx.x;
+                const bool dead = i < n && !alive[j];
+                if (i < n) {
+                    A.xyzq[i] = make_float4(x[j], y[j], alive[j] ? z[j] : -1.0f - z[j], q[j][0]);
+                    if (K > 1) A.q1[i] = q[j][1];
                 }
-                if (lane == 0) st_state(A.tile_state + tile, ((uint64_t)(epoch | FLAG_P) << 32) | (excl + total));
+                const uint32_t ball = __ballot_sync(0xffffffffu, dead);
+                if (ball) {
+                    uint32_t base = 0;
+                    if (lane == 0) base = (uint32_t)atomicAdd((unsigned long long *)(A.ctrl + 4), (unsigned long long)__popc(ball));
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    if (dead) A.holes[base + __popc(ball & ((1u << lane) - 1u))] = (uint32_t)i;
+                }
             }
-            if (lane == 0) {
-                s_excl = excl;
-                if (tile == n_tiles - 1) A.ctrl[2] = (uint64_t)excl + total;
-                __threadfence();
-            }
-        }
-        __syncthreads();
+        } else {
+            __syncthreads();  // also orders every thread's input loads before the publication below
+            if (warp == 0) {
+                // exclusive scan of the 32 part counts (index order = item-major), tile total
+                const uint32_t cnt = s_woff[lane];
+                uint32_t inc = cnt;
 #pragma unroll
-        for (int j = 0; j < kItems; ++j) {
-            if (alive[j]) {
-                const uint64_t dst = (uint64_t)s_excl + s_woff[j * (kStepThreads / 32) + warp] + rank[j];
-                A.xyzq[dst] = make_float4(x[j], y[j], z[j], q[j][0]);
-                if (K > 1) A.q1[dst] = q[j][1];
-                A.pid[dst] = pid[j];
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += t;
+                }
+                s_woff[lane] = inc - cnt;
+                const uint32_t total = __shfl_sync(0xffffffffu, inc, 31);
+                uint32_t excl = 0;
+                if (lane == 0) {
+                    __threadfence();
+                    st_state(A.tile_state + tile, ((uint64_t)(epoch | (tile == 0 ? FLAG_P : FLAG_A)) << 32) | total);
+                }
+                if (tile > 0) {
+                    // warp-wide look-back: lane l inspects tile (look - l)
+                    int look = (int)tile - 1;
+                    for (;;) {
+                        const int t = look - lane;
+                        uint64_t st = 0;
+                        uint32_t flag = FLAG_P, val = 0;
+                        if (t >= 0) {
+                            do { st = ld_state(A.tile_state + t); } while (((uint32_t)(st >> 32) & ~3u) != epoch);
+                            flag = (uint32_t)(st >> 32) & 3u;
+                            val = (uint32_t)st;
+                        }
+                        const uint32_t pmask = __ballot_sync(0xffffffffu, flag == FLAG_P);
+                        const int first_p = pmask ? __ffs(pmask) - 1 : 31;  // t < 0 lanes count as P with value 0; no P: all 32 aggregates count
+                        uint32_t contrib = (lane <= first_p) ? val : 0u;
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
+                        excl += contrib;
+                        if (pmask) break;
+                        look -= 32;
+                    }
+                    if (lane == 0) st_state(A.tile_state + tile, ((uint64_t)(epoch | FLAG_P) << 32) | (excl + total));
+                }
+                if (lane == 0) {
+                    s_excl = excl;
+                    if (tile == n_tiles - 1) A.ctrl[2] = (uint64_t)excl + total;
+                    __threadfence();
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int j = 0; j < kItems; ++j) {
+                if (alive[j]) {
+                    const uint64_t dst = (uint64_t)s_excl + s_woff[j * (kStepThreads / 32) + warp] + rank[j];
+                    A.xyzq[dst] = make_float4(x[j], y[j], z[j], q[j][0]);
+                    if (K > 1) A.q1[dst] = q[j][1];
+                    A.pid[dst] = pid[j];
+                }
             }
         }
         if (A.mask) {
@@ -533,6 +555,7 @@ __global__ void __launch_bounds__(256) inject_kernel(const __grid_constant__ Inj
     if (gtid == 0) {
         A.ctrl[0] = running;
         A.ctrl[1] = 0;
+        A.ctrl[4] = 0; A.ctrl[5] = 0; A.ctrl[6] = 0;  // hole list and fill counters of the coming step
         A.ctrl[3] += running;  // cumulative particle-steps (timing hooks)
         if (A.log_slot) *A.log_slot = running - n_prev;
     }
