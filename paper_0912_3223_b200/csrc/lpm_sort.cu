@@ -26,12 +26,21 @@ __global__ void __launch_bounds__(256) sort_key_kernel(const float4 *__restrict_
                                                        const uint64_t *__restrict__ n_dev = nullptr)
 {
     if (n_dev) n = *n_dev;  // (n is a by-value parameter: a local copy)
-    for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n; l += (uint64_t)gridDim.x * blockDim.x) {
-        const float4 p = xyzq[l];
-        uint32_t key = n_keys - 1;
-        if (p.z >= 0.0f) key = g.nlev ? corner_of<true>(g, p.x, p.y, p.z).o : corner_of<false>(g, p.x, p.y, p.z).o;
-        keys[l] = key;
-        atomicAdd(hist + key, 1u);
+    // lanes of a warp that share a key count with ONE atomic: next to the source thousands of particles share a
+    // cell, and same-address atomics are served at only ~6.5e8/s
+    const uint64_t n_round = (n + 31) & ~(uint64_t)31;
+    const int lane = threadIdx.x & 31;
+    for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n_round; l += (uint64_t)gridDim.x * blockDim.x) {
+        const bool live = l < n;
+        uint32_t key = 0xffffffffu;
+        if (live) {
+            const float4 p = xyzq[l];
+            key = n_keys - 1;
+            if (p.z >= 0.0f) key = g.nlev ? corner_of<true>(g, p.x, p.y, p.z).o : corner_of<false>(g, p.x, p.y, p.z).o;
+            keys[l] = key;
+        }
+        const uint32_t peers = __match_any_sync(0xffffffffu, key);
+        if (live && lane == __ffs(peers) - 1) atomicAdd(hist + key, (uint32_t)__popc(peers));
     }
 }
 

@@ -350,11 +350,16 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             const int cj = min(max(__float2int_rd((y - A.mg.y0) * A.mg.inv_dy), 0), A.mg.ny - 1);
             A.mask[(cj / kMaskTile) * A.mask_ntx + ci / kMaskTile] = 1;
         }
-        if (A.keys_out && in_range) {
-            // pass 1 of the coming gather-locality sort, for free: the new position is in registers
-            const uint32_t key = (valid && z >= 0.0f) ? corner_of<ZLEV>(A.mg, x, y, z).o : A.n_keys - 1u;
-            A.keys_out[l] = key;
-            atomicAdd(A.hist_out + key, 1u);
+        if (A.keys_out) {
+            // pass 1 of the coming gather-locality sort, for free: the new position is in registers; the lanes of
+            // a warp that share a key (most of them, in a sorted warp) count with one atomic
+            uint32_t key = 0xffffffffu;
+            if (in_range) {
+                key = (valid && z >= 0.0f) ? corner_of<ZLEV>(A.mg, x, y, z).o : A.n_keys - 1u;
+                A.keys_out[l] = key;
+            }
+            const uint32_t peers = __match_any_sync(0xffffffffu, key);
+            if (in_range && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(A.hist_out + key, (uint32_t)__popc(peers));
         }
         if (A.any_dep) {
             __syncthreads();
