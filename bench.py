@@ -152,12 +152,15 @@ def born_steps(w, s0: int, s1: int) -> float:
 
 
 # ------------------------------------------------------------------ the oracle legs
-def oracle_leg(name: str, scale: float, interval: int, warmup: int, steps: int, budget_s: float):
+def oracle_leg(name: str, scale: float, interval: int, warmup: int, steps: int, budget_s: float, threads: int = 0):
     """Run the fp64 oracle (as it stands) on a bounded sample of the workload: every
     ORACLE_STRIDE-th particle id (exact subset: particles are independent and Philox is keyed by
     the id), the same intervals as the CUDA arm.  Returns particle-steps/s over the timed part."""
     from oracle import oracle as orc
     from workloads import make
+    all_threads = orc.num_threads()
+    if threads:
+        orc.set_num_threads(threads)
     if name == "c5":
         w = make(name, scale=scale * ORACLE_SCALE_C5)
         sample = f"c5 at 1/{int(1 / ORACLE_SCALE_C5)} scale (injection rate and capacity), same grids/met/cadence"
@@ -184,7 +187,10 @@ def oracle_leg(name: str, scale: float, interval: int, warmup: int, steps: int, 
     dt = time.perf_counter() - t0
     units = live if name == "c5" else born_steps(w, warmup * interval, (warmup + done) * interval)
     sample += f"; {done} interval(s) of {interval} model steps after {warmup} warm-up interval(s)"
-    return units / dt, dt, done, orc.num_threads(), sample
+    used = orc.num_threads()
+    if threads:
+        orc.set_num_threads(all_threads)
+    return units / dt, dt, done, used, sample
 
 
 # ------------------------------------------------------------------ the CUDA arm
@@ -400,6 +406,10 @@ def run_ours(args):
     if not args.no_cpu_baseline:
         v, dt, done, cores, sample = oracle_leg(args.workload, args.scale, interval, 0 if args.workload != "c5" else 0, W + K, 20.0)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt}
+        # the paper's own baseline was ONE thread: the same sample on one thread, at most ~8 s
+        v1, dt1, done1, _, _ = oracle_leg(args.workload, args.scale, interval, 0, W + K, 8.0, threads=1)
+        cpu["value_1_thread"] = v1
+        cpu["intervals_1_thread"] = done1
 
     sim_hours = K * interval * w.dt / 3600.0
     line = {
