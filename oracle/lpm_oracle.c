@@ -60,6 +60,9 @@ typedef struct {
     const float *surface;  /* kz_mode 1: borrowed, [nt][ny][nx][4] = (u*, 1/L, Hz, unused), x fastest         */
     const double *z_levels; /* NULL: uniform levels z0 + (k + 1/2) dz; else borrowed, mgrid.nz ascending heights of
                              * the met levels ("vertical weather information is nonlinear")     */
+    int32_t drift;          /* 1: LABELLED DEPARTURE from the paper: z' gets the drift correction
+                             * + dKz/dz * dt of the well-mixed random walk; kz_mode 0 only                      */
+    int32_t pad3_;
 } orc_config;
 
 typedef struct {
@@ -211,6 +214,32 @@ static void sample_snapshot(const orc_grid *g, const double *levels, const float
             }
 }
 
+/* SURVEY 8(f)4, not in the paper: d/dz of the trilinear interpolant of component 3 (Kz) of one snapshot at (x, y, z):
+ * the slope between the two bracketing levels, weighted bilinearly in x and y; 0 outside the open hull of the
+ * level heights (where the interpolant is clamped, i.e. constant in z) and on a single-level grid. */
+static double snapshot_dkz_dz(const orc_grid *g, const double *levels, const float *snap, double x, double y, double z)
+{
+    int32_t i0, i1, j0, j1, k0, k1;
+    double fx, fy, fz, lo, hi, h;
+    if (g->nz < 2) return 0.0;
+    if (levels) { lo = levels[0]; hi = levels[g->nz - 1]; }
+    else { lo = g->z0 + 0.5 * g->dz; hi = g->z0 + ((double)g->nz - 0.5) * g->dz; }
+    if (!(z > lo && z < hi)) return 0.0;
+    axis_weights(x, g->x0, g->dx, g->nx, &i0, &i1, &fx);
+    axis_weights(y, g->y0, g->dy, g->ny, &j0, &j1, &fy);
+    if (levels) { level_weights(z, levels, g->nz, &k0, &k1, &fz); h = levels[k1] - levels[k0]; }
+    else { axis_weights(z, g->z0, g->dz, g->nz, &k0, &k1, &fz); h = g->dz; }
+    const int32_t I[2] = {i0, i1}, J[2] = {j0, j1};
+    const double wx[2] = {1.0 - fx, fx}, wy[2] = {1.0 - fy, fy};
+    double d = 0.0;
+    for (int jj = 0; jj < 2; ++jj)
+        for (int ii = 0; ii < 2; ++ii) {
+            size_t c0 = ((size_t)k0 * g->ny + J[jj]) * g->nx + I[ii], c1 = ((size_t)k1 * g->ny + J[jj]) * g->nx + I[ii];
+            d += wy[jj] * wx[ii] * ((double)snap[4 * c1 + 3] - (double)snap[4 * c0 + 3]);
+        }
+    return d / h;
+}
+
 /* time weight: s = clamp(floor((t-t0)/dT), 0, nt-2); a = clamp((t-T_s)/dT, 0, 1), rounded to
  * fp32 (the fp32 value is the parameter of both sides, DESIGN.md §3 R4). nt == 1: s = 0, a = 0. */
 void orc_time_weight(int32_t nt, double t0, double dt_snap, double t, int32_t *s_out, float *a_out)
@@ -242,6 +271,18 @@ void orc_sample_met_levels(const orc_grid *g, const double *levels, int32_t nt, 
     } else {
         for (int c = 0; c < 4; ++c) out[c] = A[c];
     }
+}
+
+double orc_dkz_dz(const orc_grid *g, const double *levels, int32_t nt, double t0, double dt_snap, const float *fields, double t,
+                  double x, double y, double z)
+{
+    int32_t s; float a;
+    size_t snap_elems = (size_t)g->nx * g->ny * g->nz * 4;
+    orc_time_weight(nt, t0, dt_snap, t, &s, &a);
+    double d0 = snapshot_dkz_dz(g, levels, fields + (size_t)s * snap_elems, x, y, z);
+    if (nt <= 1) return d0;
+    double d1 = snapshot_dkz_dz(g, levels, fields + (size_t)(s + 1) * snap_elems, x, y, z);
+    return (1.0 - (double)a) * d0 + (double)a * d1;
 }
 
 void orc_sample_met(const orc_grid *g, int32_t nt, double t0, double dt_snap, const float *fields,
@@ -461,12 +502,20 @@ static void step_particle(orc_sim *s, uint64_t i, uint64_t n, double t_n, int ra
         orc_sample_surface(&c->mgrid, c->nt, c->t0, c->dt_snap, c->surface, t_n, s->x[i], s->y[i], sf);
         Kz = orc_kz_eq3(sf[0], sf[1], sf[2], s->z[i]);
     }
+    double drift = 0.0;
+    if (c->drift == 1 && c->kz_mode == 0 && !(Kz < c->kz_min)) { /* SURVEY 8(f)4 departure; a floored Kz is constant in z */
+        drift = orc_dkz_dz(&c->mgrid, c->z_levels, c->nt, c->t0, c->dt_snap, c->fields, t_n, s->x[i], s->y[i], s->z[i]) * c->dt;
+        const orc_grid *mg = &c->mgrid;
+        double zlo = c->z_levels ? c->z_levels[0] : mg->z0 + 0.5 * mg->dz;
+        double zhi = c->z_levels ? c->z_levels[mg->nz - 1] : mg->z0 + ((double)mg->nz - 0.5) * mg->dz;
+        if (fabs(s->z[i] - zlo) < c->frag_delta || fabs(s->z[i] - zhi) < c->frag_delta) s->fragile[i] = 1; /* slope switches on / off there */
+    }
     if (Kz < c->kz_min) Kz = c->kz_min;
 
     /* R5: Eq.(1) + Eq.(2) */
     double xn = s->x[i] + u * c->dt + (double)s->sigma_h * nrm[0];
     double yn = s->y[i] + v * c->dt + (double)s->sigma_h * nrm[1];
-    double zn = s->z[i] + w * c->dt + sqrt(2.0 * Kz * c->dt) * nrm[2];
+    double zn = s->z[i] + w * c->dt + drift + sqrt(2.0 * Kz * c->dt) * nrm[2];
 
     /* R6: reflection at the ground and at the mixing height (north_star; paper silent) */
     if (zn < 0.0) zn = -zn;

@@ -45,7 +45,8 @@ class Config(C.Structure):
                 ("rx0", C.c_double), ("rx1", C.c_double), ("ry0", C.c_double), ("ry1", C.c_double),
                 ("rt0", C.c_double), ("rt1", C.c_double),
                 ("frag_delta", C.c_double), ("face_delta", C.c_double),
-                ("dep_mode", C.c_int32), ("kz_mode", C.c_int32), ("surface", C.c_void_p), ("z_levels", C.c_void_p)]
+                ("dep_mode", C.c_int32), ("kz_mode", C.c_int32), ("surface", C.c_void_p), ("z_levels", C.c_void_p),
+                ("drift", C.c_int32), ("pad3_", C.c_int32)]
 
 
 class Source(C.Structure):
@@ -102,6 +103,9 @@ def lib():
                                      C.c_double, C.c_double, C.c_double, C.c_double, C.c_void_p]
         L.orc_sample_met_levels.argtypes = [C.POINTER(Grid), C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_void_p,
                                             C.c_double, C.c_double, C.c_double, C.c_double, C.c_void_p]
+        L.orc_dkz_dz.argtypes = [C.POINTER(Grid), C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_void_p,
+                                 C.c_double, C.c_double, C.c_double, C.c_double]
+        L.orc_dkz_dz.restype = C.c_double
         L.orc_kz_eq3.argtypes = [C.c_double] * 4
         L.orc_kz_eq3.restype = C.c_double
         L.orc_sample_surface.argtypes = [C.POINTER(Grid), C.c_int32, C.c_double, C.c_double, C.c_void_p,
@@ -164,6 +168,12 @@ def sample_met(grid, nt, t0, dt_snap, fields, t, x, y, z, z_levels=None):
     return out
 
 
+def dkz_dz(grid, nt, t0, dt_snap, fields, t, x, y, z, z_levels=None):
+    f = np.ascontiguousarray(fields, dtype=np.float32)
+    lv = None if z_levels is None else np.ascontiguousarray(z_levels, dtype=np.float64)
+    return lib().orc_dkz_dz(C.byref(_grid(grid)), None if lv is None else lv.ctypes.data, nt, t0, dt_snap, _p(f), t, x, y, z)
+
+
 def kz_eq3(ustar, inv_L, Hz, z):
     return lib().orc_kz_eq3(ustar, inv_L, Hz, z)
 
@@ -184,7 +194,7 @@ class OracleSim:
     """The fp64 oracle run of a `workloads.Workload`."""
 
     def __init__(self, w, frag_delta: float = 0.05, face_delta: float = 0.0, bin_every: Optional[int] = None,
-                 dep_mode: int = 0):
+                 dep_mode: int = 0, drift: bool = False):
         self.w = w
         self.K = w.K
         self._fields = np.ascontiguousarray(w.fields(), dtype=np.float32)
@@ -207,6 +217,7 @@ class OracleSim:
             cfg.rt0, cfg.rt1 = w.rain.t_start, w.rain.t_end
         cfg.frag_delta, cfg.face_delta = frag_delta, face_delta
         cfg.dep_mode = dep_mode
+        cfg.drift = 1 if drift else 0
         self._levels = None
         if getattr(w, "z_levels", None) is not None:
             self._levels = np.ascontiguousarray(w.z_levels, dtype=np.float64)

@@ -496,3 +496,47 @@ def test_nonuniform_levels_reproduce_piecewise_linear_profiles():
         a = orc.sample_met(g, 1, 0.0, 3600.0, f, 0.0, 130.0, 310.0, float(z), z_levels=zu)
         b = orc.sample_met(g, 1, 0.0, 3600.0, f, 0.0, 130.0, 310.0, float(z))
         np.testing.assert_allclose(a, b, rtol=1e-13, atol=1e-15)
+
+
+# ------------------------------------------------------------------ P19: drift-corrected walk (S§8(f)4, labelled departure)
+def test_dkz_dz_is_the_slope_of_the_interpolant():
+    g = Grid(5, 4, 6, 0.0, 0.0, 0.0, 100.0, 100.0, 50.0)
+    zl = np.array([10.0, 40.0, 90.0, 170.0, 300.0, 520.0])
+    for levels, zc in ((None, g.z0 + (np.arange(g.nz) + 0.5) * g.dz), (zl, zl)):
+        prof = np.array([1.0, 4.0, 5.5, 5.0, 9.0, 2.0])
+        f = np.zeros((2, g.nz, g.ny, g.nx, 4), dtype=np.float32)
+        f[0, ..., 3] = prof[:, None, None]
+        f[1, ..., 3] = 3.0 * prof[:, None, None]
+        t, a = 900.0, 0.25
+        for k in range(g.nz - 1):
+            z = 0.3 * zc[k] + 0.7 * zc[k + 1]
+            want = (1 + 2 * a) * (prof[k + 1] - prof[k]) / (zc[k + 1] - zc[k])
+            got = orc.dkz_dz(g, 2, 0.0, 3600.0, f, t, 210.0, 170.0, float(z), z_levels=levels)
+            assert got == pytest.approx(want, rel=1e-12)
+            eps = 1e-3                                                    # and it IS the derivative of the sampled value
+            hi = orc.sample_met(g, 2, 0.0, 3600.0, f, t, 210.0, 170.0, float(z + eps), z_levels=levels)[3]
+            lo = orc.sample_met(g, 2, 0.0, 3600.0, f, t, 210.0, 170.0, float(z - eps), z_levels=levels)[3]
+            assert got == pytest.approx((hi - lo) / (2 * eps), rel=1e-7)
+        for z in (zc[0] - 1.0, zc[0], zc[-1], zc[-1] + 5.0):              # clamped: constant in z
+            assert orc.dkz_dz(g, 2, 0.0, 3600.0, f, t, 210.0, 170.0, float(z), z_levels=levels) == 0.0
+
+
+def test_drift_correction_keeps_a_uniform_cloud_well_mixed():
+    """Kz growing linearly with height, reflection at 0 and H: the paper's walk (no drift term) piles particles up where
+    Kz is small; with the + dKz/dz dt term a uniform cloud stays uniform (the well-mixed condition)."""
+    H, nz, n = 500.0, 25, 40000
+    g = Grid(4, 4, nz, -200.0, -200.0, 0.0, 100.0, 100.0, H / nz)
+    met = lambda t, Z, Y, X: (0.0, 0.0, 0.0, 2.0 + 0.04 * Z)
+    rng = np.random.default_rng(21)
+    z0 = rng.uniform(0.0, H, n)
+    hist = {}
+    for drift in (False, True):
+        w = custom(met, grid=g, n=n, dt=10.0, H=H, kz_min=0.0, n_steps=400)
+        o = orc.OracleSim(w.replace(release=None), bin_every=0, drift=drift)
+        o.set_particles(np.zeros(n), np.zeros(n), z0.copy(), np.ones((1, n)), pid=np.arange(n))
+        o.step(400)
+        hist[drift] = np.histogram(o.particles()["z"], bins=10, range=(0.0, H))[0]
+    expect = n / 10
+    chi2 = ((hist[True] - expect) ** 2 / expect).sum()
+    assert chi2 < 40.0, (chi2, hist[True])                               # 9 degrees of freedom (+ O(dt) scheme error)
+    assert hist[False][0] > 1.5 * expect and hist[False][-1] < 0.7 * expect, hist[False]
