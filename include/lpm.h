@@ -109,7 +109,10 @@ typedef struct {
                                * Bernoulli trial per nuclide and sink per step from Philox stream 1, an
                                * event deposits the nuclide's whole activity once; a particle that
                                * carries nothing any more becomes inactive (status 2)                */
-    int32_t reserved;
+    int32_t drift;            /* 1: LABELLED DEPARTURE from the paper: z' also gets + dKz/dz * dt,
+                               * the drift correction of the well-mixed random walk, with dKz/dz the z-slope of
+                               * the sampled (gridded) Kz at X_old; 0 (default) is the paper's Eq.(1)(2).
+                               * Not with kz_mode 1 (INVALID_ARG)                                    */
 } lpm_params;
 
 typedef struct {

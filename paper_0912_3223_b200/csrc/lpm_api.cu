@@ -277,6 +277,7 @@ void base_args(const lpm_handle *h, StepArgs &A)
     A.dep_stride = (uint64_t)h->cg.nx * h->cg.ny;
     A.bern = h->prm.dep_mode == 1 ? 1 : 0;
     A.eq3 = h->met.kz_mode == 1 ? 1 : 0;
+    A.drift = h->prm.drift == 1 ? 1 : 0;
     A.surf = A.eq3 ? (const float4 *)(h->ws + h->L.surf) : nullptr;
     A.any_dep = (!A.bern && (h->dry_mode != kDryNone || h->rain_on)) ? 1 : 0;
     for (int w = 0; w < 2 * LPM_MAX_NUCLIDES; ++w) {
@@ -487,7 +488,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         return LPM_ERR_INVALID_ARG;
     if (!(p->dt > 0) || p->capacity == 0 || p->capacity >= (1ull << 32) || !(met->H_mix > 0) || met->Kh < 0 ||
         (met->nt > 1 && !(met->dt_snap > 0)) || p->bin_every < 0 || p->steps_per_launch < 0 || !(p->h_dep > 0) || p->dep_mode < 0 ||
-        p->dep_mode > 1)
+        p->dep_mode > 1 || p->drift < 0 || p->drift > 1 || (p->drift == 1 && met->kz_mode == 1))
         return LPM_ERR_INVALID_ARG;
     int ndev = 0, dev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return LPM_ERR_NO_DEVICE;
@@ -529,7 +530,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         h->wet_scale[k] = keep_dry * (double)h->p_wet[k];
     }
     h->dry_mode = !any_dry ? kDryNone : (eligible_everywhere ? kDryUniform : kDryLayer);
-    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode, p->dep_mode == 1, met->kz_mode == 1, met->z_levels_host != nullptr);
+    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode, p->dep_mode == 1, met->kz_mode == 1, met->z_levels_host != nullptr || p->drift == 1);
     if (cudaMemsetAsync(ws, 0, L.total, h->st) != cudaSuccess) { delete h; return LPM_ERR_CUDA; }
     h->launches++;
     *out = h;

@@ -129,7 +129,8 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
 {
     // a0 + a2: weather at X_old, t_n
     const Corner c = corner_of<ZLEV>(A.mg, x, y, z);
-    const float4 m = trilinear(A.blend + (uint64_t)e.buf * A.snap_cells, c, A.mg);
+    float dkz = 0.0f;  // drift-corrected walk (labelled departure): dKz/dz of the sampled field
+    const float4 m = trilinear(A.blend + (uint64_t)e.buf * A.snap_cells, c, A.mg, ZLEV && A.drift != 0, &dkz);
     // Kz: the interpolated gridded field (R4), or Eq.(3) per particle from the 2-D fields of this step (R12)
     const float kz = fmaxf(EQ3 ? kz_eq3(A.surf + (uint64_t)e.buf * (uint32_t)(A.mg.nx * A.mg.ny), c, A.mg, z) : m.w, A.kz_min);
 
@@ -142,6 +143,7 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
     x = fmaf(A.sigma_h, n0, fmaf(m.x, A.dt, x));
     y = fmaf(A.sigma_h, n1, fmaf(m.y, A.dt, y));
     z = fmaf(sqrt_nr(2.0f * A.dt * kz), n2, fmaf(m.z, A.dt, z));
+    if (ZLEV && A.drift && !(m.w < A.kz_min)) z = fmaf(dkz, A.dt, z);  // (a floored Kz is constant in z)
 
     // a4: reflection (R6), lateral boundary (R7)
     z = fabsf(z);
@@ -596,7 +598,7 @@ static StepKernel pick(int K, bool compact, int dry, bool bern, bool eq3, bool z
 
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int blocks, cudaStream_t st)
 {
-    pick(K, compact, a.dry_mode, a.bern != 0, a.eq3 != 0, a.mg.nlev != 0)<<<blocks, kStepThreads, 0, st>>>(a);
+    pick(K, compact, a.dry_mode, a.bern != 0, a.eq3 != 0, a.mg.nlev != 0 || a.drift != 0)<<<blocks, kStepThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 

@@ -622,6 +622,29 @@ def test_full_size_sampled_against_oracle(lpm, orc, name, stride, steps, nt):
     assert abs(float(dep.sum().item()) * cg.dx * cg.dy / (lg[0][2] + lg[0][3] + lg[1][2] + lg[1][3] - lg[0][6] - lg[1][6]) - 1) < 1e-6
 
 
+@pytest.mark.parametrize("levels", [False, True])
+def test_drift_corrected_walk(lpm, orc, levels):
+    """S§8(f)4, labelled departure: + dKz/dz dt.  One step from an identical state (T1-class) and 500 steps (T3-class) on
+    c2's met with uniform and with non-uniform levels."""
+    w = make("c2", scale=0.01, n_steps=500).replace(nt=3)
+    if levels:
+        zl = np.array([10.0, 30.0, 60.0, 100.0, 150.0, 210.0, 280.0, 360.0, 450.0, 550.0, 660.0, 780.0, 910.0, 1050.0, 1200.0])
+        g = w.mgrid
+        w = w.replace(mgrid=Grid(g.nx, g.ny, len(zl), g.x0, g.y0, g.z0, g.dx, g.dy, g.dz), z_levels=zl)
+    sim, o = lpm.Simulation(w, drift=True), orc.OracleSim(w, drift=True)
+    sim.step(500)
+    o.step(500)
+    gp, p = sim.get_particles_host(), o.particles()
+    assert gp["x"].shape[0] == p["x"].shape[0] > 5000
+    frag = np.isin(p["pid"], o.fragile_pids())
+    assert frag.mean() < 0.2
+    _n_step_compare(gp, p, w, frag, 0.999, f"drift levels={levels}")
+    # the term really acts: the same run without it differs by metres
+    plain = lpm.Simulation(w)
+    plain.step(500)
+    assert np.abs(plain.get_particles_host()["z"] - gp["z"]).mean() > 1.0
+
+
 def test_full_rate_c5_properties(lpm):
     """C5 at BASELINE's full injection rate (4e4 particles per step, record sort on): properties that hold at any
     size - survivors have unique ids and lie inside the domain, the ledger closes, counts = live in-grid particles."""
