@@ -251,7 +251,8 @@ def run_ours(args):
 
     # ---------------- leg 1: inputs resident in HBM ----------------
     fields_dev = fields_host.to("cuda", non_blocking=True)
-    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode)
+    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode, texel_pairs=args.texel_pairs)
+    pairs = sim.texel_pairs
     conc_dev = torch.empty((w.K, g.nz, g.ny, g.nx), dtype=torch.float32, device="cuda")
     dep_dev = torch.empty((w.K, g.ny, g.nx), dtype=torch.float32, device="cuda")
     for _ in range(W):
@@ -292,7 +293,7 @@ def run_ours(args):
 
     # ---------------- leg 2: end to end through the host-buffer C-ABI calls ----------------
     fields_dev.zero_()
-    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode)
+    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode, texel_pairs=args.texel_pairs)
     sim.upload_meteo(0, fields_host[0:1])
     uploaded = 0
     h2d = d2h = 0
@@ -376,9 +377,10 @@ def run_ours(args):
                      "peak_source": pk["source"], "frac": k_rate * hbm_per_ps / (pk["hbm_gbs"] * 1e9)},
         # what ncu shows to be the binding unit (profiles/r01c_*): the L1 data pipe, one 32-byte sector per gathered
         # texel; achieved = gathers issued per second against the probe's L1-resident gather rate
-        "l1_gather_side": {"gathers_per_particle_step": 8, "achieved_per_s": 8.0 * k_rate,
+        # (z-pair texels, B8: 4 gathers of one 32-byte sector each instead of 8 of 16 bytes)
+        "l1_gather_side": {"gathers_per_particle_step": 4 if pairs else 8, "achieved_per_s": (4.0 if pairs else 8.0) * k_rate,
                            "peak_per_s": probes.get("l1_gather_sectors_per_s"),
-                           "frac": 8.0 * k_rate / probes["l1_gather_sectors_per_s"] if probes.get("l1_gather_sectors_per_s") else None,
+                           "frac": (4.0 if pairs else 8.0) * k_rate / probes["l1_gather_sectors_per_s"] if probes.get("l1_gather_sectors_per_s") else None,
                            "note": "upper bound of the sector count: lanes that share a texel share a sector"},
     }
     bpp = 12 + 4 * w.K
@@ -419,7 +421,7 @@ def run_ours(args):
         "config": {"workload": f"{args.workload} (BASELINE.json configs[{ {'c1': 0, 'c2': 1, 'c2_eq3': 1, 'c3': 2, 'c3_hdep80': 2, 'c4': 3, 'c5': 4}[args.workload] }])",
                    "particles_per_gpu": w.capacity, "nuclides": w.K, "model_steps_per_bench_step": interval, "dt_s": w.dt,
                    "conc_grid": [g.nx, g.ny, g.nz], "met_grid": [w.mgrid.nx, w.mgrid.ny, w.mgrid.nz], "met_snapshots": w.nt,
-                   "scale": args.scale, "dep_mode": args.dep_mode, "l2": "particle store larger than L2, no flush" if w.capacity * state_bytes > 126e6 else "inputs fit L2 (small config)",
+                   "scale": args.scale, "dep_mode": args.dep_mode, "met_texels": "z-pair, 32 B (DESIGN.md B8)" if pairs else "16 B", "l2": "particle store larger than L2, no flush" if w.capacity * state_bytes > 126e6 else "inputs fit L2 (small config)",
                    "parallelism": f"pid-strided ensemble x{world}, grids all-reduced per output" if world > 1 else "single GPU"},
         "sim_hours_per_s": sim_hours / (ms * 1e-3),
         "e2e": {"value": units / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
@@ -464,6 +466,7 @@ def main():
     ap.add_argument("--workload", default="c4", choices=("c1", "c2", "c2_eq3", "c3", "c3_hdep80", "c4", "c5"))
     ap.add_argument("--scale", type=float, default=1.0, help="particle-count scale of the workload (1.0 = BASELINE size)")
     ap.add_argument("--dep-mode", type=int, default=0, choices=(0, 1), help="0 expected-mass deposition (default), 1 Bernoulli deposition (S 8(f)1)")
+    ap.add_argument("--texel-pairs", type=int, default=0, choices=(-1, 0, 1), help="lpm_params.texel_pairs: 0 auto (default), 1 z-pair texels, -1 16-byte texels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probes", action="store_true", help="skip the lpm_probe micro-benchmarks (measured peaks)")
     args = ap.parse_args()

@@ -113,6 +113,14 @@ typedef struct {
                                * the drift correction of the well-mixed random walk, with dKz/dz the z-slope of
                                * the sampled (gridded) Kz at X_old; 0 (default) is the paper's Eq.(1)(2).
                                * Not with kz_mode 1 (INVALID_ARG)                                    */
+    int32_t texel_pairs;      /* layout of the time-blended met buffers the step kernel gathers from (B8):
+                               * -1 = one 16-byte texel F(k) per met cell (8 gathers per step); 1 = 32-byte
+                               * texels {F(k), F(k+1)}: 4 gathers per step, twice the bytes per blended cell;
+                               * 0 = auto: pairs when capacity >= 16 x the met cells (the blending kernel's
+                               * extra writes are then small beside the step kernel's gain).  Results are
+                               * bit-identical either way.  Pairs need the default physics on the
+                               * slot-addressed store: compact = 0, nt > 1, dep_mode 0, kz_mode 0, uniform
+                               * levels, drift 0 (auto: 16-byte texels otherwise; 1: INVALID_ARG)     */
 } lpm_params;
 
 typedef struct {
@@ -226,6 +234,9 @@ int32_t lpm_injected(lpm_handle *h, uint64_t step, uint64_t *n_host);
 const char *lpm_last_error(lpm_handle *h);
 /* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
 int32_t lpm_launch_count(lpm_handle *h, uint64_t *n_host);
+/* *on_host = 1 when this handle's blended met buffers hold 32-byte z-pair texels (lpm_params.texel_pairs, after the
+ * auto rule), else 0 */
+int32_t lpm_texel_pairs(lpm_handle *h, int32_t *on_host);
 
 /* ---- host-buffer entry points (end-to-end use: weather arrives from, results go to, host memory) */
 

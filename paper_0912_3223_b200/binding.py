@@ -28,6 +28,7 @@ SYMBOLS = (
     "lpm_set_particles", "lpm_ledger", "lpm_injected", "lpm_last_error", "lpm_launch_count", "lpm_test_philox",
     "lpm_test_normals", "lpm_test_sample", "lpm_upload_meteo", "lpm_concentration_host", "lpm_deposition_host",
     "lpm_set_timing", "lpm_get_timing", "lpm_probe", "lpm_test_box_muller", "lpm_dose", "lpm_test_curand_philox",
+    "lpm_texel_pairs",
 )
 
 
@@ -56,7 +57,7 @@ class lpm_nuclide(C.Structure):
 class lpm_params(C.Structure):
     _fields_ = [("dt", C.c_double), ("seed", C.c_uint64), ("capacity", C.c_uint64), ("boundary_mode", C.c_int32),
                 ("compact", C.c_int32), ("h_dep", C.c_double), ("bin_every", C.c_int32), ("steps_per_launch", C.c_int32),
-                ("gather_sort", C.c_int32), ("dose", C.c_int32), ("dep_mode", C.c_int32), ("drift", C.c_int32)]
+                ("gather_sort", C.c_int32), ("dose", C.c_int32), ("dep_mode", C.c_int32), ("drift", C.c_int32), ("texel_pairs", C.c_int32)]
 
 
 class lpm_source(C.Structure):
@@ -107,6 +108,7 @@ def load():
     L.lpm_deposition_host.argtypes = [vp, vp]
     L.lpm_set_timing.argtypes = [vp, i32]
     L.lpm_get_timing.argtypes = [vp, C.POINTER(dbl)]
+    L.lpm_texel_pairs.argtypes = [vp, C.POINTER(i32)]
     L.lpm_probe.argtypes = [i32, u64, vp, u64, i32, C.POINTER(dbl), vp]
     L.lpm_test_box_muller.argtypes = [vp, u64, vp, vp]
     L.lpm_test_curand_philox.argtypes = [u64, u64, u64, u64, vp, vp]
@@ -133,11 +135,16 @@ def _grid(g) -> lpm_grid:
 
 
 def workspace_bytes(cgrid, capacity: int, n_nuclides: int, compact: bool, mgrid=None, nt: int = 1, gather_sort: int = 0,
-                    dose: bool = False, kz_mode: int = 0) -> int:
-    p = lpm_params(dt=1.0, capacity=capacity, compact=1 if compact else 0, h_dep=1.0, gather_sort=gather_sort, dose=1 if dose else 0)
+                    dose: bool = False, kz_mode: int = 0, dep_mode: int = 0, drift: bool = False, texel_pairs: int = 0,
+                    z_levels=None) -> int:
+    p = lpm_params(dt=1.0, capacity=capacity, compact=1 if compact else 0, h_dep=1.0, gather_sort=gather_sort, dose=1 if dose else 0,
+                   dep_mode=dep_mode, drift=1 if drift else 0, texel_pairs=texel_pairs)
     out = C.c_uint64()
     g = _grid(cgrid)
     met = lpm_meteo(grid=_grid(mgrid if mgrid is not None else cgrid), nt=nt, kz_mode=kz_mode)
+    if z_levels is not None:   # only its presence matters for the size
+        lev = np.ascontiguousarray(z_levels, dtype=np.float64)
+        met.z_levels_host = lev.ctypes.data
     rc = load().lpm_workspace_bytes(C.byref(g), C.byref(met), C.byref(p), n_nuclides, C.byref(out))
     if rc:
         raise LpmError(rc, "lpm_workspace_bytes")
@@ -168,7 +175,7 @@ class Simulation:
     """
 
     def __init__(self, w, *, steps_per_launch: int = 0, bin_every: Optional[int] = None, fields_dev=None,
-                 stream=None, auto_release: bool = True, gather_sort: int = 0, dose: bool = False, dep_mode: int = 0, drift: bool = False):
+                 stream=None, auto_release: bool = True, gather_sort: int = 0, dose: bool = False, dep_mode: int = 0, drift: bool = False, texel_pairs: int = 0):
         torch = _require_cuda()
         L = load()
         self._L = L
@@ -186,7 +193,8 @@ class Simulation:
         self.surface_dev = None
         if kz_mode == 1:
             self.surface_dev = torch.from_numpy(np.ascontiguousarray(w.surface(), dtype=np.float32)).to(self.device)
-        nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact, w.mgrid, w.nt, gather_sort, dose, kz_mode)
+        nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact, w.mgrid, w.nt, gather_sort, dose, kz_mode, dep_mode, drift, texel_pairs,
+                                 getattr(w, "z_levels", None))
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         cg = _grid(w.cgrid)
         met = lpm_meteo(grid=_grid(w.mgrid), nt=w.nt, t0=w.t0, dt_snap=w.dt_snap, fields_dev=fields_dev.data_ptr(),
@@ -200,7 +208,8 @@ class Simulation:
         prm = lpm_params(dt=w.dt, seed=w.seed, capacity=w.capacity,
                          boundary_mode=1 if w.boundary_mode == "absorb" else 0, compact=1 if w.compact else 0,
                          h_dep=w.h_dep, bin_every=w.bin_every if bin_every is None else bin_every,
-                         steps_per_launch=steps_per_launch, gather_sort=gather_sort, dose=1 if dose else 0, dep_mode=dep_mode, drift=1 if drift else 0)
+                         steps_per_launch=steps_per_launch, gather_sort=gather_sort, dose=1 if dose else 0, dep_mode=dep_mode, drift=1 if drift else 0,
+                         texel_pairs=texel_pairs)
         h = C.c_void_p()
         with torch.cuda.stream(self.stream):
             rc = L.lpm_create(C.byref(cg), C.byref(met), nucs, w.K, C.byref(prm), self.workspace.data_ptr(), nbytes,
@@ -295,6 +304,12 @@ class Simulation:
         self._ck(self._L.lpm_get_timing(self._h, out), "lpm_get_timing")
         return dict(step_ms=out[0], step_launches=int(out[1]), bin_ms=out[2], bin_launches=int(out[3]),
                     particle_steps=out[4], binned_particles=out[5], sort_ms=out[6], sort_launches=int(out[7]))
+
+    @property
+    def texel_pairs(self) -> bool:
+        on = C.c_int32()
+        self._ck(self._L.lpm_texel_pairs(self._h, C.byref(on)), "lpm_texel_pairs")
+        return bool(on.value)
 
     @property
     def num_active(self) -> int:

@@ -32,7 +32,7 @@ struct Layout {
 
 uint64_t up(uint64_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
-Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K, bool compact, bool sort, bool dose)
+Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K, bool compact, bool sort, bool dose, bool zpair)
 {
     Layout L{};
     const uint64_t cells3 = (uint64_t)g.nx * g.ny * g.nz, cells2 = (uint64_t)g.nx * g.ny;
@@ -51,7 +51,7 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     L.stage = o; o += up(4 * cells3 * K);  // fp32 read-out staging for the *_host entry points
     L.pair = o; o += met.nt > 1 ? up(32ull * met.grid.nx * met.grid.ny * met.grid.nz) : 0;  // (F_s, F_s+1) per met cell
     const uint64_t mcells = (uint64_t)met.grid.nx * met.grid.ny * met.grid.nz;
-    L.blend = o; o += up(16ull * mcells * (met.nt > 1 ? kBlendDepth : 1) + 16);  // z-fastest F(t_n), one buffer per fused step (+ 1 pad texel)
+    L.blend = o; o += up((zpair ? 32ull : 16ull) * mcells * (met.nt > 1 ? kBlendDepth : 1) + 32);  // z-fastest F(t_n), one buffer per fused step (+ 1 pad texel)
     L.keys = o; o += sort ? up(4 * cap) : 0;            // gather-locality pass: met-cell key per slot
     L.perm = o; o += sort && !compact ? up(4 * cap) : 0;  //   slots in met-cell order (slot-addressed store)
     L.hist = o; o += sort ? up(4 * (mcells + 1)) : 0;   //   per-cell counts / offsets
@@ -97,6 +97,19 @@ bool sort_enabled(const lpm_params *p)
     return p->gather_sort >= 0;
 }
 
+// B8: z-pair texels in the blended buffers.  The physics they are instantiated for, and the auto rule.
+constexpr uint64_t kPairAutoRatio = 16;
+bool zpair_possible(const lpm_meteo *met, const lpm_params *p)
+{
+    return !p->compact && met->nt > 1 && p->dep_mode == 0 && met->kz_mode == 0 && met->z_levels_host == nullptr && p->drift == 0;
+}
+bool zpair_enabled(const lpm_meteo *met, const lpm_params *p)
+{
+    if (p->texel_pairs < 0 || !zpair_possible(met, p)) return false;
+    if (p->texel_pairs > 0) return true;
+    return p->capacity >= kPairAutoRatio * (uint64_t)met->grid.nx * met->grid.ny * met->grid.nz;
+}
+
 bool grid_ok(const lpm_grid *g)
 {
     return g && g->nx > 0 && g->ny > 0 && g->nz > 0 && g->dx > 0 && g->dy > 0 && g->dz > 0 &&
@@ -111,6 +124,7 @@ struct lpm_handle {
     lpm_nuclide nuc[LPM_MAX_NUCLIDES];
     lpm_params prm;
     bool has_levels;
+    bool zpair;   // B8: the blended buffers hold 32-byte z-pair texels
     float zlev[kMaxLevels];   // non-uniform level heights (fp32 parameters), copied from meteo.z_levels_host
     int K;
     cudaStream_t st;
@@ -267,6 +281,7 @@ void base_args(const lpm_handle *h, StepArgs &A)
     A.q1 = h->K > 1 ? (float *)(h->ws + h->L.q1) : nullptr;
     A.pid = h->prm.compact ? (uint32_t *)(h->ws + h->L.pid) : nullptr;
     A.blend = (const float4 *)(h->ws + h->L.blend);
+    A.zpair = h->zpair ? 1 : 0;
     const lpm_grid &mg = h->met.grid;
     A.snap_cells = (uint64_t)mg.nx * mg.ny * mg.nz;
     A.mg = gridf(mg, true, h->has_levels ? h->zlev : nullptr);
@@ -419,7 +434,7 @@ int ensure_blend(lpm_handle *h, StepArgs &A, int m, int m_max)
             box.src_j[box.n_src] = sj < 0 ? 0 : (sj > g.ny - 1 ? g.ny - 1 : sj);
             box.n_src++;
         }
-        CK(launch_blend(h->ws + h->L.pair, blend, A.snap_cells, cnt, a, &box, h->st));
+        CK(launch_blend(h->ws + h->L.pair, blend, A.snap_cells, cnt, a, &box, h->zpair, h->st));
         h->launches++;
         if (h->met.kz_mode == 1) {  // R12: the 2-D fields (u*, 1/L, Hz) of the same steps
             const uint64_t c2 = (uint64_t)g.nx * g.ny;
@@ -458,7 +473,7 @@ int32_t lpm_workspace_bytes(const lpm_grid *g, const lpm_meteo *met, const lpm_p
 {
     if (!grid_ok(g) || !met || !grid_ok(&met->grid) || met->nt < 1 || !p || !bytes || K < 1 || K > LPM_MAX_NUCLIDES || p->capacity == 0 || p->capacity >= (1ull << 32))
         return LPM_ERR_INVALID_ARG;
-    *bytes = make_layout(*g, *met, p->capacity, K, p->compact != 0, sort_enabled(p), p->dose != 0).total;
+    *bytes = make_layout(*g, *met, p->capacity, K, p->compact != 0, sort_enabled(p), p->dose != 0, zpair_enabled(met, p)).total;
     return LPM_OK;
 }
 
@@ -488,7 +503,8 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         return LPM_ERR_INVALID_ARG;
     if (!(p->dt > 0) || p->capacity == 0 || p->capacity >= (1ull << 32) || !(met->H_mix > 0) || met->Kh < 0 ||
         (met->nt > 1 && !(met->dt_snap > 0)) || p->bin_every < 0 || p->steps_per_launch < 0 || !(p->h_dep > 0) || p->dep_mode < 0 ||
-        p->dep_mode > 1 || p->drift < 0 || p->drift > 1 || (p->drift == 1 && met->kz_mode == 1))
+        p->dep_mode > 1 || p->drift < 0 || p->drift > 1 || (p->drift == 1 && met->kz_mode == 1) || p->texel_pairs < -1 || p->texel_pairs > 1 ||
+        (p->texel_pairs == 1 && !zpair_possible(met, p)))
         return LPM_ERR_INVALID_ARG;
     int ndev = 0, dev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return LPM_ERR_NO_DEVICE;
@@ -496,13 +512,14 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return LPM_ERR_NO_DEVICE;
     if (prop.major != 10) return LPM_ERR_NO_DEVICE;
 
-    const Layout L = make_layout(*cg, *met, p->capacity, K, p->compact != 0, sort_enabled(p), p->dose != 0);
+    const Layout L = make_layout(*cg, *met, p->capacity, K, p->compact != 0, sort_enabled(p), p->dose != 0, zpair_enabled(met, p));
     if (ws_bytes < L.total) return LPM_ERR_WORKSPACE_TOO_SMALL;
 
     lpm_handle *h = new (std::nothrow) lpm_handle();
     if (!h) return LPM_ERR_INVALID_ARG;
     h->cg = *cg; h->met = *met; h->prm = *p; h->K = K;
     h->has_levels = met->z_levels_host != nullptr;
+    h->zpair = zpair_enabled(met, p);
     if (h->has_levels) for (int k = 0; k < met->grid.nz; ++k) h->zlev[k] = (float)met->z_levels_host[k];
     h->met.z_levels_host = nullptr;  // copied: the caller's array is not needed after lpm_create
     for (int k = 0; k < K; ++k) h->nuc[k] = nuc[k];
@@ -530,7 +547,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         h->wet_scale[k] = keep_dry * (double)h->p_wet[k];
     }
     h->dry_mode = !any_dry ? kDryNone : (eligible_everywhere ? kDryUniform : kDryLayer);
-    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode, p->dep_mode == 1, met->kz_mode == 1, met->z_levels_host != nullptr || p->drift == 1);
+    h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode, p->dep_mode == 1, met->kz_mode == 1, met->z_levels_host != nullptr || p->drift == 1, h->zpair);
     if (cudaMemsetAsync(ws, 0, L.total, h->st) != cudaSuccess) { delete h; return LPM_ERR_CUDA; }
     h->launches++;
     *out = h;
@@ -1042,6 +1059,13 @@ int32_t lpm_get_timing(lpm_handle *h, double *out)
     return LPM_OK;
 }
 
+int32_t lpm_texel_pairs(lpm_handle *h, int32_t *on)
+{
+    if (!h || !on) return LPM_ERR_INVALID_ARG;
+    *on = h->zpair ? 1 : 0;
+    return LPM_OK;
+}
+
 int32_t lpm_launch_count(lpm_handle *h, uint64_t *n)
 {
     if (!h || !n) return LPM_ERR_INVALID_ARG;
@@ -1121,7 +1145,7 @@ int32_t lpm_test_sample(const lpm_meteo *met, double t, const void *xyz, uint64_
         BlendBox box{};
         box.nx = g.nx; box.ny = g.ny; box.nz = g.nz;
         rc = launch_pair_repack(f + (uint64_t)sn * cells, f + (uint64_t)(sn + 1) * cells, pair, g.nx, g.ny, g.nz, nullptr, s);
-        if (rc == cudaSuccess) rc = launch_blend(pair, blend, cells, 1, &e.a, &box, s);
+        if (rc == cudaSuccess) rc = launch_blend(pair, blend, cells, 1, &e.a, &box, false, s);
     } else {
         rc = launch_transpose(f, blend, g.nx, g.ny, g.nz, s);
     }

@@ -64,6 +64,7 @@ struct StepArgs {
     uint64_t dep_stride;
     float dep_scale[2 * LPM_MAX_NUCLIDES];       // fixed-point scales of the CTA-private deposit sums (powers of two): [2k] dry, [2k+1] wet
     double dep_inv_scale[2 * LPM_MAX_NUCLIDES];  // their inverses
+    int32_t zpair, pad4_;                    // the blended buffers hold z-pair texels (32 B: both z corners), B8
     int32_t eq3, drift;                      // kz_mode 1: Kz from Eq.(3) per particle; drift: + dKz/dz dt (departure from the paper)
     int32_t any_dep, bern;                   // some sink deposits through the tables; dep_mode 1: Bernoulli deposition (R11)
     // physics
@@ -133,7 +134,7 @@ struct BinArgs {
 
 // launchers implemented in the .cu files; all return the cudaError of the launch
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int grid_blocks, cudaStream_t st);
-int step_max_blocks_per_sm(int K, bool compact, int dry_mode, bool bern, bool eq3, bool zlev);
+int step_max_blocks_per_sm(int K, bool compact, int dry_mode, bool bern, bool eq3, bool zlev, bool zpair);
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
                                 uint32_t *perm, cudaStream_t st);
@@ -162,7 +163,7 @@ struct BlendBox {
     int32_t n_src;
     int32_t src_i[LPM_MAX_RELEASES], src_j[LPM_MAX_RELEASES];   // source columns (newborn particles)
 };
-cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, const BlendBox *box, cudaStream_t st);
+cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, const BlendBox *box, bool zpair, cudaStream_t st);
 cudaError_t launch_bin(const BinArgs &a, int blocks, cudaStream_t st);
 cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3, int K, const double *scale, cudaStream_t st);
 cudaError_t launch_dose_accum(const double *conc, double *dose, uint64_t cells3, int K, const double *scale, cudaStream_t st);

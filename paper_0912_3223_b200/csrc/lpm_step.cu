@@ -122,7 +122,7 @@ __device__ __forceinline__ void deposit_at(const StepArgs &A, float x, float y, 
 // One model step of one particle.  Returns false when the particle left the domain (ABSORB).
 // Source order = intended issue order: the eight gathers go out first and the ~150 instructions of
 // Philox + Box-Muller run while they are in flight.
-template <int K, int DRY, bool BERN, bool EQ3, bool ZLEV>
+template <int K, int DRY, bool BERN, bool EQ3, bool ZLEV, bool ZP = false>
 __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e, uint32_t step_lo,
                                           uint32_t pid_lo, float &x, float &y, float &z,
                                           float (&q)[K], Acc<K> &acc, DepTab<K> &dep)
@@ -130,7 +130,7 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
     // a0 + a2: weather at X_old, t_n
     const Corner c = corner_of<ZLEV>(A.mg, x, y, z);
     float dkz = 0.0f;  // drift-corrected walk (labelled departure): dKz/dz of the sampled field
-    const float4 m = trilinear(A.blend + (uint64_t)e.buf * A.snap_cells, c, A.mg, ZLEV && A.drift != 0, &dkz);
+    const float4 m = trilinear<ZP>(A.blend + (ZP ? 2ull : 1ull) * (uint64_t)e.buf * A.snap_cells, c, A.mg, ZLEV && A.drift != 0, &dkz);
     // Kz: the interpolated gridded field (R4), or Eq.(3) per particle from the 2-D fields of this step (R12)
     const float kz = fmaxf(EQ3 ? kz_eq3(A.surf + (uint64_t)e.buf * (uint32_t)(A.mg.nx * A.mg.ny), c, A.mg, z) : m.w, A.kz_min);
 
@@ -277,7 +277,7 @@ __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &ac
 #endif
 static_assert(sizeof(StepArgs) <= 32764, "StepArgs must fit the kernel-parameter space (32764 B since CUDA 12.1 on sm_70+)");
 
-template <int K, int DRY, bool BERN, bool EQ3, bool ZLEV>
+template <int K, int DRY, bool BERN, bool EQ3, bool ZLEV, bool ZP = false>
 __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel(const __grid_constant__ StepArgs A)
 {
     __shared__ uint32_t s_ticket;
@@ -341,7 +341,7 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             bool alive = true;
             const uint32_t step0 = (uint32_t)A.step0;
             for (int s = 0; s < A.m_steps; ++s)
-                if (alive & (s >= s_begin)) alive = step_once<K, DRY, BERN, EQ3, ZLEV>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, T);
+                if (alive & (s >= s_begin)) alive = step_once<K, DRY, BERN, EQ3, ZLEV, ZP>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, T);
             if (!alive) z = -1.0f - z;  // exit position kept, slot marked inactive
             A.xyzq[slot] = make_float4(x, y, z, q[0]);
             if (K > 1) A.q1[slot] = q[1];
@@ -590,22 +590,31 @@ static StepKernel pick_kb(bool compact, int dry, bool eq3, bool zlev)
     return zlev ? pick_dry<K, BERN, false, true>(compact, dry) : pick_dry<K, BERN, false, false>(compact, dry);
 }
 
-static StepKernel pick(int K, bool compact, int dry, bool bern, bool eq3, bool zlev)
+// z-pair texels: default physics, slot-addressed store only (6 more instantiations, not 96)
+template <int K>
+static StepKernel pick_zp(int dry)
 {
+    if (dry == kDryNone) return step_slots_kernel<K, kDryNone, false, false, false, true>;
+    return dry == kDryUniform ? step_slots_kernel<K, kDryUniform, false, false, false, true> : step_slots_kernel<K, kDryLayer, false, false, false, true>;
+}
+
+static StepKernel pick(int K, bool compact, int dry, bool bern, bool eq3, bool zlev, bool zpair = false)
+{
+    if (zpair) return K == 1 ? pick_zp<1>(dry) : pick_zp<2>(dry);
     if (K == 1) return bern ? pick_kb<1, true>(compact, dry, eq3, zlev) : pick_kb<1, false>(compact, dry, eq3, zlev);
     return bern ? pick_kb<2, true>(compact, dry, eq3, zlev) : pick_kb<2, false>(compact, dry, eq3, zlev);
 }
 
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int blocks, cudaStream_t st)
 {
-    pick(K, compact, a.dry_mode, a.bern != 0, a.eq3 != 0, a.mg.nlev != 0 || a.drift != 0)<<<blocks, kStepThreads, 0, st>>>(a);
+    pick(K, compact, a.dry_mode, a.bern != 0, a.eq3 != 0, a.mg.nlev != 0 || a.drift != 0, a.zpair != 0)<<<blocks, kStepThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 
-int step_max_blocks_per_sm(int K, bool compact, int dry, bool bern, bool eq3, bool zlev)
+int step_max_blocks_per_sm(int K, bool compact, int dry, bool bern, bool eq3, bool zlev, bool zpair)
 {
     int nb = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick(K, compact, dry, bern, eq3, zlev), kStepThreads, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, pick(K, compact, dry, bern, eq3, zlev, zpair), kStepThreads, 0);
     return nb;
 }
 
@@ -688,6 +697,7 @@ struct BlendArgs {
     int32_t m;
     float a[kBlendDepth];
     BlendBox box;
+    int32_t zpair;   // write z-pair texels {F(k), F(k+1)} (32 B) instead of F(k) (16 B)
 };
 
 // Only the columns a particle can reach are blended: a tile of 8 x 8 met columns is processed if a
@@ -735,15 +745,31 @@ __global__ void __launch_bounds__(256) blend_kernel(const __grid_constant__ Blen
             asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                 : "=f"(tx.a.x), "=f"(tx.a.y), "=f"(tx.a.z), "=f"(tx.a.w), "=f"(tx.b.x), "=f"(tx.b.y), "=f"(tx.b.z), "=f"(tx.b.w)
                 : "l"(B.pair + o));
+            if (!B.zpair) {
 #pragma unroll 4
-            for (int s = 0; s < B.m; ++s) B.out[(uint64_t)s * B.cells + o] = lerp4(tx.a, tx.b, B.a[s]);
+                for (int s = 0; s < B.m; ++s) B.out[(uint64_t)s * B.cells + o] = lerp4(tx.a, tx.b, B.a[s]);
+            } else {
+                Texel2 ty;  // the next level of the same column (the top level pairs with itself)
+                const uint64_t o1 = (r % nz) + 1u < nz ? o + 1 : o;
+                asm("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                    : "=f"(ty.a.x), "=f"(ty.a.y), "=f"(ty.a.z), "=f"(ty.a.w), "=f"(ty.b.x), "=f"(ty.b.y), "=f"(ty.b.z), "=f"(ty.b.w)
+                    : "l"(B.pair + o1));
+#pragma unroll 4
+                for (int s = 0; s < B.m; ++s) {
+                    TexelZ w;
+                    w.lo = lerp4(tx.a, tx.b, B.a[s]);
+                    w.hi = lerp4(ty.a, ty.b, B.a[s]);
+                    ((TexelZ *)B.out)[(uint64_t)s * B.cells + o] = w;
+                }
+            }
         }
     }
 }
 
-cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, const BlendBox *box, cudaStream_t st)
+cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, const float *a, const BlendBox *box, bool zpair, cudaStream_t st)
 {
     BlendArgs B;
+    B.zpair = zpair ? 1 : 0;
     B.pair = (const Texel2 *)pair; B.out = out; B.cells = cells; B.m = m;
     for (int s = 0; s < kBlendDepth; ++s) B.a[s] = s < m ? a[s] : 0.0f;
     B.box = *box;

@@ -52,6 +52,27 @@ def test_workspace_bytes_monotone_and_errors():
         lpm.workspace_bytes(w.cgrid, 10, 3, False)
 
 
+def test_workspace_bytes_texel_pairs_rule():
+    """lpm_params.texel_pairs (B8): 16 more bytes per met cell and fused step when on; auto from
+    capacity >= 16 x met cells; never for the physics the pair kernels are not instantiated for."""
+    w = make("c2")
+    mc = w.mgrid.nx * w.mgrid.ny * w.mgrid.nz
+    kw = dict(mgrid=w.mgrid, nt=3)
+    off = lpm.workspace_bytes(w.cgrid, 1000, 1, False, texel_pairs=-1, **kw)
+    on = lpm.workspace_bytes(w.cgrid, 1000, 1, False, texel_pairs=1, **kw)
+    assert on - off == 16 * 16 * mc
+    assert lpm.workspace_bytes(w.cgrid, 1000, 1, False, **kw) == off                                  # auto, small ensemble
+    big, cap = lpm.workspace_bytes(w.cgrid, 16 * mc, 1, False, **kw), lpm.workspace_bytes(w.cgrid, 16 * mc, 1, False, texel_pairs=-1, **kw)
+    assert big - cap == 16 * 16 * mc                                                                # auto, large ensemble
+    assert lpm.workspace_bytes(w.cgrid, 16 * mc - 1, 1, False, **kw) == lpm.workspace_bytes(w.cgrid, 16 * mc - 1, 1, False, texel_pairs=-1, **kw)
+    for no in (dict(dep_mode=1), dict(drift=True), dict(kz_mode=1), dict(z_levels=np.linspace(0.0, 1000.0, w.mgrid.nz))):
+        a = lpm.workspace_bytes(w.cgrid, 16 * mc, 1, False, texel_pairs=1, **kw, **no)
+        b = lpm.workspace_bytes(w.cgrid, 16 * mc, 1, False, texel_pairs=-1, **kw, **no)
+        assert a == b, no
+    assert lpm.workspace_bytes(w.cgrid, 16 * mc, 1, False, mgrid=w.mgrid, nt=1, texel_pairs=1) == \
+        lpm.workspace_bytes(w.cgrid, 16 * mc, 1, False, mgrid=w.mgrid, nt=1, texel_pairs=-1)
+
+
 def test_no_device_is_an_error_not_a_fallback():
     import torch
     if torch.cuda.is_available():

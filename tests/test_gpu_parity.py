@@ -323,6 +323,32 @@ def test_fused_equals_unfused_bitwise(lpm):
     assert res[0][2] > res[2][2] * 5
 
 
+@pytest.mark.parametrize("name,scale,nt", [("c3", 2e-3, 3), ("c2", 0.02, 3), ("c3_hdep80", 2e-3, 3)])
+def test_texel_pairs_bitwise(lpm, name, scale, nt):
+    """DESIGN.md B8: the 32-byte z-pair texel layout gathers the same eight values, so the particle state and the
+    counts are bit-identical to the 16-byte layout; the auto rule picks it from capacity >= 16 x met cells."""
+    w = make(name, scale=scale, n_steps=700).replace(nt=nt)
+    res = []
+    for tp in (-1, 1):
+        sim = lpm.Simulation(w, texel_pairs=tp)
+        assert sim.texel_pairs == (tp == 1)
+        sim.step(700)
+        p = sim.get_particles()
+        res.append((p["xyzq"].cpu().numpy().copy(), None if p["q1"] is None else p["q1"].cpu().numpy().copy(), sim.counts().cpu().numpy().copy(),
+                    sim.concentration().cpu().numpy().copy(), np.array(sim.ledger())))
+    np.testing.assert_array_equal(res[0][0], res[1][0])
+    if res[0][1] is not None:
+        np.testing.assert_array_equal(res[0][1], res[1][1])
+    np.testing.assert_array_equal(res[0][2], res[1][2])
+    np.testing.assert_allclose(res[0][3], res[1][3], rtol=1e-6)
+    np.testing.assert_allclose(res[0][4], res[1][4], rtol=1e-9)
+    assert not lpm.Simulation(w).texel_pairs                                   # auto: small ensemble, 16-byte texels
+    with pytest.raises(lpm.LpmError):
+        lpm.Simulation(w.replace(compact=True), texel_pairs=1)                 # pairs are for the slot-addressed store
+    with pytest.raises(lpm.LpmError):
+        lpm.Simulation(w, texel_pairs=1, dep_mode=1)
+
+
 # ------------------------------------------------------------------ a8: binning fed identical positions
 @pytest.mark.parametrize("name", ["c2", "c3", "c4"])
 def test_binning_identical_positions(lpm, orc, name):
@@ -586,6 +612,7 @@ def test_full_size_sampled_against_oracle(lpm, orc, name, stride, steps, nt):
     the run, so the oracle computes those trajectories one by one; plus properties that hold at any size."""
     w = make(name, scale=1.0, n_steps=steps).replace(nt=nt)
     sim = lpm.Simulation(w)
+    assert sim.texel_pairs == (name == "c4")                # the auto rule of lpm_params.texel_pairs (B8)
     sim.step(steps)
     p = sim.get_particles()
     n = p["n"]
