@@ -49,7 +49,7 @@ LANE_OPS_STATIC, LANE_OPS_TIME = 250.0, 310.0
 SMS, LANES_PER_SM = 148, 128          # 4 SMSP x 32 lanes: one warp instruction per clock per SMSP
 LAUNCH_STEPS = 16                     # model steps fused per step-kernel launch (csrc kMaxFused)
 # dram__bytes_read.sum + dram__bytes_write.sum of one captured step-kernel launch, bytes (profiles/r01c_c4_step_kernel_ncu.md)
-NCU_TRAFFIC = {"c4": 3.586e9 + 1.934e9}   # launch 171 of `bench.py --steps 1 --warmup 3`: 16 steps x 3.16e7 particles
+NCU_TRAFFIC = {"c4": 4.069e9 + 1.985e9}   # launch 171 of `bench.py --steps 1 --warmup 3`: 16 steps x 3.16e7 particles, z-pair texels (profiles/r01c_c4_step_kernel_ncu.md, r01d)
 ORACLE_STRIDE = {"c1": 1, "c2": 40, "c2_eq3": 40, "c3": 400, "c3_hdep80": 400, "c4": 4000, "c5": 1}
 ORACLE_SCALE_C5 = 1.0e-3              # c5 cannot be pid-strided (capacity couples particles): 1/1000 scale
 
