@@ -15,7 +15,9 @@
  * the exact Gaussian puff / folded normal (P4), 2^(-t/T) decay (P5), mass ledger (P6), affine
  * reproduction of the interpolation (P7), well-mixed reflection (P8), brute-force binning (P9),
  * closed-form deposition (P10, P11), compaction (P12), schedule (P13), independent numpy trace
- * (P14), geometric-series dose of a resting decaying cloud (P15).  PARITY UNPINNED (no printed value or implementation exists to compare against): the
+ * (P14), geometric-series dose of a resting decaying cloud (P15), Bernoulli deposition (P16), Eq.(3) (P17), levels (P18),
+ * drift slope (P19), ground decay: airborne + ground = emitted 2^(-t/T) and the sum of separately decayed increments (P20).
+ * PARITY UNPINNED (no printed value or implementation exists to compare against): the
  * dry-deposition rate law p_dry = 1-exp(-vd dt/h_dep) and h_dep, and the treatment of ground,
  * top and lateral boundaries (the paper gives none: L84-86 "out of scope of this paper").
  *
@@ -110,6 +112,7 @@ typedef struct orc_sim {
     uint64_t *frag_pids; uint64_t n_frag, frag_cap; /* pids ever flagged fragile (T3) */
     uint64_t bin_step;
     double *dose;     /* [K][nz][ny][nx] time-integrated concentration, Bq s m^-3; NULL = not accumulated */
+    double *ground, *ground_slack; /* [K][ny][nx] deposited activity that keeps decaying on the ground (R13); NULL = off */
 } orc_sim;
 
 /* ------------------------------------------------------------------ R1: Philox4x32-10
@@ -400,7 +403,7 @@ void orc_destroy(orc_sim *s)
     free(s->x); free(s->y); free(s->z); free(s->pid); free(s->status); free(s->fragile);
     free(s->dcell); free(s->nearface); free(s->moved);
     for (int k = 0; k < ORC_MAXK; ++k) { free(s->m[k]); free(s->inc_dry[k]); free(s->inc_wet[k]); free(s->inc_dec[k]); }
-    free(s->conc_sum); free(s->cnt); free(s->dep); free(s->dep_slack); free(s->inj_log); free(s->frag_pids); free(s->dose);
+    free(s->conc_sum); free(s->cnt); free(s->dep); free(s->dep_slack); free(s->inj_log); free(s->frag_pids); free(s->dose); free(s->ground); free(s->ground_slack);
     free(s);
 }
 
@@ -611,6 +614,7 @@ static void add_slack(orc_sim *s, int k, int64_t ci, int64_t cj, double v)
     const orc_grid *cg = &s->cfg.cgrid;
     if (ci < 0 || cj < 0 || ci >= cg->nx || cj >= cg->ny) return;
     s->dep_slack[((size_t)k * cg->ny + cj) * cg->nx + ci] += v;
+    if (s->ground_slack) s->ground_slack[((size_t)k * cg->ny + cj) * cg->nx + ci] += v;
 }
 
 /* R10 / PAPER.md L108: "Activities or masses of particles are summarized on a rectangular grid" */
@@ -671,6 +675,7 @@ int32_t orc_step(orc_sim *s, int32_t n_steps)
                 if (d == 0.0) continue;
                 if (s->dcell[i] >= 0) {
                     s->dep[(size_t)k * cg->nx * cg->ny + (size_t)s->dcell[i]] += d;
+                    if (s->ground) s->ground[(size_t)k * cg->nx * cg->ny + (size_t)s->dcell[i]] += d;
                     int64_t ci = s->dcell[i] % cg->nx, cj = s->dcell[i] / cg->nx;
                     uint8_t nf = s->nearface[i];
                     if (nf) {
@@ -694,6 +699,17 @@ int32_t orc_step(orc_sim *s, int32_t n_steps)
                     }
                 }
             }
+        }
+        /* R13 (SURVEY 8(c) R8 "a read-out-time option", 8(f)3 "ground-decay of the deposition map"): what lies on the
+         * ground decays like what is in the air.  The increments of step n were evaluated at t_n (R8: the mass at the
+         * start of the step), so they decay over this step too: ground(t_{n+1}) = (ground(t_n) + increments) exp(-lambda dt) */
+        if (s->ground) {
+            size_t c2 = (size_t)cg->nx * cg->ny;
+            for (int k = 0; k < c->K; ++k)
+                for (size_t i = 0; i < c2; ++i) {
+                    s->ground[(size_t)k * c2 + i] *= s->f_decay[k];
+                    s->ground_slack[(size_t)k * c2 + i] *= s->f_decay[k];
+                }
         }
         /* A16: stable compaction of exited particles (BASELINE config 5) */
         if (c->compact) {
@@ -816,6 +832,32 @@ void orc_deposition(const orc_sim *s, double *out, double *slack)
     for (size_t i = 0; i < n; ++i) {
         out[i] = s->dep[i] / A;
         if (slack) slack[i] = s->dep_slack[i] / A;
+    }
+}
+
+/* R13: from now on also keep the deposition map whose content decays on the ground.  Call before the first deposit
+ * (it starts from the undecayed map as it stands, which is only right while that map is empty or freshly deposited). */
+void orc_enable_ground_decay(orc_sim *s)
+{
+    const orc_grid *g = &s->cfg.cgrid;
+    size_t n = (size_t)g->nx * g->ny * s->cfg.K;
+    if (s->ground) return;
+    s->ground = malloc(n * sizeof(double));
+    s->ground_slack = malloc(n * sizeof(double));
+    if (!s->ground || !s->ground_slack) abort();
+    memcpy(s->ground, s->dep, n * sizeof(double));
+    memcpy(s->ground_slack, s->dep_slack, n * sizeof(double));
+}
+
+/* the ground-decayed deposition [K][ny][nx] in Bq m^-2 at the current time, and its face slack */
+void orc_deposition_ground(const orc_sim *s, double *out, double *slack)
+{
+    const orc_grid *g = &s->cfg.cgrid;
+    size_t n = (size_t)g->nx * g->ny * s->cfg.K;
+    double A = g->dx * g->dy;
+    for (size_t i = 0; i < n; ++i) {
+        out[i] = s->ground ? s->ground[i] / A : 0.0;
+        if (slack) slack[i] = s->ground_slack ? s->ground_slack[i] / A : 0.0;
     }
 }
 

@@ -89,6 +89,8 @@ def lib():
         L.orc_counts.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_enable_dose.argtypes = [C.c_void_p]
         L.orc_dose.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_enable_ground_decay.argtypes = [C.c_void_p]
+        L.orc_deposition_ground.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_deposition.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_injected.argtypes = [C.c_void_p, C.c_uint64]
         L.orc_injected.restype = C.c_uint64
@@ -335,6 +337,17 @@ class OracleSim:
         out = np.zeros((self.K, g.ny, g.nx))
         slack = np.zeros((self.K, g.ny, g.nx)) if with_slack else None
         lib().orc_deposition(self._h, _p(out), _p(slack))
+        return (out, slack) if with_slack else out
+
+    def enable_ground_decay(self):
+        lib().orc_enable_ground_decay(self._h)
+
+    def deposition_ground(self, with_slack=False):
+        """deposition map whose content keeps decaying on the ground [K][ny][nx], Bq m^-2 at the current time (R13)"""
+        g = self.w.cgrid
+        out = np.zeros((self.K, g.ny, g.nx))
+        slack = np.zeros((self.K, g.ny, g.nx)) if with_slack else None
+        lib().orc_deposition_ground(self._h, _p(out), _p(slack))
         return (out, slack) if with_slack else out
 
     def injected(self, step):

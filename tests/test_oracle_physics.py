@@ -540,3 +540,61 @@ def test_drift_correction_keeps_a_uniform_cloud_well_mixed():
     chi2 = ((hist[True] - expect) ** 2 / expect).sum()
     assert chi2 < 40.0, (chi2, hist[True])                               # 9 degrees of freedom (+ O(dt) scheme error)
     assert hist[False][0] > 1.5 * expect and hist[False][-1] < 0.7 * expect, hist[False]
+
+
+# ------------------------------------------------------------------ P20: ground decay of the deposition map (S§8(f)3, R13)
+def test_ground_decay_total_activity_follows_the_decay_law():
+    """A puff that moves, diffuses and deposits (dry everywhere + a rain box), everything on the map: with the ground
+    activity decaying too, airborne + ground = emitted * 2^(-t/T) at every step, whatever the particles did; for a
+    resting cloud the one cell holds m0 f^N (1 - (1-p)^N) (closed forms)."""
+    T_half, dt, N = 2400.0, 10.0, 60
+    nuc = [Nuclide("X", T_half, vd=0.5, lambda_wet=2.0e-3)]
+    g = Grid(40, 40, 4, -2000.0, -2000.0, 0.0, 100.0, 100.0, 50.0)
+    w = custom(uniform_met(u=1.5, v=-0.5, kz=2.0), grid=g, n=400, nuclides=nuc, dt=dt, Kh=20.0, H=200.0, activity=[7.0e5], n_steps=N,
+               rain=RainBox(-500.0, 600.0, -400.0, 500.0, 100.0, 400.0))
+    o = orc.OracleSim(w)
+    o.enable_ground_decay()
+    A = g.dx * g.dy
+    for n in range(1, N + 1):
+        o.step(1)
+        if n % 12 == 0:
+            air = o.particles()["m"].sum()
+            tot = air + o.deposition_ground().sum() * A
+            assert tot == pytest.approx(7.0e5 * 2.0 ** (-n * dt / T_half), rel=1e-12)
+    led = np.array(o.ledger())
+    assert led[0][6] == 0.0 and led[0][3] > 0.0                               # nothing fell off the map; it did rain
+    assert o.deposition_ground().sum() < o.deposition().sum()
+    # resting cloud
+    w = custom(uniform_met(), grid=g, n=50, nuclides=[Nuclide("X", T_half, vd=0.5)], dt=dt, H=200.0, activity=[3.0e4], n_steps=N,
+               src=(130.0, -270.0, 20.0))
+    o = orc.OracleSim(w)
+    o.enable_ground_decay()
+    o.step(N)
+    p, f = float(o.p_dry(0)), 2.0 ** (-dt / T_half)
+    d = o.deposition_ground()
+    i, j = int((130.0 - g.x0) // g.dx), int((-270.0 - g.y0) // g.dy)
+    assert d[0, j, i] * A == pytest.approx(3.0e4 * f ** N * (1 - (1 - p) ** N), rel=1e-12)
+    assert d.sum() == pytest.approx(d[0, j, i], rel=1e-15)
+
+
+def test_ground_decay_is_the_sum_of_increments_each_decayed_from_its_own_step():
+    """Definition, re-run step by step on a continuous release with layer deposition and rain, two nuclides: the increments
+    of step n (differences of the undecayed map) decay from t_n: ground(t_N) = sum_n inc_n exp(-lambda (t_N - t_n))."""
+    dt, N = 10.0, 90
+    nuc = [Nuclide("A", 1800.0, vd=0.02, lambda_wet=1.0e-3), Nuclide("B", 5.0e4, vd=0.05, lambda_wet=3.0e-4)]
+    g = Grid(30, 30, 6, -1500.0, -1500.0, 0.0, 100.0, 100.0, 50.0)
+    w = custom(uniform_met(u=2.0, v=1.0, kz=3.0), grid=g, n=600, nuclides=nuc, dt=dt, Kh=30.0, H=300.0, h_dep=80.0, activity=[1.0e6, 4.0e5],
+               t_rel=(0.0, 600.0), n_steps=N, rain=RainBox(-200.0, 900.0, -300.0, 800.0, 200.0, 700.0))
+    o = orc.OracleSim(w)
+    o.enable_ground_decay()
+    prev = o.deposition()
+    want = np.zeros_like(prev)
+    lam = np.array([math.log(2.0) / n_.half_life_s for n_ in nuc])[:, None, None]
+    for n in range(N):
+        o.step(1)
+        cur = o.deposition()
+        want += (cur - prev) * np.exp(-lam * (N - n) * dt)
+        prev = cur
+    got = o.deposition_ground()
+    assert got.sum() > 0
+    np.testing.assert_allclose(got, want, rtol=1e-9, atol=1e-12 * got.max())
