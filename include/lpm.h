@@ -121,6 +121,11 @@ typedef struct {
                                * bit-identical either way.  Pairs need the default physics on the
                                * slot-addressed store: compact = 0, nt > 1, dep_mode 0, kz_mode 0, uniform
                                * levels, drift 0 (auto: 16-byte texels otherwise; 1: INVALID_ARG)     */
+    int32_t ground_decay;     /* 1: what has been deposited keeps decaying on the ground with its nuclide's half-life
+                               * (SURVEY 8(c) R8 "a read-out-time option", 8(f)3; R13): the increments of step n
+                               * decay from t_n on, and lpm_deposition* return the map as it is at the current time.
+                               * 0 (default): the map is the cumulative deposited activity, never decayed.  The ledger
+                               * (what left the air) is the same either way                            */
 } lpm_params;
 
 typedef struct {

@@ -57,7 +57,7 @@ class lpm_nuclide(C.Structure):
 class lpm_params(C.Structure):
     _fields_ = [("dt", C.c_double), ("seed", C.c_uint64), ("capacity", C.c_uint64), ("boundary_mode", C.c_int32),
                 ("compact", C.c_int32), ("h_dep", C.c_double), ("bin_every", C.c_int32), ("steps_per_launch", C.c_int32),
-                ("gather_sort", C.c_int32), ("dose", C.c_int32), ("dep_mode", C.c_int32), ("drift", C.c_int32), ("texel_pairs", C.c_int32)]
+                ("gather_sort", C.c_int32), ("dose", C.c_int32), ("dep_mode", C.c_int32), ("drift", C.c_int32), ("texel_pairs", C.c_int32), ("ground_decay", C.c_int32)]
 
 
 class lpm_source(C.Structure):
@@ -175,7 +175,8 @@ class Simulation:
     """
 
     def __init__(self, w, *, steps_per_launch: int = 0, bin_every: Optional[int] = None, fields_dev=None,
-                 stream=None, auto_release: bool = True, gather_sort: int = 0, dose: bool = False, dep_mode: int = 0, drift: bool = False, texel_pairs: int = 0):
+                 stream=None, auto_release: bool = True, gather_sort: int = 0, dose: bool = False, dep_mode: int = 0, drift: bool = False, texel_pairs: int = 0,
+                 ground_decay: bool = False):
         torch = _require_cuda()
         L = load()
         self._L = L
@@ -209,7 +210,7 @@ class Simulation:
                          boundary_mode=1 if w.boundary_mode == "absorb" else 0, compact=1 if w.compact else 0,
                          h_dep=w.h_dep, bin_every=w.bin_every if bin_every is None else bin_every,
                          steps_per_launch=steps_per_launch, gather_sort=gather_sort, dose=1 if dose else 0, dep_mode=dep_mode, drift=1 if drift else 0,
-                         texel_pairs=texel_pairs)
+                         texel_pairs=texel_pairs, ground_decay=1 if ground_decay else 0)
         h = C.c_void_p()
         with torch.cuda.stream(self.stream):
             rc = L.lpm_create(C.byref(cg), C.byref(met), nucs, w.K, C.byref(prm), self.workspace.data_ptr(), nbytes,

@@ -152,6 +152,8 @@ struct lpm_handle {
     uint64_t csort_step;  // compact store: step of the last physical sort
     bool bbox_valid;      // the mask tiles hold the met columns of the particles as the last step launch left them
     double dep_bound[LPM_MAX_NUCLIDES];  // largest activity a particle can carry (fixed-point scale of the deposit tables)
+    double lam_dt[LPM_MAX_NUCLIDES];     // lambda_k dt
+    uint64_t dep_ref[LPM_MAX_NUCLIDES];  // R13 (ground_decay): the map of nuclide k holds activity referred to this step's time
     bool binned;
     int sms, occ;
     uint64_t launches;
@@ -301,7 +303,9 @@ void base_args(const lpm_handle *h, StepArgs &A)
         // bound: an increment outside [2^17, 2^20) / S takes the direct fp64 RED.
         const int k = w / 2;
         const double frac = k < h->K ? (w & 1 ? (double)h->p_wet[k] : (double)h->p_dry[k]) : 0.0;
-        const double inc_max = (k < h->K ? h->dep_bound[k] : 0.0) * frac;
+        // (ground decay: the increments of a launch grow by up to exp(lambda dt kMaxFused) relative to its first step)
+        const double grow = h->prm.ground_decay && k < h->K ? exp(h->lam_dt[k] * kMaxFused) : 1.0;
+        const double inc_max = (k < h->K ? h->dep_bound[k] : 0.0) * frac * grow;
         int e = 0;
         if (inc_max > 0.0) { frexp(1048576.0 / inc_max, &e); e -= 1; }
         if (e > 100) e = 100;
@@ -503,7 +507,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         return LPM_ERR_INVALID_ARG;
     if (!(p->dt > 0) || p->capacity == 0 || p->capacity >= (1ull << 32) || !(met->H_mix > 0) || met->Kh < 0 ||
         (met->nt > 1 && !(met->dt_snap > 0)) || p->bin_every < 0 || p->steps_per_launch < 0 || !(p->h_dep > 0) || p->dep_mode < 0 ||
-        p->dep_mode > 1 || p->drift < 0 || p->drift > 1 || (p->drift == 1 && met->kz_mode == 1) || p->texel_pairs < -1 || p->texel_pairs > 1 ||
+        p->dep_mode > 1 || p->drift < 0 || p->drift > 1 || (p->drift == 1 && met->kz_mode == 1) || p->texel_pairs < -1 || p->texel_pairs > 1 || p->ground_decay < 0 || p->ground_decay > 1 ||
         (p->texel_pairs == 1 && !zpair_possible(met, p)))
         return LPM_ERR_INVALID_ARG;
     int ndev = 0, dev = 0;
@@ -541,6 +545,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         any_dry |= h->p_dry[k] > 0.0f;
         const double lam_dt = nuc[k].half_life_s > 0 ? M_LN2 * p->dt / nuc[k].half_life_s : 0.0;
         h->f_decay[k] = exp(-lam_dt);
+        h->lam_dt[k] = lam_dt;
         const double keep_dry = uniform ? 1.0 - (double)h->p_dry[k] : 1.0;
         h->ln_rho[k] = -lam_dt + (uniform ? log1p(-(double)h->p_dry[k]) : 0.0);
         h->dec_scale[k] = -expm1(-lam_dt) * keep_dry;
@@ -630,11 +635,39 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
         A.step0 = h->step;
         for (int s = 0; s < m; ++s) {
             fill_entry(h, h->step + s, A.tab[s]);
-            for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) A.tab[s].Gps[k] = A.tab[s].Gp[k] * A.dep_scale[2 * k];
+            for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) {
+                // table units of the deposit increments; R13: Er = growth since the first step of the launch (1 without ground decay)
+                StepEntry &e = A.tab[s];
+                const double Er = h->prm.ground_decay && k < h->K ? exp(h->lam_dt[k] * s) : 1.0;
+                const double sd = (double)A.dep_scale[2 * k] * Er, sw = (double)A.dep_scale[2 * k + 1] * Er;
+                e.Gps[k] = (float)((double)e.Gp[k] * sd);
+                e.Pd[k] = (float)((double)h->p_dry[k] * sd);
+                e.Pw[k] = (float)((double)(float)h->wet_scale[k] * sw);
+                e.Oid[k] = (float)(1.0 / sd);
+                e.Oiw[k] = (float)(1.0 / sw);
+                e.Eg[k] = Er;   // x E0 below, once the launch's first step is final
+            }
             // a launch stays inside one met interval: the pair buffer holds snapshots (s, s+1)
             if ((A.tab[s].snap & 0xffff) != (A.tab[0].snap & 0xffff)) { m = s; break; }
         }
         A.m_steps = m;
+        if (h->prm.ground_decay) {
+            // R13: the map of nuclide k holds activity referred to step dep_ref[k]; an increment of step n enters as
+            // inc * exp(lambda (t_n - t_ref)) = inc * E0 * Er(n).  Move the reference before E0 grows large.
+            for (int k = 0; k < h->K; ++k) {
+                double age = h->lam_dt[k] * (double)(h->step - h->dep_ref[k]);
+                if (age > 4.0) {
+                    CK(launch_dep_rebase((double *)(h->ws + h->L.dep) + (uint64_t)k * A.dep_stride, A.dep_stride, exp(-age), h->st));
+                    h->launches++;
+                    h->dep_ref[k] = h->step;
+                    age = 0.0;
+                }
+                const double E0 = exp(age);
+                A.dep_inv_scale[2 * k] = E0 / (double)A.dep_scale[2 * k];
+                A.dep_inv_scale[2 * k + 1] = E0 / (double)A.dep_scale[2 * k + 1];
+                for (int s = 0; s < m; ++s) A.tab[s].Eg[k] *= E0;
+            }
+        }
         {
             const int rc = ensure_blend(h, A, m, m_max);
             if (rc) return rc;
@@ -814,8 +847,10 @@ static int dep_out(lpm_handle *h, float *o32, double *o64)
 {
     if (!h || (!o32 && !o64)) return fail(h, LPM_ERR_INVALID_ARG, "lpm_deposition: null");
     if (h->sticky) return h->sticky;
-    CK(launch_dep_readout((const double *)(h->ws + h->L.dep), o32, o64, (uint64_t)h->cg.nx * h->cg.ny, h->K,
-                          1.0 / (h->cg.dx * h->cg.dy), h->st));
+    double scale[LPM_MAX_NUCLIDES] = {0, 0};
+    for (int k = 0; k < h->K; ++k)   // per cell area; R13: the ground decay since the map's reference time
+        scale[k] = (h->prm.ground_decay ? exp(-h->lam_dt[k] * (double)(h->step - h->dep_ref[k])) : 1.0) / (h->cg.dx * h->cg.dy);
+    CK(launch_dep_readout((const double *)(h->ws + h->L.dep), o32, o64, (uint64_t)h->cg.nx * h->cg.ny, h->K, scale, h->st));
     h->launches++;
     return LPM_OK;
 }

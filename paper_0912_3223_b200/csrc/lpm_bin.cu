@@ -95,20 +95,34 @@ cudaError_t launch_dose_accum(const double *conc, double *dose, uint64_t cells3,
     return cudaGetLastError();
 }
 
-__global__ void dep_readout_kernel(const double *__restrict__ dep, float *out32, double *out64, uint64_t total, double inv_area)
+__global__ void dep_readout_kernel(const double *__restrict__ dep, float *out32, double *out64, uint64_t cells2, uint64_t total, double s0, double s1)
 {
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
-        const double v = dep[i] * inv_area;
+        const double v = dep[i] * (i < cells2 ? s0 : s1);
         if (out32) out32[i] = (float)v;
         if (out64) out64[i] = v;
     }
 }
 
-cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, double inv_area, cudaStream_t st)
+// scale[k] = 1 / cell area, times the ground-decay factor of nuclide k since the map's reference time (R13)
+cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, const double *scale, cudaStream_t st)
 {
     const uint64_t total = cells2 * K;
     int blocks = (int)((total + 255) / 256 < 148 * 8 ? (total + 255) / 256 : 148 * 8);
-    dep_readout_kernel<<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(dep, out_f32, out_f64, total, inv_area);
+    dep_readout_kernel<<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(dep, out_f32, out_f64, cells2, total, scale[0], K > 1 ? scale[1] : 0.0);
+    return cudaGetLastError();
+}
+
+// R13: move the reference time of one nuclide's ground-decaying map (keeps the stored values of the order of the activities)
+__global__ void dep_rebase_kernel(double *dep, uint64_t cells2, double factor)
+{
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < cells2; i += (uint64_t)gridDim.x * blockDim.x) dep[i] *= factor;
+}
+
+cudaError_t launch_dep_rebase(double *dep, uint64_t cells2, double factor, cudaStream_t st)
+{
+    int blocks = (int)((cells2 + 255) / 256 < 148 * 8 ? (cells2 + 255) / 256 : 148 * 8);
+    dep_rebase_kernel<<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(dep, cells2, factor);
     return cudaGetLastError();
 }
 

@@ -21,6 +21,11 @@ struct StepEntry {
     float Gf[LPM_MAX_NUCLIDES];  // (float)G_k(t_n), the factor the per-step fp32 arithmetic uses
     float Gp[LPM_MAX_NUCLIDES];  // (float)(G_k(t_n) * p_dry,k): uniform dry deposit of one step per unit q
     float Gps[LPM_MAX_NUCLIDES]; // Gp * S_dry,k: the same in the fixed-point units of the deposit tables
+    // deposit increments per unit activity in table units: p * S * Er, with Er = exp(lambda_k (t_n - t_launch)) when the
+    // map decays on the ground (R13: it is kept referred to a fixed time, so later increments weigh more), else 1
+    float Pd[LPM_MAX_NUCLIDES], Pw[LPM_MAX_NUCLIDES];
+    float Oid[LPM_MAX_NUCLIDES], Oiw[LPM_MAX_NUCLIDES];  // 1 / (S * Er): table units back to activity (off-map ledger)
+    double Eg[LPM_MAX_NUCLIDES];                         // exp(lambda_k (t_n - t_ref)): direct deposits (Bernoulli form)
     float a;                     // time weight between snapshot `snap` and `snap + 1`
     int32_t snap;                // bits 0..15 snapshot index, bit 16 = raining
     uint32_t buf;                // which time-blended met buffer holds F(t_n) (a0)
@@ -167,7 +172,8 @@ cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, c
 cudaError_t launch_bin(const BinArgs &a, int blocks, cudaStream_t st);
 cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3, int K, const double *scale, cudaStream_t st);
 cudaError_t launch_dose_accum(const double *conc, double *dose, uint64_t cells3, int K, const double *scale, cudaStream_t st);
-cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, double inv_area, cudaStream_t st);
+cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, const double *scale, cudaStream_t st);
+cudaError_t launch_dep_rebase(double *dep, uint64_t cells2, double factor, cudaStream_t st);
 cudaError_t launch_airborne(const float4 *xyzq, const float *q1, uint64_t n, const uint64_t *n_dev, int K, double *out2, cudaStream_t st);
 cudaError_t launch_export(const float4 *xyzq, const float *q1, uint64_t n, const uint64_t *n_dev, float4 *out, uint8_t *status, cudaStream_t st);
 cudaError_t launch_import(float4 *xyzq, uint64_t n, const uint8_t *status, cudaStream_t st);

@@ -86,16 +86,16 @@ __device__ __forceinline__ void dep_add(const StepArgs &A, DepTab<K> &T, int slo
 // add one particle-step's deposit to the map cell of the NEW (x, y); vd[k], vw[k] = dry and wet
 // increment of nuclide k in the fixed-point units of their sums
 template <int K, bool WET>
-__device__ __forceinline__ void deposit_at(const StepArgs &A, float x, float y, const float (&vd)[K], const float (&vw)[K], Acc<K> &acc,
-                                           DepTab<K> &T)
+__device__ __forceinline__ void deposit_at(const StepArgs &A, const StepEntry &e, float x, float y, const float (&vd)[K], const float (&vw)[K],
+                                           Acc<K> &acc, DepTab<K> &T)
 {
     const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
     const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
     if ((ci | cj) < 0) {  // off the map: ledger only
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            acc.off[k] += vd[k] * (float)A.dep_inv_scale[2 * k];
-            if (WET) acc.off[k] += vw[k] * (float)A.dep_inv_scale[2 * k + 1];
+            acc.off[k] += vd[k] * e.Oid[k];
+            if (WET) acc.off[k] += vw[k] * e.Oiw[k];
         }
         return;
     }
@@ -184,7 +184,7 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
                         const double act = (double)q[k] * e.G[k];
                         const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
                         const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
-                        if ((ci | cj) >= 0) atomicAdd(A.dep + (uint32_t)(cj * A.cg.nx + ci) + k * A.dep_stride, act);
+                        if ((ci | cj) >= 0) atomicAdd(A.dep + (uint32_t)(cj * A.cg.nx + ci) + k * A.dep_stride, act * e.Eg[k]);
                         else atomicAdd(A.ledger + k * 8 + 6, act);
                         atomicAdd(A.ledger + k * 8 + (d ? 2 : 3), act);
                         q[k] = 0.0f;
@@ -207,7 +207,7 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
             float vd[K];
 #pragma unroll
             for (int k = 0; k < K; ++k) vd[k] = q[k] * e.Gps[k];
-            deposit_at<K, false>(A, x, y, vd, vd, acc, dep);
+            deposit_at<K, false>(A, e, x, y, vd, vd, acc, dep);
         }
         return true;
     }
@@ -223,7 +223,7 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
         if (dry_here) {
             acc.dry[k] += act;
             if (DRY == kDryLayer) {
-                vd[k] = act * A.p_dry[k] * A.dep_scale[2 * k];
+                vd[k] = act * e.Pd[k];
                 q[k] = fmaf(-q[k], A.p_dry[k], q[k]);
                 act = q[k] * G;
             } else {
@@ -231,7 +231,7 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
             }
         }
         if (wet_here) {
-            vw[k] = act * A.wet_scale_f[k] * A.dep_scale[2 * k + 1];
+            vw[k] = act * e.Pw[k];
             acc.wet[k] += act;
             q[k] = fmaf(-q[k], A.p_wet[k], q[k]);
             act = q[k] * G;
@@ -240,7 +240,7 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
     }
 
     // a6: deposit at the cell of the NEW (x, y)
-    if (dry_here | wet_here) deposit_at<K, true>(A, x, y, vd, vw, acc, dep);
+    if (dry_here | wet_here) deposit_at<K, true>(A, e, x, y, vd, vw, acc, dep);
     return true;
 }
 

@@ -441,6 +441,60 @@ def test_deposition_map_end_to_end_with_slack(lpm, orc):
         assert abs(dg[k].sum() / do[k].sum() - 1) < 1e-5
 
 
+# ------------------------------------------------------------------ S§8(f)3 / R13: the deposition map decays on the ground
+@pytest.mark.parametrize("name,dep_mode", [("c3", 0), ("c3_hdep80", 0), ("c3", 1)])
+def test_ground_decay_of_the_deposition_map(lpm, orc, name, dep_mode):
+    """lpm_params.ground_decay: map vs the oracle's ground-decayed map within 1e-5 + face slack, with half-lives short
+    enough that the decay matters (1 h and 10 min against 6.4 h of run: the 10-min map moves its reference time several
+    times, and its increments grow by 20 % inside one 16-step launch); the undecayed ledger is unchanged."""
+    steps = 2300
+    w = make(name, scale=1.0, n_steps=steps)
+    w.release.pid_stride = 4000
+    nuc = [Nuclide("A", 3600.0, vd=w.nuclides[0].vd, lambda_wet=w.nuclides[0].lambda_wet),
+           Nuclide("B", 600.0, vd=w.nuclides[1].vd, lambda_wet=w.nuclides[1].lambda_wet)]
+    w = w.replace(nt=8, capacity=2500, nuclides=nuc)
+    sim = lpm.Simulation(w, ground_decay=True, dep_mode=dep_mode)
+    ref = lpm.Simulation(w, dep_mode=dep_mode)
+    o = orc.OracleSim(w, face_delta=1.5, dep_mode=dep_mode)
+    o.enable_ground_decay()
+    for s in (sim, ref, o):
+        s.step(steps)
+    dg = sim.deposition(f64=True).cpu().numpy()
+    do, slack = o.deposition_ground(with_slack=True)
+    assert do.sum() > 0 and do.sum() < 0.8 * o.deposition().sum()
+    if dep_mode == 0:
+        excess = np.maximum(np.abs(dg - do) - (1e-5 * do + 1.0001 * slack + 1e-30), 0.0)
+        assert excess.sum() <= 2e-3 * do.sum()
+        for k in range(2):
+            assert abs(dg[k].sum() / do[k].sum() - 1) < 1e-5
+    else:
+        # Bernoulli events are whole-particle deposits: identical decisions, so the maps agree wherever no event lay
+        # within the position tolerance of a cell face; compare the totals and the bulk of the cells
+        for k in range(2):
+            assert abs(dg[k].sum() / do[k].sum() - 1) < 2e-3
+        same = np.abs(dg - do) <= 1e-5 * do + 1e-30
+        assert same.mean() > 0.999
+    np.testing.assert_allclose(sim.ledger(), ref.ledger(), rtol=1e-7, atol=0)       # what left the air does not depend on it (fp32 off-map sums)
+    f32 = sim.deposition().cpu().numpy()
+    np.testing.assert_allclose(f32, dg, rtol=1e-6, atol=0)
+
+
+def test_ground_decay_total_activity_law(lpm):
+    """P20 on the GPU: a puff that deposits dry and wet, everything on the map: airborne + ground = emitted 2^(-t/T)."""
+    T_half, dt, N = 2400.0, 10.0, 60
+    nuc = [Nuclide("X", T_half, vd=0.5, lambda_wet=2.0e-3)]
+    g = Grid(40, 40, 4, -2000.0, -2000.0, 0.0, 100.0, 100.0, 50.0)
+    w = custom(uniform_met(u=1.5, v=-0.5, kz=2.0), grid=g, n=4000, nuclides=nuc, dt=dt, Kh=20.0, H=200.0, activity=[7.0e5], n_steps=N,
+               rain=RainBox(-500.0, 600.0, -400.0, 500.0, 100.0, 400.0))
+    for spl in (0, 1, 5):
+        sim = lpm.Simulation(w, ground_decay=True, steps_per_launch=spl)
+        sim.step(N)
+        led = sim.ledger()
+        ground = float(sim.deposition(f64=True).sum().item()) * g.dx * g.dy
+        assert led[0][6] == 0.0 and led[0][3] > 0.0
+        assert abs((led[0][1] + ground) / (7.0e5 * 2.0 ** (-N * dt / T_half)) - 1) < 2e-6, (spl, led[0][1], ground)
+
+
 # ------------------------------------------------------------------ S§8(f)3: time-integrated concentration
 def test_dose_grid(lpm, orc):
     """(f)3: resting decaying cloud (no wind, no diffusion): the dose grid equals the oracle's cell by cell to
