@@ -53,7 +53,7 @@ Layout make_layout(const lpm_grid &g, const lpm_meteo &met, uint64_t cap, int K,
     const uint64_t mcells = (uint64_t)met.grid.nx * met.grid.ny * met.grid.nz;
     L.blend = o; o += up((zpair ? 32ull : 16ull) * mcells * (met.nt > 1 ? kBlendDepth : 1) + 32);  // z-fastest F(t_n), one buffer per fused step (+ 1 pad texel)
     L.keys = o; o += sort ? up(4 * cap) : 0;            // gather-locality pass: met-cell key per slot
-    L.perm = o; o += sort && !compact ? up(4 * cap) : 0;  //   slots in met-cell order (slot-addressed store)
+    L.perm = o; o += sort && !compact ? 2 * up(4 * cap) : 0;  //   slots in met-cell order (slot-addressed store): current list + the one being built
     L.hist = o; o += sort ? up(4 * (mcells + 1)) : 0;   //   per-cell counts / offsets
     L.partial = o; o += sort ? up(4 * sort_partial_entries(mcells)) : 0;
     L.alt_xyzq = o; o += sort && compact ? up(16 * cap) : 0;           //   compact store: the records themselves are sorted,
@@ -125,6 +125,7 @@ struct lpm_handle {
     lpm_params prm;
     bool has_levels;
     bool zpair;   // B8: the blended buffers hold 32-byte z-pair texels
+    int perm_cur; // which half of L.perm holds the current slot list
     float zlev[kMaxLevels];   // non-uniform level heights (fp32 parameters), copied from meteo.z_levels_host
     int K;
     cudaStream_t st;
@@ -746,7 +747,7 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                 if (sort_enabled(&h->prm) && A.n_prev > 0 && (h->prm.gather_sort > 0 || A.n_prev >= kSortAutoMin)) {
                     // the list is kept for `period` model steps (one release: the perm buffer is its own);
                     // particles born since the last sort are walked in slot order behind it
-                    uint32_t *perm = (uint32_t *)(h->ws + h->L.perm);
+                    uint32_t *perm = (uint32_t *)(h->ws + h->L.perm) + (uint64_t)h->perm_cur * (up(4 * h->prm.capacity) / 4);
                     const bool single = h->rel.size() == 1;
                     const uint64_t period = h->prm.gather_sort > 0 ? (uint64_t)h->prm.gather_sort : (uint64_t)kSortPeriod;
                     const uint32_t n_keys = (uint32_t)A.snap_cells + 1u;
@@ -754,7 +755,11 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                     if (!single || !h->perm_valid || h->step - h->perm_step >= period || h->perm_n > A.n_prev) {
                         const int sspan = span_open(h, 2, (double)A.n_prev);
                         if (single && h->keys_ready && h->keys_n == A.n_prev && h->keys_step == h->step) {
-                            CK(launch_sort_finish(keys, A.n_prev, n_keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->st));
+                            // the keys stand in the order of the current list (written by the previous launch): build the other one
+                            h->perm_cur ^= 1;
+                            uint32_t *next = (uint32_t *)(h->ws + h->L.perm) + (uint64_t)h->perm_cur * (up(4 * h->prm.capacity) / 4);
+                            CK(launch_sort_finish(keys, A.n_prev, n_keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->perm_n, next, h->st));
+                            perm = next;
                             h->launches += 4;
                         } else {
                             CK(launch_sort_by_cell(A.xyzq + r.base, A.n_prev, A.mg, keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->st));

@@ -143,8 +143,8 @@ int step_max_blocks_per_sm(int K, bool compact, int dry_mode, bool bern, bool eq
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
                                 uint32_t *perm, cudaStream_t st);
-cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, uint32_t *perm,
-                               cudaStream_t st);
+cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, const uint32_t *list_old,
+                               uint64_t n_old, uint32_t *perm, cudaStream_t st);
 cudaError_t launch_fill_holes(float4 *xyzq, float *q1, uint32_t *pid, uint64_t *ctrl, const uint32_t *holes, uint32_t *src, uint32_t *dst,
                               cudaStream_t st);
 cudaError_t launch_sort_records(float4 *xyzq, float *q1, uint32_t *pid, const uint64_t *n_dev, uint64_t capacity, GridF g, uint32_t *keys,

@@ -110,21 +110,25 @@ __global__ void __launch_bounds__(256) scan_apply_kernel(uint32_t *__restrict__ 
     }
 }
 
-// pass 3: scatter slot indices; lanes of a warp that share a key claim their range with one atomic
+// pass 3: scatter slot indices; lanes of a warp that share a key claim their range with one atomic.
+// keys[pos] belongs to the slot list_old[pos] (pos < n_old: the keys were written in the order of the previous list by
+// the step kernel, so neighbours in `pos` are neighbours in space: the atomics aggregate and the writes to the new list
+// fall into a few lines per warp), or to slot pos (no previous list, and the particles born behind it).
 __global__ void __launch_bounds__(256) sort_scatter_kernel(const uint32_t *__restrict__ keys, uint64_t n, uint32_t *__restrict__ offs,
-                                                           uint32_t *__restrict__ perm)
+                                                           const uint32_t *__restrict__ list_old, uint64_t n_old, uint32_t *__restrict__ perm)
 {
     const uint64_t n_round = (n + 31) & ~(uint64_t)31;
     const int lane = threadIdx.x & 31;
     for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n_round; l += (uint64_t)gridDim.x * blockDim.x) {
         const bool live = l < n;
         const uint32_t key = live ? keys[l] : 0xffffffffu;
+        const uint32_t slot = (live && l < n_old) ? list_old[l] : (uint32_t)l;
         const uint32_t peers = __match_any_sync(0xffffffffu, key);
         const int leader = __ffs(peers) - 1;
         uint32_t base = 0;
         if (live && lane == leader) base = atomicAdd(offs + key, (uint32_t)__popc(peers));
         base = __shfl_sync(0xffffffffu, base, leader);
-        if (live) perm[base + __popc(peers & ((1u << lane) - 1u))] = (uint32_t)l;
+        if (live) perm[base + __popc(peers & ((1u << lane) - 1u))] = slot;
     }
 }
 
@@ -232,8 +236,8 @@ cudaError_t launch_sort_records(float4 *xyzq, float *q1, uint32_t *pid, const ui
 
 // passes 2 + 3 on keys and a histogram that are already there (written by sort_key_kernel, or by the
 // step kernel itself at the end of the launch that precedes a sort)
-cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, uint32_t *perm,
-                               cudaStream_t st)
+cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, const uint32_t *list_old,
+                               uint64_t n_old, uint32_t *perm, cudaStream_t st)
 {
     const uint32_t m = n_keys;
     const uint64_t want = (n + 255) / 256;
@@ -242,7 +246,7 @@ cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys
     scan_totals_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
     scan_partials_kernel<<<1, 256, 0, st>>>(partial, nb);
     scan_apply_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
-    sort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, hist, perm);
+    sort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, hist, list_old, list_old ? n_old : 0, perm);
     return cudaGetLastError();
 }
 
@@ -255,7 +259,7 @@ cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_
     const uint64_t want = (n + 255) / 256;
     const int blocks = (int)(want < 148 * 8 ? (want ? want : 1) : 148 * 8);
     sort_key_kernel<<<blocks, 256, 0, st>>>(xyzq, n, g, n_keys, keys, hist);
-    return launch_sort_finish(keys, n, n_keys, hist, partial, perm, st);
+    return launch_sort_finish(keys, n, n_keys, hist, partial, nullptr, 0, perm, st);
 }
 
 uint64_t sort_partial_entries(uint64_t n_cells) { return (n_cells + 1 + kScanBlock - 1) / kScanBlock + 1; }

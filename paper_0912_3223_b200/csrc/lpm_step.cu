@@ -301,14 +301,14 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
         __syncthreads();
         const uint32_t tile = s_ticket;
         if (tile >= n_tiles) break;
-        uint64_t l;
+        uint64_t l, pos;   // slot (relative to the release block) and its position in the list
         bool valid;
         if (tile < t_old) {
-            const uint64_t idx = (uint64_t)tile * kStepThreads + threadIdx.x;
-            valid = idx < A.n_perm;
-            l = valid ? A.perm[idx] : 0ull;
+            pos = (uint64_t)tile * kStepThreads + threadIdx.x;
+            valid = pos < A.n_perm;
+            l = valid ? A.perm[pos] : 0ull;
         } else {
-            l = first_new + (uint64_t)(tile - t_old) * kStepThreads + threadIdx.x;
+            l = pos = first_new + (uint64_t)(tile - t_old) * kStepThreads + threadIdx.x;
             valid = l < A.n;
         }
         const bool in_range = valid;
@@ -354,11 +354,12 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
         }
         if (A.keys_out) {
             // pass 1 of the coming gather-locality sort, for free: the new position is in registers; the lanes of
-            // a warp that share a key (most of them, in a sorted warp) count with one atomic
+            // a warp that share a key (most of them, in a sorted warp) count with one atomic.  The keys are stored in
+            // LIST order (coalesced here, and the scatter pass then walks spatial neighbours: lpm_sort.cu)
             uint32_t key = 0xffffffffu;
             if (in_range) {
                 key = (valid && z >= 0.0f) ? corner_of<ZLEV>(A.mg, x, y, z).o : A.n_keys - 1u;
-                A.keys_out[l] = key;
+                A.keys_out[pos] = key;
             }
             const uint32_t peers = __match_any_sync(0xffffffffu, key);
             if (in_range && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(A.hist_out + key, (uint32_t)__popc(peers));
