@@ -126,6 +126,7 @@ struct lpm_handle {
     bool has_levels;
     bool zpair;   // B8: the blended buffers hold 32-byte z-pair texels
     int perm_cur; // which half of L.perm holds the current slot list
+    bool sort_by_slot;  // fused sort keys indexed by slot (large ensembles), else by list position
     float zlev[kMaxLevels];   // non-uniform level heights (fp32 parameters), copied from meteo.z_levels_host
     int K;
     cudaStream_t st;
@@ -525,6 +526,9 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     h->cg = *cg; h->met = *met; h->prm = *p; h->K = K;
     h->has_levels = met->z_levels_host != nullptr;
     h->zpair = zpair_enabled(met, p);
+    // many particles per met cell: young particles of one cell are neighbours in the store, and the slot-order scatter keeps
+    // each cell's slots ascending (coalesced state records in the step kernel); otherwise the cheaper list-order scatter
+    h->sort_by_slot = !p->compact && p->capacity >= kPairAutoRatio * (uint64_t)met->grid.nx * met->grid.ny * met->grid.nz;
     if (h->has_levels) for (int k = 0; k < met->grid.nz; ++k) h->zlev[k] = (float)met->z_levels_host[k];
     h->met.z_levels_host = nullptr;  // copied: the caller's array is not needed after lpm_create
     for (int k = 0; k < K; ++k) h->nuc[k] = nuc[k];
@@ -755,11 +759,16 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                     if (!single || !h->perm_valid || h->step - h->perm_step >= period || h->perm_n > A.n_prev) {
                         const int sspan = span_open(h, 2, (double)A.n_prev);
                         if (single && h->keys_ready && h->keys_n == A.n_prev && h->keys_step == h->step) {
-                            // the keys stand in the order of the current list (written by the previous launch): build the other one
-                            h->perm_cur ^= 1;
-                            uint32_t *next = (uint32_t *)(h->ws + h->L.perm) + (uint64_t)h->perm_cur * (up(4 * h->prm.capacity) / 4);
-                            CK(launch_sort_finish(keys, A.n_prev, n_keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->perm_n, next, h->st));
-                            perm = next;
+                            if (h->sort_by_slot) {
+                                // keys indexed by slot: the scatter walks the slots in order, each cell's slots end up ascending
+                                CK(launch_sort_finish(keys, A.n_prev, n_keys, hist, (uint32_t *)(h->ws + h->L.partial), nullptr, 0, perm, h->st));
+                            } else {
+                                // the keys stand in the order of the current list (written by the previous launch): build the other one
+                                h->perm_cur ^= 1;
+                                uint32_t *next = (uint32_t *)(h->ws + h->L.perm) + (uint64_t)h->perm_cur * (up(4 * h->prm.capacity) / 4);
+                                CK(launch_sort_finish(keys, A.n_prev, n_keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->perm_n, next, h->st));
+                                perm = next;
+                            }
                             h->launches += 4;
                         } else {
                             CK(launch_sort_by_cell(A.xyzq + r.base, A.n_prev, A.mg, keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->st));
@@ -777,6 +786,7 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                     if (single && h->step + (uint64_t)m - h->perm_step >= period) {
                         CK(cudaMemsetAsync(hist, 0, 4ull * n_keys, h->st));
                         A.keys_out = keys; A.hist_out = hist; A.n_keys = n_keys;
+                        A.keys_by_slot = h->sort_by_slot ? 1 : 0;
                         h->keys_ready = true;
                         h->keys_n = n;
                         h->keys_step = h->step + (uint64_t)m;

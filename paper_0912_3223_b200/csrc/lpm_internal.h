@@ -69,7 +69,7 @@ struct StepArgs {
     uint64_t dep_stride;
     float dep_scale[2 * LPM_MAX_NUCLIDES];       // fixed-point scales of the CTA-private deposit sums (powers of two): [2k] dry, [2k+1] wet
     double dep_inv_scale[2 * LPM_MAX_NUCLIDES];  // their inverses
-    int32_t zpair, pad4_;                    // the blended buffers hold z-pair texels (32 B: both z corners), B8
+    int32_t zpair, keys_by_slot;             // the blended buffers hold z-pair texels (32 B: both z corners), B8; fused sort keys indexed by slot, not by list position
     int32_t eq3, drift;                      // kz_mode 1: Kz from Eq.(3) per particle; drift: + dKz/dz dt (departure from the paper)
     int32_t any_dep, bern;                   // some sink deposits through the tables; dep_mode 1: Bernoulli deposition (R11)
     // physics

@@ -355,11 +355,12 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
         if (A.keys_out) {
             // pass 1 of the coming gather-locality sort, for free: the new position is in registers; the lanes of
             // a warp that share a key (most of them, in a sorted warp) count with one atomic.  The keys are stored in
-            // LIST order (coalesced here, and the scatter pass then walks spatial neighbours: lpm_sort.cu)
+            // LIST order (coalesced here, and the scatter pass then walks spatial neighbours: lpm_sort.cu), or by slot
+            // for large ensembles (sort row: the slot-order scatter leaves each cell's slots ascending)
             uint32_t key = 0xffffffffu;
             if (in_range) {
                 key = (valid && z >= 0.0f) ? corner_of<ZLEV>(A.mg, x, y, z).o : A.n_keys - 1u;
-                A.keys_out[pos] = key;
+                A.keys_out[A.keys_by_slot ? l : pos] = key;
             }
             const uint32_t peers = __match_any_sync(0xffffffffu, key);
             if (in_range && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(A.hist_out + key, (uint32_t)__popc(peers));
