@@ -526,9 +526,6 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     h->cg = *cg; h->met = *met; h->prm = *p; h->K = K;
     h->has_levels = met->z_levels_host != nullptr;
     h->zpair = zpair_enabled(met, p);
-    // many particles per met cell: young particles of one cell are neighbours in the store, and the slot-order scatter keeps
-    // each cell's slots ascending (coalesced state records in the step kernel); otherwise the cheaper list-order scatter
-    h->sort_by_slot = !p->compact && p->capacity >= kPairAutoRatio * (uint64_t)met->grid.nx * met->grid.ny * met->grid.nz;
     if (h->has_levels) for (int k = 0; k < met->grid.nz; ++k) h->zlev[k] = (float)met->z_levels_host[k];
     h->met.z_levels_host = nullptr;  // copied: the caller's array is not needed after lpm_create
     for (int k = 0; k < K; ++k) h->nuc[k] = nuc[k];
@@ -557,6 +554,12 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         h->wet_scale[k] = keep_dry * (double)h->p_wet[k];
     }
     h->dry_mode = !any_dry ? kDryNone : (eligible_everywhere ? kDryUniform : kDryLayer);
+    // Scatter order of the gather sort.  Many particles per met cell AND per-step deposits through the CTA-private tables:
+    // the slot-order scatter keeps each cell's slots ascending, i.e. sorted by age, and particles of one age sit together
+    // (same map cell, neighbouring state records), which the step kernel gains more from than the scatter costs.  Otherwise
+    // (Bernoulli deposition, no dry deposition, smaller ensembles) the cheaper list-order scatter.
+    h->sort_by_slot = !p->compact && p->dep_mode == 0 && h->dry_mode != kDryNone &&
+                      p->capacity >= kPairAutoRatio * (uint64_t)met->grid.nx * met->grid.ny * met->grid.nz;
     h->occ = step_max_blocks_per_sm(K, p->compact != 0, h->dry_mode, p->dep_mode == 1, met->kz_mode == 1, met->z_levels_host != nullptr || p->drift == 1, h->zpair);
     if (cudaMemsetAsync(ws, 0, L.total, h->st) != cudaSuccess) { delete h; return LPM_ERR_CUDA; }
     h->launches++;
