@@ -495,6 +495,40 @@ def test_ground_decay_total_activity_law(lpm):
         assert abs((led[0][1] + ground) / (7.0e5 * 2.0 ** (-N * dt / T_half)) - 1) < 2e-6, (spl, led[0][1], ground)
 
 
+def test_ground_decay_in_the_compact_store(lpm, orc):
+    """R13 with the compacting store (one step per launch, ABSORB): a short-lived nuclide with dry deposition on a c5-class
+    run shrunk around the source; ground map vs the oracle's within 1e-5 + face slack, totals to 1e-5."""
+    w = make("c5", scale=2e-3, n_steps=900).replace(nt=3)
+    small = Grid(60, 60, 25, -4.6e4, -6.0e3, 0.0, 200.0, 200.0, 50.0)
+    w = w.replace(capacity=60_000, mgrid=small, cgrid=small, nuclides=[Nuclide("S", 900.0, vd=0.02)])
+    sim = lpm.Simulation(w, ground_decay=True)
+    o = orc.OracleSim(w, face_delta=1.5)
+    o.enable_ground_decay()
+    sim.step(900)
+    o.step(900)
+    dg = sim.deposition(f64=True).cpu().numpy()
+    do, slack = o.deposition_ground(with_slack=True)
+    assert do.sum() > 0 and do.sum() < 0.7 * o.deposition().sum()
+    excess = np.maximum(np.abs(dg - do) - (1e-5 * do + 1.0001 * slack + 1e-30), 0.0)
+    assert excess.sum() <= 2e-3 * do.sum()
+    assert abs(dg.sum() / do.sum() - 1) < 1e-4            # (particles near the absorbing boundary may differ: fragile)
+
+
+def test_texel_pairs_single_level_and_tiny_grids(lpm):
+    """B8 degenerate grids: one met level (the pair's upper half repeats the level), 2 x 2 columns; bit-identical."""
+    for g in (Grid(12, 9, 1, -600.0, -450.0, 0.0, 100.0, 100.0, 400.0), Grid(2, 2, 3, -500.0, -500.0, 0.0, 500.0, 500.0, 100.0)):
+        met = lambda t, Z, Y, X: (1.0 + 0.001 * X + 0.0005 * t / 10.0, -0.5 + 0.002 * Y, 0.0, 1.0 + 0.01 * Z)
+        w = custom(met, grid=g, nt=3, dt_snap=600.0, n=3000, dt=10.0, Kh=5.0, H=300.0, n_steps=100, t_rel=(0.0, 500.0),
+                   nuclides=[Nuclide("X", 3600.0, vd=0.01)], activity=[1.0e6])
+        res = []
+        for tp in (-1, 1):
+            sim = lpm.Simulation(w, texel_pairs=tp)
+            assert sim.texel_pairs == (tp == 1)
+            sim.step(100)
+            res.append(sim.get_particles()["xyzq"].cpu().numpy().copy())
+        np.testing.assert_array_equal(res[0], res[1])
+
+
 # ------------------------------------------------------------------ S§8(f)3: time-integrated concentration
 def test_dose_grid(lpm, orc):
     """(f)3: resting decaying cloud (no wind, no diffusion): the dose grid equals the oracle's cell by cell to
