@@ -251,7 +251,8 @@ def run_ours(args):
 
     # ---------------- leg 1: inputs resident in HBM ----------------
     fields_dev = fields_host.to("cuda", non_blocking=True)
-    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode, texel_pairs=args.texel_pairs)
+    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode, texel_pairs=args.texel_pairs, gather_sort=args.gather_sort,
+                         steps_per_launch=args.steps_per_launch)
     pairs = sim.texel_pairs
     conc_dev = torch.empty((w.K, g.nz, g.ny, g.nx), dtype=torch.float32, device="cuda")
     dep_dev = torch.empty((w.K, g.ny, g.nx), dtype=torch.float32, device="cuda")
@@ -293,7 +294,8 @@ def run_ours(args):
 
     # ---------------- leg 2: end to end through the host-buffer C-ABI calls ----------------
     fields_dev.zero_()
-    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode, texel_pairs=args.texel_pairs)
+    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode, texel_pairs=args.texel_pairs, gather_sort=args.gather_sort,
+                         steps_per_launch=args.steps_per_launch)
     sim.upload_meteo(0, fields_host[0:1])
     uploaded = 0
     h2d = d2h = 0
@@ -360,7 +362,7 @@ def run_ours(args):
     peak = SMS * LANES_PER_SM * pk["sm_max_mhz"] * 1e6 / 1e12
     state_bytes = 16 + 4 * (w.K - 1) + (4 if w.compact else 0)
     k_rate = (k_units / world) / (step_ms * 1e-3) if step_ms > 0 else 0.0      # particle-steps/s inside the step kernel
-    fused = 1 if w.compact else LAUNCH_STEPS
+    fused = 1 if w.compact else (min(args.steps_per_launch, LAUNCH_STEPS) if args.steps_per_launch > 0 else LAUNCH_STEPS)
     hbm_per_ps = 2.0 * (state_bytes + (0 if w.compact else 4)) / fused          # state read + written once per launch (+ list entry)
     roofline = {
         "kernel": "step_compact_kernel" if w.compact else "step_slots_kernel", "bound": "alu",
@@ -421,7 +423,7 @@ def run_ours(args):
         "config": {"workload": f"{args.workload} (BASELINE.json configs[{ {'c1': 0, 'c2': 1, 'c2_eq3': 1, 'c3': 2, 'c3_hdep80': 2, 'c4': 3, 'c5': 4}[args.workload] }])",
                    "particles_per_gpu": w.capacity, "nuclides": w.K, "model_steps_per_bench_step": interval, "dt_s": w.dt,
                    "conc_grid": [g.nx, g.ny, g.nz], "met_grid": [w.mgrid.nx, w.mgrid.ny, w.mgrid.nz], "met_snapshots": w.nt,
-                   "scale": args.scale, "dep_mode": args.dep_mode, "met_texels": "z-pair, 32 B (DESIGN.md B8)" if pairs else "16 B", "l2": "particle store larger than L2, no flush" if w.capacity * state_bytes > 126e6 else "inputs fit L2 (small config)",
+                   "scale": args.scale, "dep_mode": args.dep_mode, "met_texels": "z-pair, 32 B (DESIGN.md B8)" if pairs else "16 B", "gather_sort": args.gather_sort, "steps_per_launch": args.steps_per_launch, "l2": "particle store larger than L2, no flush" if w.capacity * state_bytes > 126e6 else "inputs fit L2 (small config)",
                    "parallelism": f"pid-strided ensemble x{world}, grids all-reduced per output" if world > 1 else "single GPU"},
         "sim_hours_per_s": sim_hours / (ms * 1e-3),
         "e2e": {"value": units / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
@@ -467,6 +469,8 @@ def main():
     ap.add_argument("--scale", type=float, default=1.0, help="particle-count scale of the workload (1.0 = BASELINE size)")
     ap.add_argument("--dep-mode", type=int, default=0, choices=(0, 1), help="0 expected-mass deposition (default), 1 Bernoulli deposition (S 8(f)1)")
     ap.add_argument("--texel-pairs", type=int, default=0, choices=(-1, 0, 1), help="lpm_params.texel_pairs: 0 auto (default), 1 z-pair texels, -1 16-byte texels")
+    ap.add_argument("--gather-sort", type=int, default=0, help="lpm_params.gather_sort: 0 auto (every 32 steps), p > 0 every p steps, -1 never")
+    ap.add_argument("--steps-per-launch", type=int, default=0, help="lpm_params.steps_per_launch: 0 auto (16), m fuses up to min(m, 16) steps per launch")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-probes", action="store_true", help="skip the lpm_probe micro-benchmarks (measured peaks)")
     args = ap.parse_args()

@@ -98,7 +98,8 @@ typedef struct {
                                * min(m, 16) steps per launch with the particle state in registers */
     int32_t gather_sort;      /* gather-locality pass (slots listed in the order of the lower-corner met
                                * cell of their trilinear stencil): 0 = auto (from 65536 particles, every
-                               * 32 steps), p > 0 = always, every p model steps (1 = before every launch),
+                               * 32 to 64 steps: about the time the horizontal walk needs to cross a met
+                               * cell), p > 0 = always, every p model steps (1 = before every launch),
                                * -1 = never.  Results per particle do not depend on it.  With compact = 1
                                * the records themselves are sorted (the id travels with the particle), so
                                * the store is then in met-cell order, not in id order.             */

@@ -127,6 +127,7 @@ struct lpm_handle {
     bool zpair;   // B8: the blended buffers hold 32-byte z-pair texels
     int perm_cur; // which half of L.perm holds the current slot list
     bool sort_by_slot;  // fused sort keys indexed by slot (large ensembles), else by list position
+    int sort_period;    // model steps between two gather sorts when gather_sort = 0 (auto)
     float zlev[kMaxLevels];   // non-uniform level heights (fp32 parameters), copied from meteo.z_levels_host
     int K;
     cudaStream_t st;
@@ -537,6 +538,16 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     h->pair_snap = -1;
     // R5 / R8 constants: double formula, rounded once to fp32 where the kernels consume fp32
     h->sigma_h = (float)sqrt(2.0 * met->Kh * p->dt);
+    {
+        // Auto period of the gather sort: what un-sorts a warp is the horizontal random walk (advection moves neighbours
+        // together), so the list is worth keeping for about as many steps as the walk needs to cross a met cell,
+        // (dx / sigma_h)^2; measured optima 32 (c3: 31), 48-64 (c4: 62), 64 (c2: 250, c5: 100) -> 0.8 x that, in whole
+        // launches of kMaxFused steps, between 32 and 64.
+        const double dmin = met->grid.dx < met->grid.dy ? met->grid.dx : met->grid.dy;
+        const double cross = h->sigma_h > 0.0f ? 0.8 * (dmin / h->sigma_h) * (dmin / h->sigma_h) : 1e9;
+        int per = cross > 1e6 ? 64 : (int)(cross / kMaxFused + 0.5) * kMaxFused;
+        h->sort_period = per < kSortPeriod ? kSortPeriod : (per > 2 * kSortPeriod ? 2 * kSortPeriod : per);
+    }
     // uniform dry deposition folds into the scalar G only in the expected-mass form; Bernoulli trials (R11) are per particle
     const bool eligible_everywhere = p->h_dep >= met->H_mix;
     const bool uniform = eligible_everywhere && p->dep_mode != 1;
@@ -710,7 +721,7 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                 for (int k = 0; k < h->K; ++k) sp.q[k] = (float)(r.emit[k] / A.tab[0].G[k]);
             }
             if (sort_enabled(&h->prm)) {
-                const uint64_t period = h->prm.gather_sort > 0 ? (uint64_t)h->prm.gather_sort : (uint64_t)kSortPeriod;
+                const uint64_t period = h->prm.gather_sort > 0 ? (uint64_t)h->prm.gather_sort : (uint64_t)h->sort_period;
                 if (h->step - h->csort_step >= period) {
                     const int sspan = span_open(h, 2, 0.0);
                     CK(launch_sort_records(A.xyzq, A.q1, A.pid, A.ctrl + 2, h->prm.capacity, A.mg, (uint32_t *)(h->ws + h->L.keys),
@@ -756,7 +767,7 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                     // particles born since the last sort are walked in slot order behind it
                     uint32_t *perm = (uint32_t *)(h->ws + h->L.perm) + (uint64_t)h->perm_cur * (up(4 * h->prm.capacity) / 4);
                     const bool single = h->rel.size() == 1;
-                    const uint64_t period = h->prm.gather_sort > 0 ? (uint64_t)h->prm.gather_sort : (uint64_t)kSortPeriod;
+                    const uint64_t period = h->prm.gather_sort > 0 ? (uint64_t)h->prm.gather_sort : (uint64_t)h->sort_period;
                     const uint32_t n_keys = (uint32_t)A.snap_cells + 1u;
                     uint32_t *keys = (uint32_t *)(h->ws + h->L.keys), *hist = (uint32_t *)(h->ws + h->L.hist);
                     if (!single || !h->perm_valid || h->step - h->perm_step >= period || h->perm_n > A.n_prev) {

@@ -11,7 +11,7 @@ namespace lpm {
 constexpr int kMaxFused = 16;        // model steps fused into one launch (table lives in kernel params)
 constexpr int kBlendDepth = kMaxFused;  // time-blended met buffers kept: one per fused step
 constexpr int kMaxLevels = 64;       // non-uniform vertical met levels held in the kernel parameters
-constexpr int kSortPeriod = 32;      // model steps between two gather-locality sorts of a release
+constexpr int kSortPeriod = 32;      // least number of model steps between two gather-locality sorts of a release (auto: 32..64)
 constexpr int kStepThreads = 256;    // CTA size of the step kernel
 constexpr int kScanTile = 4 * kStepThreads;  // particles per look-back tile (compaction): 4 per thread
 
