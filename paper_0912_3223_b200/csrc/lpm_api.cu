@@ -547,6 +547,8 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         const double cross = h->sigma_h > 0.0f ? 0.8 * (dmin / h->sigma_h) * (dmin / h->sigma_h) : 1e9;
         int per = cross > 1e6 ? 64 : (int)(cross / kMaxFused + 0.5) * kMaxFused;
         h->sort_period = per < kSortPeriod ? kSortPeriod : (per > 2 * kSortPeriod ? 2 * kSortPeriod : per);
+        // compact store: the record order also feeds the binning kernel's atomics (c5: 50 % of its roofline at 32, 45 % at 64)
+        if (p->compact) h->sort_period = kSortPeriod;
     }
     // uniform dry deposition folds into the scalar G only in the expected-mass form; Bernoulli trials (R11) are per particle
     const bool eligible_everywhere = p->h_dep >= met->H_mix;
