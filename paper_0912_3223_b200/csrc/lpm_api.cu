@@ -978,6 +978,19 @@ int32_t lpm_set_particles(lpm_handle *h, const void *xyzq, const float *q1, cons
         h->rel.push_back(r);
         h->next_base = n;
     }
+    if (h->prm.ground_decay) {
+        // R13: the clock may jump (restart from a checkpoint): bring each map to the present first, then regard it as
+        // the ground activity at the new step index
+        for (int k = 0; k < h->K; ++k) {
+            const double age = h->lam_dt[k] * (double)(h->step - h->dep_ref[k]);
+            if (age > 0.0) {
+                const uint64_t c2 = (uint64_t)h->cg.nx * h->cg.ny;
+                CK(launch_dep_rebase((double *)(h->ws + h->L.dep) + (uint64_t)k * c2, c2, exp(-age), h->st));
+                h->launches++;
+            }
+            h->dep_ref[k] = step_index;
+        }
+    }
     h->step = step_index;
     h->binned = false;
     h->perm_valid = false;

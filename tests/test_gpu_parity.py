@@ -479,6 +479,29 @@ def test_ground_decay_of_the_deposition_map(lpm, orc, name, dep_mode):
     np.testing.assert_allclose(f32, dg, rtol=1e-6, atol=0)
 
 
+def test_ground_decay_survives_a_clock_jump(lpm):
+    """lpm_set_particles may move the step index (restart): the ground map is brought to the present first and then
+    regarded as the ground activity at the new step, so a read-out right after the jump returns the same map."""
+    T_half, dt = 600.0, 10.0
+    g = Grid(20, 20, 4, -1000.0, -1000.0, 0.0, 100.0, 100.0, 50.0)
+    w = custom(uniform_met(u=1.0, kz=1.0), grid=g, n=2000, nuclides=[Nuclide("X", T_half, vd=0.5)], dt=dt, Kh=10.0, H=200.0, activity=[1.0e6],
+               n_steps=200)
+    sim = lpm.Simulation(w, ground_decay=True)
+    sim.step(100)
+    before = sim.deposition(f64=True).cpu().numpy().copy()
+    p = sim.get_particles()
+    for new_step in (5, 4000):                                            # backwards and far forwards
+        sim.set_particles(p["xyzq"], step_index=new_step)
+        after = sim.deposition(f64=True).cpu().numpy()
+        assert np.isfinite(after).all()
+        np.testing.assert_allclose(after, before, rtol=1e-12, atol=0)
+    sim.step(60)                                                          # and it keeps decaying from there
+    later = sim.deposition(f64=True).cpu().numpy()
+    assert np.isfinite(later).all() and later.sum() > 0
+    untouched = before[0] > 0
+    assert (later[0][untouched] >= before[0][untouched] * 2.0 ** (-60 * dt / T_half) * (1 - 1e-9)).all()
+
+
 def test_ground_decay_total_activity_law(lpm):
     """P20 on the GPU: a puff that deposits dry and wet, everything on the map: airborne + ground = emitted 2^(-t/T)."""
     T_half, dt, N = 2400.0, 10.0, 60
