@@ -226,7 +226,9 @@ int32_t lpm_get_particles(lpm_handle *h, void *xyzq_dev, float *q1_dev, uint32_t
                           uint8_t *status_dev, uint64_t *n_host);
 /* Replace the particle state by n slots (all treated as already born; pid_dev NULL = 0..n-1;
  * status_dev NULL = all active) and set the step index.  Registered releases keep running only
- * in compact mode (append); in slot-addressed mode they are dropped. */
+ * in compact mode (append); in slot-addressed mode they are dropped.  The output grids are kept; with
+ * ground_decay = 1 the deposition map is first brought to the present and then regarded as the ground
+ * activity at the new step index. */
 int32_t lpm_set_particles(lpm_handle *h, const void *xyzq_dev, const float *q1_dev,
                           const uint32_t *pid_dev, const uint8_t *status_dev, uint64_t n,
                           uint64_t step_index);
