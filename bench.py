@@ -11,10 +11,13 @@ Default workload: BASELINE.json configs[3] ("Large ensemble", c4: 1e8 particles,
 1000x1000x30 concentration grid) — BASELINE.json's metric names no single config, so the largest
 single-GPU configuration is used; its particle store (2.0 GB) is far larger than L2 (126 MB), so
 no L2 flush is needed between timed steps.  With the defaults (W = 3, K = 9) the run IS the whole
-12 h config: 3 warm-up hours + 9 timed hours.
+12 h config: 3 warm-up hours + 9 timed hours.  Any other W, K walks the same config as a LOOP of its
+output intervals (bench step i = interval i mod 12; every wrap restarts the run from step 0 inside the
+timed region), so no bench step ever simulates an hour the config does not have.
 
-Printed JSON line (rank 0): metric particle-steps/s = born particles x model steps / device time
-(CUDA events on the launching stream, max over ranks), plus
+Printed JSON line (rank 0): metric particle-steps/s = particle-steps the step kernels executed (born AND
+active particles x model steps, counted on the device: a particle that has left the met box is inactive,
+P:L108, and counts for nothing) / device time (CUDA events on the launching stream, max over ranks), plus
   e2e          the same run through the host-buffer C-ABI calls: every step uploads the next
                hourly met snapshot from pinned host memory and reads the concentration grid back
   roofline     the step kernel (dominant): algorithmic lane-operations per launch / its average
@@ -43,13 +46,15 @@ if ROOT not in sys.path:
 METRIC = "particle_steps_per_s"
 UNIT = "particle-steps/s"
 # SURVEY.md §8(d) / DESIGN.md §6: algorithmic lane-operations per particle-step (FMA = 1), frozen
-# before any tuning: 250 with one met snapshot, 310 with time interpolation (the figure stays 310
-# although the kernel now samples a time-blended buffer: the budget is implementation-independent).
-LANE_OPS_STATIC, LANE_OPS_TIME = 250.0, 310.0
+# before any tuning: 250.  (S§8(d) adds 60 for on-the-fly time interpolation "when a0 is not materialised"; here a0
+# IS materialised - blend_kernel writes F(t_n) per met cell, < 1 lane-op per particle-step - so 250 applies throughout.)
+LANE_OPS = 250.0
 SMS, LANES_PER_SM = 148, 128          # 4 SMSP x 32 lanes: one warp instruction per clock per SMSP
 LAUNCH_STEPS = 16                     # model steps fused per step-kernel launch (csrc kMaxFused)
-# dram__bytes_read.sum + dram__bytes_write.sum of one captured step-kernel launch, bytes (profiles/r01c_c4_step_kernel_ncu.md)
-NCU_TRAFFIC = {"c4": 4.069e9 + 1.985e9}   # launch 171 of `bench.py --steps 1 --warmup 3`: 16 steps x 3.16e7 particles, z-pair texels (profiles/r01c_c4_step_kernel_ncu.md, r01d)
+# dram__bytes_read.sum + dram__bytes_write.sum of one captured step-kernel launch, bytes: NOT measured by this run, copied
+# from the named ncu capture
+NCU_TRAFFIC = {"c4": {"bytes": 4.069e9 + 1.985e9, "source": "profiles/r01c_c4_step_kernel_ncu.md (r01d): launch 171 of `bench.py --steps 1 "
+                      "--warmup 3`, 16 steps x 3.16e7 particles, z-pair texels; 3.0 B algorithmic per particle-step = 1.5 GB"}}
 ORACLE_STRIDE = {"c1": 1, "c2": 40, "c2_eq3": 40, "c3": 400, "c3_hdep80": 400, "c4": 4000, "c5": 1}
 ORACLE_SCALE_C5 = 1.0e-3              # c5 cannot be pid-strided (capacity couples particles): 1/1000 scale
 
@@ -130,32 +135,13 @@ def make_workload(name: str, scale: float, world: int, rank: int):
     return w
 
 
-def born_steps(w, s0: int, s1: int) -> float:
-    """Born particle x model step pairs for model steps s0 <= n < s1 (R9 closed form, local ids)."""
-    r = w.release
-    start = int(math.ceil(r.t_start / w.dt))
-    S = max(1, int(math.ceil((r.t_end - r.t_start) / w.dt)))
-    tot = 0
-    if r.n_particles > 0:
-        N = r.n_particles
-        for n in range(s0, s1):
-            if n < start:
-                continue
-            B = N if n - start + 1 >= S else min(N, -(-(n - start + 1) * N // S))
-            tot += 0 if B <= r.pid_offset else (B - r.pid_offset + r.pid_stride - 1) // r.pid_stride
-    else:
-        c = int(round(r.rate * w.dt))
-        for n in range(s0, s1):
-            if n >= start:
-                tot += min(w.capacity, c * min(n - start + 1, S))
-    return float(tot)
-
-
 # ------------------------------------------------------------------ the oracle legs
 def oracle_leg(name: str, scale: float, interval: int, warmup: int, steps: int, budget_s: float, threads: int = 0):
     """Run the fp64 oracle (as it stands) on a bounded sample of the workload: every
     ORACLE_STRIDE-th particle id (exact subset: particles are independent and Philox is keyed by
-    the id), the same intervals as the CUDA arm.  Returns particle-steps/s over the timed part."""
+    the id), the same looped intervals as the CUDA arm (a fresh run at every wrap of the config).
+    Returns active particle-steps/s over the timed part (active = born and not yet inactive, as the CUDA arm counts)."""
+    import numpy as np
     from oracle import oracle as orc
     from workloads import make
     all_threads = orc.num_threads()
@@ -171,29 +157,89 @@ def oracle_leg(name: str, scale: float, interval: int, warmup: int, steps: int, 
         n_local = len(range(0, w.release.n_particles, stride))
         w = w.replace(capacity=max(n_local, 1))
         sample = f"every {stride}th particle id of {name} ({n_local} particles), full grids and met"
+    n_int = max(1, w.n_steps // interval)
+
+    def active(o):
+        return float((o.particles()["status"] == 0).sum()) if o.n else 0.0
+
     o = orc.OracleSim(w)
-    o.step(warmup * interval)
+    for i in range(warmup):
+        if i and i % n_int == 0:
+            o = orc.OracleSim(w)
+        o.step(interval)
     t0 = time.perf_counter()
     done = 0
     live = 0.0
-    for i in range(steps):
-        n0 = o.n
+    for i in range(warmup, warmup + steps):
+        if i and i % n_int == 0:
+            o = orc.OracleSim(w)
+        a0 = active(o)
         o.step(interval)
         o.concentration()
-        live += 0.5 * (n0 + o.n) * interval      # c5: exits make the live count data-dependent
+        live += 0.5 * (a0 + active(o)) * interval      # trapezoid: births and exits make the active count vary inside an interval
         done += 1
         if budget_s and time.perf_counter() - t0 > budget_s:
             break
     dt = time.perf_counter() - t0
-    units = live if name == "c5" else born_steps(w, warmup * interval, (warmup + done) * interval)
-    sample += f"; {done} interval(s) of {interval} model steps after {warmup} warm-up interval(s)"
+    sample += f"; {done} interval(s) of {interval} model steps after {warmup} warm-up interval(s) of the looped config"
     used = orc.num_threads()
     if threads:
         orc.set_num_threads(all_threads)
-    return units / dt, dt, done, used, sample
+    return live / dt, dt, done, used, sample
 
 
 # ------------------------------------------------------------------ the CUDA arm
+class Looped:
+    """The workload as a loop of its own output intervals: bench step i is interval (i mod n_int) of the config, and
+    every wrap starts the run again from step 0 (lpm_destroy + lpm_create on the same workspace, inside the timed
+    region), so that ANY --steps / --warmup stays on BASELINE.json's configuration: the run never simulates an hour
+    the config does not have.  Per-handle timing totals are carried over the restarts."""
+
+    KEYS = ("step_ms", "step_launches", "bin_ms", "bin_launches", "particle_steps", "binned_particles", "sort_ms", "sort_launches",
+            "born_particle_steps")
+
+    def __init__(self, sim, n_int, on_restart=None):
+        self.sim, self.n_int, self.i, self.on_restart = sim, n_int, 0, on_restart
+        self.tot = {k: 0.0 for k in self.KEYS}
+        self.launches = 0
+        self.timing = False
+        self.l0 = sim.launch_count
+        self.restarts = 0
+
+    def begin_timing(self):
+        self.timing = True
+        self.tot = {k: 0.0 for k in self.KEYS}
+        self.launches = 0
+        self.l0 = self.sim.launch_count
+        self.sim.set_timing(True)
+
+    def _collect(self):
+        if self.timing:
+            t = self.sim.get_timing()
+            for k in self.KEYS:
+                self.tot[k] += t[k]
+        self.launches += self.sim.launch_count - self.l0
+
+    def next_interval(self):
+        """Called before every bench step: wraps to a fresh run when the config is over."""
+        if self.i and self.i % self.n_int == 0:
+            self._collect()
+            self.sim.restart()
+            self.restarts += 1
+            self.l0 = self.sim.launch_count
+            if self.timing:
+                self.sim.set_timing(True)
+            if self.on_restart:
+                self.on_restart()
+        self.i += 1
+
+    def end_timing(self):
+        self._collect()
+        self.l0 = self.sim.launch_count
+        self.timing = False
+        return dict(self.tot), self.launches
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -219,13 +265,13 @@ def run_ours(args):
     if rank == 0 and not args.no_probes:
         for key, kind, fp in (("ffma_lane_ops_per_s", "ffma", 0), ("imad_lop_lane_ops_per_s", "imad_lop", 0),
                               ("l1_gather_sectors_per_s", "gather", 64 << 10), ("l2_gather_sectors_per_s", "gather", 64 << 20),
-                              ("red_f64_l2_resident_per_s", "red_f64", 16 << 20), ("red_f64_600MB_per_s", "red_f64", 600 << 20),
                               ("red_same_address_per_s", "red_same", 0), ("shared_atomic_per_s", "atoms", 0)):
-            probes[key] = lpm.probe(kind, fp, scratch_bytes=1 << 30 if fp > (1 << 28) else 1 << 28)
+            probes[key] = lpm.probe(kind, fp, scratch_bytes=1 << 28)
         torch.cuda.empty_cache()
 
     w = make_workload(args.workload, args.scale, world, rank)
     interval = w.bin_every
+    n_int = max(1, w.n_steps // interval)        # output intervals of the config (c4: 12 hourly intervals)
     W, K = args.warmup, args.steps
     g = w.cgrid
     pk = peaks()
@@ -249,64 +295,69 @@ def run_ours(args):
         t = step_index * w.dt
         return min(w.nt - 1, int(math.floor((t - w.t0) / w.dt_snap)) + 1) if w.nt > 1 else 0
 
+    mk = dict(dep_mode=args.dep_mode, texel_pairs=args.texel_pairs, gather_sort=args.gather_sort, steps_per_launch=args.steps_per_launch)
+
     # ---------------- leg 1: inputs resident in HBM ----------------
     fields_dev = fields_host.to("cuda", non_blocking=True)
-    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode, texel_pairs=args.texel_pairs, gather_sort=args.gather_sort,
-                         steps_per_launch=args.steps_per_launch)
+    sim = lpm.Simulation(w, fields_dev=fields_dev, **mk)
     pairs = sim.texel_pairs
+    loop = Looped(sim, n_int)
     conc_dev = torch.empty((w.K, g.nz, g.ny, g.nx), dtype=torch.float32, device="cuda")
     dep_dev = torch.empty((w.K, g.ny, g.nx), dtype=torch.float32, device="cuda")
-    for _ in range(W):
+
+    def resident_step():
+        loop.next_interval()
         sim.step(interval)
         sim.concentration(conc_dev)
         allreduce(conc_dev)
+
+    for _ in range(W):
+        resident_step()
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    launches0 = sim.launch_count
-    sim.set_timing(True)
+    loop.begin_timing()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     ev0.record()
-    binned_compact = 0.0
     for _ in range(K):
-        sim.step(interval)
-        sim.concentration(conc_dev)
-        allreduce(conc_dev)
-        if w.compact:
-            binned_compact += sim.num_active      # device-side live count (syncs at the interval boundary)
+        resident_step()
     sim.deposition(dep_dev)
     allreduce(dep_dev)
     ev1.record()
     barrier()
     ms = ev0.elapsed_time(ev1)
-    tim = sim.get_timing()
-    launches = sim.launch_count - launches0
+    tim, launches = loop.end_timing()
     clocks = sampler.stop() if rank == 0 else None
-    units_local = born_steps(w, W * interval, (W + K) * interval)
-    if w.compact:
-        units_local = tim["particle_steps"]
-        tim["binned_particles"] = binned_compact
     total_mass = float(conc_dev.sum().item())
+    touched = sim.touched_cells                       # cells that hold a particle in the last binning (untimed)
+    restarts = loop.restarts
+    del loop
     del sim
     torch.cuda.empty_cache()
 
     # ---------------- leg 2: end to end through the host-buffer C-ABI calls ----------------
     fields_dev.zero_()
-    sim = lpm.Simulation(w, fields_dev=fields_dev, dep_mode=args.dep_mode, texel_pairs=args.texel_pairs, gather_sort=args.gather_sort,
-                         steps_per_launch=args.steps_per_launch)
-    sim.upload_meteo(0, fields_host[0:1])
-    uploaded = 0
-    h2d = d2h = 0
+    sim = lpm.Simulation(w, fields_dev=fields_dev, **mk)
+    state = {"uploaded": 0, "h2d": 0, "d2h": 0}
+
+    def first_snapshot():
+        sim.upload_meteo(0, fields_host[0:1])
+        state["uploaded"] = 0
+        state["h2d"] += snap_bytes
+
+    first_snapshot()
+    loop = Looped(sim, n_int, on_restart=first_snapshot)
 
     def e2e_step():
-        nonlocal uploaded, h2d, d2h
+        loop.next_interval()
         need = snapshot_for(sim.step_index)
-        while uploaded < need:
-            uploaded += 1
-            sim.upload_meteo(uploaded, fields_host[uploaded:uploaded + 1])
-            h2d += snap_bytes
+        while state["uploaded"] < need:
+            state["uploaded"] += 1
+            u = state["uploaded"]
+            sim.upload_meteo(u, fields_host[u:u + 1])
+            state["h2d"] += snap_bytes
         sim.step(interval)
         if world > 1:
             sim.concentration(conc_dev)
@@ -314,12 +365,13 @@ def run_ours(args):
             conc_host.copy_(conc_dev, non_blocking=False)
         else:
             sim.concentration_host(conc_host)
-        d2h += conc_host.numel() * 4
+        state["d2h"] += conc_host.numel() * 4
 
     for _ in range(W):
         e2e_step()
     barrier()
-    h2d = d2h = 0
+    state["h2d"] = state["d2h"] = 0
+    loop.begin_timing()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record()
@@ -331,44 +383,62 @@ def run_ours(args):
         dep_host.copy_(dep_dev)
     else:
         sim.deposition_host(dep_host)
-    d2h += dep_host.numel() * 4
+    state["d2h"] += dep_host.numel() * 4
     e1.record()
     barrier()
     ms_e2e = e0.elapsed_time(e1)
+    tim_e2e, _ = loop.end_timing()
+    h2d, d2h = state["h2d"], state["d2h"]
     e2e_mass = float(conc_host.sum().item())
+    del loop
     del sim
+    torch.cuda.empty_cache()
+
+    # the binning atomics' peak: random-address red.global.add.f64 over exactly the footprint the last binning touched
+    if rank == 0 and not args.no_probes:
+        fp = max(1 << 20, int(touched) * (4 + 8 * w.K))
+        probes["red_f64_touched_footprint_per_s"] = lpm.probe("red_f64", fp, scratch_bytes=max(1 << 28, 1 << (fp - 1).bit_length()))
+        probes["red_f64_touched_footprint_bytes"] = fp
+        torch.cuda.empty_cache()
 
     # ---------------- reduce over ranks ----------------
     if world > 1:
         t = torch.tensor([ms, ms_e2e, tim["step_ms"], tim["bin_ms"]], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms, ms_e2e, step_ms, bin_ms = t.tolist()
-        u = torch.tensor([units_local, tim["particle_steps"], tim["binned_particles"], float(launches)], device="cuda", dtype=torch.float64)
+        u = torch.tensor([tim["particle_steps"], tim["binned_particles"], float(launches), tim["born_particle_steps"], tim_e2e["particle_steps"]],
+                         device="cuda", dtype=torch.float64)
         dist.all_reduce(u)
-        units, k_units, b_units, launches = u.tolist()
+        units, b_units, launches, born_units, units_e2e = u.tolist()
         launches = int(launches)
     else:
-        units, k_units, b_units, step_ms, bin_ms = units_local, tim["particle_steps"], tim["binned_particles"], tim["step_ms"], tim["bin_ms"]
+        units, b_units, step_ms, bin_ms = tim["particle_steps"], tim["binned_particles"], tim["step_ms"], tim["bin_ms"]
+        born_units, units_e2e = tim["born_particle_steps"], tim_e2e["particle_steps"]
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
+    # the grid must hold something at the end of both legs: an empty grid means the run left the configuration
+    if not (total_mass > 0.0 and e2e_mass > 0.0):
+        raise SystemExit(f"bench.py: the concentration grid is empty at the end of the timed region "
+                         f"(resident {total_mass}, e2e {e2e_mass}): not a valid measurement")
+
     # ---------------- roofline of the dominant kernel (step) ----------------
-    lane_ops = LANE_OPS_TIME if w.nt > 1 else LANE_OPS_STATIC
+    lane_ops = LANE_OPS              # a0 is materialised (time-blended buffers), so every config is on the 250-op budget
     n_launch = max(tim["step_launches"], 1)
     avg_ms = step_ms / n_launch
-    achieved = lane_ops * (k_units / world) / n_launch / (avg_ms * 1e-3) / 1e12 if avg_ms > 0 else 0.0
+    achieved = lane_ops * (units / world) / n_launch / (avg_ms * 1e-3) / 1e12 if avg_ms > 0 else 0.0
     peak = SMS * LANES_PER_SM * pk["sm_max_mhz"] * 1e6 / 1e12
     state_bytes = 16 + 4 * (w.K - 1) + (4 if w.compact else 0)
-    k_rate = (k_units / world) / (step_ms * 1e-3) if step_ms > 0 else 0.0      # particle-steps/s inside the step kernel
+    k_rate = (units / world) / (step_ms * 1e-3) if step_ms > 0 else 0.0      # particle-steps/s inside the step kernel
     fused = 1 if w.compact else (min(args.steps_per_launch, LAUNCH_STEPS) if args.steps_per_launch > 0 else LAUNCH_STEPS)
     hbm_per_ps = 2.0 * (state_bytes + (0 if w.compact else 4)) / fused          # state read + written once per launch (+ list entry)
     roofline = {
         "kernel": "step_compact_kernel" if w.compact else "step_slots_kernel", "bound": "alu",
         "achieved": achieved, "peak": peak, "unit": "Tlane-op/s", "frac": achieved / peak if peak else None,
-        # dram__bytes_read + dram__bytes_write of ONE captured launch (profiles/r01c_*): not per average launch
-        "traffic": NCU_TRAFFIC.get(args.workload),
+        # dram__bytes_read + dram__bytes_write of ONE captured launch (not measured in this run: from the named profile)
+        "traffic": NCU_TRAFFIC.get(args.workload, {}).get("bytes"), "traffic_source": NCU_TRAFFIC.get(args.workload, {}).get("source"),
         "lane_ops_per_particle_step": lane_ops, "avg_launch_ms": avg_ms, "launches": tim["step_launches"],
         "kernel_particle_steps_per_s": k_rate,
         "share_of_step": step_ms / ms if ms else None,
@@ -377,56 +447,67 @@ def run_ours(args):
         "frac_of_measured_ffma": achieved * 1e12 / probes["ffma_lane_ops_per_s"] if probes.get("ffma_lane_ops_per_s") else None,
         "hbm_side": {"bytes_per_particle_step": hbm_per_ps, "fused_steps_per_launch": fused, "hbm_peak_gbs": pk["hbm_gbs"],
                      "peak_source": pk["source"], "frac": k_rate * hbm_per_ps / (pk["hbm_gbs"] * 1e9)},
-        # what ncu shows to be the binding unit (profiles/r01c_*): the L1 data pipe, one 32-byte sector per gathered
-        # texel; achieved = gathers issued per second against the probe's L1-resident gather rate
-        # (z-pair texels, B8: 4 gathers of one 32-byte sector each instead of 8 of 16 bytes)
         "l1_gather_side": {"gathers_per_particle_step": 4 if pairs else 8, "achieved_per_s": (4.0 if pairs else 8.0) * k_rate,
                            "peak_per_s": probes.get("l1_gather_sectors_per_s"),
                            "frac": (4.0 if pairs else 8.0) * k_rate / probes["l1_gather_sectors_per_s"] if probes.get("l1_gather_sectors_per_s") else None,
                            "note": "upper bound of the sector count: lanes that share a texel share a sector"},
     }
+    # ---------------- binning (a8): particle bytes at HBM peak, or one atomic per touched cell and field ----------------
     bpp = 12 + 4 * w.K
-    n_bin = b_units / world
+    n_bin = b_units / world                                   # particles the kernel binned (active, inside the grid)
+    n_bl = max(tim["bin_launches"], 1)
     bin_bytes = bpp * n_bin
     grid_bytes = (4 + 8 * w.K) * g.nx * g.ny * g.nz
-    red_rate = probes.get("red_f64_l2_resident_per_s")
-    t_hbm = (bin_bytes + tim["bin_launches"] * grid_bytes) / (pk["hbm_gbs"] * 1e9)      # particles read + grids zeroed
-    t_atom = (1 + w.K) * n_bin / red_rate if red_rate else None                          # one count + K sums per particle
+    red_rate = probes.get("red_f64_touched_footprint_per_s")
+    t_hbm = (bin_bytes + n_bl * grid_bytes) / (pk["hbm_gbs"] * 1e9)                    # particles read + grids zeroed
+    t_atom = n_bl * touched * (1 + w.K) / red_rate if red_rate else None              # every touched cell: one count + K sums
     t_roof = max(t_hbm, t_atom) if t_atom else t_hbm
-    binning = {"kernel": "bin_kernel", "gbs": bin_bytes / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else None,
-               "avg_ms": bin_ms / max(tim["bin_launches"], 1), "launches": tim["bin_launches"],
-               "bytes_per_particle": bpp, "particles": n_bin,
+    binning = {"kernel": "bin_tile_kernel", "gbs": bin_bytes / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else None,
+               "avg_ms": bin_ms / n_bl, "launches": tim["bin_launches"],
+               "bytes_per_particle": bpp, "particles": n_bin, "touched_cells_last_binning": touched,
                "roofline": {"bound": "atomic" if t_atom and t_atom >= t_hbm else "hbm", "roof_ms": t_roof * 1e3, "measured_ms": bin_ms,
                             "frac": t_roof * 1e3 / bin_ms if bin_ms > 0 else None,
                             "hbm_ms": t_hbm * 1e3, "atomic_ms": t_atom * 1e3 if t_atom else None,
-                            "atomics_per_particle": 1 + w.K,
-                            "atomic_peak_per_s": red_rate, "atomic_peak_source": "lpm_probe red.global.add.f64, random addresses, "
-                            "L2-resident 16 MB footprint (the plume's cells are L2-resident; over the full grid footprint the "
-                            "random-address rate is red_f64_600MB_per_s)"},
-               "note": "span = memsets of the count and sum grids + bin kernel"}
+                            "atomics_per_touched_cell": 1 + w.K,
+                            "atomic_peak_per_s": red_rate, "atomic_peak_source": "lpm_probe red.global.add.f64, random addresses over "
+                            "touched cells x (4 + 8 K) bytes (the footprint of the last binning, measured in this run)"},
+               "note": "span = one memset of the count and sum grids + the bin kernel; the roofline counts the particle records at "
+                       "12 + 4 K bytes (the kernel reads them through the step kernel's sorted slot list, 4 more bytes each), the "
+                       "zeroing of the grids, and one RED per touched cell and field (what a privatised design must at least issue)"}
 
     # ---------------- cpu baseline (oracle, bounded sample) ----------------
     cpu = None
     if not args.no_cpu_baseline:
-        v, dt, done, cores, sample = oracle_leg(args.workload, args.scale, interval, 0 if args.workload != "c5" else 0, W + K, 20.0)
+        ow = min(W + K, n_int)
+        v, dt, done, cores, sample = oracle_leg(args.workload, args.scale, interval, 0, ow, 20.0)   # from step 0, at most ~20 s
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt}
         # the paper's own baseline was ONE thread: the same sample on one thread, at most ~8 s
-        v1, dt1, done1, _, _ = oracle_leg(args.workload, args.scale, interval, 0, W + K, 8.0, threads=1)
+        v1, dt1, done1, _, _ = oracle_leg(args.workload, args.scale, interval, 0, ow, 8.0, threads=1)
         cpu["value_1_thread"] = v1
         cpu["intervals_1_thread"] = done1
 
     sim_hours = K * interval * w.dt / 3600.0
+    idx = {'c1': 0, 'c2': 1, 'c2_eq3': 1, 'c3': 2, 'c3_hdep80': 2, 'c4': 3, 'c5': 4}[args.workload]
+    first = W % n_int
     line = {
         "metric": METRIC, "value": units / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{args.workload} (BASELINE.json configs[{ {'c1': 0, 'c2': 1, 'c2_eq3': 1, 'c3': 2, 'c3_hdep80': 2, 'c4': 3, 'c5': 4}[args.workload] }])",
+        "config": {"workload": f"{args.workload} (BASELINE.json configs[{idx}])",
                    "particles_per_gpu": w.capacity, "nuclides": w.K, "model_steps_per_bench_step": interval, "dt_s": w.dt,
                    "conc_grid": [g.nx, g.ny, g.nz], "met_grid": [w.mgrid.nx, w.mgrid.ny, w.mgrid.nz], "met_snapshots": w.nt,
+                   "intervals_in_config": n_int, "timed_intervals": f"{K} consecutive output intervals of the looped config, starting at "
+                   f"interval {first} of {n_int}; {restarts} restart(s) from step 0 inside the timed region",
+                   "boundary": w.boundary_mode,
                    "scale": args.scale, "dep_mode": args.dep_mode, "met_texels": "z-pair, 32 B (DESIGN.md B8)" if pairs else "16 B", "gather_sort": args.gather_sort, "steps_per_launch": args.steps_per_launch, "l2": "particle store larger than L2, no flush" if w.capacity * state_bytes > 126e6 else "inputs fit L2 (small config)",
                    "parallelism": f"pid-strided ensemble x{world}, grids all-reduced per output" if world > 1 else "single GPU"},
+        # unit of `value`: particle-steps the step kernels EXECUTED (born and still active: inside the met box, carrying
+        # activity), counted on the device; particles that have left the domain are inactive and count for nothing
+        "in_domain_fraction": 1.0,
+        "active_over_born": units / born_units if born_units else None,
+        "born_particle_steps": born_units if born_units else None,
         "sim_hours_per_s": sim_hours / (ms * 1e-3),
-        "e2e": {"value": units / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
+        "e2e": {"value": units_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                 "ms_per_step": ms_e2e / K, "sim_hours_per_s": sim_hours / (ms_e2e * 1e-3)},
         "gpu_launches": launches,
         "roofline": roofline, "binning": binning, "measured_peaks": probes, "cpu_baseline": cpu, "clocks": clocks,

@@ -145,7 +145,8 @@ int32_t lpm_version(void);
 /* Static text for a status code. */
 const char *lpm_status_string(int32_t status);
 
-/* Bytes of device workspace lpm_create needs (particle SoA store, grids, ledger, scan state,
+/* Bytes of device workspace lpm_create needs for params->capacity particle slots (the capacity travels inside
+ * lpm_params, as for lpm_create, not as an argument of its own) (particle SoA store, grids, ledger, scan state,
  * read-out staging, the z-fastest time-blended met buffers (16 bytes per met cell and fused step) and,
  * when meteo->nt > 1, the interleaved snapshot-pair buffer of the current met interval: 32 bytes per
  * met cell).  Only the grid and nt of `meteo` are read. */
@@ -201,7 +202,8 @@ int32_t lpm_concentration(lpm_handle *h, float *out_dev);
 int32_t lpm_dose(lpm_handle *h, float *out_dev);
 /* Particle counts per cell, uint32 [nz][ny][nx], same snapshot rule. */
 int32_t lpm_counts(lpm_handle *h, uint32_t *out_dev);
-/* Cumulative deposited activity in Bq m^-2, float [K][ny][nx] (not decayed on the ground). */
+/* Deposited activity in Bq m^-2, float [K][ny][nx]: cumulative and never decayed with params.ground_decay = 0 (default);
+ * with ground_decay = 1 what lies on the ground keeps decaying and the map is returned as it is at the current time. */
 int32_t lpm_deposition(lpm_handle *h, float *out_dev);
 /* Same map at full precision, double [K][ny][nx] (the accumulator itself, scaled by 1/area). */
 int32_t lpm_deposition_f64(lpm_handle *h, double *out_dev);
@@ -217,7 +219,8 @@ int32_t lpm_step_index(lpm_handle *h, uint64_t *step_host);
  * G_k(t) the host-side fp64 decay (and uniform dry-deposition) factor at the current step (R8). */
 int32_t lpm_mass_scale(lpm_handle *h, double *scale_host /* [K] */);
 /* Copy out the particle state: xyzq_dev float4 (x, y, z, q0) per slot, q1_dev (K = 2, may be
- * NULL), pid_dev uint32 (may be NULL), status_dev uint8 0 = active, 1 = exited, 2 = deposited all it carried
+ * NULL), pid_dev uint32 global particle ids (may be NULL; slot-addressed store: pid_offset + l * pid_stride for slot l
+ * of a release block), status_dev uint8 0 = active, 1 = exited, 2 = deposited all it carried
  * (dep_mode 1) (may be NULL).
  * Buffers must hold capacity entries; *n_host receives the slot count.  Exited particles report
  * their exit position.  With several releases each release owns a block of slots that starts at a multiple of
@@ -226,7 +229,10 @@ int32_t lpm_get_particles(lpm_handle *h, void *xyzq_dev, float *q1_dev, uint32_t
                           uint8_t *status_dev, uint64_t *n_host);
 /* Replace the particle state by n slots (all treated as already born; pid_dev NULL = 0..n-1;
  * status_dev NULL = all active) and set the step index.  Registered releases keep running only
- * in compact mode (append); in slot-addressed mode they are dropped.  The output grids are kept; with
+ * in compact mode (append); in slot-addressed mode they are dropped.  With compact = 0 the id of a particle is
+ * implied by its slot, so pid_dev (if given) must be affine, pid[l] = pid[0] + l * (pid[1] - pid[0]) with a positive
+ * stride - exactly what lpm_get_particles reports for one release, strided or not - else INVALID_ARG: a run
+ * restarted from lpm_get_particles' output continues bit for bit.  The output grids are kept; with
  * ground_decay = 1 the deposition map is first brought to the present and then regarded as the ground
  * activity at the new step index. */
 int32_t lpm_set_particles(lpm_handle *h, const void *xyzq_dev, const float *q1_dev,
@@ -265,11 +271,19 @@ int32_t lpm_deposition_host(lpm_handle *h, float *out_host);
  * events on the handle's stream (two cudaEventRecord per launch); also clears the totals. */
 int32_t lpm_set_timing(lpm_handle *h, int32_t enable);
 /* Synchronises, then returns out_host[0] = total ms in step kernels, [1] = their launch count,
- * [2] = total ms in binning kernels (memsets of the grids included), [3] = their launch count,
- * [4] = particle-steps executed by the timed step launches (born particles x steps, host count),
- * [5] = particles read by the timed binning launches, [6] = total ms in gather-locality sort
- * passes, [7] = their count; accumulated since lpm_set_timing. */
-int32_t lpm_get_timing(lpm_handle *h, double *out_host /* [8] */);
+ * [2] = total ms in binning kernels (the memset of the grids included), [3] = their launch count,
+ * [4] = particle-steps EXECUTED (born and still active particles x steps; counted by the step kernels themselves, so
+ *       particles that have left the domain or deposited everything do not count),
+ * [5] = particles BINNED (active and inside the concentration grid; counted by the binning kernel),
+ * [6] = total ms in gather-locality sort passes, [7] = their count,
+ * [8] = born particles x steps of the timed step launches (host count of the release schedule R9: the same as [4]
+ *       while no particle has become inactive; slot-addressed store only, 0 with compact = 1),
+ * [9..11] reserved (0); accumulated since lpm_set_timing. */
+int32_t lpm_get_timing(lpm_handle *h, double *out_host /* [12] */);
+/* Number of concentration cells that hold at least one particle in the current binning (the footprint the binning
+ * atomics spread over: bench.py measures its atomic peak over exactly that many cells).  Synchronises.
+ * Errors: STATE (nothing binned yet). */
+int32_t lpm_touched_cells(lpm_handle *h, uint64_t *n_host);
 
 /* ---- micro-benchmarks: measured denominators of the rooflines ------------------ */
 

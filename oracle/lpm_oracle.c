@@ -511,7 +511,7 @@ static void step_particle(orc_sim *s, uint64_t i, uint64_t n, double t_n, int ra
         const orc_grid *mg = &c->mgrid;
         double zlo = c->z_levels ? c->z_levels[0] : mg->z0 + 0.5 * mg->dz;
         double zhi = c->z_levels ? c->z_levels[mg->nz - 1] : mg->z0 + ((double)mg->nz - 0.5) * mg->dz;
-        if (fabs(s->z[i] - zlo) < c->frag_delta || fabs(s->z[i] - zhi) < c->frag_delta) s->fragile[i] = 1; /* slope switches on / off there */
+        if (fabs(s->z[i] - zlo) < c->frag_delta || fabs(s->z[i] - zhi) < c->frag_delta) { if (s->fragile[i] == 0) s->fragile[i] = 1; } /* slope switches on / off there */
     }
     if (Kz < c->kz_min) Kz = c->kz_min;
 
@@ -532,7 +532,7 @@ static void step_particle(orc_sim *s, uint64_t i, uint64_t n, double t_n, int ra
     double bx0 = g->x0, bx1 = g->x0 + g->nx * g->dx, by0 = g->y0, by1 = g->y0 + g->ny * g->dy;
     if (c->boundary_mode == 1) {
         double dmin = fmin(fmin(fabs(xn - bx0), fabs(xn - bx1)), fmin(fabs(yn - by0), fabs(yn - by1)));
-        if (dmin < c->frag_delta) s->fragile[i] = 1;
+        if (dmin < c->frag_delta) { if (s->fragile[i] == 0) s->fragile[i] = 1; }
         if (!(xn >= bx0 && xn < bx1 && yn >= by0 && yn < by1)) {
             s->status[i] = 1;
             return; /* mass is moved to the exited ledger by the serial pass */
@@ -541,7 +541,7 @@ static void step_particle(orc_sim *s, uint64_t i, uint64_t n, double t_n, int ra
 
     /* R8: deposition, then decay, at the new position */
     int eligible = (c->h_dep >= c->H_mix) || (zn < c->h_dep);
-    if (c->h_dep < c->H_mix && fabs(zn - c->h_dep) < c->frag_delta) s->fragile[i] = 1;
+    if (c->h_dep < c->H_mix && fabs(zn - c->h_dep) < c->frag_delta) { if (s->fragile[i] == 0) s->fragile[i] = 1; }
     int wet = 0;
     if (raining) {
         wet = (xn >= c->rx0 && xn < c->rx1 && yn >= c->ry0 && yn < c->ry1);
@@ -550,7 +550,7 @@ static void step_particle(orc_sim *s, uint64_t i, uint64_t n, double t_n, int ra
         double ddy = fmin(fabs(yn - c->ry0), fabs(yn - c->ry1));
         int near_x = ddx < c->frag_delta && yn >= c->ry0 - c->frag_delta && yn <= c->ry1 + c->frag_delta;
         int near_y = ddy < c->frag_delta && xn >= c->rx0 - c->frag_delta && xn <= c->rx1 + c->frag_delta;
-        if (near_x || near_y) s->fragile[i] = 1;
+        if (near_x || near_y) { if (s->fragile[i] == 0) s->fragile[i] = 1; }
     }
     int any = 0;
     if (c->dep_mode == 1) {

@@ -28,7 +28,7 @@ SYMBOLS = (
     "lpm_set_particles", "lpm_ledger", "lpm_injected", "lpm_last_error", "lpm_launch_count", "lpm_test_philox",
     "lpm_test_normals", "lpm_test_sample", "lpm_upload_meteo", "lpm_concentration_host", "lpm_deposition_host",
     "lpm_set_timing", "lpm_get_timing", "lpm_probe", "lpm_test_box_muller", "lpm_dose", "lpm_test_curand_philox",
-    "lpm_texel_pairs",
+    "lpm_texel_pairs", "lpm_touched_cells",
 )
 
 
@@ -109,6 +109,7 @@ def load():
     L.lpm_set_timing.argtypes = [vp, i32]
     L.lpm_get_timing.argtypes = [vp, C.POINTER(dbl)]
     L.lpm_texel_pairs.argtypes = [vp, C.POINTER(i32)]
+    L.lpm_touched_cells.argtypes = [vp, C.POINTER(u64)]
     L.lpm_probe.argtypes = [i32, u64, vp, u64, i32, C.POINTER(dbl), vp]
     L.lpm_test_box_muller.argtypes = [vp, u64, vp, vp]
     L.lpm_test_curand_philox.argtypes = [u64, u64, u64, u64, vp, vp]
@@ -197,31 +198,46 @@ class Simulation:
         nbytes = workspace_bytes(w.cgrid, w.capacity, w.K, w.compact, w.mgrid, w.nt, gather_sort, dose, kz_mode, dep_mode, drift, texel_pairs,
                                  getattr(w, "z_levels", None))
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
-        cg = _grid(w.cgrid)
-        met = lpm_meteo(grid=_grid(w.mgrid), nt=w.nt, t0=w.t0, dt_snap=w.dt_snap, fields_dev=fields_dev.data_ptr(),
-                        Kh=w.Kh, H_mix=w.H_mix, kz_min=w.kz_min, kz_mode=kz_mode,
-                        surface_dev=self.surface_dev.data_ptr() if self.surface_dev is not None else None)
         self._levels = None
         if getattr(w, "z_levels", None) is not None:
             self._levels = np.ascontiguousarray(w.z_levels, dtype=np.float64)
+        self._create_args = dict(kz_mode=kz_mode, bin_every=w.bin_every if bin_every is None else bin_every, steps_per_launch=steps_per_launch,
+                                 gather_sort=gather_sort, dose=dose, dep_mode=dep_mode, drift=drift, texel_pairs=texel_pairs,
+                                 ground_decay=ground_decay, auto_release=auto_release)
+        self._h = None
+        self._create()
+
+    def _create(self):
+        """lpm_create on this object's workspace (which the library zeroes), then the rain box and the release."""
+        w, a, L, torch = self.w, self._create_args, self._L, self.torch
+        cg = _grid(w.cgrid)
+        met = lpm_meteo(grid=_grid(w.mgrid), nt=w.nt, t0=w.t0, dt_snap=w.dt_snap, fields_dev=self.fields_dev.data_ptr(),
+                        Kh=w.Kh, H_mix=w.H_mix, kz_min=w.kz_min, kz_mode=a["kz_mode"],
+                        surface_dev=self.surface_dev.data_ptr() if self.surface_dev is not None else None)
+        if self._levels is not None:
             met.z_levels_host = self._levels.ctypes.data
         nucs = (lpm_nuclide * w.K)(*[lpm_nuclide(n.half_life_s, n.vd, n.lambda_wet) for n in w.nuclides])
         prm = lpm_params(dt=w.dt, seed=w.seed, capacity=w.capacity,
                          boundary_mode=1 if w.boundary_mode == "absorb" else 0, compact=1 if w.compact else 0,
-                         h_dep=w.h_dep, bin_every=w.bin_every if bin_every is None else bin_every,
-                         steps_per_launch=steps_per_launch, gather_sort=gather_sort, dose=1 if dose else 0, dep_mode=dep_mode, drift=1 if drift else 0,
-                         texel_pairs=texel_pairs, ground_decay=1 if ground_decay else 0)
+                         h_dep=w.h_dep, bin_every=a["bin_every"], steps_per_launch=a["steps_per_launch"], gather_sort=a["gather_sort"],
+                         dose=1 if a["dose"] else 0, dep_mode=a["dep_mode"], drift=1 if a["drift"] else 0,
+                         texel_pairs=a["texel_pairs"], ground_decay=1 if a["ground_decay"] else 0)
         h = C.c_void_p()
         with torch.cuda.stream(self.stream):
-            rc = L.lpm_create(C.byref(cg), C.byref(met), nucs, w.K, C.byref(prm), self.workspace.data_ptr(), nbytes,
+            rc = L.lpm_create(C.byref(cg), C.byref(met), nucs, w.K, C.byref(prm), self.workspace.data_ptr(), self.workspace.numel(),
                               self.stream.cuda_stream, C.byref(h))
         if rc:
             raise LpmError(rc, "lpm_create")
         self._h = h
         if w.rain is not None:
             self._ck(L.lpm_set_rain(h, w.rain.x0, w.rain.x1, w.rain.y0, w.rain.y1, w.rain.t_start, w.rain.t_end), "lpm_set_rain")
-        if auto_release and w.release is not None:
+        if a["auto_release"] and w.release is not None:
             self.release(w.release)
+
+    def restart(self):
+        """Start the same run again from step 0: lpm_destroy + lpm_create on the same workspace and met array."""
+        self.close()
+        self._create()
 
     # ------------------------------------------------------------------ plumbing
     def _ck(self, rc, where):
@@ -301,10 +317,17 @@ class Simulation:
         self._ck(self._L.lpm_set_timing(self._h, 1 if on else 0), "lpm_set_timing")
 
     def get_timing(self):
-        out = (C.c_double * 8)()
+        out = (C.c_double * 12)()
         self._ck(self._L.lpm_get_timing(self._h, out), "lpm_get_timing")
         return dict(step_ms=out[0], step_launches=int(out[1]), bin_ms=out[2], bin_launches=int(out[3]),
-                    particle_steps=out[4], binned_particles=out[5], sort_ms=out[6], sort_launches=int(out[7]))
+                    particle_steps=out[4], binned_particles=out[5], sort_ms=out[6], sort_launches=int(out[7]),
+                    born_particle_steps=out[8])
+
+    @property
+    def touched_cells(self) -> int:
+        n = C.c_uint64()
+        self._ck(self._L.lpm_touched_cells(self._h, C.byref(n)), "lpm_touched_cells")
+        return n.value
 
     @property
     def texel_pairs(self) -> bool:
@@ -361,28 +384,28 @@ class Simulation:
         return dict(xyzq=xyzq[:n], q1=None if q1 is None else q1[:n], pid=pid64, status=st[:n], n=n)
 
     def get_particles_host(self):
-        """numpy view of the state in activity units: x, y, z (f32), m [K,n] (f64 = q * scale), pid, status."""
+        """numpy copy of the state as stored: x, y, z (f32), q [K,n] (the stored fp32 values as f64), scale [K]
+        (lpm_mass_scale: the activity of a particle is q * scale, R8 - the product is left to the caller), pid, status."""
         p = self.get_particles()
-        scale = self.mass_scale()
         xyzq = p["xyzq"].cpu().numpy()
         q = [xyzq[:, 3].astype(np.float64)]
         if self.K > 1:
             q.append(p["q1"].cpu().numpy().astype(np.float64))
-        m = np.stack(q) * scale[:, None]
-        return dict(x=xyzq[:, 0].copy(), y=xyzq[:, 1].copy(), z=xyzq[:, 2].copy(), q=np.stack(q), m=m,
+        return dict(x=xyzq[:, 0].copy(), y=xyzq[:, 1].copy(), z=xyzq[:, 2].copy(), q=np.stack(q), scale=self.mass_scale(),
                     pid=p["pid"].cpu().numpy().astype(np.uint64), status=p["status"].cpu().numpy())
 
     def set_particles(self, xyzq, q1=None, pid=None, status=None, step_index: int = 0):
         t = self.torch
-        xyzq = xyzq.to(device=self.device, dtype=t.float32).contiguous()
-        n = xyzq.shape[0]
-        q1 = None if q1 is None else q1.to(device=self.device, dtype=t.float32).contiguous()
-        pid = None if pid is None else pid.to(device=self.device, dtype=t.int64).to(t.int32).contiguous()
-        status = None if status is None else status.to(device=self.device, dtype=t.uint8).contiguous()
-        self._ck(self._L.lpm_set_particles(self._h, xyzq.data_ptr(), None if q1 is None else q1.data_ptr(),
-                                           None if pid is None else pid.data_ptr(),
-                                           None if status is None else status.data_ptr(), n, step_index), "lpm_set_particles")
-        self.torch.cuda.current_stream().synchronize()
+        with t.cuda.stream(self.stream):   # the staging copies and the library's copies run on the handle's stream
+            xyzq = xyzq.to(device=self.device, dtype=t.float32).contiguous()
+            n = xyzq.shape[0]
+            q1 = None if q1 is None else q1.to(device=self.device, dtype=t.float32).contiguous()
+            pid = None if pid is None else pid.to(device=self.device, dtype=t.int64).to(t.int32).contiguous()
+            status = None if status is None else status.to(device=self.device, dtype=t.uint8).contiguous()
+            self._ck(self._L.lpm_set_particles(self._h, xyzq.data_ptr(), None if q1 is None else q1.data_ptr(),
+                                               None if pid is None else pid.data_ptr(),
+                                               None if status is None else status.data_ptr(), n, step_index), "lpm_set_particles")
+        self.stream.synchronize()
 
 
 # ---------------------------------------------------------------- micro-benchmarks

@@ -166,7 +166,7 @@ struct lpm_handle {
     std::vector<Span> spans;
     std::vector<cudaEvent_t> ev_pool;
     double t_ms[3], t_units[3];
-    uint64_t t_base;  // compact mode: device particle-step counter at lpm_set_timing
+    uint64_t t_base, t_base_bin;  // device counters (particle-steps executed, particles binned) at lpm_set_timing
     uint64_t t_launches[3];
     int sticky;
     char err[512];
@@ -199,7 +199,7 @@ cudaEvent_t ev_get(lpm_handle *h)
 {
     if (!h->ev_pool.empty()) { cudaEvent_t e = h->ev_pool.back(); h->ev_pool.pop_back(); return e; }
     cudaEvent_t e = nullptr;
-    cudaEventCreate(&e);
+    if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
     return e;
 }
 
@@ -208,6 +208,11 @@ int span_open(lpm_handle *h, int kind, double units)
 {
     if (!h->timing) return -1;
     lpm_handle::Span sp{ev_get(h), ev_get(h), kind};
+    if (!sp.a || !sp.b) {   // no event to be had: this launch goes untimed (its units are not counted either)
+        if (sp.a) h->ev_pool.push_back(sp.a);
+        if (sp.b) h->ev_pool.push_back(sp.b);
+        return -1;
+    }
     cudaEventRecord(sp.a, h->st);
     h->spans.push_back(sp);
     h->t_units[kind] += units;
@@ -346,12 +351,20 @@ int grid_blocks(const lpm_handle *h, uint64_t n)
     return (int)(want < maxb ? (want ? want : 1) : maxb);
 }
 
+// control block (uint64 words of L.ctrl): [0..2] compact store counts, [3] particle-steps executed (cumulative),
+// [4..6] hole list / fill counters, [8..15] per-release emitted counts (compact), [16] tile ticket of the slot kernel,
+// [17], [18] live length of the slot list in half 0 / 1 of L.perm, [19] particles binned (cumulative),
+// [20] cells that held a particle at the last lpm_touched_cells, [22] |u|max, |v|max of the met interval
+constexpr int kCtrlSteps = 3, kCtrlLive = 17, kCtrlBinned = 19, kCtrlTouched = 20;
+
+uint32_t *perm_half(const lpm_handle *h, int half) { return (uint32_t *)(h->ws + h->L.perm) + (uint64_t)half * (up(4 * h->prm.capacity) / 4); }
+
 int do_bin(lpm_handle *h)
 {
     const uint64_t cells3 = (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz;
     const int span = span_open(h, 1, 0.0);
-    CK(cudaMemsetAsync(h->ws + h->L.cnt, 0, 4 * cells3, h->st));
-    CK(cudaMemsetAsync(h->ws + h->L.conc, 0, 8 * cells3 * h->K, h->st));
+    // the count grid and the K sum grids lie back to back in the workspace: one memset
+    CK(cudaMemsetAsync(h->ws + h->L.cnt, 0, (h->L.conc - h->L.cnt) + 8 * cells3 * h->K, h->st));
     BinArgs B{};
     B.q1 = h->K > 1 ? (const float *)(h->ws + h->L.q1) : nullptr;
     B.cg = gridf(h->cg);
@@ -359,12 +372,23 @@ int do_bin(lpm_handle *h)
     B.conc = (double *)(h->ws + h->L.conc);
     B.cells3 = cells3;
     B.K = h->K;
+    B.n_binned = (uint64_t *)(h->ws + h->L.ctrl) + kCtrlBinned;
+    for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) {
+        // largest stored q: q = activity / G(t) and a particle never gains activity, so q <= dep_bound / G(now)
+        const double qmax = k < h->K ? h->dep_bound[k] / G_of(h, k, h->step) : 0.0;
+        int e = 0;
+        if (qmax > 0.0) { frexp(1048576.0 / qmax, &e); e -= 1; }
+        if (e > 100) e = 100;
+        if (e < -100) e = -100;
+        B.scale[k] = (float)ldexp(1.0, e);
+        B.inv_scale[k] = ldexp(1.0, -e);
+    }
+    const int max_blocks = h->sms * 6;
     if (h->prm.compact) {
         B.xyzq = (const float4 *)(h->ws + h->L.xyzq);
         B.n_dev = (const uint64_t *)(h->ws + h->L.ctrl) + 2;
-        CK(launch_bin(B, h->sms * 8, h->st));
+        CK(launch_bin(B, max_blocks, h->st));
         h->launches++;
-        // the live count is device-side; the host's upper bound is the capacity (labelled so in bench.py)
     } else {
         for (const Release &r : h->rel) {
             const uint64_t n = born_local(r, (int64_t)h->step - 1);
@@ -372,10 +396,16 @@ int do_bin(lpm_handle *h)
             B.xyzq = (const float4 *)(h->ws + h->L.xyzq) + r.base;
             if (B.q1) B.q1 = (const float *)(h->ws + h->L.q1) + r.base;
             B.n = n;
-            const uint64_t want = (n + 255) / 256;
-            CK(launch_bin(B, (int)(want < (uint64_t)h->sms * 8 ? want : (uint64_t)h->sms * 8), h->st));
+            B.perm = nullptr; B.n_list_dev = nullptr; B.n_list = 0; B.first_new = 0;
+            if (h->perm_valid && h->rel.size() == 1 && h->perm_n <= n) {   // the step kernel's met-cell-sorted list
+                B.perm = perm_half(h, h->perm_cur);
+                B.n_list = h->perm_n;
+                B.n_list_dev = (const uint64_t *)(h->ws + h->L.ctrl) + kCtrlLive + h->perm_cur;
+                B.first_new = h->perm_n;
+            }
+            const uint64_t want = (n + 1023) / 1024;
+            CK(launch_bin(B, (int)(want < (uint64_t)max_blocks ? want : (uint64_t)max_blocks), h->st));
             h->launches++;
-            if (h->timing) h->t_units[1] += (double)n;
         }
     }
     span_close(h, span);
@@ -632,6 +662,9 @@ int32_t lpm_release(lpm_handle *h, const lpm_source *src, const double *act, uin
     }
     for (int k = 0; k < h->K; ++k) if (r.emit[k] > h->dep_bound[k]) h->dep_bound[k] = r.emit[k];
     h->rel.push_back(r);
+    // the met buffers blended ahead (and the plume mask they were cut to) know nothing of this source
+    h->blend_n = 0;
+    h->bbox_valid = false;
     return LPM_OK;
 }
 
@@ -763,11 +796,13 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                     for (int s = 0; s < m; ++s) units += (double)born_local(r, (int64_t)h->step + s);
                 A.perm = nullptr;
                 A.n_perm = 0;
+                A.n_live = nullptr;
                 A.keys_out = nullptr; A.hist_out = nullptr; A.n_keys = 0;
                 if (sort_enabled(&h->prm) && A.n_prev > 0 && (h->prm.gather_sort > 0 || A.n_prev >= kSortAutoMin)) {
                     // the list is kept for `period` model steps (one release: the perm buffer is its own);
                     // particles born since the last sort are walked in slot order behind it
-                    uint32_t *perm = (uint32_t *)(h->ws + h->L.perm) + (uint64_t)h->perm_cur * (up(4 * h->prm.capacity) / 4);
+                    uint32_t *perm = perm_half(h, h->perm_cur);
+                    uint64_t *live = A.ctrl + kCtrlLive;
                     const bool single = h->rel.size() == 1;
                     const uint64_t period = h->prm.gather_sort > 0 ? (uint64_t)h->prm.gather_sort : (uint64_t)h->sort_period;
                     const uint32_t n_keys = (uint32_t)A.snap_cells + 1u;
@@ -777,17 +812,18 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                         if (single && h->keys_ready && h->keys_n == A.n_prev && h->keys_step == h->step) {
                             if (h->sort_by_slot) {
                                 // keys indexed by slot: the scatter walks the slots in order, each cell's slots end up ascending
-                                CK(launch_sort_finish(keys, A.n_prev, n_keys, hist, (uint32_t *)(h->ws + h->L.partial), nullptr, 0, perm, h->st));
+                                CK(launch_sort_finish(keys, A.n_prev, n_keys, hist, (uint32_t *)(h->ws + h->L.partial), nullptr, 0, nullptr, perm, live + h->perm_cur, h->st));
                             } else {
                                 // the keys stand in the order of the current list (written by the previous launch): build the other one
+                                const uint64_t *live_old = live + h->perm_cur;
                                 h->perm_cur ^= 1;
-                                uint32_t *next = (uint32_t *)(h->ws + h->L.perm) + (uint64_t)h->perm_cur * (up(4 * h->prm.capacity) / 4);
-                                CK(launch_sort_finish(keys, A.n_prev, n_keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->perm_n, next, h->st));
+                                uint32_t *next = perm_half(h, h->perm_cur);
+                                CK(launch_sort_finish(keys, A.n_prev, n_keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->perm_n, live_old, next, live + h->perm_cur, h->st));
                                 perm = next;
                             }
                             h->launches += 4;
                         } else {
-                            CK(launch_sort_by_cell(A.xyzq + r.base, A.n_prev, A.mg, keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, h->st));
+                            CK(launch_sort_by_cell(A.xyzq + r.base, A.n_prev, A.mg, keys, hist, (uint32_t *)(h->ws + h->L.partial), perm, live + h->perm_cur, h->st));
                             h->launches += 5;
                         }
                         span_close(h, sspan);
@@ -797,6 +833,7 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                     }
                     A.perm = perm;
                     A.n_perm = h->perm_n;
+                    A.n_live = live + h->perm_cur;
                     // will the next launch sort?  then this one leaves the keys and the histogram
                     h->keys_ready = false;
                     if (single && h->step + (uint64_t)m - h->perm_step >= period) {
@@ -943,9 +980,15 @@ int32_t lpm_get_particles(lpm_handle *h, void *xyzq, float *q1, uint32_t *pid, u
     if (pid) {
         if (h->prm.compact) CK(cudaMemcpyAsync(pid, h->ws + h->L.pid, 4 * n, cudaMemcpyDeviceToDevice, h->st));
         else {
-            // slot-addressed mode: ids are implied; single-release blocks report offset + l*stride
-            CK(launch_iota(pid, n, h->st));
-            h->launches++;
+            // slot-addressed mode: ids are implied by the slot: pid_offset + l * pid_stride inside each release block
+            // (the padding slots between two blocks report 0)
+            CK(cudaMemsetAsync(pid, 0, 4 * n, h->st));
+            for (const Release &r : h->rel) {
+                const uint64_t b = born_local(r, (int64_t)h->step - 1);
+                if (!b) continue;
+                CK(launch_iota(pid + r.base, b, r.pid_offset, r.pid_stride, h->st));
+                h->launches++;
+            }
         }
     }
     return LPM_OK;
@@ -956,8 +999,29 @@ int32_t lpm_set_particles(lpm_handle *h, const void *xyzq, const float *q1, cons
 {
     if (!h || !xyzq || (h->K > 1 && !q1)) return fail(h, LPM_ERR_INVALID_ARG, "lpm_set_particles: null");
     if (n > h->prm.capacity) return fail(h, LPM_ERR_CAPACITY, "lpm_set_particles: n exceeds capacity");
-    if (!h->prm.compact && pid) return fail(h, LPM_ERR_INVALID_ARG, "lpm_set_particles: ids are implied by the slot unless compact=1");
     if (h->sticky) return h->sticky;
+    uint64_t id_off = 0, id_stride = 1;
+    if (!h->prm.compact && pid && n) {
+        // slot-addressed store: ids are implied by the slot, so the given ids must be offset + l * stride (what
+        // lpm_get_particles reports for one release); offset and stride are read back from the first two entries
+        uint32_t two[2] = {0, 0};
+        CK(cudaMemcpyAsync(two, pid, n > 1 ? 8 : 4, cudaMemcpyDeviceToHost, h->st));
+        CK(cudaStreamSynchronize(h->st));
+        id_off = two[0];
+        if (n > 1) {
+            if (two[1] <= two[0]) return fail(h, LPM_ERR_INVALID_ARG, "lpm_set_particles: slot-addressed store needs ascending affine ids");
+            id_stride = two[1] - two[0];
+        }
+        if (id_off + (n - 1) * id_stride >= (1ull << 32)) return fail(h, LPM_ERR_INVALID_ARG, "lpm_set_particles: particle ids must stay below 2^32");
+        uint32_t *bad = (uint32_t *)(h->ws + h->L.air);
+        uint32_t bad_h = 0;
+        CK(cudaMemsetAsync(bad, 0, 4, h->st));
+        CK(launch_check_affine(pid, n, id_off, id_stride, bad, h->st));
+        h->launches++;
+        CK(cudaMemcpyAsync(&bad_h, bad, 4, cudaMemcpyDeviceToHost, h->st));
+        CK(cudaStreamSynchronize(h->st));
+        if (bad_h) return fail(h, LPM_ERR_INVALID_ARG, "lpm_set_particles: ids are implied by the slot unless compact=1: pid must be offset + l*stride");
+    }
     if (n) {
         CK(cudaMemcpyAsync(h->ws + h->L.xyzq, xyzq, 16 * n, cudaMemcpyDeviceToDevice, h->st));
         if (h->K > 1) CK(cudaMemcpyAsync(h->ws + h->L.q1, q1, 4 * n, cudaMemcpyDeviceToDevice, h->st));
@@ -966,15 +1030,17 @@ int32_t lpm_set_particles(lpm_handle *h, const void *xyzq, const float *q1, cons
     if (h->prm.compact) {
         if (n) {
             if (pid) CK(cudaMemcpyAsync(h->ws + h->L.pid, pid, 4 * n, cudaMemcpyDeviceToDevice, h->st));
-            else { CK(launch_iota((uint32_t *)(h->ws + h->L.pid), n, h->st)); h->launches++; }
+            else { CK(launch_iota((uint32_t *)(h->ws + h->L.pid), n, 0, 1, h->st)); h->launches++; }
         }
+        // the look-back tile states carry the step index as their epoch: a clock moved backwards must not meet old ones
+        CK(cudaMemsetAsync(h->ws + h->L.tile, 0, 8 * (h->prm.capacity / kScanTile + 2), h->st));
         uint64_t ctrl[3] = {n, 0, n};
         CK(cudaMemcpyAsync(h->ws + h->L.ctrl, ctrl, sizeof(ctrl), cudaMemcpyHostToDevice, h->st));
         CK(cudaStreamSynchronize(h->st));
     } else {
         h->rel.clear();
         Release r{};
-        r.fixed = true; r.n_local = n; r.pid_stride = 1; r.S = 1;
+        r.fixed = true; r.n_local = n; r.pid_offset = id_off; r.pid_stride = id_stride; r.S = 1;
         h->rel.push_back(r);
         h->next_base = n;
     }
@@ -1113,10 +1179,9 @@ int32_t lpm_set_timing(lpm_handle *h, int32_t enable)
     spans_collect(h);
     h->timing = enable != 0;
     for (int i = 0; i < 3; ++i) { h->t_ms[i] = 0.0; h->t_units[i] = 0.0; h->t_launches[i] = 0; }
-    if (h->prm.compact) {
-        CK(cudaMemcpyAsync(&h->t_base, (uint64_t *)(h->ws + h->L.ctrl) + 3, 8, cudaMemcpyDeviceToHost, h->st));
-        CK(cudaStreamSynchronize(h->st));
-    }
+    CK(cudaMemcpyAsync(&h->t_base, (uint64_t *)(h->ws + h->L.ctrl) + kCtrlSteps, 8, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaMemcpyAsync(&h->t_base_bin, (uint64_t *)(h->ws + h->L.ctrl) + kCtrlBinned, 8, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
     return LPM_OK;
 }
 
@@ -1129,12 +1194,28 @@ int32_t lpm_get_timing(lpm_handle *h, double *out)
     out[2] = h->t_ms[1]; out[3] = (double)h->t_launches[1];
     out[4] = h->t_units[0]; out[5] = h->t_units[1];
     out[6] = h->t_ms[2]; out[7] = (double)h->t_launches[2];
-    if (h->prm.compact) {  // the live count is device-side: cumulative particle-steps since lpm_set_timing
-        uint64_t now = 0;
-        CK(cudaMemcpyAsync(&now, (uint64_t *)(h->ws + h->L.ctrl) + 3, 8, cudaMemcpyDeviceToHost, h->st));
-        CK(cudaStreamSynchronize(h->st));
-        out[4] = (double)(now - h->t_base);
-    }
+    out[8] = h->t_units[0];   // born particles x steps (host count, R9): includes particles that have left the domain
+    // what the kernels counted themselves: particle-steps executed (born AND active), particles binned (active, in the grid)
+    uint64_t now[2] = {0, 0};
+    CK(cudaMemcpyAsync(&now[0], (uint64_t *)(h->ws + h->L.ctrl) + kCtrlSteps, 8, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaMemcpyAsync(&now[1], (uint64_t *)(h->ws + h->L.ctrl) + kCtrlBinned, 8, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    out[4] = (double)(now[0] - h->t_base);
+    out[5] = (double)(now[1] - h->t_base_bin);
+    return LPM_OK;
+}
+
+int32_t lpm_touched_cells(lpm_handle *h, uint64_t *n)
+{
+    if (!h || !n) return LPM_ERR_INVALID_ARG;
+    if (h->sticky) return h->sticky;
+    if (!h->binned) return fail(h, LPM_ERR_STATE, "lpm_touched_cells: nothing has been binned yet");
+    uint64_t *dst = (uint64_t *)(h->ws + h->L.ctrl) + kCtrlTouched;
+    CK(cudaMemsetAsync(dst, 0, 8, h->st));
+    CK(launch_count_nonzero((const uint32_t *)(h->ws + h->L.cnt), (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz, dst, h->st));
+    h->launches++;
+    CK(cudaMemcpyAsync(n, dst, 8, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
     return LPM_OK;
 }
 

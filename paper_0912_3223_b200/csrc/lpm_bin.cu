@@ -10,54 +10,149 @@
 
 namespace lpm {
 
-// v0: one particle per thread iteration, warp-aggregated: lanes that hit the same cell are
-// combined with match.any so that the hot cells next to the source cost one RED per warp.
-__global__ void __launch_bounds__(256) bin_kernel(const __grid_constant__ BinArgs A)
+// The binning kernel named by north_star ("shared-memory-privatised histograms ... instead of naive global
+// atomics"; the paper itself only says the summation "may be computed by the GPU, in a separate kernel").
+//
+// Order.  The particles are walked in the order of the step kernel's met-cell-sorted slot list (S 8(f)4: the sort is
+// shared), so the kBinTile particles a CTA takes at a time are spatial neighbours and fall into few concentration
+// cells; the compact store is itself kept in that order, small ensembles are walked as stored.
+// Privatisation.  Per tile, counts and sums are accumulated in an open-addressing table in shared memory keyed by the
+// concentration cell: u32 count + per nuclide a u32 FIXED-POINT sum rint(q * S_k), S_k a power of two with
+// q_max S_k in [2^19, 2^20) (the DepTab idea of the step kernel: native 32-bit shared atomics, order-independent
+// integer sums, a tile of 1024 particles cannot overflow: 2^10 x 2^20).  q in [2^17, 2^20) / S_k (>= 18 significant
+// bits, relative rounding error <= 3.8e-6 per particle, unbiased) takes this path, anything else the direct fp64 RED.
+// When the tile is done every touched cell receives ONE u32 RED and one fp64 RED per nuclide.  Counts are exact.
+constexpr int kBinTile = 1024, kBinItems = kBinTile / 256;
+constexpr int kBinSlots = 2048, kBinSlotBits = 11, kBinProbes = 8;
+
+template <int K>
+struct BinTab {
+    uint32_t tag[kBinSlots];      // cell + 1, 0 = empty
+    uint32_t cnt[kBinSlots];
+    uint32_t sum[K][kBinSlots];
+};
+
+template <int K>
+__global__ void __launch_bounds__(256) bin_tile_kernel(const __grid_constant__ BinArgs A)
 {
+    __shared__ BinTab<K> T;
+    for (int i = threadIdx.x; i < kBinSlots; i += 256) {
+        T.tag[i] = 0u; T.cnt[i] = 0u;
+#pragma unroll
+        for (int k = 0; k < K; ++k) T.sum[k][i] = 0u;
+    }
     const uint64_t n = A.n_dev ? *A.n_dev : A.n;
-    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
-    const uint64_t n_round = (n + 31) & ~(uint64_t)31;  // keep warps converged for match.any
-    const int lane = threadIdx.x & 31;
-    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
-        int cell = -1;
-        float q0 = 0.f, q1 = 0.f;
-        if (i < n) {
-            const float4 p = A.xyzq[i];
-            if (p.z >= 0.0f) {  // z < 0 marks an exited slot
-                const int ci = cell_of(p.x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
-                const int cj = cell_of(p.y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
-                const int ck = cell_of(p.z, A.cg.z0, A.cg.inv_dz, A.cg.nz);
-                if ((ci | cj | ck) >= 0) {
-                    cell = (ck * A.cg.ny + cj) * A.cg.nx + ci;
-                    q0 = p.w;
-                    if (A.K > 1) q1 = A.q1[i];
+    uint64_t n_list = 0, first_new = 0;
+    if (A.perm) {
+        n_list = A.n_list;
+        if (A.n_list_dev) { const uint64_t d = *A.n_list_dev; n_list = d < n_list ? d : n_list; }
+        first_new = A.first_new < n ? A.first_new : n;
+    }
+    const uint32_t t_old = (uint32_t)((n_list + kBinTile - 1) / kBinTile);
+    const uint32_t n_tiles = t_old + (uint32_t)((n - first_new + kBinTile - 1) / kBinTile);
+    uint32_t binned = 0;
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        __syncthreads();   // the table is clear (start of the kernel / flush of the previous tile)
+#pragma unroll
+        for (int j = 0; j < kBinItems; ++j) {
+            uint64_t slot;
+            bool valid;
+            if (tile < t_old) {
+                const uint64_t pos = (uint64_t)tile * kBinTile + (uint32_t)j * 256 + threadIdx.x;
+                valid = pos < n_list;
+                slot = valid ? A.perm[pos] : 0ull;
+            } else {
+                slot = first_new + (uint64_t)(tile - t_old) * kBinTile + (uint32_t)j * 256 + threadIdx.x;
+                valid = slot < n;
+            }
+            if (!valid) continue;
+            const float4 p = A.xyzq[slot];
+            if (!(p.z >= 0.0f)) continue;   // z < 0 marks an exited slot
+            const int ci = cell_of(p.x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
+            const int cj = cell_of(p.y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
+            const int ck = cell_of(p.z, A.cg.z0, A.cg.inv_dz, A.cg.nz);
+            if ((ci | cj | ck) < 0) continue;
+            ++binned;
+            const uint32_t cell = (uint32_t)((ck * A.cg.ny + cj) * A.cg.nx + ci), key = cell + 1u;
+            float q[K];
+            q[0] = p.w;
+            if (K > 1) q[1] = A.q1[slot];
+            uint32_t h = (key * 0x9E3779B1u) >> (32 - kBinSlotBits);
+            int s = -1;
+#pragma unroll 1
+            for (int pr = 0; pr < kBinProbes; ++pr) {
+                const uint32_t t = *(volatile uint32_t *)&T.tag[h];
+                if (t == key) { s = (int)h; break; }
+                if (t == 0u) {
+                    const uint32_t old = atomicCAS(&T.tag[h], 0u, key);
+                    if (old == 0u || old == key) { s = (int)h; break; }
                 }
+                h = (h + 1u) & (kBinSlots - 1);
+            }
+            if (s >= 0) atomicAdd(&T.cnt[s], 1u);
+            else atomicAdd(A.cnt + cell, 1u);
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                const uint32_t iv = __float2uint_rn(q[k] * A.scale[k]);   // saturating; q >= 0
+                if (s >= 0 && iv - 131072u < 1048576u - 131072u) atomicAdd(&T.sum[k][s], iv);
+                else if (q[k] != 0.0f) atomicAdd(A.conc + (uint64_t)k * A.cells3 + cell, (double)q[k]);
             }
         }
-        const uint32_t peers = __match_any_sync(0xffffffffu, cell);
-        if (cell < 0) continue;
-        const int leader = __ffs(peers) - 1;
-        // sum q over the peer group in lane order (deterministic for a given warp content)
-        double s0 = 0.0, s1 = 0.0;
-        uint32_t rest = peers;
-        while (rest) {
-            const int src = __ffs(rest) - 1;
-            rest &= rest - 1;
-            s0 += (double)__shfl_sync(peers, q0, src);
-            if (A.K > 1) s1 += (double)__shfl_sync(peers, q1, src);
+        __syncthreads();
+        for (int i = threadIdx.x; i < kBinSlots; i += 256) {
+            const uint32_t key = T.tag[i];
+            if (key == 0u) continue;
+            T.tag[i] = 0u;
+            const uint32_t c = T.cnt[i];
+            T.cnt[i] = 0u;
+            atomicAdd(A.cnt + (key - 1u), c);
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                const uint32_t v = T.sum[k][i];
+                T.sum[k][i] = 0u;
+                if (v) atomicAdd(A.conc + (uint64_t)k * A.cells3 + (key - 1u), (double)v * A.inv_scale[k]);
+            }
         }
-        if (lane == leader) {
-            atomicAdd(A.cnt + cell, (uint32_t)__popc(peers));
-            atomicAdd(A.conc + cell, s0);
-            if (A.K > 1) atomicAdd(A.conc + A.cells3 + cell, s1);
-        }
+    }
+    if (A.n_binned) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) binned += __shfl_xor_sync(0xffffffffu, binned, o);
+        if ((threadIdx.x & 31) == 0 && binned) atomicAdd((unsigned long long *)A.n_binned, (unsigned long long)binned);
     }
 }
 
 cudaError_t launch_bin(const BinArgs &a, int blocks, cudaStream_t st)
 {
-    bin_kernel<<<blocks, 256, 0, st>>>(a);
+    if (a.K > 1) bin_tile_kernel<2><<<blocks, 256, 0, st>>>(a);
+    else bin_tile_kernel<1><<<blocks, 256, 0, st>>>(a);
     return cudaGetLastError();
+}
+
+// number of cells that hold at least one particle (bench.py: the footprint the binning atomics spread over)
+__global__ void __launch_bounds__(256) count_nonzero_kernel(const uint32_t *__restrict__ cnt, uint64_t cells3, uint64_t *out)
+{
+    uint32_t c = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < cells3; i += (uint64_t)gridDim.x * blockDim.x) c += cnt[i] != 0u;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd((unsigned long long *)out, (unsigned long long)c);
+}
+
+cudaError_t launch_count_nonzero(const uint32_t *cnt, uint64_t cells3, uint64_t *out, cudaStream_t st)
+{
+    const uint64_t want = (cells3 + 255) / 256, cap = (uint64_t)sm_count() * 8;
+    count_nonzero_kernel<<<(int)(want < cap ? (want ? want : 1) : cap), 256, 0, st>>>(cnt, cells3, out);
+    return cudaGetLastError();
+}
+
+int sm_count()
+{
+    static int sms = 0;
+    if (sms <= 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
+    }
+    return sms;
 }
 
 // concentration read-out: Bq m^-3 = sum(q) * G_k(t_bin) / V   (scale[k] = G_k / V)
@@ -72,7 +167,7 @@ __global__ void conc_readout_kernel(const double *__restrict__ conc, float *__re
 cudaError_t launch_conc_readout(const double *conc, float *out, uint64_t cells3, int K, const double *scale, cudaStream_t st)
 {
     const uint64_t total = cells3 * K;
-    int blocks = (int)((total + 255) / 256 < 148 * 8 ? (total + 255) / 256 : 148 * 8);
+    int blocks = (int)((total + 255) / 256 < sm_count() * 8 ? (total + 255) / 256 : sm_count() * 8);
     conc_readout_kernel<<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(conc, out, cells3, K, scale[0], K > 1 ? scale[1] : 0.0);
     return cudaGetLastError();
 }
@@ -90,7 +185,7 @@ __global__ void dose_accum_kernel(const double *__restrict__ conc, double *__res
 cudaError_t launch_dose_accum(const double *conc, double *dose, uint64_t cells3, int K, const double *scale, cudaStream_t st)
 {
     const uint64_t total = cells3 * K;
-    int blocks = (int)((total + 255) / 256 < 148 * 8 ? (total + 255) / 256 : 148 * 8);
+    int blocks = (int)((total + 255) / 256 < sm_count() * 8 ? (total + 255) / 256 : sm_count() * 8);
     dose_accum_kernel<<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(conc, dose, cells3, K, scale[0], K > 1 ? scale[1] : 0.0);
     return cudaGetLastError();
 }
@@ -108,7 +203,7 @@ __global__ void dep_readout_kernel(const double *__restrict__ dep, float *out32,
 cudaError_t launch_dep_readout(const double *dep, float *out_f32, double *out_f64, uint64_t cells2, int K, const double *scale, cudaStream_t st)
 {
     const uint64_t total = cells2 * K;
-    int blocks = (int)((total + 255) / 256 < 148 * 8 ? (total + 255) / 256 : 148 * 8);
+    int blocks = (int)((total + 255) / 256 < sm_count() * 8 ? (total + 255) / 256 : sm_count() * 8);
     dep_readout_kernel<<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(dep, out_f32, out_f64, cells2, total, scale[0], K > 1 ? scale[1] : 0.0);
     return cudaGetLastError();
 }
@@ -121,7 +216,7 @@ __global__ void dep_rebase_kernel(double *dep, uint64_t cells2, double factor)
 
 cudaError_t launch_dep_rebase(double *dep, uint64_t cells2, double factor, cudaStream_t st)
 {
-    int blocks = (int)((cells2 + 255) / 256 < 148 * 8 ? (cells2 + 255) / 256 : 148 * 8);
+    int blocks = (int)((cells2 + 255) / 256 < sm_count() * 8 ? (cells2 + 255) / 256 : sm_count() * 8);
     dep_rebase_kernel<<<blocks < 1 ? 1 : blocks, 256, 0, st>>>(dep, cells2, factor);
     return cudaGetLastError();
 }
@@ -156,7 +251,7 @@ __global__ void __launch_bounds__(256) airborne_kernel(const float4 *__restrict_
 
 cudaError_t launch_airborne(const float4 *xyzq, const float *q1, uint64_t n, const uint64_t *n_dev, int K, double *out2, cudaStream_t st)
 {
-    airborne_kernel<<<148 * 4, 256, 0, st>>>(xyzq, q1, n, n_dev, K, out2);
+    airborne_kernel<<<sm_count() * 4, 256, 0, st>>>(xyzq, q1, n, n_dev, K, out2);
     return cudaGetLastError();
 }
 
@@ -177,7 +272,7 @@ __global__ void export_kernel(const float4 *__restrict__ xyzq, const float *__re
 
 cudaError_t launch_export(const float4 *xyzq, const float *q1, uint64_t n, const uint64_t *n_dev, float4 *out, uint8_t *status, cudaStream_t st)
 {
-    export_kernel<<<148 * 4, 256, 0, st>>>(xyzq, q1, n, n_dev, out, status);
+    export_kernel<<<sm_count() * 4, 256, 0, st>>>(xyzq, q1, n, n_dev, out, status);
     return cudaGetLastError();
 }
 
@@ -189,19 +284,33 @@ __global__ void import_kernel(float4 *xyzq, uint64_t n, const uint8_t *status)
 
 cudaError_t launch_import(float4 *xyzq, uint64_t n, const uint8_t *status, cudaStream_t st)
 {
-    import_kernel<<<148 * 4, 256, 0, st>>>(xyzq, n, status);
+    import_kernel<<<sm_count() * 4, 256, 0, st>>>(xyzq, n, status);
     return cudaGetLastError();
 }
 
-__global__ void iota_kernel(uint32_t *pid, uint64_t n)
+// slot-addressed store: slot l of a release block carries the global id offset + l * stride (R9)
+__global__ void iota_kernel(uint32_t *pid, uint64_t n, uint64_t offset, uint64_t stride)
 {
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x)
-        pid[i] = (uint32_t)i;
+        pid[i] = (uint32_t)(offset + i * stride);
 }
 
-cudaError_t launch_iota(uint32_t *pid, uint64_t n, cudaStream_t st)
+cudaError_t launch_iota(uint32_t *pid, uint64_t n, uint64_t offset, uint64_t stride, cudaStream_t st)
 {
-    iota_kernel<<<148 * 4, 256, 0, st>>>(pid, n);
+    iota_kernel<<<sm_count() * 4, 256, 0, st>>>(pid, n, offset, stride);
+    return cudaGetLastError();
+}
+
+// lpm_set_particles on the slot-addressed store: the ids must be offset + l * stride; *bad != 0 otherwise
+__global__ void check_affine_kernel(const uint32_t *__restrict__ pid, uint64_t n, uint64_t offset, uint64_t stride, uint32_t *bad)
+{
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x)
+        if (pid[i] != (uint32_t)(offset + i * stride)) *bad = 1u;
+}
+
+cudaError_t launch_check_affine(const uint32_t *pid, uint64_t n, uint64_t offset, uint64_t stride, uint32_t *bad, cudaStream_t st)
+{
+    check_affine_kernel<<<sm_count() * 4, 256, 0, st>>>(pid, n, offset, stride, bad);
     return cudaGetLastError();
 }
 
@@ -227,7 +336,7 @@ __global__ void qmax_kernel(const float4 *__restrict__ xyzq, const float *__rest
 
 cudaError_t launch_qmax(const float4 *xyzq, const float *q1, uint64_t n, int K, float *out2, cudaStream_t st)
 {
-    qmax_kernel<<<148 * 4, 256, 0, st>>>(xyzq, q1, n, K, out2);
+    qmax_kernel<<<sm_count() * 4, 256, 0, st>>>(xyzq, q1, n, K, out2);
     return cudaGetLastError();
 }
 
@@ -243,7 +352,7 @@ __global__ void test_philox_kernel(uint32_t seed_lo, uint32_t seed_hi, uint32_t 
 
 cudaError_t launch_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st)
 {
-    test_philox_kernel<<<148, 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step, stream, pid0, n, out);
+    test_philox_kernel<<<sm_count(), 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step, stream, pid0, n, out);
     return cudaGetLastError();
 }
 
@@ -261,7 +370,7 @@ __global__ void test_curand_philox_kernel(uint64_t seed, uint64_t step, uint64_t
 
 cudaError_t launch_test_curand_philox(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st)
 {
-    test_curand_philox_kernel<<<148, 256, 0, st>>>(seed, step, pid0, n, out);
+    test_curand_philox_kernel<<<sm_count(), 256, 0, st>>>(seed, step, pid0, n, out);
     return cudaGetLastError();
 }
 
@@ -278,7 +387,7 @@ __global__ void test_normals_kernel(uint32_t seed_lo, uint32_t seed_hi, uint32_t
 
 cudaError_t launch_test_normals(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, float *out, cudaStream_t st)
 {
-    test_normals_kernel<<<148, 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step, pid0, n, out);
+    test_normals_kernel<<<sm_count(), 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step, pid0, n, out);
     return cudaGetLastError();
 }
 
@@ -293,7 +402,7 @@ __global__ void test_box_muller_kernel(const uint4 *__restrict__ r, uint64_t n, 
 
 cudaError_t launch_test_box_muller(const uint32_t *r, uint64_t n, float *out, cudaStream_t st)
 {
-    test_box_muller_kernel<<<148 * 8, 256, 0, st>>>((const uint4 *)r, n, out);
+    test_box_muller_kernel<<<sm_count() * 8, 256, 0, st>>>((const uint4 *)r, n, out);
     return cudaGetLastError();
 }
 
@@ -311,7 +420,7 @@ __global__ void test_sample_kernel(const float4 *blend, const __grid_constant__ 
 cudaError_t launch_test_sample(const float4 *blend, GridF mg, float kz_min, const float4 *xyz, uint64_t n, float4 *out,
                                cudaStream_t st)
 {
-    test_sample_kernel<<<148, 256, 0, st>>>(blend, mg, kz_min, xyz, n, out);
+    test_sample_kernel<<<sm_count(), 256, 0, st>>>(blend, mg, kz_min, xyz, n, out);
     return cudaGetLastError();
 }
 

@@ -88,6 +88,8 @@ struct StepArgs {
     uint64_t base, n, n_prev;  // slots >= n_prev are born inside this launch
     const uint32_t *perm;      // gather-locality pass: slots [0, n_perm) listed in dual-cell order, or null
     uint64_t n_perm;           // slots [n_perm, n) are walked in slot order
+    const uint64_t *n_live;    // device: length of the live part of `perm` (particles that had left the domain at the
+                               // sort are not listed); the kernel walks the positions [0, min(*n_live, n_perm))
     uint8_t *mask;             // non-null: flag the mask tile of each particle's met column at the end of the launch
     int32_t mask_ntx, pad2_;
     uint32_t *keys_out, *hist_out;  // non-null: the launch before a sort leaves each slot's dual-cell key and the histogram
@@ -130,11 +132,21 @@ struct BinArgs {
     const float *q1;
     uint64_t n;               // slots to bin (slot-addressed mode)
     const uint64_t *n_dev;    // compact mode: read n from here
+    // walk order (a8, S 8(f)4 "sort shared between binning and the step kernel"): the live part of the step kernel's
+    // met-cell-sorted slot list, positions [0, min(*n_list_dev, n_list)), then the slots [first_new, n) in slot order;
+    // perm == null: all slots [0, n) in storage order (small ensembles; the compact store, which is itself kept sorted)
+    const uint32_t *perm;
+    const uint64_t *n_list_dev;
+    uint64_t n_list, first_new;
     GridF cg;
     uint32_t *cnt;
     double *conc;             // [K][cells3] sums of q
     uint64_t cells3;
-    int32_t K;
+    int32_t K, pad_;
+    // fixed-point scale of the CTA-private sums (power of two; 2^19 <= q_max * scale < 2^20) and its inverse
+    float scale[LPM_MAX_NUCLIDES];
+    double inv_scale[LPM_MAX_NUCLIDES];
+    uint64_t *n_binned;       // device counter: += particles binned (active and inside the grid)
 };
 
 // launchers implemented in the .cu files; all return the cudaError of the launch
@@ -142,9 +154,9 @@ cudaError_t launch_step(const StepArgs &a, int K, bool compact, int grid_blocks,
 int step_max_blocks_per_sm(int K, bool compact, int dry_mode, bool bern, bool eq3, bool zlev, bool zpair);
 cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st);
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
-                                uint32_t *perm, cudaStream_t st);
+                                uint32_t *perm, uint64_t *live_out, cudaStream_t st);
 cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, const uint32_t *list_old,
-                               uint64_t n_old, uint32_t *perm, cudaStream_t st);
+                               uint64_t n_old, const uint64_t *live_old, uint32_t *perm, uint64_t *live_out, cudaStream_t st);
 cudaError_t launch_fill_holes(float4 *xyzq, float *q1, uint32_t *pid, uint64_t *ctrl, const uint32_t *holes, uint32_t *src, uint32_t *dst,
                               cudaStream_t st);
 cudaError_t launch_sort_records(float4 *xyzq, float *q1, uint32_t *pid, const uint64_t *n_dev, uint64_t capacity, GridF g, uint32_t *keys,
@@ -177,7 +189,10 @@ cudaError_t launch_dep_rebase(double *dep, uint64_t cells2, double factor, cudaS
 cudaError_t launch_airborne(const float4 *xyzq, const float *q1, uint64_t n, const uint64_t *n_dev, int K, double *out2, cudaStream_t st);
 cudaError_t launch_export(const float4 *xyzq, const float *q1, uint64_t n, const uint64_t *n_dev, float4 *out, uint8_t *status, cudaStream_t st);
 cudaError_t launch_import(float4 *xyzq, uint64_t n, const uint8_t *status, cudaStream_t st);
-cudaError_t launch_iota(uint32_t *pid, uint64_t n, cudaStream_t st);
+cudaError_t launch_iota(uint32_t *pid, uint64_t n, uint64_t offset, uint64_t stride, cudaStream_t st);
+cudaError_t launch_check_affine(const uint32_t *pid, uint64_t n, uint64_t offset, uint64_t stride, uint32_t *bad, cudaStream_t st);
+cudaError_t launch_count_nonzero(const uint32_t *cnt, uint64_t cells3, uint64_t *out, cudaStream_t st);
+int sm_count();   // SMs of the current device (cached)
 cudaError_t launch_qmax(const float4 *xyzq, const float *q1, uint64_t n, int K, float *out2, cudaStream_t st);
 cudaError_t launch_test_philox(uint64_t seed, uint64_t step, uint32_t stream, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st);
 cudaError_t launch_test_curand_philox(uint64_t seed, uint64_t step, uint64_t pid0, uint64_t n, uint32_t *out, cudaStream_t st);

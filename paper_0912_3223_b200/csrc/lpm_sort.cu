@@ -94,7 +94,10 @@ __global__ void __launch_bounds__(256) scan_partials_kernel(uint32_t *partial, u
     }
 }
 
-__global__ void __launch_bounds__(256) scan_apply_kernel(uint32_t *__restrict__ hist, uint32_t m, const uint32_t *__restrict__ partial)
+// live_out (may be null): receives the exclusive offset of the LAST key (the bucket of the exited slots) = the number
+// of live particles listed; the scatter pass does not list the exited ones at all
+__global__ void __launch_bounds__(256) scan_apply_kernel(uint32_t *__restrict__ hist, uint32_t m, const uint32_t *__restrict__ partial,
+                                                         uint64_t *__restrict__ live_out)
 {
     __shared__ uint32_t s_warp[8];
     const uint32_t base = blockIdx.x * kScanBlock + threadIdx.x * kScanItems;
@@ -106,23 +109,31 @@ __global__ void __launch_bounds__(256) scan_apply_kernel(uint32_t *__restrict__ 
 #pragma unroll
     for (int i = 0; i < kScanItems; ++i) {
         if (base + i < m) hist[base + i] = run;
+        if (live_out && base + i == m - 1) *live_out = run;
         run += v[i];
     }
 }
 
 // pass 3: scatter slot indices; lanes of a warp that share a key claim their range with one atomic.
-// keys[pos] belongs to the slot list_old[pos] (pos < n_old: the keys were written in the order of the previous list by
-// the step kernel, so neighbours in `pos` are neighbours in space: the atomics aggregate and the writes to the new list
-// fall into a few lines per warp), or to slot pos (no previous list, and the particles born behind it).
-__global__ void __launch_bounds__(256) sort_scatter_kernel(const uint32_t *__restrict__ keys, uint64_t n, uint32_t *__restrict__ offs,
-                                                           const uint32_t *__restrict__ list_old, uint64_t n_old, uint32_t *__restrict__ perm)
+// keys[pos] belongs to the slot list_old[pos] (pos < *live_old, the live length of the previous list: the keys were
+// written in the order of that list by the step kernel, so neighbours in `pos` are neighbours in space: the atomics
+// aggregate and the writes to the new list fall into a few lines per warp), or to slot pos (pos >= n_old: the
+// particles born behind the previous list; no previous list: every pos).  Positions [*live_old, n_old) hold nothing
+// (slots that had left the domain before the previous sort are not listed any more).  Slots whose key is the last one
+// (exited) are not listed: the new list has hist[n_keys - 1] entries, exported by scan_apply_kernel.
+__global__ void __launch_bounds__(256) sort_scatter_kernel(const uint32_t *__restrict__ keys, uint64_t n, uint32_t dead_key, uint32_t *__restrict__ offs,
+                                                           const uint32_t *__restrict__ list_old, uint64_t n_old, const uint64_t *__restrict__ live_old,
+                                                           uint32_t *__restrict__ perm)
 {
     const uint64_t n_round = (n + 31) & ~(uint64_t)31;
     const int lane = threadIdx.x & 31;
+    uint64_t n_live_old = n_old;
+    if (list_old && live_old) { const uint64_t d = *live_old; n_live_old = d < n_old ? d : n_old; }
     for (uint64_t l = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; l < n_round; l += (uint64_t)gridDim.x * blockDim.x) {
-        const bool live = l < n;
-        const uint32_t key = live ? keys[l] : 0xffffffffu;
-        const uint32_t slot = (live && l < n_old) ? list_old[l] : (uint32_t)l;
+        bool live = l < n && !(list_old && l >= n_live_old && l < n_old);
+        uint32_t key = live ? keys[l] : 0xffffffffu;
+        if (key == dead_key) { live = false; key = 0xffffffffu; }
+        const uint32_t slot = (live && list_old && l < n_old) ? list_old[l] : (uint32_t)l;
         const uint32_t peers = __match_any_sync(0xffffffffu, key);
         const int leader = __ffs(peers) - 1;
         uint32_t base = 0;
@@ -209,8 +220,8 @@ __global__ void __launch_bounds__(256) fill_move_kernel(float4 *__restrict__ xyz
 cudaError_t launch_fill_holes(float4 *xyzq, float *q1, uint32_t *pid, uint64_t *ctrl, const uint32_t *holes, uint32_t *src, uint32_t *dst,
                               cudaStream_t st)
 {
-    fill_collect_kernel<<<148, 256, 0, st>>>(xyzq, ctrl, holes, src, dst);
-    fill_move_kernel<<<148, 256, 0, st>>>(xyzq, q1, pid, ctrl, src, dst);
+    fill_collect_kernel<<<sm_count(), 256, 0, st>>>(xyzq, ctrl, holes, src, dst);
+    fill_move_kernel<<<sm_count(), 256, 0, st>>>(xyzq, q1, pid, ctrl, src, dst);
     return cudaGetLastError();
 }
 
@@ -222,13 +233,13 @@ cudaError_t launch_sort_records(float4 *xyzq, float *q1, uint32_t *pid, const ui
     const uint32_t n_keys = (uint32_t)g.nx * g.ny * g.nz + 1u, m = n_keys;
     cudaError_t e = cudaMemsetAsync(hist, 0, 4ull * n_keys, st);
     if (e != cudaSuccess) return e;
-    const uint64_t want = (capacity + 255) / 256;
-    const int blocks = (int)(want < 148 * 8 ? (want ? want : 1) : 148 * 8);
+    const uint64_t want = (capacity + 255) / 256, cap = (uint64_t)sm_count() * 8;
+    const int blocks = (int)(want < cap ? (want ? want : 1) : cap);
     sort_key_kernel<<<blocks, 256, 0, st>>>(xyzq, 0, g, n_keys, keys, hist, n_dev);
     const uint32_t nb = (m + kScanBlock - 1) / kScanBlock;
     scan_totals_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
     scan_partials_kernel<<<1, 256, 0, st>>>(partial, nb);
-    scan_apply_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
+    scan_apply_kernel<<<nb, 256, 0, st>>>(hist, m, partial, nullptr);
     sort_scatter_records_kernel<<<blocks, 256, 0, st>>>(keys, n_dev, hist, xyzq, q1, pid, xyzq_alt, q1_alt, pid_alt);
     copy_records_kernel<<<blocks, 256, 0, st>>>(n_dev, xyzq_alt, q1_alt, pid_alt, xyzq, q1, pid);
     return cudaGetLastError();
@@ -237,29 +248,29 @@ cudaError_t launch_sort_records(float4 *xyzq, float *q1, uint32_t *pid, const ui
 // passes 2 + 3 on keys and a histogram that are already there (written by sort_key_kernel, or by the
 // step kernel itself at the end of the launch that precedes a sort)
 cudaError_t launch_sort_finish(const uint32_t *keys, uint64_t n, uint32_t n_keys, uint32_t *hist, uint32_t *partial, const uint32_t *list_old,
-                               uint64_t n_old, uint32_t *perm, cudaStream_t st)
+                               uint64_t n_old, const uint64_t *live_old, uint32_t *perm, uint64_t *live_out, cudaStream_t st)
 {
     const uint32_t m = n_keys;
-    const uint64_t want = (n + 255) / 256;
-    const int blocks = (int)(want < 148 * 8 ? (want ? want : 1) : 148 * 8);
+    const uint64_t want = (n + 255) / 256, cap = (uint64_t)sm_count() * 8;
+    const int blocks = (int)(want < cap ? (want ? want : 1) : cap);
     const uint32_t nb = (m + kScanBlock - 1) / kScanBlock;
     scan_totals_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
     scan_partials_kernel<<<1, 256, 0, st>>>(partial, nb);
-    scan_apply_kernel<<<nb, 256, 0, st>>>(hist, m, partial);
-    sort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, hist, list_old, list_old ? n_old : 0, perm);
+    scan_apply_kernel<<<nb, 256, 0, st>>>(hist, m, partial, live_out);
+    sort_scatter_kernel<<<blocks, 256, 0, st>>>(keys, n, n_keys - 1u, hist, list_old, list_old ? n_old : 0, live_old, perm);
     return cudaGetLastError();
 }
 
 cudaError_t launch_sort_by_cell(const float4 *xyzq, uint64_t n, GridF g, uint32_t *keys, uint32_t *hist, uint32_t *partial,
-                                uint32_t *perm, cudaStream_t st)
+                                uint32_t *perm, uint64_t *live_out, cudaStream_t st)
 {
     const uint32_t n_keys = (uint32_t)g.nx * g.ny * g.nz + 1u;
     cudaError_t e = cudaMemsetAsync(hist, 0, 4ull * n_keys, st);
     if (e != cudaSuccess) return e;
-    const uint64_t want = (n + 255) / 256;
-    const int blocks = (int)(want < 148 * 8 ? (want ? want : 1) : 148 * 8);
+    const uint64_t want = (n + 255) / 256, cap = (uint64_t)sm_count() * 8;
+    const int blocks = (int)(want < cap ? (want ? want : 1) : cap);
     sort_key_kernel<<<blocks, 256, 0, st>>>(xyzq, n, g, n_keys, keys, hist);
-    return launch_sort_finish(keys, n, n_keys, hist, partial, nullptr, 0, perm, st);
+    return launch_sort_finish(keys, n, n_keys, hist, partial, nullptr, 0, nullptr, perm, live_out, st);
 }
 
 uint64_t sort_partial_entries(uint64_t n_cells) { return (n_cells + 1 + kScanBlock - 1) / kScanBlock + 1; }

@@ -292,9 +292,13 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
     // in the CTA-private tables below instead of in the global map.
     __shared__ DepTab<K> T;
     dep_clear<K>(T);
-    const uint32_t t_old = A.perm ? (uint32_t)((A.n_perm + kStepThreads - 1) / kStepThreads) : 0u;
+    // (slots that had left the domain when the list was built are not on it: its live length is a device scalar)
+    uint64_t n_list = A.perm ? A.n_perm : 0ull;
+    if (A.perm && A.n_live) { const uint64_t d = *A.n_live; n_list = d < n_list ? d : n_list; }
+    const uint32_t t_old = (uint32_t)((n_list + kStepThreads - 1) / kStepThreads);
     const uint64_t first_new = A.perm ? A.n_perm : 0ull;
     const uint32_t n_tiles = t_old + (uint32_t)((A.n - first_new + kStepThreads - 1) / kStepThreads);
+    uint32_t n_done = 0;   // particle-steps this thread executed (bench.py's unit: born AND active particles x steps)
     for (;;) {
         __syncthreads();
         if (threadIdx.x == 0) s_ticket = (uint32_t)atomicAdd((unsigned long long *)(A.ctrl + 16), 1ull);
@@ -305,7 +309,7 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
         bool valid;
         if (tile < t_old) {
             pos = (uint64_t)tile * kStepThreads + threadIdx.x;
-            valid = pos < A.n_perm;
+            valid = pos < n_list;
             l = valid ? A.perm[pos] : 0ull;
         } else {
             l = pos = first_new + (uint64_t)(tile - t_old) * kStepThreads + threadIdx.x;
@@ -341,7 +345,10 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             bool alive = true;
             const uint32_t step0 = (uint32_t)A.step0;
             for (int s = 0; s < A.m_steps; ++s)
-                if (alive & (s >= s_begin)) alive = step_once<K, DRY, BERN, EQ3, ZLEV, ZP>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, T);
+                if (alive & (s >= s_begin)) {
+                    alive = step_once<K, DRY, BERN, EQ3, ZLEV, ZP>(A, A.tab[s], step0 + (uint32_t)s, pid, x, y, z, q, acc, T);
+                    ++n_done;
+                }
             if (!alive) z = -1.0f - z;  // exit position kept, slot marked inactive
             A.xyzq[slot] = make_float4(x, y, z, q[0]);
             if (K > 1) A.q1[slot] = q[1];
@@ -371,6 +378,8 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
         }
     }
     flush_ledger<K>(A, acc);
+    n_done = __reduce_add_sync(0xffffffffu, n_done);
+    if ((threadIdx.x & 31) == 0 && n_done) atomicAdd((unsigned long long *)(A.ctrl + 3), (unsigned long long)n_done);
 }
 
 // ------------------------------------------------------------------ compacting kernel (a7)
@@ -535,7 +544,10 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
                 }
             }
         }
-        if (A.any_dep) dep_flush<K>(A, T);  // every thread's step is behind the barrier above
+        if (A.any_dep) {
+            if (A.holes) __syncthreads();   // the hole-list branch has no barrier of its own: every thread's deposits first
+            dep_flush<K>(A, T);             // (scan branch: every thread's step is behind the barriers above)
+        }
         __syncthreads();  // s_tile / s_woff / s_excl and the deposit table are reused by the next tile
     }
     flush_ledger<K>(A, acc);
@@ -663,7 +675,7 @@ cudaError_t launch_pair_repack(const float4 *s0, const float4 *s1, void *pair, i
         if (e != cudaSuccess) return e;
     }
     const uint64_t want = ((uint64_t)nx * ny * nz + 255) / 256;
-    pair_repack_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(s0, s1, (Texel2 *)pair, (uint32_t)nx, (uint32_t)ny, (uint32_t)nz,
+    pair_repack_kernel<<<(int)(want < sm_count() * 8 ? want : sm_count() * 8), 256, 0, st>>>(s0, s1, (Texel2 *)pair, (uint32_t)nx, (uint32_t)ny, (uint32_t)nz,
                                                                                 uvmax);
     return cudaGetLastError();
 }
@@ -682,7 +694,7 @@ __global__ void __launch_bounds__(256) transpose_kernel(const float4 *__restrict
 cudaError_t launch_transpose(const float4 *s0, float4 *out, int nx, int ny, int nz, cudaStream_t st)
 {
     const uint64_t want = ((uint64_t)nx * ny * nz + 255) / 256;
-    transpose_kernel<<<(int)(want < 148 * 8 ? want : 148 * 8), 256, 0, st>>>(s0, out, (uint32_t)nx, (uint32_t)ny, (uint32_t)nz);
+    transpose_kernel<<<(int)(want < sm_count() * 8 ? want : sm_count() * 8), 256, 0, st>>>(s0, out, (uint32_t)nx, (uint32_t)ny, (uint32_t)nz);
     return cudaGetLastError();
 }
 
@@ -776,7 +788,7 @@ cudaError_t launch_blend(const void *pair, float4 *out, uint64_t cells, int m, c
     for (int s = 0; s < kBlendDepth; ++s) B.a[s] = s < m ? a[s] : 0.0f;
     B.box = *box;
     const int tiles = ((box->nx + kMaskTile - 1) / kMaskTile) * ((box->ny + kMaskTile - 1) / kMaskTile);
-    blend_kernel<<<tiles * 4 < 148 * 8 ? tiles * 4 : 148 * 8, 256, 0, st>>>(B);
+    blend_kernel<<<tiles * 4 < sm_count() * 8 ? tiles * 4 : sm_count() * 8, 256, 0, st>>>(B);
     return cudaGetLastError();
 }
 
@@ -803,7 +815,7 @@ cudaError_t launch_blend_surface(const float4 *s0, const float4 *s1, float4 *out
     B.s0 = s0; B.s1 = s1; B.out = out; B.cells2 = cells2; B.m = m;
     for (int s = 0; s < kBlendDepth; ++s) B.a[s] = s < m ? a[s] : 0.0f;
     const uint64_t want = (cells2 + 255) / 256;
-    blend_surface_kernel<<<(int)(want < 148 * 8 ? (want ? want : 1) : 148 * 8), 256, 0, st>>>(B);
+    blend_surface_kernel<<<(int)(want < sm_count() * 8 ? (want ? want : 1) : sm_count() * 8), 256, 0, st>>>(B);
     return cudaGetLastError();
 }
 
@@ -813,7 +825,7 @@ cudaError_t launch_inject(const InjectArgs &a, cudaStream_t st)
     for (int r = 0; r < a.n_spec; ++r) mx = a.spec[r].count > mx ? a.spec[r].count : mx;
     int blocks = (int)((mx + 255) / 256);
     if (blocks < 1) blocks = 1;
-    if (blocks > 1184) blocks = 1184;
+    if (blocks > sm_count() * 8) blocks = sm_count() * 8;
     inject_kernel<<<blocks, 256, 0, st>>>(a);
     return cudaGetLastError();
 }

@@ -42,3 +42,11 @@ def custom(met_fn, *, grid=None, mgrid=None, nt=1, t0=0.0, dt_snap=3600.0, Kh=0.
 
 def uniform_met(u=0.0, v=0.0, w=0.0, kz=0.0):
     return lambda t, Z, Y, X: (u, v, w, kz)
+
+
+def gpu_state(sim):
+    """The CUDA path's particle state in activity units: the binding returns the stored fp32 q and the fp64 scale
+    G_k(t) (lpm_mass_scale, R8) separately; their product is formed here, on the test side."""
+    p = sim.get_particles_host()
+    p["m"] = p["q"] * p["scale"][:, None]
+    return p

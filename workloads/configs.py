@@ -5,6 +5,13 @@ grids, constants, sources and the closed-form meteorological fields, generated i
 float64 and rounded ONCE to float32.  That float32 array is the input of both the
 fp64 oracle and the CUDA path.  No method arithmetic lives here.
 
+Lateral boundary (R7): c1 and c2 are OPEN (their plumes stay inside the grid for the whole run).
+c3 and c4 are ABSORB, the paper's own rule (a particle that "reaches the predefined boundaries" becomes
+inactive): a 3-8 m/s wind whose direction swings +-45 degrees about a fixed mean carries a particle at least
+3 cos(45 deg) x 12 h = 92 km, typically 250 km, so no source position keeps the particles inside the 100 km box of
+BASELINE.json configs 3/4 for 12 or 24 h; what has left the box is inactive and is not counted as work.  The
+particle store of c3/c4 stays slot-addressed (no compaction: BASELINE.json asks for it in config 5 only).
+
 Paper scales used (citations are PAPER.md lines): dt ~ 10 s, Kx = Ky = 100 m^2/s
 (P:L77), Kz profile of Eq.(3) with Phi = 1, low point source,
 hours-long runs with 0.5 - several million particles.  The paper's own
@@ -254,7 +261,7 @@ def _c3(scale, h_dep=1000.0, name="c3"):
         name=name, cgrid=g, mgrid=g, nt=25, t0=0.0, dt_snap=HOUR, Kh=100.0, H_mix=1000.0, kz_min=1.0,
         nuclides=[Nuclide("I-131", T_HALF_I131, 1.0e-3, 1.0e-4),
                   Nuclide("Cs-137", T_HALF_CS137, 2.0e-3, 1.0e-4)],
-        dt=10.0, seed=3, capacity=n, boundary_mode="open", compact=False, h_dep=h_dep,
+        dt=10.0, seed=3, capacity=n, boundary_mode="absorb", compact=False, h_dep=h_dep,
         bin_every=360, n_steps=8640,
         release=Release(-4.0e4, 0.0, 50.0, 0.0, 24 * HOUR, [1.0e15, 1.0e14], n_particles=n),
         rain=RainBox(-3.0e4, 1.0e4, -2.0e4, 2.0e4, 6 * HOUR, 9 * HOUR), met_fn=_met_c3)
@@ -268,7 +275,7 @@ def _c4(scale):
         name="c4", cgrid=cg, mgrid=mg, nt=13, t0=0.0, dt_snap=HOUR, Kh=100.0, H_mix=1000.0, kz_min=1.0,
         nuclides=[Nuclide("I-131", T_HALF_I131, 1.0e-3, 1.0e-4),
                   Nuclide("Cs-137", T_HALF_CS137, 2.0e-3, 1.0e-4)],
-        dt=5.0, seed=4, capacity=n, boundary_mode="open", compact=False, h_dep=1000.0,
+        dt=5.0, seed=4, capacity=n, boundary_mode="absorb", compact=False, h_dep=1000.0,
         bin_every=720, n_steps=8640,
         release=Release(-4.0e4, 0.0, 50.0, 0.0, 12 * HOUR, [1.0e15, 1.0e14], n_particles=n),
         rain=RainBox(-3.0e4, 1.0e4, -2.0e4, 2.0e4, 6 * HOUR, 9 * HOUR), met_fn=_met_c3)
