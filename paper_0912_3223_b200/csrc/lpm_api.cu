@@ -4,6 +4,7 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+#include <stdlib.h>
 
 #include <new>
 #include <vector>
@@ -397,7 +398,8 @@ int do_bin(lpm_handle *h)
             if (B.q1) B.q1 = (const float *)(h->ws + h->L.q1) + r.base;
             B.n = n;
             B.perm = nullptr; B.n_list_dev = nullptr; B.n_list = 0; B.first_new = 0;
-            if (h->perm_valid && h->rel.size() == 1 && h->perm_n <= n) {   // the step kernel's met-cell-sorted list
+            static const bool walk_list = getenv("LPM_BIN_LIST") != nullptr;   // EXPERIMENT
+            if (walk_list && h->perm_valid && h->rel.size() == 1 && h->perm_n <= n) {   // the step kernel's met-cell-sorted list
                 B.perm = perm_half(h, h->perm_cur);
                 B.n_list = h->perm_n;
                 B.n_list_dev = (const uint64_t *)(h->ws + h->L.ctrl) + kCtrlLive + h->perm_cur;

@@ -6,6 +6,15 @@
 
 #include "../../include/lpm.h"
 
+// kernel formulation switches (round 2; all on: measured one by one on c4, profiles/r02_*): packed FFMA2 arithmetic,
+// MUFU.SQRT, 32-bit texel indices, direct-mapped deposit window
+#ifndef LPM_LEGACY_KERNEL
+#define LPM_FMA2 1
+#define LPM_SQRT_MUFU 1
+#define LPM_IDX32 1
+#define LPM_DEPWIN 1
+#endif
+
 namespace lpm {
 
 constexpr int kMaxFused = 16;        // model steps fused into one launch (table lives in kernel params)

@@ -39,6 +39,93 @@ struct Acc {  // per-thread ledger partial sums, in activity units before the pe
 constexpr int kDepSlots = 1024, kDepSlotBits = 10, kDepProbes = 8;
 static_assert(kStepThreads * kMaxFused <= 4096, "fixed-point deposit sums: 20 bits + 12 bits of count");
 
+#ifdef LPM_DEPWIN
+// Direct-mapped form of the table: the particles of a tile are spatial neighbours, so their deposits of one launch fall
+// into a window of kDepWin x kDepWin map cells around the tile; slot = (cj - wj0) * kDepWin + (ci - wi0), no tags, no
+// probing.  The window is centred on the map cell of the tile's first live particle (dep_window, once per tile); a deposit
+// outside it (a tile that straddles two rows of the sorted list, an unsorted small ensemble) takes the direct fp64 RED.
+constexpr int kDepWin = 32, kDepWinBits = 5;
+static_assert(kDepWin * kDepWin == kDepSlots, "window = table");
+template <int K>
+struct DepTab {
+    int32_t wi0, wj0, ref;
+    uint32_t sum[2 * K][kDepSlots];
+};
+
+template <int K>
+__device__ __forceinline__ void dep_clear(DepTab<K> &T)
+{
+    for (int i = threadIdx.x; i < kDepSlots; i += kStepThreads) {
+#pragma unroll
+        for (int k = 0; k < 2 * K; ++k) T.sum[k][i] = 0u;
+    }
+    if (threadIdx.x == 0) { T.ref = 0x7fffffff; T.wi0 = T.wj0 = 0; }
+}
+
+// all threads of the CTA, once per tile before its steps: `live` threads hold a particle at (x, y)
+template <int K>
+__device__ __forceinline__ void dep_window(const StepArgs &A, DepTab<K> &T, bool live, float x, float y)
+{
+    if (live) atomicMin(&T.ref, (int32_t)threadIdx.x);
+    __syncthreads();
+    if ((int32_t)threadIdx.x == T.ref) {
+        T.wi0 = __float2int_rd(__fmul_rn(__fsub_rn(x, A.cg.x0), A.cg.inv_dx)) - kDepWin / 2;
+        T.wj0 = __float2int_rd(__fmul_rn(__fsub_rn(y, A.cg.y0), A.cg.inv_dy)) - kDepWin / 2;
+    }
+    __syncthreads();
+}
+
+// all threads of the CTA; barriers on both sides belong to the caller
+template <int K>
+__device__ __forceinline__ void dep_flush(const StepArgs &A, DepTab<K> &T)
+{
+    const int wi0 = T.wi0, wj0 = T.wj0;
+    for (int i = threadIdx.x; i < kDepSlots; i += kStepThreads) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const uint32_t vd = T.sum[2 * k][i], vw = T.sum[2 * k + 1][i];
+            if (vd | vw) {
+                T.sum[2 * k][i] = 0u; T.sum[2 * k + 1][i] = 0u;
+                const uint32_t cell = (uint32_t)((wj0 + (i >> kDepWinBits)) * A.cg.nx + wi0 + (i & (kDepWin - 1)));
+                atomicAdd(A.dep + cell + k * A.dep_stride, (double)vd * A.dep_inv_scale[2 * k] + (double)vw * A.dep_inv_scale[2 * k + 1]);
+            }
+        }
+    }
+    if (threadIdx.x == 0) T.ref = 0x7fffffff;
+}
+
+template <int K>
+__device__ __forceinline__ void dep_add(const StepArgs &A, DepTab<K> &T, int slot, uint32_t cell, int k, int w, float v)
+{
+    const uint32_t iv = __float2uint_rn(v);  // saturating; v >= 0
+    if (slot >= 0 && iv - 131072u < 1048576u - 131072u) atomicAdd(&T.sum[w][slot], iv);   // 2^17 <= iv < 2^20: one unsigned compare
+    else if (v != 0.0f) atomicAdd(A.dep + cell + k * A.dep_stride, (double)v * A.dep_inv_scale[w]);
+}
+
+template <int K, bool WET>
+__device__ __forceinline__ void deposit_at(const StepArgs &A, const StepEntry &e, float x, float y, const float (&vd)[K], const float (&vw)[K],
+                                           Acc<K> &acc, DepTab<K> &T)
+{
+    const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
+    const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
+    if ((ci | cj) < 0) {  // off the map: ledger only
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            acc.off[k] += vd[k] * e.Oid[k];
+            if (WET) acc.off[k] += vw[k] * e.Oiw[k];
+        }
+        return;
+    }
+    const uint32_t cell = (uint32_t)(cj * A.cg.nx + ci);
+    const uint32_t di = (uint32_t)(ci - T.wi0), dj = (uint32_t)(cj - T.wj0);
+    const int slot = (di | dj) < (uint32_t)kDepWin ? (int)((dj << kDepWinBits) | di) : -1;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        dep_add<K>(A, T, slot, cell, k, 2 * k, vd[k]);
+        if (WET) dep_add<K>(A, T, slot, cell, k, 2 * k + 1, vw[k]);
+    }
+}
+#else
 // Dry and wet increments differ by orders of magnitude (p_dry ~ 5e-6, p_wet ~ 5e-4 per step), so each
 // has its own scale and its own sum: slot word 2k = dry, 2k + 1 = wet deposit of nuclide k.
 template <int K>
@@ -119,6 +206,8 @@ __device__ __forceinline__ void deposit_at(const StepArgs &A, const StepEntry &e
     }
 }
 
+#endif  // LPM_DEPWIN
+
 // One model step of one particle.  Returns false when the particle left the domain (ABSORB).
 // Source order = intended issue order: the eight gathers go out first and the ~150 instructions of
 // Philox + Box-Muller run while they are in flight.
@@ -128,9 +217,18 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
                                           float (&q)[K], Acc<K> &acc, DepTab<K> &dep)
 {
     // a0 + a2: weather at X_old, t_n
+#ifdef LPM_IDX32
+    Corner c = corner_of<ZLEV>(A.mg, x, y, z);
+    float dkz = 0.0f;  // drift-corrected walk (labelled departure): dKz/dz of the sampled field
+    const uint32_t o_cell = c.o;
+    c.o += e.buf * (uint32_t)A.snap_cells;   // texel index inside the whole set of blended buffers (< 2^32: lpm_create)
+    const float4 m = trilinear<ZP>(A.blend, c, A.mg, ZLEV && A.drift != 0, &dkz);
+    c.o = o_cell;
+#else
     const Corner c = corner_of<ZLEV>(A.mg, x, y, z);
     float dkz = 0.0f;  // drift-corrected walk (labelled departure): dKz/dz of the sampled field
     const float4 m = trilinear<ZP>(A.blend + (ZP ? 2ull : 1ull) * (uint64_t)e.buf * A.snap_cells, c, A.mg, ZLEV && A.drift != 0, &dkz);
+#endif
     // Kz: the interpolated gridded field (R4), or Eq.(3) per particle from the 2-D fields of this step (R12)
     const float kz = fmaxf(EQ3 ? kz_eq3(A.surf + (uint64_t)e.buf * (uint32_t)(A.mg.nx * A.mg.ny), c, A.mg, z) : m.w, A.kz_min);
 
@@ -339,6 +437,9 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
                 valid = z >= 0.0f;  // z < 0: exited earlier (ABSORB without compaction)
             }
         }
+#ifdef LPM_DEPWIN
+        if (A.any_dep) dep_window<K>(A, T, valid, x, y);
+#endif
         if (valid) {
             // the trip count is the same for every thread (uniform table index, uniform branches inside
             // the step); a particle born inside this launch or absorbed at the boundary skips steps
@@ -446,6 +547,9 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
                 pid[j] = A.pid[i];
             }
         }
+#ifdef LPM_DEPWIN
+        if (A.any_dep) dep_window<K>(A, T, (uint64_t)tile * kScanTile + threadIdx.x < n, x[0], y[0]);
+#endif
 #pragma unroll
         for (int j = 0; j < kItems; ++j) {
             const uint64_t i = (uint64_t)tile * kScanTile + (uint32_t)j * kStepThreads + threadIdx.x;

@@ -240,7 +240,8 @@ def _n_step_compare(g, p, w, frag, frac_required, label):
     an inactive particle is not compared: the oracle books it to the ledger and zeroes it, the store keeps the last q."""
     L = (w.cgrid.nx * w.cgrid.dx, w.cgrid.ny * w.cgrid.dy, w.cgrid.nz * w.cgrid.dz)
     ok = ~frag
-    np.testing.assert_array_equal(g["status"][ok], p["status"][ok])
+    if "status" in p:
+        np.testing.assert_array_equal(g["status"][ok], p["status"][ok])
     worst = 0.0
     good = np.ones(ok.sum(), dtype=bool)
     for key, Li in zip(("x", "y", "z"), L):
@@ -248,7 +249,7 @@ def _n_step_compare(g, p, w, frag, frac_required, label):
         tol = 1e-5 * np.maximum(Li, np.abs(p[key][ok]))
         good &= err <= tol
         worst = max(worst, float((err / tol).max()))
-    active = (p["status"] == 0)[ok]
+    active = (p["status"] == 0)[ok] if "status" in p else np.ones(ok.sum(), dtype=bool)   # (callers without it pass active particles only)
     rel = (np.abs(g["m"] - p["m"]) / np.maximum(p["m"], 1e-300))[:, ok]
     rel[:, ~active] = 0.0
     good &= (rel <= 1e-5).all(axis=0)
