@@ -12,6 +12,11 @@
 // The paper's kernel staged particle state in shared memory and sampled hardware textures
 // (P:L110-114); neither survives on B200: there is no reuse to stage, and texture filtering's
 // fixed-point weights cannot meet the 1e-5 parity bar.
+//
+// Bounding experiments (profiles/r02_*; NOT part of the product, results are wrong with either):
+//   nvcc ... -DLPM_BOUND_NO_DEPOSIT   the step without the deposit scatter a6 (the ledger is still kept)
+//   nvcc ... -DLPM_BOUND_NO_GATHER    the step with the eight met texels replaced by values made up in registers (no gathers)
+// build a library with one of them next to the product:  nvcc <flags of build.py> -D... -c csrc/lpm_step.cu, link with the other objects.
 #include "lpm_device.cuh"
 
 namespace lpm {
@@ -44,7 +49,7 @@ static_assert(kStepThreads * kMaxFused <= 4096, "fixed-point deposit sums: 20 bi
 // into a window of kDepWin x kDepWin map cells around the tile; slot = (cj - wj0) * kDepWin + (ci - wi0), no tags, no
 // probing.  The window is centred on the map cell of the tile's first live particle (dep_window, once per tile); a deposit
 // outside it (a tile that straddles two rows of the sorted list, an unsorted small ensemble) takes the direct fp64 RED.
-constexpr int kDepWin = 32, kDepWinBits = 5;
+constexpr int kDepWin = 32, kDepWinBits = 5, kDepSwz = 5;
 static_assert(kDepWin * kDepWin == kDepSlots, "window = table");
 template <int K>
 struct DepTab {
@@ -86,7 +91,8 @@ __device__ __forceinline__ void dep_flush(const StepArgs &A, DepTab<K> &T)
             const uint32_t vd = T.sum[2 * k][i], vw = T.sum[2 * k + 1][i];
             if (vd | vw) {
                 T.sum[2 * k][i] = 0u; T.sum[2 * k + 1][i] = 0u;
-                const uint32_t cell = (uint32_t)((wj0 + (i >> kDepWinBits)) * A.cg.nx + wi0 + (i & (kDepWin - 1)));
+                const int dj = i >> kDepWinBits, di = ((i & (kDepWin - 1)) - kDepSwz * dj) & (kDepWin - 1);   // undo the bank swizzle
+                const uint32_t cell = (uint32_t)((wj0 + dj) * A.cg.nx + wi0 + di);
                 atomicAdd(A.dep + cell + k * A.dep_stride, (double)vd * A.dep_inv_scale[2 * k] + (double)vw * A.dep_inv_scale[2 * k + 1]);
             }
         }
@@ -118,7 +124,10 @@ __device__ __forceinline__ void deposit_at(const StepArgs &A, const StepEntry &e
     }
     const uint32_t cell = (uint32_t)(cj * A.cg.nx + ci);
     const uint32_t di = (uint32_t)(ci - T.wi0), dj = (uint32_t)(cj - T.wj0);
-    const int slot = (di | dj) < (uint32_t)kDepWin ? (int)((dj << kDepWinBits) | di) : -1;
+    // slot = row dj, column (di + kDepSwz dj) mod 32: the shared-memory bank of a slot is its column, and the particles of
+    // a warp cover a block of a few x few map cells - unswizzled, the cells of one map column would share a bank and
+    // their atomics be served one after the other (ncu r02a: 8.8 wavefronts per ATOMS, 16 % of the L1 data pipe)
+    const int slot = (di | dj) < (uint32_t)kDepWin ? (int)((dj << kDepWinBits) | ((di + kDepSwz * dj) & (kDepWin - 1))) : -1;
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         dep_add<K>(A, T, slot, cell, k, 2 * k, vd[k]);
@@ -305,7 +314,9 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
             float vd[K];
 #pragma unroll
             for (int k = 0; k < K; ++k) vd[k] = q[k] * e.Gps[k];
+#ifndef LPM_BOUND_NO_DEPOSIT
             deposit_at<K, false>(A, e, x, y, vd, vd, acc, dep);
+#endif
         }
         return true;
     }
@@ -338,7 +349,9 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
     }
 
     // a6: deposit at the cell of the NEW (x, y)
+#ifndef LPM_BOUND_NO_DEPOSIT
     if (dry_here | wet_here) deposit_at<K, true>(A, e, x, y, vd, vw, acc, dep);
+#endif
     return true;
 }
 
