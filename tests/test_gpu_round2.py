@@ -1,0 +1,333 @@
+"""GPU parity tests added in round 2 (VERDICT r1 "close the parity holes"): end-to-end concentration
+fields, c5 on its own domain at 1/100 rate, checkpoint / restart with strided ids, the compact store's hole-list path
+with deposition, a release registered in mid-run, the looped bench restart, and the device-side unit counters."""
+import math
+
+import numpy as np
+import pytest
+
+from helpers import custom, gpu_state, uniform_met
+from workloads import Grid, Nuclide, RainBox, Release, make
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def lpm():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_0912_3223_b200.build import build
+    build()
+    import paper_0912_3223_b200 as m
+    return m
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import oracle
+    return oracle
+
+
+# ------------------------------------------------------------------ S§8(c) T3: end-to-end concentration fields
+def _conc_face_slack(p, g, K, delta):
+    """Activity of the oracle's active particles that sit within `delta` of a face of their concentration cell: it may
+    legitimately be binned into the neighbour across that face by a run whose positions differ by less than delta.
+    Returned per cell [K][nz][ny][nx] in activity units (own cell and every neighbour across the near faces)."""
+    act = p["status"] == 0
+    x, y, z = p["x"][act], p["y"][act], p["z"][act]
+    m = p["m"][:, act]
+    gx, gy, gz = (x - g.x0) / g.dx, (y - g.y0) / g.dy, (z - g.z0) / g.dz
+    ci, cj, ck = np.floor(gx).astype(np.int64), np.floor(gy).astype(np.int64), np.floor(gz).astype(np.int64)
+    offs = []
+    for c, gg, d in ((ci, gx, g.dx), (cj, gy, g.dy), (ck, gz, g.dz)):
+        f = gg - c
+        offs.append(((f * d < delta), ((1.0 - f) * d < delta)))
+    near = offs[0][0] | offs[0][1] | offs[1][0] | offs[1][1] | offs[2][0] | offs[2][1]
+    slack = np.zeros((K, g.nz, g.ny, g.nx))
+    idx = np.flatnonzero(near)
+    for dk in (-1, 0, 1):
+        for dj in (-1, 0, 1):
+            for di in (-1, 0, 1):
+                sel = np.ones(len(idx), dtype=bool)
+                for d, (lo, hi) in zip((di, dj, dk), offs):
+                    if d == -1:
+                        sel &= lo[idx]
+                    elif d == 1:
+                        sel &= hi[idx]
+                ii, jj, kk = ci[idx][sel] + di, cj[idx][sel] + dj, ck[idx][sel] + dk
+                ok = (ii >= 0) & (ii < g.nx) & (jj >= 0) & (jj < g.ny) & (kk >= 0) & (kk < g.nz)
+                for k in range(K):
+                    np.add.at(slack[k], (kk[ok], jj[ok], ii[ok]), m[k][idx][sel][ok])
+    return slack
+
+
+@pytest.mark.parametrize("name,scale,stride,steps,nt", [
+    ("c2", 0.1, 1, 1440, 3),            # the whole 2 h run, 1e5 particles
+    ("c3", 1.0, 10, 2520, 9),           # 7 h: dry deposition, the first hour of rain, particles leaving the domain
+    ("c4", 1.0, 20, 1440, 3),           # 2 h on the 1000 x 1000 x 30 grid of 100 m cells
+])
+def test_concentration_field_end_to_end(lpm, orc, name, scale, stride, steps, nt):
+    """The paper's own comparison (Fig. 4: relative difference per cell, poorly populated cells masked out):
+    after N steps the concentration field of the CUDA path equals the oracle's on every cell with count >= 100 to
+    1e-5 relative + face slack (activity of oracle particles within 1.5 m of a cell face: 1e-5 of the 100 km domain
+    is 1 m of position tolerance).  The 0.1 % of particles T3 lets outside the position band may sit in a wrong cell:
+    their total (missing in one cell, extra in another) stays below 2e-3 of the binned activity."""
+    w = make(name, scale=scale, n_steps=steps)
+    w.release.pid_stride = stride
+    n_local = len(range(0, w.release.n_particles, stride))
+    w = w.replace(nt=nt, capacity=n_local, bin_every=steps)
+    sim, o = lpm.Simulation(w), orc.OracleSim(w)
+    sim.step(steps)
+    o.step(steps)
+    g = w.cgrid
+    V = g.dx * g.dy * g.dz
+    cg, co = sim.concentration().cpu().numpy().astype(np.float64) * V, o.concentration() * V      # activity per cell
+    ng, no = sim.counts().cpu().numpy().astype(np.int64), o.counts().astype(np.int64)
+    slack = _conc_face_slack(o.particles(), g, w.K, 1.5)
+    big = no >= 100
+    assert big.sum() >= 10, big.sum()
+    tot_ok = 0
+    for k in range(w.K):
+        tol = 1e-5 * co[k] + 1.0001 * slack[k] + 3e-7 * co[k]                  # (+ the fp32 read-out of the CUDA path)
+        excess = np.maximum(np.abs(cg[k] - co[k]) - tol, 0.0)
+        assert excess[big].sum() <= 2e-3 * co[k][big].sum(), (k, excess[big].sum() / co[k][big].sum())
+        clean = big & (slack[k] == 0.0)
+        if clean.sum():
+            rel = np.abs(cg[k][clean] / co[k][clean] - 1.0)
+            tot_ok += int((rel <= 1.1e-5).sum())
+            assert (rel <= 1.1e-5).mean() >= 0.99, (k, rel.max())
+        rel_all = np.abs(cg[k][big] / co[k][big] - 1.0)
+        # the paper's figure of merit (~90 % of the cells differ by < 2.5 % on its hardware)
+        assert (rel_all < 0.025).mean() >= 0.999, (k, (rel_all < 0.025).mean())
+        assert abs(cg[k].sum() / co[k].sum() - 1.0) < 1e-5
+    # counts: equal except where a particle sits within the position tolerance of a face
+    assert abs(int(ng.sum()) - int(no.sum())) <= 2 + 1e-4 * no.sum()
+    assert np.abs(ng - no)[big].sum() <= 2e-3 * no[big].sum()
+    print(f"[conc e2e {name}] cells>=100: {big.sum()}, particles {no.sum()}, count L1 diff {np.abs(ng - no).sum()}")
+
+
+# ------------------------------------------------------------------ c5 on its OWN domain (S§8(d): 1/100-scale full-rate run)
+@pytest.mark.parametrize("gather_sort", [-1, 0])
+def test_c5_own_domain_hundredth_scale(lpm, orc, gather_sort):
+    """BASELINE.json config 5 on its own 500 x 500 x 25 grid of 200 m / 50 m cells at 1/100 of the rate and capacity
+    (400 particles per step, 5e5 slots: S§8(d)), through the capacity plateau (reached at step 1250: injection is
+    throttled to the exits from then on, highest ids skipped) and well into the phase in which particles leave the domain.
+    Both compaction forms: the stable look-back scan (gather_sort = -1) and the unordered hole-fill store with the
+    physical record sort (auto).  Compared with the oracle: the injected log, the set of live ids, the state of every
+    common id (T3), the ledger, the counts."""
+    from test_gpu_parity import _n_step_compare
+    steps = 6000
+    w = make("c5", scale=0.01, n_steps=steps).replace(nt=5)
+    assert int(round(w.release.rate * w.dt)) == 400 and w.capacity == 500_000
+    assert (w.cgrid.nx, w.cgrid.ny, w.cgrid.nz, w.cgrid.dx, w.cgrid.dz) == (500, 500, 25, 200.0, 50.0) and w.boundary_mode == "absorb" and w.compact
+    o = getattr(test_c5_own_domain_hundredth_scale, "_oracle", None)
+    if o is None:                                     # one oracle run serves both parametrisations (it takes about a minute)
+        o = orc.OracleSim(w)
+        o.step(steps)
+        test_c5_own_domain_hundredth_scale._oracle = o
+    sim = lpm.Simulation(w, gather_sort=gather_sort)
+    sim.step(steps)
+    inj_g = np.array([sim.injected(s) for s in range(0, steps, 7)] + [sim.injected(s) for s in range(1240, 1260)])
+    inj_o = np.array([o.injected(s) for s in range(0, steps, 7)] + [o.injected(s) for s in range(1240, 1260)])
+    gp, p = gpu_state(sim), o.particles()
+    frag = o.fragile_pids()
+    led_o = o.ledger()
+    n_exit = int(round(led_o[0][5] / (w.release.total_activity[0] / (400 * 21600)) / 0.9))     # rough number of exits so far
+    assert len(p["pid"]) <= 500_000 and led_o[0][5] > 0 and n_exit > 2000, (len(p["pid"]), n_exit)
+    assert sim.num_active == len(gp["pid"]) and len(np.unique(gp["pid"])) == len(gp["pid"])
+    # the throttle: full at step 1250 (400 x 1250), nothing injected while full, then as many as left
+    assert list(inj_g[-20:]) == list(inj_o[-20:]) and inj_o[-20:].sum() == 400 * 10
+    # at the plateau every step injects what the previous step's exits left free.  After thousands of steps in Kz of up to
+    # 200 m2/s the two position sets differ by centimetres (T3 allows a metre), so a particle may cross the boundary one
+    # step apart on the two sides: the injected counts of those two steps then differ by one each, with opposite signs
+    same = inj_g == inj_o
+    n_off = int((~same).sum())
+    assert same.mean() >= 0.9 and np.abs(inj_g.astype(np.int64) - inj_o.astype(np.int64)).max() <= 8, (same.mean(),)
+    assert sim.num_active == o.n == 500_000            # both sides sit at the capacity
+    if gather_sort < 0:
+        assert np.all(np.diff(gp["pid"].astype(np.int64)) > 0)          # stable form: ids strictly increasing
+    diff = np.setxor1d(gp["pid"], p["pid"])
+    # (the log was sampled every 7th step: about 7 n_off steps differ in all, each moving one exit and one injected id)
+    assert len(diff) <= 4 + 2 * len(frag) + 4 * 7 * n_off, (len(diff), len(frag), n_off)
+    common, gi, pi = np.intersect1d(gp["pid"], p["pid"], return_indices=True)
+    assert len(common) > 0.99 * len(p["pid"])
+    gg = {k: gp[k][gi] for k in ("x", "y", "z")}
+    gg["m"] = gp["m"][:, gi]
+    pp = {k: p[k][pi] for k in ("x", "y", "z")}
+    pp["m"] = p["m"][:, pi]
+    _n_step_compare(gg, pp, w, np.isin(common, frag), 0.999, f"c5 own domain, gather_sort={gather_sort}")
+    lg = sim.ledger()
+    assert abs(lg[0][0] / led_o[0][0] - 1) < 1e-4 and abs(lg[0][5] / led_o[0][5] - 1) < 2e-3
+    assert abs((lg[0][1] + lg[0][4] + lg[0][5]) / lg[0][0] - 1) < 1e-5
+    cg, co = sim.counts().cpu().numpy().astype(np.int64), o.counts().astype(np.int64)
+    assert abs(int(cg.sum()) - int(co.sum())) <= 4 + 2 * len(frag) + 4 * 7 * n_off and np.abs(cg - co).sum() <= 4e-3 * co.sum()
+
+
+# ------------------------------------------------------------------ checkpoint / restart keeps the particle ids
+def test_restart_from_checkpoint_strided_bitwise(lpm):
+    """lpm_get_particles reports the global ids (offset + l * stride) of a strided release and lpm_set_particles takes them
+    back: step, get, set, step equals the uninterrupted run bit for bit (Philox stays keyed by the real id)."""
+    w = make("c3", scale=1.0, n_steps=900)
+    w.release.pid_stride, w.release.pid_offset = 700, 3
+    n_local = len(range(3, w.release.n_particles, 700))
+    w = w.replace(nt=4, capacity=n_local, bin_every=0)
+    a = lpm.Simulation(w)
+    a.step(900)
+    ref = a.get_particles()
+    b = lpm.Simulation(w)
+    b.step(400)
+    ck = b.get_particles()
+    n = ck["n"]
+    np.testing.assert_array_equal(ck["pid"].cpu().numpy(), 3 + 700 * np.arange(n))
+    # a fresh handle continues from the checkpoint; the release must not run again, so only the particles born so far move on:
+    # compare them with the same slots of the uninterrupted run at a step where no newer particle matters
+    c = lpm.Simulation(w, auto_release=False)
+    c.set_particles(ck["xyzq"], ck["q1"], pid=ck["pid"], status=ck["status"], step_index=400)
+    c.step(500)
+    got = c.get_particles()
+    np.testing.assert_array_equal(got["pid"].cpu().numpy(), ck["pid"].cpu().numpy())
+    np.testing.assert_array_equal(got["xyzq"].cpu().numpy(), ref["xyzq"][:n].cpu().numpy())
+    np.testing.assert_array_equal(got["q1"].cpu().numpy(), ref["q1"][:n].cpu().numpy())
+    # ids that are not affine are refused on the slot-addressed store
+    bad = ck["pid"].clone()
+    bad[5] += 1
+    with pytest.raises(lpm.LpmError) as e:
+        c.set_particles(ck["xyzq"], ck["q1"], pid=bad, step_index=400)
+    assert e.value.status == -1
+
+
+# ------------------------------------------------------------------ hole-list compaction with deposition
+def test_compact_hole_list_with_deposition(lpm, orc):
+    """compact = 1 with the unordered (hole-list) store AND sinks that go through the CTA-private deposit table: the map
+    must hold exactly what the ledger says was deposited on it (a table flushed while other warps still deposit would
+    orphan increments), equal the stable-scan form, and match the oracle."""
+    w = make("c5", scale=2e-3, n_steps=700).replace(nt=3)
+    small = Grid(60, 60, 25, -4.6e4, -6.0e3, 0.0, 200.0, 200.0, 50.0)
+    w = w.replace(capacity=70_000, mgrid=small, cgrid=small, nuclides=[Nuclide("S", 8.02 * 86400.0, vd=0.02, lambda_wet=2.0e-4)],
+                  rain=RainBox(-4.4e4, -3.9e4, -3.0e3, 3.0e3, 200.0, 1200.0))
+    res = []
+    for gs in (8, -1):                                   # 8: hole list + record sort every 8 steps; -1: stable scan
+        sim = lpm.Simulation(w, gather_sort=gs)
+        sim.step(700)
+        led = sim.ledger()
+        dep = sim.deposition(f64=True).cpu().numpy()
+        on_map = led[0][2] + led[0][3] - led[0][6]
+        assert led[0][2] > 0 and led[0][3] > 0
+        assert abs(dep.sum() * 200.0 * 200.0 / on_map - 1) < 1e-6, (gs, dep.sum() * 4e4, on_map)
+        res.append((dep, led))
+    np.testing.assert_allclose(res[0][0], res[1][0], rtol=2e-5, atol=res[1][0].max() * 1e-9)
+    np.testing.assert_allclose(res[0][1], res[1][1], rtol=1e-6)
+    o = orc.OracleSim(w, face_delta=1.5)
+    o.step(700)
+    do, slack = o.deposition(with_slack=True)
+    excess = np.maximum(np.abs(res[0][0] - do) - (1e-5 * do + 1.0001 * slack + 1e-30), 0.0)
+    assert excess.sum() <= 2e-3 * do.sum()
+    lo = o.ledger()
+    for f in (2, 3, 4):
+        assert abs(res[0][1][0][f] / lo[0][f] - 1) < 5e-5, (f, res[0][1][0][f], lo[0][f])
+
+
+# ------------------------------------------------------------------ a release registered in mid-run
+@pytest.mark.parametrize("compact", [False, True])
+def test_release_registered_mid_run_far_from_the_plume(lpm, orc, compact):
+    """The met buffers are blended ahead for up to 16 steps and only for the columns the plume (and the registered
+    sources) can reach.  A second release registered between two lpm_step calls, starting inside the current blend
+    window and 30 km away from the plume, must still see the right weather: lpm_release invalidates the window."""
+    g = Grid(200, 200, 12, -5.0e4, -5.0e4, 0.0, 500.0, 500.0, 100.0)
+
+    def met(t, Z, Y, X):       # varies in space and time, so stale or unblended columns show up at once
+        return 3.0 + 2.0e-5 * X + t / 3600.0, -1.0 + 3.0e-5 * Y - 0.5 * t / 3600.0, 0.0, 5.0 + 0.01 * Z
+
+    first = Release(-3.0e4, -3.0e4, 50.0, 0.0, 2000.0, [1.0e9], n_particles=0 if compact else 4000, rate=2.0 if compact else 0.0)
+    w = custom(met, grid=g, nt=3, dt_snap=3600.0, n=0, dt=10.0, Kh=50.0, H=1000.0, kz_min=1.0, nuclides=[Nuclide("X", 8.02 * 86400.0)],
+               n_steps=300, boundary="absorb" if compact else "open", compact=compact, capacity=20_000)
+    w.release = None
+    # one step per launch in both stores, so that the blend-ahead window (16 steps) spans several lpm_step calls
+    sim = lpm.Simulation(w, steps_per_launch=1, auto_release=False)
+    o = orc.OracleSim(w)
+    sim.release(first)
+    o.release(first)
+    sim.step(37)                                         # the blend window now covers steps 32..47
+    o.step(37)
+    second = Release(2.0e4, 1.0e4, 80.0, 400.0, 1500.0, [2.0e9], n_particles=0 if compact else 3000, rate=3.0 if compact else 0.0,
+                     pid_offset=1_000_000 if compact else 0)    # (count mode: the offset selects a shard of the ids 0..N-1, so both releases use 0..)
+    sim.release(second)                                  # starts at step 40: inside the window, 64 km from the first source
+    o.release(second)
+    sim.step(163)
+    o.step(163)
+    gp, p = gpu_state(sim), o.particles()
+    # match by particle id (the slot-addressed store keeps one padded block of slots per release; unborn and padding slots report id 0)
+    valid = np.ones(len(gp["pid"]), dtype=bool)
+    if not compact:
+        valid = (gp["pid"] > 0) | (gp["x"] != 0.0)
+    # the two clouds stay 50 km apart (x < 0 and x > 0): that tells the releases apart where their ids coincide
+    key_g = gp["pid"][valid] + np.where(gp["x"][valid] > 0, 1 << 40, 0).astype(np.uint64)
+    key_o = p["pid"] + np.where(p["x"] > 0, 1 << 40, 0).astype(np.uint64)
+    common, gi, pi = np.intersect1d(key_g, key_o, return_indices=True)
+    gi = np.flatnonzero(valid)[gi]
+    assert len(common) == len(p["pid"]) > 500
+    assert (p["x"] > 0).sum() > 300
+    for key, L in (("x", 1.0e5), ("y", 1.0e5), ("z", 1200.0)):
+        err = np.abs(gp[key][gi].astype(np.float64) - p[key][pi])
+        assert (err <= 1e-5 * np.maximum(L, np.abs(p[key][pi]))).all(), (key, err.max())
+
+
+# ------------------------------------------------------------------ bench.py's loop: restart() = a fresh run
+def test_restart_equals_a_fresh_simulation(lpm):
+    w = make("c3", scale=2e-3, n_steps=400).replace(nt=3, bin_every=200)
+    a = lpm.Simulation(w)
+    a.step(400)
+    ref = (a.get_particles()["xyzq"].cpu().numpy().copy(), a.concentration().cpu().numpy().copy(), a.deposition(f64=True).cpu().numpy().copy(), a.ledger())
+    a.step(130)                                          # move on, then start again on the same workspace
+    a.restart()
+    assert a.step_index == 0 and a.num_active == 0
+    a.step(400)
+    np.testing.assert_array_equal(a.get_particles()["xyzq"].cpu().numpy(), ref[0])
+    # (the fp64 sums receive one RED per tile and cell: their order may change the last bit of the fp32 read-out)
+    np.testing.assert_allclose(a.concentration().cpu().numpy(), ref[1], rtol=1e-6, atol=0)
+    np.testing.assert_allclose(a.deposition(f64=True).cpu().numpy(), ref[2], rtol=1e-12)
+    np.testing.assert_allclose(a.ledger(), ref[3], rtol=1e-9)
+
+
+# ------------------------------------------------------------------ exited slots leave the sorted list; device-side unit counters
+def test_absorbed_slots_leave_the_sorted_list_and_the_unit_count(lpm, orc):
+    """Slot-addressed store with ABSORB (c3 / c4 since round 2): particles that left the domain are dropped from the
+    gather-locality list at the next sort and cost nothing afterwards.  The state is bit-identical with and without the
+    list, the step kernels' own count of executed particle-steps equals the oracle's count of active particle-steps, and the
+    binning kernel's count equals the number of active in-grid particles."""
+    w = make("c3", scale=1.0, n_steps=1200)
+    w.release.pid_stride = 250
+    small = Grid(48, 40, 30, -4.6e4, -5.0e3, 0.0, 250.0, 250.0, 40.0)       # 12 x 10 km around the source: exits from about step 150
+    w = w.replace(nt=3, capacity=len(range(0, w.release.n_particles, 250)), mgrid=small, cgrid=small, bin_every=400)
+    res = []
+    for gs in (16, -1):
+        sim = lpm.Simulation(w, gather_sort=gs)
+        sim.set_timing(True)
+        sim.step(1200)
+        t = sim.get_timing()
+        p = sim.get_particles()
+        res.append((p["xyzq"].cpu().numpy().copy(), p["status"].cpu().numpy().copy(), t, sim.counts().cpu().numpy().copy(), sim.ledger()))
+    np.testing.assert_array_equal(res[0][0], res[1][0])
+    np.testing.assert_array_equal(res[0][1], res[1][1])
+    np.testing.assert_array_equal(res[0][3], res[1][3])
+    assert res[0][2]["particle_steps"] == res[1][2]["particle_steps"]
+    assert (res[0][1] == 1).mean() > 0.3                                    # a good part of the ensemble has left
+    o = orc.OracleSim(w)
+    active_steps, binned = 0, 0
+    for s in range(1200):
+        st = o.particles()["status"] if o.n else np.zeros(0)
+        n_before = o.n
+        o.step(1)
+        # a particle counts for a step it was active in at the START of the step (newborn ones included)
+        born_now = o.n - n_before
+        active_steps += int((st == 0).sum()) + born_now
+        if (s + 1) % 400 == 0:
+            binned += int(o.counts().sum())
+    frag = len(o.fragile_pids())
+    assert abs(res[0][2]["particle_steps"] - active_steps) <= 2 * frag + 2, (res[0][2]["particle_steps"], active_steps, frag)
+    assert abs(res[0][2]["binned_particles"] - binned) <= 2 * frag + 6, (res[0][2]["binned_particles"], binned)
+    assert res[0][2]["born_particle_steps"] > 1.2 * res[0][2]["particle_steps"]   # the host's born count includes the ones that left
+    lo = o.ledger()
+    for k in range(2):
+        assert abs(res[0][4][k][5] / lo[k][5] - 1) < 5e-3                   # exited activity (fragile particles may differ)
+        assert abs(sum(res[0][4][k][1:6]) / res[0][4][k][0] - 1) < 1e-5
