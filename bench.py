@@ -196,7 +196,7 @@ class Looped:
     the config does not have.  Per-handle timing totals are carried over the restarts."""
 
     KEYS = ("step_ms", "step_launches", "bin_ms", "bin_launches", "particle_steps", "binned_particles", "sort_ms", "sort_launches",
-            "born_particle_steps")
+            "born_particle_steps", "bin_fused_launch_ms", "bin_fused_launches", "bin_fused_prev_launch_ms")
 
     def __init__(self, sim, n_int, on_restart=None):
         self.sim, self.n_int, self.i, self.on_restart = sim, n_int, 0, on_restart
@@ -332,6 +332,17 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     total_mass = float(conc_dev.sum().item())
     touched = sim.touched_cells                       # cells that hold a particle in the last binning (untimed)
+    # the stand-alone binning kernel (lpm_bin_now: what a caller gets outside the cadence) on the final state, untimed region
+    sim.set_timing(True)
+    sb0, sb1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sim.bin_now()
+    sb0.record()
+    for _ in range(3):
+        sim.bin_now()
+    sb1.record()
+    torch.cuda.synchronize()
+    standalone_ms = sb0.elapsed_time(sb1) / 3.0
+    standalone_n = sim.get_timing()["binned_particles"] / 4.0
     restarts = loop.restarts
     del loop
     del sim
@@ -452,28 +463,47 @@ def run_ours(args):
                            "frac": (4.0 if pairs else 8.0) * k_rate / probes["l1_gather_sectors_per_s"] if probes.get("l1_gather_sectors_per_s") else None,
                            "note": "upper bound of the sector count: lanes that share a texel share a sector"},
     }
-    # ---------------- binning (a8): particle bytes at HBM peak, or one atomic per touched cell and field ----------------
+    # ---------------- binning (a8) ----------------
+    # roofline of ANY binning design: the particle records at HBM peak (12 + 4 K bytes each) + the zeroing of the grids, or
+    # one RED per touched cell and field at the measured random-address RED rate over exactly that footprint
     bpp = 12 + 4 * w.K
-    n_bin = b_units / world                                   # particles the kernel binned (active, inside the grid)
-    n_bl = max(tim["bin_launches"], 1)
-    bin_bytes = bpp * n_bin
     grid_bytes = (4 + 8 * w.K) * g.nx * g.ny * g.nz
     red_rate = probes.get("red_f64_touched_footprint_per_s")
-    t_hbm = (bin_bytes + n_bl * grid_bytes) / (pk["hbm_gbs"] * 1e9)                    # particles read + grids zeroed
-    t_atom = n_bl * touched * (1 + w.K) / red_rate if red_rate else None              # every touched cell: one count + K sums
-    t_roof = max(t_hbm, t_atom) if t_atom else t_hbm
-    binning = {"kernel": "bin_tile_kernel", "gbs": bin_bytes / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else None,
-               "avg_ms": bin_ms / n_bl, "launches": tim["bin_launches"],
+
+    def bin_roof(n_particles, n_launches):
+        t_hbm = (bpp * n_particles + n_launches * grid_bytes) / (pk["hbm_gbs"] * 1e9)
+        t_atom = n_launches * touched * (1 + w.K) / red_rate if red_rate else None
+        return t_hbm, t_atom, (max(t_hbm, t_atom) if t_atom else t_hbm)
+
+    n_bin = b_units / world                                   # particles binned in the timed region (active, inside the grid)
+    fused_n = tim["bin_fused_launches"]
+    if fused_n:
+        # slot-addressed store: the step launch that ends an output interval bins its particles from registers; what that
+        # costs = (those launches) - (the launches right before them), + the memset of the grids (the timed "bin" span)
+        epi_ms = tim["bin_fused_launch_ms"] - tim["bin_fused_prev_launch_ms"]
+        measured_ms = max(epi_ms, 0.0) + bin_ms
+        t_hbm, t_atom, t_roof = bin_roof(n_bin, fused_n)
+        design = "fused into the step launch that ends each output interval (CTA-private table, one RED per touched cell, field and tile)"
+    else:
+        measured_ms = bin_ms
+        t_hbm, t_atom, t_roof = bin_roof(n_bin, max(tim["bin_launches"], 1))
+        design = "stand-alone bin_tile_kernel on the compact (physically sorted) store"
+    sa_hbm, sa_atom, sa_roof = bin_roof(standalone_n, 1)
+    binning = {"kernel": "step_slots_kernel epilogue (bin_tile)" if fused_n else "bin_tile_kernel", "design": design,
+               "gbs": bpp * n_bin / (measured_ms * 1e-3) / 1e9 if measured_ms > 0 else None,
+               "measured_ms": measured_ms, "launches": fused_n or tim["bin_launches"], "memset_ms": bin_ms if fused_n else None,
+               "epilogue_ms": epi_ms if fused_n else None,
                "bytes_per_particle": bpp, "particles": n_bin, "touched_cells_last_binning": touched,
-               "roofline": {"bound": "atomic" if t_atom and t_atom >= t_hbm else "hbm", "roof_ms": t_roof * 1e3, "measured_ms": bin_ms,
-                            "frac": t_roof * 1e3 / bin_ms if bin_ms > 0 else None,
-                            "hbm_ms": t_hbm * 1e3, "atomic_ms": t_atom * 1e3 if t_atom else None,
-                            "atomics_per_touched_cell": 1 + w.K,
+               "roofline": {"bound": "atomic" if t_atom and t_atom >= t_hbm else "hbm", "roof_ms": t_roof * 1e3, "measured_ms": measured_ms,
+                            "frac": t_roof * 1e3 / measured_ms if measured_ms > 0 else None,
+                            "hbm_ms": t_hbm * 1e3, "atomic_ms": t_atom * 1e3 if t_atom else None, "atomics_per_touched_cell": 1 + w.K,
                             "atomic_peak_per_s": red_rate, "atomic_peak_source": "lpm_probe red.global.add.f64, random addresses over "
                             "touched cells x (4 + 8 K) bytes (the footprint of the last binning, measured in this run)"},
-               "note": "span = one memset of the count and sum grids + the bin kernel; the roofline counts the particle records at "
-                       "12 + 4 K bytes (the kernel reads them through the step kernel's sorted slot list, 4 more bytes each), the "
-                       "zeroing of the grids, and one RED per touched cell and field (what a privatised design must at least issue)"}
+               "standalone": {"kernel": "bin_tile_kernel (lpm_bin_now on the final state, average of 3, outside the timed region)",
+                              "ms": standalone_ms, "particles": standalone_n, "gbs": bpp * standalone_n / (standalone_ms * 1e-3) / 1e9,
+                              "roof_ms": sa_roof * 1e3, "frac": sa_roof * 1e3 / standalone_ms if standalone_ms > 0 else None},
+               "note": "fused: measured = sum over the intervals of (step launch with the epilogue - the step launch before it) + the "
+                       "memset of the grids; the two launches differ by 16 steps of births (< 0.1 % of the population)"}
 
     # ---------------- cpu baseline (oracle, bounded sample) ----------------
     cpu = None

@@ -189,7 +189,8 @@ int32_t lpm_release(lpm_handle *h, const lpm_source *src, const double *total_ac
                     uint64_t pid_stride);
 
 /* Advance n_steps model steps.  Every params.bin_every-th step the concentration
- * grid is re-binned from the particle state. */
+ * grid is re-binned from the particle state: on the slot-addressed store by the step launch that ends on that
+ * step, while the particles are still in registers; on the compact store by the stand-alone binning kernel. */
 int32_t lpm_step(lpm_handle *h, int32_t n_steps);
 
 /* ---- outputs -------------------------------------------------------------------------------- */
@@ -278,7 +279,10 @@ int32_t lpm_set_timing(lpm_handle *h, int32_t enable);
  * [6] = total ms in gather-locality sort passes, [7] = their count,
  * [8] = born particles x steps of the timed step launches (host count of the release schedule R9: the same as [4]
  *       while no particle has become inactive; slot-addressed store only, 0 with compact = 1),
- * [9..11] reserved (0); accumulated since lpm_set_timing. */
+ * [9]  = total ms of the step launches that carried the fused binning epilogue (slot-addressed store: the launch that
+ *        ends on a binning step bins its particles itself; these launches are also part of [0] and [1]),
+ * [10] = their count, [11] = total ms of the step launches directly before them (same population to within 16 steps
+ *        of births: [9] - [11] estimates what the epilogues cost); accumulated since lpm_set_timing. */
 int32_t lpm_get_timing(lpm_handle *h, double *out_host /* [12] */);
 /* Number of concentration cells that hold at least one particle in the current binning (the footprint the binning
  * atomics spread over: bench.py measures its atomic peak over exactly that many cells).  Synchronises.

@@ -163,12 +163,14 @@ struct lpm_handle {
     uint64_t launches;
     // timing hooks: event pairs around step / binning launches
     bool timing;
-    struct Span { cudaEvent_t a, b; int kind; };
+    struct Span { cudaEvent_t a, b; int kind; bool pre; };   // pre: the step launch right before one with the binning epilogue
     std::vector<Span> spans;
     std::vector<cudaEvent_t> ev_pool;
-    double t_ms[3], t_units[3];
+    double t_ms[5], t_units[5];   // kinds: 0 step launches, 1 binning (memset + stand-alone kernel), 2 sorts, 3 step launches with the fused
+                                  // binning epilogue (also counted in 0), 4 the step launches right before those (also in 0)
+    int last_step_span;           // index into spans of the latest kind-0 span, -1 = none
     uint64_t t_base, t_base_bin;  // device counters (particle-steps executed, particles binned) at lpm_set_timing
-    uint64_t t_launches[3];
+    uint64_t t_launches[5];
     int sticky;
     char err[512];
 };
@@ -208,16 +210,20 @@ cudaEvent_t ev_get(lpm_handle *h)
 int span_open(lpm_handle *h, int kind, double units)
 {
     if (!h->timing) return -1;
-    lpm_handle::Span sp{ev_get(h), ev_get(h), kind};
+    lpm_handle::Span sp{ev_get(h), ev_get(h), kind, false};
     if (!sp.a || !sp.b) {   // no event to be had: this launch goes untimed (its units are not counted either)
         if (sp.a) h->ev_pool.push_back(sp.a);
         if (sp.b) h->ev_pool.push_back(sp.b);
         return -1;
     }
     cudaEventRecord(sp.a, h->st);
+    if (kind == 3 && h->last_step_span >= 0 && h->last_step_span < (int)h->spans.size()) h->spans[h->last_step_span].pre = true;
     h->spans.push_back(sp);
     h->t_units[kind] += units;
     h->t_launches[kind]++;
+    if (kind == 3) { h->t_units[0] += units; h->t_launches[0]++; }
+    if (kind == 0) h->last_step_span = (int)h->spans.size() - 1;   // (sort and memset spans in between do not matter)
+    if (kind == 3) h->last_step_span = -1;
     return (int)h->spans.size() - 1;
 }
 void span_close(lpm_handle *h, int id)
@@ -228,11 +234,16 @@ void spans_collect(lpm_handle *h)
 {
     for (auto &sp : h->spans) {
         float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) h->t_ms[sp.kind] += (double)ms;
+        if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) {
+            h->t_ms[sp.kind] += (double)ms;
+            if (sp.kind == 3) h->t_ms[0] += (double)ms;
+            if (sp.pre) { h->t_ms[4] += (double)ms; h->t_launches[4]++; }
+        }
         h->ev_pool.push_back(sp.a);
         h->ev_pool.push_back(sp.b);
     }
     h->spans.clear();
+    h->last_step_span = -1;
 }
 
 double G_of(const lpm_handle *h, int k, uint64_t step) { return exp((double)step * h->ln_rho[k]); }
@@ -360,6 +371,21 @@ constexpr int kCtrlSteps = 3, kCtrlLive = 17, kCtrlBinned = 19, kCtrlTouched = 2
 
 uint32_t *perm_half(const lpm_handle *h, int half) { return (uint32_t *)(h->ws + h->L.perm) + (uint64_t)half * (up(4 * h->prm.capacity) / 4); }
 
+// fixed-point scale of the CTA-private concentration sums: largest power of two S with q_max S < 2^20, where the
+// largest stored q is bounded by dep_bound / G(now) (q = activity / G(t), and a particle never gains activity)
+void bin_scales(const lpm_handle *h, uint64_t step, float *scale, double *inv_scale)
+{
+    for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) {
+        const double qmax = k < h->K ? h->dep_bound[k] / G_of(h, k, step) : 0.0;
+        int e = 0;
+        if (qmax > 0.0) { frexp(1048576.0 / qmax, &e); e -= 1; }
+        if (e > 100) e = 100;
+        if (e < -100) e = -100;
+        scale[k] = (float)ldexp(1.0, e);
+        inv_scale[k] = ldexp(1.0, -e);
+    }
+}
+
 int do_bin(lpm_handle *h)
 {
     const uint64_t cells3 = (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz;
@@ -374,16 +400,7 @@ int do_bin(lpm_handle *h)
     B.cells3 = cells3;
     B.K = h->K;
     B.n_binned = (uint64_t *)(h->ws + h->L.ctrl) + kCtrlBinned;
-    for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) {
-        // largest stored q: q = activity / G(t) and a particle never gains activity, so q <= dep_bound / G(now)
-        const double qmax = k < h->K ? h->dep_bound[k] / G_of(h, k, h->step) : 0.0;
-        int e = 0;
-        if (qmax > 0.0) { frexp(1048576.0 / qmax, &e); e -= 1; }
-        if (e > 100) e = 100;
-        if (e < -100) e = -100;
-        B.scale[k] = (float)ldexp(1.0, e);
-        B.inv_scale[k] = ldexp(1.0, -e);
-    }
+    bin_scales(h, h->step, B.scale, B.inv_scale);
     const int max_blocks = h->sms * 6;
     if (h->prm.compact) {
         B.xyzq = (const float4 *)(h->ws + h->L.xyzq);
@@ -568,6 +585,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     h->sms = prop.multiProcessorCount;
     h->err[0] = 0;
     h->pair_snap = -1;
+    h->last_step_span = -1;
     // R5 / R8 constants: double formula, rounded once to fp32 where the kernels consume fp32
     h->sigma_h = (float)sqrt(2.0 * met->Kh * p->dt);
     {
@@ -683,6 +701,7 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
     base_args(h, A);
     int64_t left = n_steps;
     while (left > 0) {
+        bool fused_bin = false;
         int m = (int)(left < m_max ? left : m_max);
         if (h->prm.bin_every > 0) {
             const uint64_t to_bin = (uint64_t)h->prm.bin_every - h->step % (uint64_t)h->prm.bin_every;
@@ -782,6 +801,19 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
             span_close(h, span);
             h->launches += 2;
         } else {
+            // a8 fused: a launch that ends on a binning step bins its particles itself (lpm_step.cu: bin_tile)
+            fused_bin = h->prm.bin_every > 0 && (h->step + (uint64_t)m) % (uint64_t)h->prm.bin_every == 0;
+            A.bin_cnt = nullptr;
+            if (fused_bin) {
+                const uint64_t cells3 = (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz;
+                const int bspan = span_open(h, 1, 0.0);
+                CK(cudaMemsetAsync(h->ws + h->L.cnt, 0, (h->L.conc - h->L.cnt) + 8 * cells3 * h->K, h->st));
+                span_close(h, bspan);
+                A.bin_cnt = (uint32_t *)(h->ws + h->L.cnt);
+                A.bin_conc = (double *)(h->ws + h->L.conc);
+                A.bin_cells3 = cells3;
+                bin_scales(h, h->step + (uint64_t)m, A.bin_scale, A.bin_inv_scale);
+            }
             for (const Release &r : h->rel) {
                 const uint64_t n = born_local(r, (int64_t)h->step + m - 1);
                 if (!n) continue;
@@ -848,7 +880,7 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
                     }
                 }
                 CK(cudaMemsetAsync(A.ctrl + 16, 0, 8, h->st));  // tile ticket of the slot kernel
-                const int span = span_open(h, 0, units);
+                const int span = span_open(h, fused_bin ? 3 : 0, units);
                 CK(launch_step(A, h->K, false, grid_blocks(h, n), h->st));
                 span_close(h, span);
                 h->launches++;
@@ -857,8 +889,8 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
         h->step += (uint64_t)m;
         left -= m;
         if (h->prm.bin_every > 0 && h->step % (uint64_t)h->prm.bin_every == 0) {
-            const int rc = do_bin(h);
-            if (rc) return rc;
+            if (fused_bin) { h->bin_step = h->step; h->binned = true; }
+            else { const int rc = do_bin(h); if (rc) return rc; }
             if (h->prm.dose) {
                 // P:L108 / Fig. 2b "time integrated dosage": concentration of this binning x the interval it stands for
                 const double T = (double)h->prm.bin_every * h->prm.dt, V = h->cg.dx * h->cg.dy * h->cg.dz;
@@ -1180,7 +1212,7 @@ int32_t lpm_set_timing(lpm_handle *h, int32_t enable)
     CK(cudaStreamSynchronize(h->st));
     spans_collect(h);
     h->timing = enable != 0;
-    for (int i = 0; i < 3; ++i) { h->t_ms[i] = 0.0; h->t_units[i] = 0.0; h->t_launches[i] = 0; }
+    for (int i = 0; i < 5; ++i) { h->t_ms[i] = 0.0; h->t_units[i] = 0.0; h->t_launches[i] = 0; }
     CK(cudaMemcpyAsync(&h->t_base, (uint64_t *)(h->ws + h->L.ctrl) + kCtrlSteps, 8, cudaMemcpyDeviceToHost, h->st));
     CK(cudaMemcpyAsync(&h->t_base_bin, (uint64_t *)(h->ws + h->L.ctrl) + kCtrlBinned, 8, cudaMemcpyDeviceToHost, h->st));
     CK(cudaStreamSynchronize(h->st));
@@ -1196,6 +1228,7 @@ int32_t lpm_get_timing(lpm_handle *h, double *out)
     out[2] = h->t_ms[1]; out[3] = (double)h->t_launches[1];
     out[4] = h->t_units[0]; out[5] = h->t_units[1];
     out[6] = h->t_ms[2]; out[7] = (double)h->t_launches[2];
+    out[9] = h->t_ms[3]; out[10] = (double)h->t_launches[3]; out[11] = h->t_ms[4];
     out[8] = h->t_units[0];   // born particles x steps (host count, R9): includes particles that have left the domain
     // what the kernels counted themselves: particle-steps executed (born AND active), particles binned (active, in the grid)
     uint64_t now[2] = {0, 0};

@@ -81,6 +81,12 @@ struct StepArgs {
     int32_t zpair, keys_by_slot;             // the blended buffers hold z-pair texels (32 B: both z corners), B8; fused sort keys indexed by slot, not by list position
     int32_t eq3, drift;                      // kz_mode 1: Kz from Eq.(3) per particle; drift: + dKz/dz dt (departure from the paper)
     int32_t any_dep, bern;                   // some sink deposits through the tables; dep_mode 1: Bernoulli deposition (R11)
+    // a8 fused: non-null when this launch ends on a binning step: count grid, sum grids [K][cells3], fixed-point scales
+    uint32_t *bin_cnt;
+    double *bin_conc;
+    uint64_t bin_cells3;
+    float bin_scale[LPM_MAX_NUCLIDES];
+    double bin_inv_scale[LPM_MAX_NUCLIDES];
     // physics
     float dt, sigma_h, kz_min, H, h_dep;
     int32_t dry_mode, absorb;

@@ -379,6 +379,82 @@ __device__ __forceinline__ void flush_ledger(const StepArgs &A, const Acc<K> &ac
     }
 }
 
+// a8 fused into the step (round 2): the launch that ends on a binning step bins its particles while they are still in
+// registers - no second pass over the particle store (the stand-alone bin_tile_kernel of lpm_bin.cu reads 12 + 4 K bytes per
+// particle again and, walking the store in slot order, finds few particles of a tile in the same cell).  Here the 256
+// particles of a tile are spatial neighbours (gather-locality order), so their counts and fixed-point sums meet in a
+// CTA-private open-addressing table keyed by the concentration cell - the same table, and the same shared memory, as the
+// deposit table, which is idle once the tile's steps are done - and every touched cell receives one RED per field.
+constexpr int kBinTabSlots = 1024, kBinTabBits = 10, kBinTabProbes = 8;
+template <int K>
+struct BinTabS {
+    uint32_t tag[kBinTabSlots];      // cell + 1, 0 = empty
+    uint32_t cnt[kBinTabSlots];
+    uint32_t sum[K][kBinTabSlots];   // rint(q * S_k), S_k = StepArgs::bin_scale
+};
+template <int K>
+union TileTab {
+    DepTab<K> dep;
+    BinTabS<K> bin;
+};
+
+// all threads of the CTA, after the tile's steps and the flush of its deposit table; `live`: this thread holds an active
+// particle at (x, y, z) carrying q.  Leaves the shared memory zeroed (= an empty deposit table).
+template <int K>
+__device__ __forceinline__ uint32_t bin_tile(const StepArgs &A, BinTabS<K> &B, bool live, float x, float y, float z, const float (&q)[K])
+{
+    __syncthreads();                                   // the deposit table has been flushed: all words are zero ...
+    if (threadIdx.x < 4) B.tag[threadIdx.x] = 0u;      // ... except the window header that overlays the first tags
+    __syncthreads();
+    uint32_t binned = 0;
+    if (live) {
+        const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
+        const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
+        const int ck = cell_of(z, A.cg.z0, A.cg.inv_dz, A.cg.nz);
+        if ((ci | cj | ck) >= 0) {
+            binned = 1;
+            const uint32_t cell = (uint32_t)((ck * A.cg.ny + cj) * A.cg.nx + ci), key = cell + 1u;
+            uint32_t h = (key * 0x9E3779B1u) >> (32 - kBinTabBits);
+            int s = -1;
+#pragma unroll 1
+            for (int pr = 0; pr < kBinTabProbes; ++pr) {
+                const uint32_t t = *(volatile uint32_t *)&B.tag[h];
+                if (t == key) { s = (int)h; break; }
+                if (t == 0u) {
+                    const uint32_t old = atomicCAS(&B.tag[h], 0u, key);
+                    if (old == 0u || old == key) { s = (int)h; break; }
+                }
+                h = (h + 1u) & (kBinTabSlots - 1);
+            }
+            if (s >= 0) atomicAdd(&B.cnt[s], 1u);
+            else atomicAdd(A.bin_cnt + cell, 1u);
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                const uint32_t iv = __float2uint_rn(q[k] * A.bin_scale[k]);   // saturating; q >= 0
+                if (s >= 0 && iv - 131072u < 1048576u - 131072u) atomicAdd(&B.sum[k][s], iv);
+                else if (q[k] != 0.0f) atomicAdd(A.bin_conc + (uint64_t)k * A.bin_cells3 + cell, (double)q[k]);
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < kBinTabSlots; i += kStepThreads) {
+        const uint32_t key = B.tag[i];
+        if (key == 0u) continue;
+        B.tag[i] = 0u;
+        const uint32_t c = B.cnt[i];
+        B.cnt[i] = 0u;
+        atomicAdd(A.bin_cnt + (key - 1u), c);
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const uint32_t v = B.sum[k][i];
+            B.sum[k][i] = 0u;
+            if (v) atomicAdd(A.bin_conc + (uint64_t)k * A.bin_cells3 + (key - 1u), (double)v * A.bin_inv_scale[k]);
+        }
+    }
+    __syncthreads();
+    return binned;
+}
+
 // ------------------------------------------------------------------ slot-addressed kernel
 // Particles of one release occupy the slots base + [0, n); slot l carries global particle id
 // pid_offset + l * pid_stride, so ids (and birth steps, R9) are implied by the slot.  Persistent
@@ -401,8 +477,12 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
     // younger slots in id order (still close to the source).  The CTAs resident together therefore
     // work on one small region of the plume: their met gathers hit L1/L2, and their deposits meet
     // in the CTA-private tables below instead of in the global map.
-    __shared__ DepTab<K> T;
+    __shared__ TileTab<K> U;
+    DepTab<K> &T = U.dep;
+    for (int i = threadIdx.x; i < (int)(sizeof(U) / 4); i += kStepThreads) ((uint32_t *)&U)[i] = 0u;
+    __syncthreads();
     dep_clear<K>(T);
+    uint32_t n_binned = 0;
     // (slots that had left the domain when the list was built are not on it: its live length is a device scalar)
     uint64_t n_list = A.perm ? A.n_perm : 0ull;
     if (A.perm && A.n_live) { const uint64_t d = *A.n_live; n_list = d < n_list ? d : n_list; }
@@ -490,8 +570,16 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             __syncthreads();
             dep_flush<K>(A, T);
         }
+        if (A.bin_cnt) {   // this launch ends on a binning step (a8 fused)
+            n_binned += bin_tile<K>(A, U.bin, valid && z >= 0.0f, x, y, z, q);
+            dep_clear<K>(T);                           // window header of the deposit table (the sums are zero again)
+        }
     }
     flush_ledger<K>(A, acc);
+    if (A.bin_cnt) {
+        n_binned = __reduce_add_sync(0xffffffffu, n_binned);
+        if ((threadIdx.x & 31) == 0 && n_binned) atomicAdd((unsigned long long *)(A.ctrl + 19), (unsigned long long)n_binned);
+    }
     n_done = __reduce_add_sync(0xffffffffu, n_done);
     if ((threadIdx.x & 31) == 0 && n_done) atomicAdd((unsigned long long *)(A.ctrl + 3), (unsigned long long)n_done);
 }
