@@ -191,8 +191,7 @@ def oracle_leg(name: str, scale: float, interval: int, warmup: int, steps: int, 
 # ------------------------------------------------------------------ the CUDA arm
 class Looped:
     """The workload as a loop of its own output intervals: bench step i is interval (i mod n_int) of the config, and
-    every wrap starts the run again from step 0 (lpm_destroy + lpm_create on the same workspace, inside the timed
-    region), so that ANY --steps / --warmup stays on BASELINE.json's configuration: the run never simulates an hour
+    every wrap starts the run again from step 0 (lpm_restart on the same handle, inside the timed region), so that ANY --steps / --warmup stays on BASELINE.json's configuration: the run never simulates an hour
     the config does not have.  Per-handle timing totals are carried over the restarts."""
 
     KEYS = ("step_ms", "step_launches", "bin_ms", "bin_launches", "particle_steps", "binned_particles", "sort_ms", "sort_launches",

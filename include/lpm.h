@@ -94,8 +94,9 @@ typedef struct {
                              * is unordered (re-sorted by met cell) and holes are filled from the tail */
     double h_dep;           /* dry deposition acts where z' < h_dep; h_dep >= H_mix: everywhere */
     int32_t bin_every;      /* concentration binning cadence in steps ("n"); 0 = never   */
-    int32_t steps_per_launch; /* 0 = auto (16); 1 = one model step per kernel launch; m > 1 fuses up to
-                               * min(m, 16) steps per launch with the particle state in registers */
+    int32_t steps_per_launch; /* 0 = auto (16; 64 with a single met snapshot and no deposition: small runs are
+                               * launch-latency-bound); 1 = one model step per kernel launch; m > 1 fuses up to
+                               * min(m, 16 or 64) steps per launch with the particle state in registers */
     int32_t gather_sort;      /* gather-locality pass (slots listed in the order of the lower-corner met
                                * cell of their trilinear stencil): 0 = auto (from 65536 particles, every
                                * 32 to 64 steps: about the time the horizontal walk needs to cross a met
@@ -170,6 +171,13 @@ int32_t lpm_create(const lpm_grid *conc_grid, const lpm_meteo *meteo, const lpm_
                    uint64_t workspace_bytes, void *cuda_stream, lpm_handle **out);
 
 int32_t lpm_destroy(lpm_handle *h);
+
+/* Start the same run again from step 0 on the same handle: the registered releases, the rain box, the grids' geometry and
+ * the meteorology stay; the step index, the output grids, the deposition map, the ledger, the injected log and every
+ * cached list / blended met buffer are cleared (asynchronously; the particle store needs no clearing: a slot is
+ * initialised when its particle is born).  The results of the second run equal those of the first.
+ * Errors: STATE (the particle state was installed by lpm_set_particles: there is no release to start again), CUDA. */
+int32_t lpm_restart(lpm_handle *h);
 
 /* Axis-aligned rain box over the full column, active for t_start <= t_n < t_end, tested at the
  * start of the step ("wet deposition only occurs in case of precipitation"; G6). */

@@ -28,7 +28,7 @@ SYMBOLS = (
     "lpm_set_particles", "lpm_ledger", "lpm_injected", "lpm_last_error", "lpm_launch_count", "lpm_test_philox",
     "lpm_test_normals", "lpm_test_sample", "lpm_upload_meteo", "lpm_concentration_host", "lpm_deposition_host",
     "lpm_set_timing", "lpm_get_timing", "lpm_probe", "lpm_test_box_muller", "lpm_dose", "lpm_test_curand_philox",
-    "lpm_texel_pairs", "lpm_touched_cells",
+    "lpm_texel_pairs", "lpm_touched_cells", "lpm_restart",
 )
 
 
@@ -84,6 +84,7 @@ def load():
     L.lpm_create.argtypes = [C.POINTER(lpm_grid), C.POINTER(lpm_meteo), C.POINTER(lpm_nuclide), i32,
                              C.POINTER(lpm_params), vp, u64, vp, C.POINTER(vp)]
     L.lpm_destroy.argtypes = [vp]
+    L.lpm_restart.argtypes = [vp]
     L.lpm_set_rain.argtypes = [vp, dbl, dbl, dbl, dbl, dbl, dbl]
     L.lpm_release.argtypes = [vp, C.POINTER(lpm_source), C.POINTER(dbl), u64, dbl, u64, u64]
     L.lpm_step.argtypes = [vp, i32]
@@ -235,9 +236,8 @@ class Simulation:
             self.release(w.release)
 
     def restart(self):
-        """Start the same run again from step 0: lpm_destroy + lpm_create on the same workspace and met array."""
-        self.close()
-        self._create()
+        """lpm_restart: the same run again from step 0 on the same handle."""
+        self._ck(self._L.lpm_restart(self._h), "lpm_restart")
 
     # ------------------------------------------------------------------ plumbing
     def _ck(self, rc, where):

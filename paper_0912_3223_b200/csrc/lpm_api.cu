@@ -564,9 +564,11 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
         return LPM_ERR_INVALID_ARG;
     int ndev = 0, dev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return LPM_ERR_NO_DEVICE;
-    cudaDeviceProp prop;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return LPM_ERR_NO_DEVICE;
-    if (prop.major != 10) return LPM_ERR_NO_DEVICE;
+    // (attributes, not cudaGetDeviceProperties: that call takes milliseconds, and bench.py re-creates the handle at every wrap of a looped config)
+    int cc_major = 0, n_sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&n_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return LPM_ERR_NO_DEVICE;
+    if (cc_major != 10) return LPM_ERR_NO_DEVICE;
 
     const Layout L = make_layout(*cg, *met, p->capacity, K, p->compact != 0, sort_enabled(p), p->dose != 0, zpair_enabled(met, p));
     if (ws_bytes < L.total) return LPM_ERR_WORKSPACE_TOO_SMALL;
@@ -582,7 +584,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     h->st = (cudaStream_t)stream;
     h->ws = (char *)ws;
     h->L = L;
-    h->sms = prop.multiProcessorCount;
+    h->sms = n_sms;
     h->err[0] = 0;
     h->pair_snap = -1;
     h->last_step_span = -1;
@@ -627,6 +629,29 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     if (cudaMemsetAsync(ws, 0, L.total, h->st) != cudaSuccess) { delete h; return LPM_ERR_CUDA; }
     h->launches++;
     *out = h;
+    return LPM_OK;
+}
+
+int32_t lpm_restart(lpm_handle *h)
+{
+    if (!h) return LPM_ERR_INVALID_ARG;
+    if (h->sticky) return h->sticky;
+    for (const Release &r : h->rel) if (r.fixed) return fail(h, LPM_ERR_STATE, "lpm_restart: the state was installed by lpm_set_particles, there is no release to start again");
+    // everything that accumulates or counts; the particle store needs no clearing (a slot is initialised when its particle is born)
+    const uint64_t cells3 = (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz, cells2 = (uint64_t)h->cg.nx * h->cg.ny;
+    const Layout &L = h->L;
+    CK(cudaMemsetAsync(h->ws + L.cnt, 0, (L.conc - L.cnt) + 8 * cells3 * h->K, h->st));
+    CK(cudaMemsetAsync(h->ws + L.dep, 0, 8 * cells2 * h->K, h->st));
+    CK(cudaMemsetAsync(h->ws + L.ledger, 0, L.tile - L.ledger, h->st));    // ledger, airborne scratch, control block
+    if (h->prm.compact) CK(cudaMemsetAsync(h->ws + L.tile, 0, L.stage - L.tile, h->st));   // look-back states, injected log
+    if (h->prm.dose) CK(cudaMemsetAsync(h->ws + L.dose, 0, 8 * cells3 * h->K, h->st));
+    h->launches += 4;
+    h->step = 0; h->bin_step = 0; h->binned = false;
+    h->pair_snap = -1; h->blend_n = 0; h->blend_step0 = 0; h->bbox_valid = false;
+    h->perm_valid = false; h->perm_n = 0; h->perm_step = 0; h->perm_cur = 0; h->keys_ready = false; h->csort_step = 0;
+    for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) { h->dep_ref[k] = 0; h->dep_bound[k] = 0.0; }
+    for (const Release &r : h->rel)
+        for (int k = 0; k < h->K; ++k) if (r.emit[k] > h->dep_bound[k]) h->dep_bound[k] = r.emit[k];
     return LPM_OK;
 }
 
@@ -693,12 +718,14 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
     if (!h || n_steps < 0) return fail(h, LPM_ERR_INVALID_ARG, "lpm_step: negative step count");
     if (h->sticky) return h->sticky;
     const bool compact = h->prm.compact != 0;
-    int m_max = h->prm.steps_per_launch > 0 ? h->prm.steps_per_launch : kMaxFused;
-    if (m_max > kMaxFused) m_max = kMaxFused;
-    if (compact) m_max = 1;
-    if (h->met.nt > 1 && m_max > kBlendDepth) m_max = kBlendDepth;  // one time-blended met buffer per fused step
     StepArgs A;
     base_args(h, A);
+    // up to 16 steps per launch; up to 64 when one met buffer serves every step and no sink uses the deposit tables
+    const int m_cap = (!compact && h->met.nt == 1 && !A.any_dep) ? kMaxFusedLong : kMaxFused;
+    int m_max = h->prm.steps_per_launch > 0 ? h->prm.steps_per_launch : m_cap;
+    if (m_max > m_cap) m_max = m_cap;
+    if (compact) m_max = 1;
+    if (h->met.nt > 1 && m_max > kBlendDepth) m_max = kBlendDepth;  // one time-blended met buffer per fused step
     int64_t left = n_steps;
     while (left > 0) {
         bool fused_bin = false;

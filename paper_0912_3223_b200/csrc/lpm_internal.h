@@ -8,6 +8,9 @@
 
 // kernel formulation switches (round 2; all on: measured one by one on c4, profiles/r02_*): packed FFMA2 arithmetic,
 // MUFU.SQRT, 32-bit texel indices, direct-mapped deposit window
+#ifndef LPM_FUSED_LONG
+#define LPM_FUSED_LONG 64
+#endif
 #ifndef LPM_LEGACY_KERNEL
 #define LPM_FMA2 1
 #define LPM_SQRT_MUFU 1
@@ -18,6 +21,9 @@
 namespace lpm {
 
 constexpr int kMaxFused = 16;        // model steps fused into one launch (table lives in kernel params)
+constexpr int kMaxFusedLong = LPM_FUSED_LONG;    // ... when every step samples the same met buffer (one snapshot) and nothing goes through the
+                                     // deposit tables (their fixed-point sums hold 256 x 16 increments): small, launch-latency-bound
+                                     // runs like c1 ("fewer particles ... GPU spends most of the time on initialization")
 constexpr int kBlendDepth = kMaxFused;  // time-blended met buffers kept: one per fused step
 constexpr int kMaxLevels = 64;       // non-uniform vertical met levels held in the kernel parameters
 constexpr int kSortPeriod = 32;      // least number of model steps between two gather-locality sorts of a release (auto: 32..64)
@@ -121,7 +127,7 @@ struct StepArgs {
     // time
     uint64_t step0;
     int32_t m_steps;
-    StepEntry tab[kMaxFused];
+    StepEntry tab[kMaxFusedLong];
 };
 
 // compact mode: newborn particles of one step, appended behind the live ones
