@@ -829,7 +829,9 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps)
             h->launches += 2;
         } else {
             // a8 fused: a launch that ends on a binning step bins its particles itself (lpm_step.cu: bin_tile)
-            fused_bin = h->prm.bin_every > 0 && (h->step + (uint64_t)m) % (uint64_t)h->prm.bin_every == 0;
+            // (the epilogue is instantiated for the default physics: expected-mass deposition, gridded Kz, uniform levels, no drift)
+            fused_bin = h->prm.bin_every > 0 && (h->step + (uint64_t)m) % (uint64_t)h->prm.bin_every == 0 && !A.bern && !A.eq3 && !A.drift &&
+                        !h->has_levels;
             A.bin_cnt = nullptr;
             if (fused_bin) {
                 const uint64_t cells3 = (uint64_t)h->cg.nx * h->cg.ny * h->cg.nz;

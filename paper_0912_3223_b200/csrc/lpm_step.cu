@@ -17,6 +17,8 @@
 //   nvcc ... -DLPM_BOUND_NO_DEPOSIT   the step without the deposit scatter a6 (the ledger is still kept)
 //   nvcc ... -DLPM_BOUND_NO_GATHER    the step with the eight met texels replaced by values made up in registers (no gathers)
 // build a library with one of them next to the product:  nvcc <flags of build.py> -D... -c csrc/lpm_step.cu, link with the other objects.
+#include <type_traits>
+
 #include "lpm_device.cuh"
 
 namespace lpm {
@@ -464,7 +466,10 @@ __device__ __forceinline__ uint32_t bin_tile(const StepArgs &A, BinTabS<K> &B, b
 #endif
 static_assert(sizeof(StepArgs) <= 32764, "StepArgs must fit the kernel-parameter space (32764 B since CUDA 12.1 on sm_70+)");
 
-template <int K, int DRY, bool BERN, bool EQ3, bool ZLEV, bool ZP = false>
+// BIN: the instantiation for the launch that ends on a binning step (a8 fused; default physics only).  A separate
+// instantiation because the epilogue's registers and shared-memory union cost the step loop 5 % when compiled in
+// (measured: 7.32e10 -> 6.98e10 particle-steps/s on c4), and 44 of 45 launches do not bin.
+template <int K, int DRY, bool BERN, bool EQ3, bool ZLEV, bool ZP = false, bool BIN = false>
 __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel(const __grid_constant__ StepArgs A)
 {
     __shared__ uint32_t s_ticket;
@@ -477,12 +482,14 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
     // younger slots in id order (still close to the source).  The CTAs resident together therefore
     // work on one small region of the plume: their met gathers hit L1/L2, and their deposits meet
     // in the CTA-private tables below instead of in the global map.
-    __shared__ TileTab<K> U;
-    DepTab<K> &T = U.dep;
-    for (int i = threadIdx.x; i < (int)(sizeof(U) / 4); i += kStepThreads) ((uint32_t *)&U)[i] = 0u;
-    __syncthreads();
+    __shared__ typename std::conditional<BIN, TileTab<K>, DepTab<K>>::type U;
+    DepTab<K> &T = *reinterpret_cast<DepTab<K> *>(&U);
+    if constexpr (BIN) {
+        for (int i = threadIdx.x; i < (int)(sizeof(U) / 4); i += kStepThreads) ((uint32_t *)&U)[i] = 0u;
+        __syncthreads();
+    }
     dep_clear<K>(T);
-    uint32_t n_binned = 0;
+    [[maybe_unused]] uint32_t n_binned = 0;
     // (slots that had left the domain when the list was built are not on it: its live length is a device scalar)
     uint64_t n_list = A.perm ? A.n_perm : 0ull;
     if (A.perm && A.n_live) { const uint64_t d = *A.n_live; n_list = d < n_list ? d : n_list; }
@@ -570,13 +577,13 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             __syncthreads();
             dep_flush<K>(A, T);
         }
-        if (A.bin_cnt) {   // this launch ends on a binning step (a8 fused)
-            n_binned += bin_tile<K>(A, U.bin, valid && z >= 0.0f, x, y, z, q);
+        if constexpr (BIN) {   // this launch ends on a binning step (a8 fused)
+            n_binned += bin_tile<K>(A, *reinterpret_cast<BinTabS<K> *>(&U), valid && z >= 0.0f, x, y, z, q);
             dep_clear<K>(T);                           // window header of the deposit table (the sums are zero again)
         }
     }
     flush_ledger<K>(A, acc);
-    if (A.bin_cnt) {
+    if constexpr (BIN) {
         n_binned = __reduce_add_sync(0xffffffffu, n_binned);
         if ((threadIdx.x & 31) == 0 && n_binned) atomicAdd((unsigned long long *)(A.ctrl + 19), (unsigned long long)n_binned);
     }
@@ -809,24 +816,29 @@ static StepKernel pick_kb(bool compact, int dry, bool eq3, bool zlev)
     return zlev ? pick_dry<K, BERN, false, true>(compact, dry) : pick_dry<K, BERN, false, false>(compact, dry);
 }
 
-// z-pair texels: default physics, slot-addressed store only (6 more instantiations, not 96)
-template <int K>
+// z-pair texels and / or the fused binning epilogue: default physics, slot-addressed store only (18 more instantiations, not 96 x 4)
+template <int K, bool ZP, bool BIN>
 static StepKernel pick_zp(int dry)
 {
-    if (dry == kDryNone) return step_slots_kernel<K, kDryNone, false, false, false, true>;
-    return dry == kDryUniform ? step_slots_kernel<K, kDryUniform, false, false, false, true> : step_slots_kernel<K, kDryLayer, false, false, false, true>;
+    if (dry == kDryNone) return step_slots_kernel<K, kDryNone, false, false, false, ZP, BIN>;
+    return dry == kDryUniform ? step_slots_kernel<K, kDryUniform, false, false, false, ZP, BIN> : step_slots_kernel<K, kDryLayer, false, false, false, ZP, BIN>;
 }
 
-static StepKernel pick(int K, bool compact, int dry, bool bern, bool eq3, bool zlev, bool zpair = false)
+static StepKernel pick(int K, bool compact, int dry, bool bern, bool eq3, bool zlev, bool zpair = false, bool bin = false)
 {
-    if (zpair) return K == 1 ? pick_zp<1>(dry) : pick_zp<2>(dry);
+    if (bin) {
+        if (zpair) return K == 1 ? pick_zp<1, true, true>(dry) : pick_zp<2, true, true>(dry);
+        return K == 1 ? pick_zp<1, false, true>(dry) : pick_zp<2, false, true>(dry);
+    }
+    if (zpair) return K == 1 ? pick_zp<1, true, false>(dry) : pick_zp<2, true, false>(dry);
     if (K == 1) return bern ? pick_kb<1, true>(compact, dry, eq3, zlev) : pick_kb<1, false>(compact, dry, eq3, zlev);
     return bern ? pick_kb<2, true>(compact, dry, eq3, zlev) : pick_kb<2, false>(compact, dry, eq3, zlev);
 }
 
 cudaError_t launch_step(const StepArgs &a, int K, bool compact, int blocks, cudaStream_t st)
 {
-    pick(K, compact, a.dry_mode, a.bern != 0, a.eq3 != 0, a.mg.nlev != 0 || a.drift != 0, a.zpair != 0)<<<blocks, kStepThreads, 0, st>>>(a);
+    // (lpm_api.cu asks for the binning epilogue - bin_cnt != null - only with the physics it is instantiated for)
+    pick(K, compact, a.dry_mode, a.bern != 0, a.eq3 != 0, a.mg.nlev != 0 || a.drift != 0, a.zpair != 0, a.bin_cnt != nullptr)<<<blocks, kStepThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 
