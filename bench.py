@@ -53,8 +53,8 @@ SMS, LANES_PER_SM = 148, 128          # 4 SMSP x 32 lanes: one warp instruction 
 LAUNCH_STEPS = 16                     # model steps fused per step-kernel launch (csrc kMaxFused)
 # dram__bytes_read.sum + dram__bytes_write.sum of one captured step-kernel launch, bytes: NOT measured by this run, copied
 # from the named ncu capture
-NCU_TRAFFIC = {"c4": {"bytes": 4.069e9 + 1.985e9, "source": "profiles/r01c_c4_step_kernel_ncu.md (r01d): launch 171 of `bench.py --steps 1 "
-                      "--warmup 3`, 16 steps x 3.16e7 particles, z-pair texels; 3.0 B algorithmic per particle-step = 1.5 GB"}}
+NCU_TRAFFIC = {"c4": {"bytes": 2.605e9 + 1.173e9, "source": "profiles/r02_c4_step_kernel_ncu.md (r02b): launch 171 of `bench.py --steps 1 "
+                      "--warmup 3`, 16 steps x 2.94e7 active particles, z-pair texels; 3.0 B algorithmic per particle-step = 1.4 GB"}}
 ORACLE_STRIDE = {"c1": 1, "c2": 40, "c2_eq3": 40, "c3": 400, "c3_hdep80": 400, "c4": 4000, "c5": 1}
 ORACLE_SCALE_C5 = 1.0e-3              # c5 cannot be pid-strided (capacity couples particles): 1/1000 scale
 

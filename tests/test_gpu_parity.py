@@ -440,10 +440,17 @@ def test_deposition_map_end_to_end_with_slack(lpm, orc):
     o.step(2300)
     dg = sim.deposition(f64=True).cpu().numpy()
     do, slack = o.deposition(with_slack=True)
-    # cells whose error exceeds 1e-5 + face slack can only come from the heavy tail of particles whose
-    # position left the 1e-5 L band (T3 allows 0.1 % of them); their deposit must stay a tiny part
+    # Tolerance: every cell within 1e-5 + face slack, EXCEPT for what the particles outside the position band
+    # can move.  The slack covers particles within face_delta = 1.5 m of a map-cell face (1e-5 of the 100 km domain = 1 m of
+    # position tolerance, + margin); a particle whose position error exceeds that - T3 allows 0.1 % of them - may put its
+    # deposits into a neighbouring cell: missing in one cell, extra in another, so at most 2 x its share of the total.
+    # Hence excess <= 2 x 1e-3 x total; the same run must also show that no more than 0.1 % of the particles are that far off.
     excess = np.maximum(np.abs(dg - do) - (1e-5 * do + 1.0001 * slack + 1e-30), 0.0)
-    print(f"[dep e2e] cells over tol: {(excess > 0).sum()} of {(do > 0).sum()}, excess/total = {excess.sum() / do.sum():.3e}")
+    g, p = gpu_state(sim), o.particles()
+    far = (np.abs(g["x"] - p["x"]) > 1.5) | (np.abs(g["y"] - p["y"]) > 1.5)
+    print(f"[dep e2e] cells over tol: {(excess > 0).sum()} of {(do > 0).sum()}, excess/total = {excess.sum() / do.sum():.3e}, "
+          f"particles further than 1.5 m from the oracle's: {far.mean():.2e}")
+    assert far.mean() <= 1e-3
     assert excess.sum() <= 2e-3 * do.sum()
     g = w.cgrid
     for k in range(2):
@@ -618,7 +625,10 @@ def test_bernoulli_deposition(lpm, orc, h_dep):
     assert g["x"].shape[0] == p["x"].shape[0] > 1500
     frag = np.isin(p["pid"], o.fragile_pids())
     ok = ~frag
-    assert frag.mean() < (0.02 if h_dep >= 1000.0 else 0.15)     # the z = h_dep surface sits 30 m above the source
+    print(f"[bernoulli h_dep={h_dep}] fragile fraction {frag.mean():.4f}")
+    # measured with the oracle alone (same seed, deterministic): 0.0024 (rain-box faces only) and 0.0686 (the z = h_dep surface
+    # sits 30 m above the source, and every particle that ever came within 5 cm of it stays flagged); bound = that + a margin
+    assert frag.mean() < (0.004 if h_dep >= 1000.0 else 0.08)
     np.testing.assert_array_equal(g["status"][ok], p["status"][ok])
     assert (p["status"] == 2).sum() > 50
     for k in range(2):                                    # the same nuclides are gone from the same particles
@@ -786,7 +796,9 @@ def test_drift_corrected_walk(lpm, orc, levels):
     gp, p = gpu_state(sim), o.particles()
     assert gp["x"].shape[0] == p["x"].shape[0] > 5000
     frag = np.isin(p["pid"], o.fragile_pids())
-    assert frag.mean() < 0.2
+    # measured with the oracle alone: 0.118 (uniform levels) and 0.107: the slope of the interpolant switches on at the lowest level
+    # height (25 m / 10 m, next to the 50 m source), and a particle that came within 5 cm of it in any of the 500 steps stays flagged
+    assert frag.mean() < 0.13
     _n_step_compare(gp, p, w, frag, 0.999, f"drift levels={levels}")
     # the term really acts: the same run without it differs by metres
     plain = lpm.Simulation(w)
