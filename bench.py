@@ -264,6 +264,8 @@ def run_ours(args):
     if rank == 0 and not args.no_probes:
         for key, kind, fp in (("ffma_lane_ops_per_s", "ffma", 0), ("imad_lop_lane_ops_per_s", "imad_lop", 0),
                               ("l1_gather_sectors_per_s", "gather", 64 << 10), ("l2_gather_sectors_per_s", "gather", 64 << 20),
+                              ("l1_gather32_sectors_per_s", "gather32", 64 << 10), ("smem_gather_1440B_lane_loads_per_s", "smem_gather", 1440),
+                              ("smem_gather_16KB_lane_loads_per_s", "smem_gather", 16 << 10),
                               ("red_same_address_per_s", "red_same", 0), ("shared_atomic_per_s", "atoms", 0)):
             probes[key] = lpm.probe(kind, fp, scratch_bytes=1 << 28)
         torch.cuda.empty_cache()

@@ -311,10 +311,14 @@ int32_t lpm_touched_cells(lpm_handle *h, uint64_t *n_host);
  *   LPM_PROBE_ATOMS     conflict-free shared-memory atomicAdd (u32), atomics / s
  *   LPM_PROBE_GATHER    16-byte loads, each lane its own 32-byte sector of an L1-resident window of
  *                       footprint_bytes: L1 sectors / s (the met gather of a decorrelated warp)
+ *   LPM_PROBE_SMEM_GATHER  16-byte shared-memory loads, each lane its own texel of a window of footprint_bytes (<= 16 KB)
+ *                       staged in shared memory: lane-loads / s (the alternative to the L1 gathers: 8 per trilinear sample)
+ *   LPM_PROBE_GATHER32  32-byte loads (ld.global.nc.v8.f32), each lane its own sector of an L1-resident window: sectors / s
+ *                       (the z-pair texel gather of the step kernel: 4 per trilinear sample)
  * Errors: INVALID_ARG (null, unknown kind, scratch < 1 MiB), NO_DEVICE, CUDA. */
 typedef enum {
     LPM_PROBE_FFMA = 0, LPM_PROBE_IMAD_LOP = 1, LPM_PROBE_RED_F64 = 2, LPM_PROBE_RED_U32 = 3,
-    LPM_PROBE_RED_SAME = 4, LPM_PROBE_ATOMS = 5, LPM_PROBE_GATHER = 6
+    LPM_PROBE_RED_SAME = 4, LPM_PROBE_ATOMS = 5, LPM_PROBE_GATHER = 6, LPM_PROBE_SMEM_GATHER = 7, LPM_PROBE_GATHER32 = 8
 } lpm_probe_kind;
 int32_t lpm_probe(int32_t kind, uint64_t footprint_bytes, void *scratch_dev, uint64_t scratch_bytes, int32_t reps,
                   double *ops_per_s_host, void *cuda_stream);

@@ -409,7 +409,7 @@ class Simulation:
 
 
 # ---------------------------------------------------------------- micro-benchmarks
-PROBE_KINDS = {"ffma": 0, "imad_lop": 1, "red_f64": 2, "red_u32": 3, "red_same": 4, "atoms": 5, "gather": 6}
+PROBE_KINDS = {"ffma": 0, "imad_lop": 1, "red_f64": 2, "red_u32": 3, "red_same": 4, "atoms": 5, "gather": 6, "smem_gather": 7, "gather32": 8}
 
 
 def probe(kind: str, footprint_bytes: int = 0, scratch_bytes: int = 1 << 28, reps: int = 5) -> float:

@@ -1305,11 +1305,11 @@ static int dev_ok()
 
 int32_t lpm_probe(int32_t kind, uint64_t footprint, void *scratch, uint64_t scratch_bytes, int32_t reps, double *ops, void *st)
 {
-    if (!scratch || !ops || kind < 0 || kind > LPM_PROBE_GATHER || scratch_bytes < (1u << 20) || reps < 1 || ((uintptr_t)scratch & 15))
+    if (!scratch || !ops || kind < 0 || kind > LPM_PROBE_GATHER32 || scratch_bytes < (1u << 20) || reps < 1 || ((uintptr_t)scratch & 15))
         return LPM_ERR_INVALID_ARG;
     if (!dev_ok()) return LPM_ERR_NO_DEVICE;
     if (footprint == 0 || footprint > scratch_bytes) footprint = scratch_bytes;
-    if (kind == LPM_PROBE_GATHER && footprint > scratch_bytes - 64) footprint = scratch_bytes - 64;
+    if ((kind == LPM_PROBE_GATHER || kind == LPM_PROBE_GATHER32) && footprint > scratch_bytes - 64) footprint = scratch_bytes - 64;
     return run_probe(kind, footprint, scratch, scratch_bytes, reps, ops, (cudaStream_t)st) == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
 }
 

@@ -107,6 +107,45 @@ __global__ void __launch_bounds__(kThreads) probe_gather(const float4 *buf, uint
     if (acc == 123.456f) out[0] = acc;
 }
 
+// 7: the alternative to the L1 gathers that north_star names ("staged ... into shared memory"): 16-byte LDS gathers, every lane its own
+// texel inside a window of `texels` float4 in shared memory (a warp's block of columns x levels, staged per step): LDS.128 lane-loads
+// per second.  One trilinear sample needs 8 of them (or 4 of 32 bytes from global memory, probe 6 with 32-byte texels).
+__global__ void __launch_bounds__(kThreads) probe_smem_gather(float *out, uint32_t texels, int iters)
+{
+    __shared__ float4 win[1024];
+    for (int i = threadIdx.x; i < 1024; i += kThreads) win[i] = make_float4((float)i, 1.f, 2.f, 3.f);
+    __syncthreads();
+    uint32_t s = (blockIdx.x * kThreads + threadIdx.x) * 2654435761u + 4242u;
+    float acc = 0.f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const uint32_t i = (lcg(s) >> 8) % texels;
+            const float4 v = win[i];
+            acc += v.x + v.w;
+        }
+    }
+    if (acc == 123.456f) out[0] = acc;
+}
+
+// 8: 32-byte gathers (ld.global.nc.v8.f32), every lane its own sector of an L1-resident window: the z-pair texel gather of the step kernel
+__global__ void __launch_bounds__(kThreads) probe_gather32(const float4 *buf, uint32_t texels, float *out, int iters)
+{
+    uint32_t s = (blockIdx.x * kThreads + threadIdx.x) * 2654435761u + 77u;
+    float acc = 0.f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t i = (lcg(s) >> 8) % texels;
+            float a0, a1, a2, a3, a4, a5, a6, a7;
+            asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                         : "=f"(a0), "=f"(a1), "=f"(a2), "=f"(a3), "=f"(a4), "=f"(a5), "=f"(a6), "=f"(a7) : "l"(buf + 2ull * i));
+            acc += a0 + a7;
+        }
+    }
+    if (acc == 123.456f) out[0] = acc;
+}
+
 }  // namespace
 
 // returns operations per second in *ops (FMA lane-ops, IMAD+LOP3 lane-op pairs x2, atomics, sectors)
@@ -136,6 +175,8 @@ cudaError_t run_probe(int kind, uint64_t footprint_bytes, void *scratch_dev, uin
                 case 4: probe_red_same<<<blocks, kThreads, 0, st>>>((double *)scratch_dev, 16); per_launch = (double)threads * 16; break;
                 case 5: probe_atoms<<<blocks, kThreads, 0, st>>>((uint32_t *)scratch_dev, 512); per_launch = (double)threads * 512 * 8; break;
                 case 6: probe_gather<<<blocks, kThreads, 0, st>>>((const float4 *)scratch_dev, (uint32_t)(footprint_bytes / 16), (float *)scratch_dev + scratch_bytes / 4 - 4, 128); per_launch = (double)threads * 128 * 8; break;
+                case 7: probe_smem_gather<<<blocks, kThreads, 0, st>>>((float *)scratch_dev, (uint32_t)(footprint_bytes / 16 < 1024 ? (footprint_bytes / 16 ? footprint_bytes / 16 : 1) : 1024), 256); per_launch = (double)threads * 256 * 8; break;
+                case 8: probe_gather32<<<blocks, kThreads, 0, st>>>((const float4 *)scratch_dev, (uint32_t)(footprint_bytes / 32), (float *)scratch_dev + scratch_bytes / 4 - 4, 128); per_launch = (double)threads * 128 * 4; break;
                 default: rc = cudaErrorInvalidValue; break;
             }
             if (rc != cudaSuccess) break;
