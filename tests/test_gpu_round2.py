@@ -344,3 +344,37 @@ def test_absorbed_slots_leave_the_sorted_list_and_the_unit_count(lpm, orc):
     for k in range(2):
         assert abs(res[0][4][k][5] / lo[k][5] - 1) < 5e-3                   # exited activity (fragile particles may differ)
         assert abs(sum(res[0][4][k][1:6]) / res[0][4][k][0] - 1) < 1e-5
+
+
+# ------------------------------------------------------------------ a8 fused = a8 stand-alone
+@pytest.mark.parametrize("name,scale,nt", [("c4", 3e-3, 3), ("c3", 0.02, 3), ("c2", 0.2, 3)])
+def test_fused_binning_equals_the_standalone_kernel(lpm, orc, name, scale, nt):
+    """The step launch that ends an output interval bins its particles from registers (bin_tile epilogue); lpm_bin_now bins
+    the same state with the stand-alone kernel: identical counts, sums equal to fp64 rounding; and both equal the oracle's
+    binning of the SAME positions (counts bit-exact, concentration 1e-5)."""
+    import torch
+    w = make(name, scale=scale, n_steps=480).replace(nt=nt, bin_every=240)
+    sim = lpm.Simulation(w, gather_sort=32)           # (forced: the small ensemble still walks a sorted list)
+    sim.set_timing(True)
+    sim.step(480)
+    t = sim.get_timing()
+    assert t["bin_fused_launches"] == 2 and t["bin_launches"] == 2      # two fused binnings; the timed "bin" spans are their memsets
+    cnt_f = sim.counts().cpu().numpy().copy()
+    conc_f = sim.concentration().cpu().numpy().astype(np.float64)
+    sim.bin_now()
+    cnt_s = sim.counts().cpu().numpy()
+    conc_s = sim.concentration().cpu().numpy().astype(np.float64)
+    np.testing.assert_array_equal(cnt_f, cnt_s)
+    assert cnt_f.sum() > 1000
+    np.testing.assert_allclose(conc_f, conc_s, rtol=2e-6, atol=0)
+    # the oracle bins the CUDA path's own positions and activities
+    p = gpu_state(sim)
+    o = orc.OracleSim(w.replace(release=None, capacity=max(len(p["x"]), 1)), bin_every=0)
+    o.set_particles(p["x"].astype(np.float64), p["y"].astype(np.float64), p["z"].astype(np.float64), p["m"], pid=np.arange(len(p["x"])),
+                    status=p["status"])
+    o.set_step_index(480)
+    o.bin_now()
+    np.testing.assert_array_equal(cnt_f.view(np.uint32), o.counts())
+    oc = o.concentration()
+    nz = oc > 0
+    assert np.array_equal(nz, conc_f > 0) and np.abs(conc_f[nz] / oc[nz] - 1).max() <= 1e-5
