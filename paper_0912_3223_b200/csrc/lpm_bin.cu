@@ -53,6 +53,9 @@ __global__ void __launch_bounds__(256) bin_tile_kernel(const __grid_constant__ B
     uint32_t binned = 0;
     for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         __syncthreads();   // the table is clear (start of the kernel / flush of the previous tile)
+        // all of the thread's records first (independent loads in flight), then the table work
+        float4 pr[kBinItems];
+        float q1r[kBinItems];
 #pragma unroll
         for (int j = 0; j < kBinItems; ++j) {
             uint64_t slot;
@@ -65,8 +68,12 @@ __global__ void __launch_bounds__(256) bin_tile_kernel(const __grid_constant__ B
                 slot = first_new + (uint64_t)(tile - t_old) * kBinTile + (uint32_t)j * 256 + threadIdx.x;
                 valid = slot < n;
             }
-            if (!valid) continue;
-            const float4 p = A.xyzq[slot];
+            pr[j] = valid ? A.xyzq[slot] : make_float4(0.f, 0.f, -1.f, 0.f);    // (z < 0: nothing to bin)
+            q1r[j] = (K > 1 && valid) ? A.q1[slot] : 0.f;
+        }
+#pragma unroll
+        for (int j = 0; j < kBinItems; ++j) {
+            const float4 p = pr[j];
             if (!(p.z >= 0.0f)) continue;   // z < 0 marks an exited slot
             const int ci = cell_of(p.x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
             const int cj = cell_of(p.y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
@@ -76,11 +83,11 @@ __global__ void __launch_bounds__(256) bin_tile_kernel(const __grid_constant__ B
             const uint32_t cell = (uint32_t)((ck * A.cg.ny + cj) * A.cg.nx + ci), key = cell + 1u;
             float q[K];
             q[0] = p.w;
-            if (K > 1) q[1] = A.q1[slot];
+            if (K > 1) q[1] = q1r[j];
             uint32_t h = (key * 0x9E3779B1u) >> (32 - kBinSlotBits);
             int s = -1;
 #pragma unroll 1
-            for (int pr = 0; pr < kBinProbes; ++pr) {
+            for (int pr_ = 0; pr_ < kBinProbes; ++pr_) {
                 const uint32_t t = *(volatile uint32_t *)&T.tag[h];
                 if (t == key) { s = (int)h; break; }
                 if (t == 0u) {
