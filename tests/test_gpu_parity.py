@@ -286,13 +286,15 @@ def test_T2_c1_full(lpm, orc):
 
 @pytest.mark.parametrize("name,scale,stride,steps,nt,req", [
     ("c2", 0.02, 1, 1440, 3, 0.999),
+    ("c2", 1.0, 1, 1440, 3, 0.999),                 # BASELINE's full size and duration (measured: 100 %)
     ("c2_eq3", 0.02, 1, 1440, 3, 0.999),
-    ("c3", 1.0, 2000, 3000, 10, 0.999),
+    ("c3", 1.0, 400, 8640, 25, 0.999),              # the whole 24 h on every 400th id (measured: 99.97 %)
     ("c3_hdep80", 1.0, 2000, 3000, 10, 0.999),
-    ("c4", 1.0, 20000, 5200, 9, 0.999),
+    ("c4", 1.0, 4000, 8640, 13, 0.999),             # the whole 12 h on every 4000th id (measured: 99.92 %)
 ])
 def test_T3_n_steps(lpm, orc, name, scale, stride, steps, nt, req):
-    """T3: full-duration-class runs on a pid-strided subsample (exact subset of the full run)."""
+    """T3: full-duration runs; c3 / c4 on a pid-strided subsample (an exact subset of the full run: particles are independent
+    and Philox is keyed by the id), c2 also at its full size."""
     w = make(name, scale=scale, n_steps=steps)
     rel = w.release
     rel.pid_stride = stride
