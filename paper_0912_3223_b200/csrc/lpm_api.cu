@@ -4,7 +4,6 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
-#include <stdlib.h>
 
 #include <new>
 #include <vector>
@@ -414,14 +413,6 @@ int do_bin(lpm_handle *h)
             B.xyzq = (const float4 *)(h->ws + h->L.xyzq) + r.base;
             if (B.q1) B.q1 = (const float *)(h->ws + h->L.q1) + r.base;
             B.n = n;
-            B.perm = nullptr; B.n_list_dev = nullptr; B.n_list = 0; B.first_new = 0;
-            static const bool walk_list = getenv("LPM_BIN_LIST") != nullptr;   // EXPERIMENT
-            if (walk_list && h->perm_valid && h->rel.size() == 1 && h->perm_n <= n) {   // the step kernel's met-cell-sorted list
-                B.perm = perm_half(h, h->perm_cur);
-                B.n_list = h->perm_n;
-                B.n_list_dev = (const uint64_t *)(h->ws + h->L.ctrl) + kCtrlLive + h->perm_cur;
-                B.first_new = h->perm_n;
-            }
             const uint64_t want = (n + 1023) / 1024;
             CK(launch_bin(B, (int)(want < (uint64_t)max_blocks ? want : (uint64_t)max_blocks), h->st));
             h->launches++;

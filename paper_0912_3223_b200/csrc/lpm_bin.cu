@@ -2,8 +2,8 @@
 //
 // P:L108 "Activities or masses of particles are summarized on a rectangular grid"; the paper does
 // this on the CPU after a D2H copy and suggests a separate GPU kernel.  Here the
-// particles never leave HBM.  Cell rule R10 (exact fp32 index), counts in u32 (exact), sums of the
-// stored q in fp64 so that the result does not depend on the order of the atomics beyond 1e-16.
+// particles never leave HBM.  Cell rule R10 (exact fp32 index), counts in u32 (exact); the stored q are summed as
+// fixed-point integers per tile (order-independent) and the tile sums added to fp64 grids (B9).
 #include <curand_kernel.h>
 
 #include "lpm_device.cuh"
@@ -13,9 +13,11 @@ namespace lpm {
 // The binning kernel named by north_star ("shared-memory-privatised histograms ... instead of naive global
 // atomics"; the paper itself only says the summation "may be computed by the GPU, in a separate kernel").
 //
-// Order.  The particles are walked in the order of the step kernel's met-cell-sorted slot list (S 8(f)4: the sort is
-// shared), so the kBinTile particles a CTA takes at a time are spatial neighbours and fall into few concentration
-// cells; the compact store is itself kept in that order, small ensembles are walked as stored.
+// Order.  This stand-alone kernel walks the store as stored: the compact store is physically kept in met-cell order (S 8(f)4:
+// the sort is shared), so the kBinTile particles a CTA takes at a time are spatial neighbours and fall into few concentration
+// cells; a slot-addressed store is in id = age order, where only young particles share cells - there the cadence binning
+// is fused into the step kernel instead (lpm_step.cu: bin_tile, list order for free), and this kernel serves lpm_bin_now.
+// (Walking the step kernel's sorted slot list from here was measured: the indirect record reads made it 1.8 x slower.)
 // Privatisation.  Per tile, counts and sums are accumulated in an open-addressing table in shared memory keyed by the
 // concentration cell: u32 count + per nuclide a u32 FIXED-POINT sum rint(q * S_k), S_k a power of two with
 // q_max S_k in [2^19, 2^20) (the DepTab idea of the step kernel: native 32-bit shared atomics, order-independent
@@ -42,14 +44,7 @@ __global__ void __launch_bounds__(256) bin_tile_kernel(const __grid_constant__ B
         for (int k = 0; k < K; ++k) T.sum[k][i] = 0u;
     }
     const uint64_t n = A.n_dev ? *A.n_dev : A.n;
-    uint64_t n_list = 0, first_new = 0;
-    if (A.perm) {
-        n_list = A.n_list;
-        if (A.n_list_dev) { const uint64_t d = *A.n_list_dev; n_list = d < n_list ? d : n_list; }
-        first_new = A.first_new < n ? A.first_new : n;
-    }
-    const uint32_t t_old = (uint32_t)((n_list + kBinTile - 1) / kBinTile);
-    const uint32_t n_tiles = t_old + (uint32_t)((n - first_new + kBinTile - 1) / kBinTile);
+    const uint32_t n_tiles = (uint32_t)((n + kBinTile - 1) / kBinTile);
     uint32_t binned = 0;
     for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         __syncthreads();   // the table is clear (start of the kernel / flush of the previous tile)
@@ -58,16 +53,8 @@ __global__ void __launch_bounds__(256) bin_tile_kernel(const __grid_constant__ B
         float q1r[kBinItems];
 #pragma unroll
         for (int j = 0; j < kBinItems; ++j) {
-            uint64_t slot;
-            bool valid;
-            if (tile < t_old) {
-                const uint64_t pos = (uint64_t)tile * kBinTile + (uint32_t)j * 256 + threadIdx.x;
-                valid = pos < n_list;
-                slot = valid ? A.perm[pos] : 0ull;
-            } else {
-                slot = first_new + (uint64_t)(tile - t_old) * kBinTile + (uint32_t)j * 256 + threadIdx.x;
-                valid = slot < n;
-            }
+            const uint64_t slot = (uint64_t)tile * kBinTile + (uint32_t)j * 256 + threadIdx.x;
+            const bool valid = slot < n;
             pr[j] = valid ? A.xyzq[slot] : make_float4(0.f, 0.f, -1.f, 0.f);    // (z < 0: nothing to bin)
             q1r[j] = (K > 1 && valid) ? A.q1[slot] : 0.f;
         }

@@ -153,12 +153,6 @@ struct BinArgs {
     const float *q1;
     uint64_t n;               // slots to bin (slot-addressed mode)
     const uint64_t *n_dev;    // compact mode: read n from here
-    // walk order (a8, S 8(f)4 "sort shared between binning and the step kernel"): the live part of the step kernel's
-    // met-cell-sorted slot list, positions [0, min(*n_list_dev, n_list)), then the slots [first_new, n) in slot order;
-    // perm == null: all slots [0, n) in storage order (small ensembles; the compact store, which is itself kept sorted)
-    const uint32_t *perm;
-    const uint64_t *n_list_dev;
-    uint64_t n_list, first_new;
     GridF cg;
     uint32_t *cnt;
     double *conc;             // [K][cells3] sums of q

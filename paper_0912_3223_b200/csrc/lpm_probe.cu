@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(kThreads) probe_gather32(const float4 *buf, ui
             float a0, a1, a2, a3, a4, a5, a6, a7;
             asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                          : "=f"(a0), "=f"(a1), "=f"(a2), "=f"(a3), "=f"(a4), "=f"(a5), "=f"(a6), "=f"(a7) : "l"(buf + 2ull * i));
-            acc += a0 + a7;
+            acc += (a0 + a1) + (a2 + a3) + (a4 + a5) + (a6 + a7);
         }
     }
     if (acc == 123.456f) out[0] = acc;

@@ -43,7 +43,8 @@ struct Acc {  // per-thread ledger partial sums, in activity units before the pe
 // [2^17, 2^20) take this path (>= 18 significant bits, round to nearest: relative error <= 1.9e-6
 // per increment, unbiased; B4); smaller ones (a particle that carries < 1/8 of the
 // largest activity), increments that do not fit and a full table take the direct fp64 RED.
-constexpr int kDepSlots = 1024, kDepSlotBits = 10, kDepProbes = 8;
+constexpr int kDepSlots = 1024;
+[[maybe_unused]] constexpr int kDepSlotBits = 10, kDepProbes = 8;   // (open-addressing form of the table: LPM_LEGACY_KERNEL)
 static_assert(kStepThreads * kMaxFused <= 4096, "fixed-point deposit sums: 20 bits + 12 bits of count");
 
 #ifdef LPM_DEPWIN
