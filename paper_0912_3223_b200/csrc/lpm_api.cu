@@ -400,7 +400,7 @@ int do_bin(lpm_handle *h)
     B.K = h->K;
     B.n_binned = (uint64_t *)(h->ws + h->L.ctrl) + kCtrlBinned;
     bin_scales(h, h->step, B.scale, B.inv_scale);
-    const int max_blocks = h->sms * 6;
+    const int max_blocks = h->sms * 8;
     if (h->prm.compact) {
         B.xyzq = (const float4 *)(h->ws + h->L.xyzq);
         B.n_dev = (const uint64_t *)(h->ws + h->L.ctrl) + 2;
