@@ -490,7 +490,8 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
         __syncthreads();
     }
     dep_clear<K>(T);
-    [[maybe_unused]] uint32_t n_binned = 0;
+    __shared__ uint32_t s_binned;   // BIN: particles binned by this CTA (kept in shared memory: no register lives across the step loop)
+    if (BIN && threadIdx.x == 0) s_binned = 0u;
     // (slots that had left the domain when the list was built are not on it: its live length is a device scalar)
     uint64_t n_list = A.perm ? A.n_perm : 0ull;
     if (A.perm && A.n_live) { const uint64_t d = *A.n_live; n_list = d < n_list ? d : n_list; }
@@ -579,14 +580,16 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
             dep_flush<K>(A, T);
         }
         if constexpr (BIN) {   // this launch ends on a binning step (a8 fused)
-            n_binned += bin_tile<K>(A, *reinterpret_cast<BinTabS<K> *>(&U), valid && z >= 0.0f, x, y, z, q);
+            const uint32_t b = bin_tile<K>(A, *reinterpret_cast<BinTabS<K> *>(&U), valid && z >= 0.0f, x, y, z, q);
+            const uint32_t bw = __reduce_add_sync(0xffffffffu, b);
+            if ((threadIdx.x & 31) == 0 && bw) atomicAdd(&s_binned, bw);
             dep_clear<K>(T);                           // window header of the deposit table (the sums are zero again)
         }
     }
     flush_ledger<K>(A, acc);
     if constexpr (BIN) {
-        n_binned = __reduce_add_sync(0xffffffffu, n_binned);
-        if ((threadIdx.x & 31) == 0 && n_binned) atomicAdd((unsigned long long *)(A.ctrl + 19), (unsigned long long)n_binned);
+        __syncthreads();
+        if (threadIdx.x == 0 && s_binned) atomicAdd((unsigned long long *)(A.ctrl + 19), (unsigned long long)s_binned);
     }
     n_done = __reduce_add_sync(0xffffffffu, n_done);
     if ((threadIdx.x & 31) == 0 && n_done) atomicAdd((unsigned long long *)(A.ctrl + 3), (unsigned long long)n_done);
