@@ -5,7 +5,7 @@ grids, constants, sources and the closed-form meteorological fields, generated i
 float64 and rounded ONCE to float32.  That float32 array is the input of both the
 fp64 oracle and the CUDA path.  No method arithmetic lives here.
 
-Lateral boundary (R7): c1 and c2 are OPEN (their plumes stay inside the grid for the whole run).
+Lateral boundary (R7): c1 and c2 are OPEN (their plumes essentially stay inside the grid for the whole run).
 c3 and c4 are ABSORB, the paper's own rule (a particle that "reaches the predefined boundaries" becomes
 inactive): a 3-8 m/s wind whose direction swings +-45 degrees about a fixed mean carries a particle at least
 3 cos(45 deg) x 12 h = 92 km, typically 250 km, so no source position keeps the particles inside the 100 km box of
