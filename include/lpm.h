@@ -343,6 +343,44 @@ int32_t lpm_test_box_muller(const uint32_t *r_dev, uint64_t n, float *out_dev, v
 int32_t lpm_test_sample(const lpm_meteo *meteo, double t, const void *xyz_dev, uint64_t n,
                         void *out_dev, void *cuda_stream);
 
+/* ---- met sampling for callers that must not allocate device memory -------------------------- */
+
+/* The same operation as lpm_test_sample (R4: "interpolating ... in x, y, z and time" - the wind and Kz a
+ * particle at xyz would see at time t), with identical arguments and bit-identical results, but without a single
+ * cudaMalloc / cudaFree.  lpm_test_sample needs two temporary device buffers per call (the z-fastest snapshot pair,
+ * 32 bytes per met cell, and the time-blended field, 16 bytes per met cell) and gets them from cudaMalloc.  Some users
+ * of the sampler cannot do that:
+ *   - a process whose device memory is entirely in the hands of another allocator (a framework's caching pool that has
+ *     reserved the whole GPU, a fixed MIG / MPS memory budget): a raw cudaMalloc there fails or eats into a budget the
+ *     host application has planned to the byte;
+ *   - an operational loop (dose forecast next to a running dispersion model) in which other streams must keep going:
+ *     cudaMalloc and cudaFree synchronise the whole device, so every call would stall the model.
+ * For them the two buffers live in ONE array that is part of the library image itself (a file-scope __device__
+ * array of LPM_SAMPLE_STATIC_BYTES = 12 MiB + 256 B): every GPU on which the library's kernels are loaded holds
+ * those bytes from module load until the process exits, whether this function is ever called or not.
+ *
+ *  LIMIT      grid.nx * grid.ny * grid.nz <= LPM_SAMPLE_STATIC_MAX_CELLS (262144, e.g. 128 x 128 x 16).  A larger
+ *             met grid is refused with LPM_ERR_WORKSPACE_TOO_SMALL before anything is enqueued (the built-in array
+ *             is this call's workspace); use lpm_test_sample or a handle for those.
+ *  FIRST CALL on each device looks up the device address of the array (cudaGetSymbolAddress, with that device
+ *             current; the address is cached per device ordinal).  That look-up is a set-up step, not stream work:
+ *             make the first call on a device ahead of any stream capture you may have in mind, and with the device
+ *             you will use current.  Later calls on that device issue only kernel launches and one 16-byte memset.
+ *  SHARED     every call on a device uses the same array and finds the previous call's data in it.  The function
+ *             re-writes whatever it reads (the one texel that must be zero, the pad behind the blended field, is
+ *             cleared on every call), so calls may follow each other on ONE stream in any mix of grids and times.
+ *             Two calls whose GPU work overlaps - different streams, different host threads, different handles -
+ *             race on the array and return garbage: serialise them yourself.
+ *  ASYNC      unlike lpm_test_sample this call does not synchronise: the work is enqueued on `cuda_stream` (NULL =
+ *             default stream) and out_dev is valid once that stream has reached the end of it.  meteo->fields_dev,
+ *             xyz_dev, out_dev stay the caller's (inputs are only read); z_levels_host is copied before return.
+ *  Errors: INVALID_ARG (as lpm_test_sample; nz > 64 with z_levels_host), WORKSPACE_TOO_SMALL (the limit above),
+ *  NO_DEVICE, CUDA (including a failed address look-up).  n = 0 is a valid no-op. */
+#define LPM_SAMPLE_STATIC_MAX_CELLS 262144
+#define LPM_SAMPLE_STATIC_BYTES (48ull * LPM_SAMPLE_STATIC_MAX_CELLS + 256ull)
+int32_t lpm_sample_static(const lpm_meteo *meteo, double t, const void *xyz_dev, uint64_t n, void *out_dev,
+                          void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -5,5 +5,5 @@ CUDA kernels for sm_100a behind the C ABI of include/lpm.h (csrc/, built into li
 Importing the package is light; the shared library is loaded on first use and its absence is an
 error (there is no CPU fallback).
 """
-from .binding import (LEDGER_NAMES, box_muller_kernel, curand_philox_kernel, LpmError, Simulation, load, normals_kernel, philox_kernel, probe, sample_kernel,  # noqa: F401
+from .binding import (LEDGER_NAMES, box_muller_kernel, curand_philox_kernel, LpmError, Simulation, load, normals_kernel, philox_kernel, probe, sample_kernel, sample_static,  # noqa: F401
                       schedule_born, status_string, version, workspace_bytes)

@@ -28,7 +28,7 @@ SYMBOLS = (
     "lpm_set_particles", "lpm_ledger", "lpm_injected", "lpm_last_error", "lpm_launch_count", "lpm_test_philox",
     "lpm_test_normals", "lpm_test_sample", "lpm_upload_meteo", "lpm_concentration_host", "lpm_deposition_host",
     "lpm_set_timing", "lpm_get_timing", "lpm_probe", "lpm_test_box_muller", "lpm_dose", "lpm_test_curand_philox",
-    "lpm_texel_pairs", "lpm_touched_cells", "lpm_restart",
+    "lpm_texel_pairs", "lpm_touched_cells", "lpm_restart", "lpm_sample_static",
 )
 
 
@@ -117,6 +117,7 @@ def load():
     L.lpm_test_philox.argtypes = [u64, u64, C.c_uint32, u64, u64, vp, vp]
     L.lpm_test_normals.argtypes = [u64, u64, u64, u64, vp, vp]
     L.lpm_test_sample.argtypes = [C.POINTER(lpm_meteo), dbl, vp, u64, vp, vp]
+    L.lpm_sample_static.argtypes = [C.POINTER(lpm_meteo), dbl, vp, u64, vp, vp]
     for s in SYMBOLS:
         if getattr(L, s).restype is C.c_int:
             getattr(L, s).restype = i32
@@ -481,4 +482,38 @@ def sample_kernel(w, t, xyz):
     if rc:
         raise LpmError(rc, "lpm_test_sample")
     torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+SAMPLE_STATIC_MAX_CELLS = 262144   # LPM_SAMPLE_STATIC_MAX_CELLS of include/lpm.h
+
+
+def sample_static(w, t, xyz):
+    """lpm_sample_static: the met sampling of `sample_kernel`, for users who must not allocate on the device.
+
+    Same arguments, same result bit for bit.  The difference is where the two temporary fields of the sampling path
+    live: `sample_kernel` (lpm_test_sample) takes them from cudaMalloc on every call, this call keeps them in a 12 MiB
+    array built into the library.  That is what a caller needs whose GPU memory belongs to someone else's pool, or who
+    cannot have cudaMalloc / cudaFree stop every other stream of the device for a moment.  Limit: the met grid of `w`
+    may have at most SAMPLE_STATIC_MAX_CELLS cells (LpmError with status ERR_WORKSPACE_TOO_SMALL beyond).  All calls
+    share the one array: keep them on one stream, one after the other.  (The tensors created here are this wrapper's
+    inputs and outputs, which a real caller already owns; the C call itself allocates nothing.)"""
+    torch = _require_cuda()
+    f = torch.from_numpy(np.ascontiguousarray(w.fields())).cuda()
+    pts = np.zeros((xyz.shape[0], 4), dtype=np.float32)
+    pts[:, :3] = xyz
+    p = torch.from_numpy(pts).cuda()
+    out = torch.empty_like(p)
+    met = lpm_meteo(grid=_grid(w.mgrid), nt=w.nt, t0=w.t0, dt_snap=w.dt_snap, fields_dev=f.data_ptr(), Kh=w.Kh,
+                    H_mix=w.H_mix, kz_min=w.kz_min)
+    levels = None
+    if getattr(w, "z_levels", None) is not None:
+        levels = np.ascontiguousarray(w.z_levels, dtype=np.float64)
+        met.z_levels_host = levels.ctypes.data
+    rc = load().lpm_sample_static(C.byref(met), t, p.data_ptr(), p.shape[0], out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    if rc:
+        g = w.mgrid
+        raise LpmError(rc, "lpm_sample_static", f"(met grid {g.nx} x {g.ny} x {g.nz} = {g.nx * g.ny * g.nz} cells; the built-in scratch "
+                                                f"array holds at most {SAMPLE_STATIC_MAX_CELLS})" if rc == ERR_WORKSPACE_TOO_SMALL else "")
+    torch.cuda.synchronize()   # the C call is asynchronous; `out` is read on the host next
     return out.cpu().numpy()

@@ -5,6 +5,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1378,3 +1379,90 @@ int32_t lpm_test_sample(const lpm_meteo *met, double t, const void *xyz, uint64_
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------ lpm_sample_static: met sampling without an allocation
+//
+// For callers that cannot call cudaMalloc (all device memory owned by a host application's pool, or a loop that cannot
+// afford the device-wide synchronisation of cudaMalloc / cudaFree): the two temporaries of the sampling path live in the
+// library image.  One array per loaded module = per GPU, shared by every call, never freed.
+//   [0, 16 * (cells + 1))                       time-blended z-fastest field + the zero pad texel behind it
+//   [kStaticPairAt, kStaticPairAt + 32 * cells)  interleaved snapshot pair of the met interval (nt > 1 only)
+// g_sample_scratch is a HOST-SIDE STAND-IN for the device array: host code must never hand its name (or &name) to a
+// kernel as a pointer.  The device address comes from cudaGetSymbolAddress, once per device, below.
+static_assert(LPM_SAMPLE_STATIC_MAX_CELLS % 16 == 0, "the pair buffer starts 256-byte aligned");
+constexpr uint64_t kStaticPairAt = 16ull * LPM_SAMPLE_STATIC_MAX_CELLS + 256ull;
+static_assert(kStaticPairAt + 32ull * LPM_SAMPLE_STATIC_MAX_CELLS == LPM_SAMPLE_STATIC_BYTES, "lpm.h states the size of the array");
+static __device__ __align__(256) unsigned char g_sample_scratch[LPM_SAMPLE_STATIC_BYTES];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+unsigned char *g_static_addr[kStaticMaxDevices] = {};   // device address of g_sample_scratch on device d; null = not looked up yet
+
+// Device address of the scratch array on the CURRENT device.  First call per device: cudaGetSymbolAddress (this is the
+// set-up step lpm.h tells the caller to get out of the way early); afterwards a table look-up.
+cudaError_t static_scratch(unsigned char **p)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_addr[dev]) {
+        void *q = nullptr;
+        e = cudaGetSymbolAddress(&q, g_sample_scratch);
+        if (e != cudaSuccess) return e;
+        if (!q || ((uintptr_t)q & 255)) return cudaErrorInvalidSymbol;
+        g_static_addr[dev] = (unsigned char *)q;
+    }
+    *p = g_static_addr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int32_t lpm_sample_static(const lpm_meteo *met, double t, const void *xyz, uint64_t n, void *out, void *st)
+{
+    if (!met || !grid_ok(&met->grid) || !met->fields_dev || !xyz || !out || met->nt < 1) return LPM_ERR_INVALID_ARG;
+    const lpm_grid &g = met->grid;
+    if (met->z_levels_host && g.nz > kMaxLevels) return LPM_ERR_INVALID_ARG;
+    const uint64_t cells = (uint64_t)g.nx * g.ny * g.nz;
+    if (cells > LPM_SAMPLE_STATIC_MAX_CELLS) return LPM_ERR_WORKSPACE_TOO_SMALL;   // the built-in array is this call's workspace
+    if (!dev_ok()) return LPM_ERR_NO_DEVICE;
+    unsigned char *scratch = nullptr;
+    if (static_scratch(&scratch) != cudaSuccess) return LPM_ERR_CUDA;
+    float4 *blend = (float4 *)scratch;
+    void *pair = scratch + kStaticPairAt;
+
+    lpm_handle tmp{};
+    tmp.met = *met;
+    tmp.K = 0;
+    tmp.prm.dt = t;   // fill_entry evaluates the time weight at n * dt: dt = t, n = 1
+    StepEntry e;
+    fill_entry(&tmp, 1, e);
+    const float4 *f = (const float4 *)met->fields_dev;
+    cudaStream_t s = (cudaStream_t)st;
+    const int sn = e.snap & 0xffff;
+    // The array still holds the last call's field (perhaps of a bigger grid).  Everything below [0, 16 * cells) and the
+    // pair buffer is overwritten before it is read; the pad texel at `cells` is read with weight 0 when nz = 1 and must
+    // not hold a NaN / Inf left behind by an earlier, larger field: cleared on every call.
+    cudaError_t rc = cudaMemsetAsync(blend + cells, 0, 16, s);
+    if (rc == cudaSuccess) {
+        if (met->nt > 1) {
+            BlendBox box{};
+            box.nx = g.nx; box.ny = g.ny; box.nz = g.nz;
+            rc = launch_pair_repack(f + (uint64_t)sn * cells, f + (uint64_t)(sn + 1) * cells, pair, g.nx, g.ny, g.nz, nullptr, s);
+            if (rc == cudaSuccess) rc = launch_blend(pair, blend, cells, 1, &e.a, &box, false, s);
+        } else {
+            rc = launch_transpose(f, blend, g.nx, g.ny, g.nz, s);
+        }
+    }
+    float lev[kMaxLevels];
+    if (met->z_levels_host)
+        for (int k = 0; k < g.nz; ++k) lev[k] = (float)met->z_levels_host[k];
+    if (rc == cudaSuccess)
+        rc = launch_test_sample(blend, gridf(g, true, met->z_levels_host ? lev : nullptr), (float)met->kz_min, (const float4 *)xyz, n,
+                                (float4 *)out, s);
+    return rc == cudaSuccess ? LPM_OK : LPM_ERR_CUDA;
+}
