@@ -150,7 +150,9 @@ const char *lpm_status_string(int32_t status);
  * lpm_params, as for lpm_create, not as an argument of its own) (particle SoA store, grids, ledger, scan state,
  * read-out staging, the z-fastest time-blended met buffers (16 bytes per met cell and fused step) and,
  * when meteo->nt > 1, the interleaved snapshot-pair buffer of the current met interval: 32 bytes per
- * met cell).  Only the grid and nt of `meteo` are read. */
+ * met cell).  Only the grid and nt of `meteo` are read.  Errors: INVALID_ARG (as lpm_create for the same arguments;
+ * among them: a met grid of 2^28 cells or more with nt > 1 - the step kernel's 32-bit texel index spans all 16 blended
+ * buffers - or of 2^31 or more cells at all). */
 int32_t lpm_workspace_bytes(const lpm_grid *conc_grid, const lpm_meteo *meteo, const lpm_params *params,
                             int32_t n_nuclides, uint64_t *bytes_host);
 
@@ -175,7 +177,9 @@ int32_t lpm_destroy(lpm_handle *h);
 /* Start the same run again from step 0 on the same handle: the registered releases, the rain box, the grids' geometry and
  * the meteorology stay; the step index, the output grids, the deposition map, the ledger, the injected log and every
  * cached list / blended met buffer are cleared (asynchronously; the particle store needs no clearing: a slot is
- * initialised when its particle is born).  The results of the second run equal those of the first.
+ * initialised when its particle is born).  The results of the second run equal those of the first.  The device-side unit
+ * counters behind lpm_get_timing's [4] and [5] start again at 0 as well: after a restart they count from the restart, while
+ * the times and launch counts keep accumulating since lpm_set_timing (call lpm_set_timing again for a clean slate).
  * Errors: STATE (the particle state was installed by lpm_set_particles: there is no release to start again), CUDA. */
 int32_t lpm_restart(lpm_handle *h);
 
@@ -290,8 +294,11 @@ int32_t lpm_set_timing(lpm_handle *h, int32_t enable);
  * [9]  = total ms of the step launches that carried the fused binning epilogue (slot-addressed store: the launch that
  *        ends on a binning step bins its particles itself; these launches are also part of [0] and [1]),
  * [10] = their count, [11] = total ms of the step launches directly before them (same population to within 16 steps
- *        of births: [9] - [11] estimates what the epilogues cost); accumulated since lpm_set_timing. */
-int32_t lpm_get_timing(lpm_handle *h, double *out_host /* [12] */);
+ *        of births); [12] = born particles x steps (host count, as [8]) of the launches of [9], [13] = of the launches of
+ *        [11].  The last launch of an output interval runs bin_every mod 16 model steps when that is not 0, its
+ *        predecessor 16: compare the two per particle-step, [9] - [11] * [12] / [13] estimates what the epilogues cost
+ *        ([9] - [11] does so only when bin_every is a multiple of the fused step count); accumulated since lpm_set_timing. */
+int32_t lpm_get_timing(lpm_handle *h, double *out_host /* [14] */);
 /* Number of concentration cells that hold at least one particle in the current binning (the footprint the binning
  * atomics spread over: bench.py measures its atomic peak over exactly that many cells).  Synchronises.
  * Errors: STATE (nothing binned yet). */

@@ -318,11 +318,12 @@ class Simulation:
         self._ck(self._L.lpm_set_timing(self._h, 1 if on else 0), "lpm_set_timing")
 
     def get_timing(self):
-        out = (C.c_double * 12)()
+        out = (C.c_double * 14)()
         self._ck(self._L.lpm_get_timing(self._h, out), "lpm_get_timing")
         return dict(step_ms=out[0], step_launches=int(out[1]), bin_ms=out[2], bin_launches=int(out[3]),
                     particle_steps=out[4], binned_particles=out[5], sort_ms=out[6], sort_launches=int(out[7]),
-                    born_particle_steps=out[8], bin_fused_launch_ms=out[9], bin_fused_launches=int(out[10]), bin_fused_prev_launch_ms=out[11])
+                    born_particle_steps=out[8], bin_fused_launch_ms=out[9], bin_fused_launches=int(out[10]), bin_fused_prev_launch_ms=out[11],
+                    bin_fused_born_particle_steps=out[12], bin_fused_prev_born_particle_steps=out[13])
 
     @property
     def touched_cells(self) -> int:

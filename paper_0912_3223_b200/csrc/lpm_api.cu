@@ -117,6 +117,15 @@ bool grid_ok(const lpm_grid *g)
            (uint64_t)g->nx * g->ny * g->nz < (1ull << 31);
 }
 
+// The step kernel addresses the time-blended met buffers with ONE 32-bit texel index that includes the buffer
+// (lpm_step.cu, LPM_IDX32: c.o += e.buf * snap_cells, e.buf < kBlendDepth): with more than one snapshot all kBlendDepth
+// buffers together must stay below 2^32 texels, i.e. the met grid below 2^28 cells (a single snapshot has one buffer).
+bool met_index_ok(const lpm_meteo *met)
+{
+    const uint64_t cells = (uint64_t)met->grid.nx * met->grid.ny * met->grid.nz;
+    return met->nt <= 1 || (uint64_t)kBlendDepth * cells < (1ull << 32);
+}
+
 }  // namespace
 
 struct lpm_handle {
@@ -163,7 +172,7 @@ struct lpm_handle {
     uint64_t launches;
     // timing hooks: event pairs around step / binning launches
     bool timing;
-    struct Span { cudaEvent_t a, b; int kind; bool pre; };   // pre: the step launch right before one with the binning epilogue
+    struct Span { cudaEvent_t a, b; int kind; bool pre; double units; };   // pre: the step launch right before one with the binning epilogue
     std::vector<Span> spans;
     std::vector<cudaEvent_t> ev_pool;
     double t_ms[5], t_units[5];   // kinds: 0 step launches, 1 binning (memset + stand-alone kernel), 2 sorts, 3 step launches with the fused
@@ -210,7 +219,7 @@ cudaEvent_t ev_get(lpm_handle *h)
 int span_open(lpm_handle *h, int kind, double units)
 {
     if (!h->timing) return -1;
-    lpm_handle::Span sp{ev_get(h), ev_get(h), kind, false};
+    lpm_handle::Span sp{ev_get(h), ev_get(h), kind, false, units};
     if (!sp.a || !sp.b) {   // no event to be had: this launch goes untimed (its units are not counted either)
         if (sp.a) h->ev_pool.push_back(sp.a);
         if (sp.b) h->ev_pool.push_back(sp.b);
@@ -237,7 +246,7 @@ void spans_collect(lpm_handle *h)
         if (cudaEventElapsedTime(&ms, sp.a, sp.b) == cudaSuccess) {
             h->t_ms[sp.kind] += (double)ms;
             if (sp.kind == 3) h->t_ms[0] += (double)ms;
-            if (sp.pre) { h->t_ms[4] += (double)ms; h->t_launches[4]++; }
+            if (sp.pre) { h->t_ms[4] += (double)ms; h->t_launches[4]++; h->t_units[4] += sp.units; }
         }
         h->ev_pool.push_back(sp.a);
         h->ev_pool.push_back(sp.b);
@@ -521,6 +530,7 @@ int32_t lpm_workspace_bytes(const lpm_grid *g, const lpm_meteo *met, const lpm_p
 {
     if (!grid_ok(g) || !met || !grid_ok(&met->grid) || met->nt < 1 || !p || !bytes || K < 1 || K > LPM_MAX_NUCLIDES || p->capacity == 0 || p->capacity >= (1ull << 32))
         return LPM_ERR_INVALID_ARG;
+    if (!met_index_ok(met)) return LPM_ERR_INVALID_ARG;
     *bytes = make_layout(*g, *met, p->capacity, K, p->compact != 0, sort_enabled(p), p->dose != 0, zpair_enabled(met, p)).total;
     return LPM_OK;
 }
@@ -549,6 +559,7 @@ int32_t lpm_create(const lpm_grid *cg, const lpm_meteo *met, const lpm_nuclide *
     }
     if (met->nt < 1 || met->nt > 32767 || !met->fields_dev || ((uintptr_t)met->fields_dev & 15) || ((uintptr_t)ws & 255))
         return LPM_ERR_INVALID_ARG;
+    if (!met_index_ok(met)) return LPM_ERR_INVALID_ARG;
     if (!(p->dt > 0) || p->capacity == 0 || p->capacity >= (1ull << 32) || !(met->H_mix > 0) || met->Kh < 0 ||
         (met->nt > 1 && !(met->dt_snap > 0)) || p->bin_every < 0 || p->steps_per_launch < 0 || !(p->h_dep > 0) || p->dep_mode < 0 ||
         p->dep_mode > 1 || p->drift < 0 || p->drift > 1 || (p->drift == 1 && met->kz_mode == 1) || p->texel_pairs < -1 || p->texel_pairs > 1 || p->ground_decay < 0 || p->ground_decay > 1 ||
@@ -639,6 +650,7 @@ int32_t lpm_restart(lpm_handle *h)
     if (h->prm.dose) CK(cudaMemsetAsync(h->ws + L.dose, 0, 8 * cells3 * h->K, h->st));
     h->launches += 4;
     h->step = 0; h->bin_step = 0; h->binned = false;
+    h->t_base = 0; h->t_base_bin = 0;   // the device counters lpm_get_timing subtracts these from were zeroed with the control block
     h->pair_snap = -1; h->blend_n = 0; h->blend_step0 = 0; h->bbox_valid = false;
     h->perm_valid = false; h->perm_n = 0; h->perm_step = 0; h->perm_cur = 0; h->keys_ready = false; h->csort_step = 0;
     for (int k = 0; k < LPM_MAX_NUCLIDES; ++k) { h->dep_ref[k] = 0; h->dep_bound[k] = 0.0; }
@@ -1250,6 +1262,7 @@ int32_t lpm_get_timing(lpm_handle *h, double *out)
     out[4] = h->t_units[0]; out[5] = h->t_units[1];
     out[6] = h->t_ms[2]; out[7] = (double)h->t_launches[2];
     out[9] = h->t_ms[3]; out[10] = (double)h->t_launches[3]; out[11] = h->t_ms[4];
+    out[12] = h->t_units[3]; out[13] = h->t_units[4];
     out[8] = h->t_units[0];   // born particles x steps (host count, R9): includes particles that have left the domain
     // what the kernels counted themselves: particle-steps executed (born AND active), particles binned (active, in the grid)
     uint64_t now[2] = {0, 0};

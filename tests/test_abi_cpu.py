@@ -52,6 +52,28 @@ def test_workspace_bytes_monotone_and_errors():
         lpm.workspace_bytes(w.cgrid, 10, 3, False)
 
 
+def test_met_grid_beyond_the_32_bit_texel_index_is_refused():
+    """The step kernel folds the blended-buffer number into one 32-bit texel index (16 buffers when nt > 1): a met grid of
+    2^28 cells or more with several snapshots must be refused, not gathered from wrapped addresses.  With one snapshot
+    there is one buffer, and the limit is grid_ok's 2^31."""
+    from workloads import Grid
+    cg = Grid(8, 8, 4, 0.0, 0.0, 0.0, 100.0, 100.0, 100.0)
+    at = Grid(1024, 1024, 256, 0.0, 0.0, 0.0, 100.0, 100.0, 10.0)        # 2^28 cells
+    below = Grid(1024, 1024, 255, 0.0, 0.0, 0.0, 100.0, 100.0, 10.0)
+    with pytest.raises(lpm.LpmError):
+        lpm.workspace_bytes(cg, 1000, 1, False, mgrid=at, nt=2)
+    assert lpm.workspace_bytes(cg, 1000, 1, False, mgrid=below, nt=2) > 16 * 16 * 1024 * 1024 * 255
+    assert lpm.workspace_bytes(cg, 1000, 1, False, mgrid=at, nt=1) > 16 * 1024 * 1024 * 256
+    # straight through the C ABI: lpm_create refuses the same grid before it looks for a device
+    L = binding.load()
+    met = binding.lpm_meteo(grid=binding._grid(at), nt=2, t0=0.0, dt_snap=3600.0, fields_dev=256, Kh=1.0, H_mix=1000.0, kz_min=0.0)
+    nuc = (binding.lpm_nuclide * 1)(binding.lpm_nuclide(1.0, 0.0, 0.0))
+    prm = binding.lpm_params(dt=1.0, seed=1, capacity=16, h_dep=1000.0)
+    h = ctypes.c_void_p()
+    rc = L.lpm_create(ctypes.byref(binding._grid(cg)), ctypes.byref(met), nuc, 1, ctypes.byref(prm), 256, 1 << 40, None, ctypes.byref(h))
+    assert rc == binding.ERR_INVALID_ARG and not h.value
+
+
 def test_workspace_bytes_texel_pairs_rule():
     """lpm_params.texel_pairs (B8): 16 more bytes per met cell and fused step when on; auto from
     capacity >= 16 x met cells; never for the physics the pair kernels are not instantiated for."""

@@ -302,6 +302,33 @@ def test_restart_equals_a_fresh_simulation(lpm):
     np.testing.assert_allclose(a.ledger(), ref[3], rtol=1e-9)
 
 
+def test_unit_counters_after_a_restart(lpm):
+    """lpm_restart zeroes the control block, and with it the device-side counters of executed particle-steps and binned
+    particles; lpm_get_timing subtracts the values they had at lpm_set_timing.  Without resetting those bases a restart
+    made the difference wrap to about 1.8e19.  After a restart the counters count from the restart: the same run gives the
+    same counts.  Also: the born particle-steps of the launches that carry the binning epilogue and of their predecessors
+    (bench.py scales the predecessor's time by their ratio; bin_every = 200 = 12 x 16 + 8 makes the two launches differ)."""
+    w = make("c3", scale=2e-3, n_steps=400).replace(nt=3, bin_every=200)
+    a = lpm.Simulation(w)
+    a.step(48)
+    a.set_timing(True)              # bases taken in mid-run, not at zero
+    a.step(352)
+    t1 = a.get_timing()
+    assert 0 < t1["particle_steps"] <= t1["born_particle_steps"] < 2 ** 52 and 0 < t1["binned_particles"] < 2 ** 52
+    assert t1["bin_fused_launches"] == 2
+    f, p = t1["bin_fused_born_particle_steps"], t1["bin_fused_prev_born_particle_steps"]
+    assert 0 < f <= 1.2 * p and f + p < t1["born_particle_steps"]
+    a.restart()
+    a.step(400)
+    t2 = a.get_timing()
+    b = lpm.Simulation(w)
+    b.set_timing(True)
+    b.step(400)
+    t3 = b.get_timing()
+    assert t2["particle_steps"] == t3["particle_steps"] > t1["particle_steps"]
+    assert t2["binned_particles"] == t3["binned_particles"] > 0
+
+
 # ------------------------------------------------------------------ exited slots leave the sorted list; device-side unit counters
 def test_absorbed_slots_leave_the_sorted_list_and_the_unit_count(lpm, orc):
     """Slot-addressed store with ABSORB (c3 / c4 since round 2): particles that left the domain are dropped from the
