@@ -208,14 +208,18 @@ int32_t lpm_step(lpm_handle *h, int32_t n_steps);
 /* ---- outputs -------------------------------------------------------------------------------- */
 
 /* Concentration in Bq m^-3, float [K][nz][ny][nx], of the particle state at the current step
- * (re-bins first if the internal grid is stale). */
+ * (re-bins first if the internal grid is stale).  P:L108 "At the end of every n-th time step the activity of particles
+ * is calculated ... Activities or masses of particles are summarized on a rectangular grid"; P:L136-138 (the fields on
+ * a 3-D grid that the paper compares cell by cell). */
 int32_t lpm_concentration(lpm_handle *h, float *out_dev);
 /* Time-integrated concentration in Bq s m^-3, float [K][nz][ny][nx]: sum over the cadence binnings so far
  * of (concentration at that binning) x (bin_every * dt) (rectangle rule; needs params.dose = 1, else STATE). */
 int32_t lpm_dose(lpm_handle *h, float *out_dev);
-/* Particle counts per cell, uint32 [nz][ny][nx], same snapshot rule. */
+/* Particle counts per cell, uint32 [nz][ny][nx], same snapshot rule (the same summation with weight 1 per
+ * active particle - the sample size behind each cell of the grid of P:L136). */
 int32_t lpm_counts(lpm_handle *h, uint32_t *out_dev);
-/* Deposited activity in Bq m^-2, float [K][ny][nx]: cumulative and never decayed with params.ground_decay = 0 (default);
+/* Deposited activity in Bq m^-2, float [K][ny][nx] ("finally testing for dry and wet depositions", P:L84-86
+ * "remove from the atmosphere to the surface by dry and wet pathways"): cumulative and never decayed with params.ground_decay = 0 (default);
  * with ground_decay = 1 what lies on the ground keeps decaying and the map is returned as it is at the current time. */
 int32_t lpm_deposition(lpm_handle *h, float *out_dev);
 /* Same map at full precision, double [K][ny][nx] (the accumulator itself, scaled by 1/area). */

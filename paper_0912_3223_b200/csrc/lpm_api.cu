@@ -118,7 +118,7 @@ bool grid_ok(const lpm_grid *g)
 }
 
 // The step kernel addresses the time-blended met buffers with ONE 32-bit texel index that includes the buffer
-// (lpm_step.cu, LPM_IDX32: c.o += e.buf * snap_cells, e.buf < kBlendDepth): with more than one snapshot all kBlendDepth
+// (lpm_step.cu, step_once: c.o += e.buf * snap_cells, e.buf < kBlendDepth): with more than one snapshot all kBlendDepth
 // buffers together must stay below 2^32 texels, i.e. the met grid below 2^28 cells (a single snapshot has one buffer).
 bool met_index_ok(const lpm_meteo *met)
 {

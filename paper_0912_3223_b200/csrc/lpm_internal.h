@@ -11,12 +11,6 @@
 #ifndef LPM_FUSED_LONG
 #define LPM_FUSED_LONG 64
 #endif
-#ifndef LPM_LEGACY_KERNEL
-#define LPM_FMA2 1
-#define LPM_SQRT_MUFU 1
-#define LPM_IDX32 1
-#define LPM_DEPWIN 1
-#endif
 
 namespace lpm {
 

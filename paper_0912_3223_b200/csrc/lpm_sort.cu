@@ -1,13 +1,15 @@
 // lpm_sort.cu — gather-locality pass of the step (pulled into the hot path).
 //
-// The particle store stays in particle-id order (slot l <-> id, R9), but before a fused launch the
+// The particle store stays in particle-id order (slot l <-> id, R9), but every 32 to 64 model steps the
 // slots are listed in order of the MET CELL their particle sits in (counting sort of 4-byte slot
 // indices: histogram -> exclusive scan -> scatter).  The step kernel then walks that list, so the
-// 32 lanes of a warp sample the same or neighbouring texels: one or two L1 wavefronts per gather
-// instead of one per lane, and the texels stay in L1.  Only indices move; the 16-24 B particle
-// records are read and written in place (a scattered 16 B access per particle per launch of up to
-// 96 steps is noise).  The paper relied on the texture cache for locality; this is
-// its sm_100a counterpart.
+// 32 lanes of a warp sample the same or neighbouring texels and the texels stay in L1.  What that buys, as
+// measured (profiles/r02_c4_step_kernel_ncu.md): a 32-byte gather request of a warp touches about 19 distinct
+// sectors in about 5 distinct 128-byte lines and costs about 22 L1 wavefronts - the lanes of a warp are neighbours, not
+// twins, so the gathers are NOT down to one or two wavefronts; the gain is the L1 hit rate and the line count.
+// Only indices move; the 16-24 B particle records are read and written in place (a scattered 16 B access per
+// particle per launch of up to 16 fused steps).  The paper relied on the texture cache for locality (P:L110,
+// P:L148); this is its sm_100a counterpart.
 #include "lpm_device.cuh"
 
 namespace lpm {

@@ -44,10 +44,8 @@ struct Acc {  // per-thread ledger partial sums, in activity units before the pe
 // per increment, unbiased; B4); smaller ones (a particle that carries < 1/8 of the
 // largest activity), increments that do not fit and a full table take the direct fp64 RED.
 constexpr int kDepSlots = 1024;
-[[maybe_unused]] constexpr int kDepSlotBits = 10, kDepProbes = 8;   // (open-addressing form of the table: LPM_LEGACY_KERNEL)
 static_assert(kStepThreads * kMaxFused <= 4096, "fixed-point deposit sums: 20 bits + 12 bits of count");
 
-#ifdef LPM_DEPWIN
 // Direct-mapped form of the table: the particles of a tile are spatial neighbours, so their deposits of one launch fall
 // into a window of kDepWin x kDepWin map cells around the tile; slot = (cj - wj0) * kDepWin + (ci - wi0), no tags, no
 // probing.  The window is centred on the map cell of the tile's first live particle (dep_window, once per tile); a deposit
@@ -137,88 +135,6 @@ __device__ __forceinline__ void deposit_at(const StepArgs &A, const StepEntry &e
         if (WET) dep_add<K>(A, T, slot, cell, k, 2 * k + 1, vw[k]);
     }
 }
-#else
-// Dry and wet increments differ by orders of magnitude (p_dry ~ 5e-6, p_wet ~ 5e-4 per step), so each
-// has its own scale and its own sum: slot word 2k = dry, 2k + 1 = wet deposit of nuclide k.
-template <int K>
-struct DepTab {
-    uint32_t tag[kDepSlots];           // map cell + 1, 0 = empty
-    uint32_t sum[2 * K][kDepSlots];
-};
-
-template <int K>
-__device__ __forceinline__ void dep_clear(DepTab<K> &T)
-{
-    for (int i = threadIdx.x; i < kDepSlots; i += kStepThreads) {
-        T.tag[i] = 0u;
-#pragma unroll
-        for (int k = 0; k < 2 * K; ++k) T.sum[k][i] = 0u;
-    }
-}
-
-// all threads of the CTA; barriers on both sides belong to the caller
-template <int K>
-__device__ __forceinline__ void dep_flush(const StepArgs &A, DepTab<K> &T)
-{
-    for (int i = threadIdx.x; i < kDepSlots; i += kStepThreads) {
-        const uint32_t key = T.tag[i];
-        if (key == 0u) continue;
-        T.tag[i] = 0u;
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-            const uint32_t vd = T.sum[2 * k][i], vw = T.sum[2 * k + 1][i];
-            T.sum[2 * k][i] = 0u; T.sum[2 * k + 1][i] = 0u;
-            if (vd | vw) atomicAdd(A.dep + (key - 1u) + k * A.dep_stride, (double)vd * A.dep_inv_scale[2 * k] + (double)vw * A.dep_inv_scale[2 * k + 1]);
-        }
-    }
-}
-
-// one increment v (already scaled) into word w of the slot, or straight to the map
-template <int K>
-__device__ __forceinline__ void dep_add(const StepArgs &A, DepTab<K> &T, int slot, uint32_t cell, int k, int w, float v)
-{
-    const uint32_t iv = __float2uint_rn(v);  // saturating; v >= 0
-    if (slot >= 0 && iv - 131072u < 1048576u - 131072u) atomicAdd(&T.sum[w][slot], iv);   // 2^17 <= iv < 2^20: one unsigned compare
-    else if (v != 0.0f) atomicAdd(A.dep + cell + k * A.dep_stride, (double)v * A.dep_inv_scale[w]);
-}
-
-// add one particle-step's deposit to the map cell of the NEW (x, y); vd[k], vw[k] = dry and wet
-// increment of nuclide k in the fixed-point units of their sums
-template <int K, bool WET>
-__device__ __forceinline__ void deposit_at(const StepArgs &A, const StepEntry &e, float x, float y, const float (&vd)[K], const float (&vw)[K],
-                                           Acc<K> &acc, DepTab<K> &T)
-{
-    const int ci = cell_of(x, A.cg.x0, A.cg.inv_dx, A.cg.nx);
-    const int cj = cell_of(y, A.cg.y0, A.cg.inv_dy, A.cg.ny);
-    if ((ci | cj) < 0) {  // off the map: ledger only
-#pragma unroll
-        for (int k = 0; k < K; ++k) {
-            acc.off[k] += vd[k] * e.Oid[k];
-            if (WET) acc.off[k] += vw[k] * e.Oiw[k];
-        }
-        return;
-    }
-    const uint32_t cell = (uint32_t)(cj * A.cg.nx + ci), key = cell + 1u;
-    uint32_t h = (key * 0x9E3779B1u) >> (32 - kDepSlotBits);
-    int slot = -1;
-#pragma unroll 1
-    for (int p = 0; p < kDepProbes; ++p) {
-        const uint32_t t = *(volatile uint32_t *)&T.tag[h];
-        if (t == key) { slot = (int)h; break; }
-        if (t == 0u) {
-            const uint32_t old = atomicCAS(&T.tag[h], 0u, key);
-            if (old == 0u || old == key) { slot = (int)h; break; }
-        }
-        h = (h + 1u) & (kDepSlots - 1);
-    }
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-        dep_add<K>(A, T, slot, cell, k, 2 * k, vd[k]);
-        if (WET) dep_add<K>(A, T, slot, cell, k, 2 * k + 1, vw[k]);
-    }
-}
-
-#endif  // LPM_DEPWIN
 
 // One model step of one particle.  Returns false when the particle left the domain (ABSORB).
 // Source order = intended issue order: the eight gathers go out first and the ~150 instructions of
@@ -229,18 +145,12 @@ __device__ __forceinline__ bool step_once(const StepArgs &A, const StepEntry &e,
                                           float (&q)[K], Acc<K> &acc, DepTab<K> &dep)
 {
     // a0 + a2: weather at X_old, t_n
-#ifdef LPM_IDX32
     Corner c = corner_of<ZLEV>(A.mg, x, y, z);
     float dkz = 0.0f;  // drift-corrected walk (labelled departure): dKz/dz of the sampled field
     const uint32_t o_cell = c.o;
     c.o += e.buf * (uint32_t)A.snap_cells;   // texel index inside the whole set of blended buffers (< 2^32: lpm_create)
     const float4 m = trilinear<ZP>(A.blend, c, A.mg, ZLEV && A.drift != 0, &dkz);
     c.o = o_cell;
-#else
-    const Corner c = corner_of<ZLEV>(A.mg, x, y, z);
-    float dkz = 0.0f;  // drift-corrected walk (labelled departure): dKz/dz of the sampled field
-    const float4 m = trilinear<ZP>(A.blend + (ZP ? 2ull : 1ull) * (uint64_t)e.buf * A.snap_cells, c, A.mg, ZLEV && A.drift != 0, &dkz);
-#endif
     // Kz: the interpolated gridded field (R4), or Eq.(3) per particle from the 2-D fields of this step (R12)
     const float kz = fmaxf(EQ3 ? kz_eq3(A.surf + (uint64_t)e.buf * (uint32_t)(A.mg.nx * A.mg.ny), c, A.mg, z) : m.w, A.kz_min);
 
@@ -539,9 +449,7 @@ __global__ void __launch_bounds__(kStepThreads, LPM_STEP_MINB) step_slots_kernel
                 valid = z >= 0.0f;  // z < 0: exited earlier (ABSORB without compaction)
             }
         }
-#ifdef LPM_DEPWIN
         if (A.any_dep) dep_window<K>(A, T, valid, x, y);
-#endif
         if (valid) {
             // the trip count is the same for every thread (uniform table index, uniform branches inside
             // the step); a particle born inside this launch or absorbed at the boundary skips steps
@@ -659,9 +567,7 @@ __global__ void __launch_bounds__(kStepThreads) step_compact_kernel(const __grid
                 pid[j] = A.pid[i];
             }
         }
-#ifdef LPM_DEPWIN
         if (A.any_dep) dep_window<K>(A, T, (uint64_t)tile * kScanTile + threadIdx.x < n, x[0], y[0]);
-#endif
 #pragma unroll
         for (int j = 0; j < kItems; ++j) {
             const uint64_t i = (uint64_t)tile * kScanTile + (uint32_t)j * kStepThreads + threadIdx.x;
