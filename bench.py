@@ -195,7 +195,8 @@ class Looped:
     the config does not have.  Per-handle timing totals are carried over the restarts."""
 
     KEYS = ("step_ms", "step_launches", "bin_ms", "bin_launches", "particle_steps", "binned_particles", "sort_ms", "sort_launches",
-            "born_particle_steps", "bin_fused_launch_ms", "bin_fused_launches", "bin_fused_prev_launch_ms")
+            "born_particle_steps", "bin_fused_launch_ms", "bin_fused_launches", "bin_fused_prev_launch_ms",
+            "bin_fused_born_particle_steps", "bin_fused_prev_born_particle_steps")
 
     def __init__(self, sim, n_int, on_restart=None):
         self.sim, self.n_int, self.i, self.on_restart = sim, n_int, 0, on_restart
@@ -333,7 +334,10 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     total_mass = float(conc_dev.sum().item())
     touched = sim.touched_cells                       # cells that hold a particle in the last binning (untimed)
-    # the stand-alone binning kernel (lpm_bin_now: what a caller gets outside the cadence) on the final state, untimed region
+    # the stand-alone binning kernel (lpm_bin_now: what a caller gets outside the cadence), untimed region, on a FIXED state:
+    # the end of the config (the run started again and taken through all its intervals), not wherever the timed loop stopped
+    sim.restart()
+    sim.step(n_int * interval)
     sim.set_timing(True)
     sb0, sb1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sim.bin_now()
@@ -344,6 +348,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     standalone_ms = sb0.elapsed_time(sb1) / 3.0
     standalone_n = sim.get_timing()["binned_particles"] / 4.0
+    touched_sa = sim.touched_cells
     # fraction of the active particles that sit inside the met box: 1 by construction where leaving makes a particle inactive
     # (ABSORB: c3, c4, c5); measured on the final state of this leg where the boundary is OPEN (c1, c2)
     if w.boundary_mode == "absorb":
@@ -483,9 +488,10 @@ def run_ours(args):
     grid_bytes = (4 + 8 * w.K) * g.nx * g.ny * g.nz
     red_rate = probes.get("red_f64_touched_footprint_per_s")
 
-    def bin_roof(n_particles, n_launches):
-        t_hbm = (bpp * n_particles + n_launches * grid_bytes) / (pk["hbm_gbs"] * 1e9)
-        t_atom = n_launches * touched * (1 + w.K) / red_rate if red_rate else None
+    def bin_roof(n_particles, n_launches, cells=None, memset=True):
+        cells = touched if cells is None else cells
+        t_hbm = (bpp * n_particles + (n_launches * grid_bytes if memset else 0)) / (pk["hbm_gbs"] * 1e9)
+        t_atom = n_launches * cells * (1 + w.K) / red_rate if red_rate else None
         return t_hbm, t_atom, (max(t_hbm, t_atom) if t_atom else t_hbm)
 
     n_bin = b_units / world                                   # particles binned in the timed region (active, inside the grid)
@@ -506,7 +512,14 @@ def run_ours(args):
         measured_ms = bin_ms
         t_hbm, t_atom, t_roof = bin_roof(n_bin, max(tim["bin_launches"], 1))
         design = "stand-alone bin_tile_kernel on the compact (physically sorted) store"
-    sa_hbm, sa_atom, sa_roof = bin_roof(standalone_n, 1)
+    sa_hbm, sa_atom, sa_roof = bin_roof(standalone_n, 1, cells=touched_sa)
+    # the kernel work alone: particle records at HBM peak or one RED per touched cell and field, against the epilogue time -
+    # no grid memset in the roof or in the measured time (where zeroing dominates the other fraction says nothing about the kernel)
+    ko = None
+    if fused_n and epi_ms > 0:
+        k_hbm, k_atom, k_roof = bin_roof(n_bin, fused_n, memset=False)
+        ko = {"roof_ms": k_roof * 1e3, "measured_ms": epi_ms, "frac": k_roof * 1e3 / epi_ms, "hbm_ms": k_hbm * 1e3,
+              "atomic_ms": k_atom * 1e3 if k_atom else None, "per_binning_ms": epi_ms / fused_n}
     binning = {"kernel": "step_slots_kernel epilogue (bin_tile)" if fused_n else "bin_tile_kernel", "design": design,
                "gbs": bpp * n_bin / (measured_ms * 1e-3) / 1e9 if measured_ms > 0 else None,
                "measured_ms": measured_ms, "launches": fused_n or tim["bin_launches"], "memset_ms": bin_ms if fused_n else None,
@@ -517,7 +530,9 @@ def run_ours(args):
                             "hbm_ms": t_hbm * 1e3, "atomic_ms": t_atom * 1e3 if t_atom else None, "atomics_per_touched_cell": 1 + w.K,
                             "atomic_peak_per_s": red_rate, "atomic_peak_source": "lpm_probe red.global.add.f64, random addresses over "
                             "touched cells x (4 + 8 K) bytes (the footprint of the last binning, measured in this run)"},
-               "standalone": {"kernel": "bin_tile_kernel (lpm_bin_now on the final state, average of 3, outside the timed region)",
+               "kernel_only": ko,
+               "standalone": {"kernel": "bin_tile_kernel (lpm_bin_now on the state at the END of the config, average of 3, outside the timed region)",
+                              "touched_cells": touched_sa,
                               "ms": standalone_ms, "particles": standalone_n, "gbs": bpp * standalone_n / (standalone_ms * 1e-3) / 1e9,
                               "roof_ms": sa_roof * 1e3, "frac": sa_roof * 1e3 / standalone_ms if standalone_ms > 0 else None},
                "note": "fused: measured = sum over the intervals of (step launch with the epilogue - the step launch before it x epilogue_unit_ratio, "
@@ -590,6 +605,23 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def spawn_ranks(n):
+    """`python bench.py --gpus N` without torchrun: start the N ranks ourselves (the same launch the driver uses: one rank per
+    GPU under torch.distributed.run, rendezvous on 127.0.0.1) and wait for them; rank 0 prints the JSON line."""
+    import socket
+    import subprocess
+    import torch
+    have = torch.cuda.device_count()
+    if have < n:
+        raise SystemExit(f"bench.py: --gpus {n} but only {have} CUDA device(s) are visible")
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -609,6 +641,8 @@ def main():
         print(f"note: --warmup {args.warmup} < 3; timing rules ask for at least 3", file=sys.stderr)
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args.gpus)
     else:
         run_ours(args)
 

@@ -65,13 +65,17 @@ def _conc_face_slack(p, g, K, delta):
     ("c2", 0.1, 1, 1440, 3),            # the whole 2 h run, 1e5 particles
     ("c3", 1.0, 10, 2520, 9),           # 7 h: dry deposition, the first hour of rain, particles leaving the domain
     ("c4", 1.0, 20, 1440, 3),           # 2 h on the 1000 x 1000 x 30 grid of 100 m cells
+    ("c4", 1.0, 100, 8640, 13),         # the WHOLE 12 h of BASELINE config 4 on every 100th id: rain, exits, all 13 snapshots
 ])
 def test_concentration_field_end_to_end(lpm, orc, name, scale, stride, steps, nt):
     """The paper's own comparison (Fig. 4: relative difference per cell, poorly populated cells masked out):
     after N steps the concentration field of the CUDA path equals the oracle's on every cell with count >= 100 to
     1e-5 relative + face slack (activity of oracle particles within 1.5 m of a cell face: 1e-5 of the 100 km domain
-    is 1 m of position tolerance).  The 0.1 % of particles T3 lets outside the position band may sit in a wrong cell:
-    their total (missing in one cell, extra in another) stays below 2e-3 of the binned activity."""
+    is 1 m of position tolerance).  The 0.1 % of particles T3 lets outside the position band ("far": position off by
+    more than the 1.5 m the slack covers, another status, or activity off by more than 1e-5 - identified here particle by
+    particle, the premise far <= 1e-3 asserted) may sit in a wrong cell: their total (missing in one cell, extra in
+    another) stays below 2e-3 of the binned activity, and that aggregate is the bar ONLY for cells a far particle touches.
+    EVERY other cell with count >= 100 and no slack must agree to 1e-5 (+ the fp32 read-out): 100 % of them, not 99 %."""
     w = make(name, scale=scale, n_steps=steps)
     w.release.pid_stride = stride
     n_local = len(range(0, w.release.n_particles, stride))
@@ -86,16 +90,34 @@ def test_concentration_field_end_to_end(lpm, orc, name, scale, stride, steps, nt
     slack = _conc_face_slack(o.particles(), g, w.K, 1.5)
     big = no >= 100
     assert big.sum() >= 10, big.sum()
+    # far particles, and the cells they touch in either run
+    gp, p = gpu_state(sim), o.particles()
+    assert np.array_equal(gp["pid"], p["pid"])
+    act_o, act_g = p["status"] == 0, gp["status"] == 0
+    dpos = np.max([np.abs(gp[a].astype(np.float64) - p[a]) for a in ("x", "y", "z")], axis=0)
+    mrel = (np.abs(gp["m"] - p["m"]) / np.maximum(p["m"], 1e-300)).max(axis=0)
+    far = (act_o != act_g) | (act_o & act_g & ((dpos > 1.5) | (mrel > 1e-5)))
+    assert far.mean() <= 1e-3, far.mean()
+    touch = np.zeros((g.nz, g.ny, g.nx), dtype=bool)
+    for src, act in ((p, act_o), (gp, act_g)):
+        sel = far & act
+        ii = np.floor((src["x"][sel].astype(np.float64) - g.x0) / g.dx).astype(np.int64)
+        jj = np.floor((src["y"][sel].astype(np.float64) - g.y0) / g.dy).astype(np.int64)
+        kk = np.floor((src["z"][sel].astype(np.float64) - g.z0) / g.dz).astype(np.int64)
+        okc = (ii >= 0) & (ii < g.nx) & (jj >= 0) & (jj < g.ny) & (kk >= 0) & (kk < g.nz)
+        touch[kk[okc], jj[okc], ii[okc]] = True
     tot_ok = 0
     for k in range(w.K):
         tol = 1e-5 * co[k] + 1.0001 * slack[k] + 3e-7 * co[k]                  # (+ the fp32 read-out of the CUDA path)
         excess = np.maximum(np.abs(cg[k] - co[k]) - tol, 0.0)
         assert excess[big].sum() <= 2e-3 * co[k][big].sum(), (k, excess[big].sum() / co[k][big].sum())
-        clean = big & (slack[k] == 0.0)
+        assert excess[big & ~touch].sum() <= 1e-9 * co[k][big].sum(), (k, excess[big & ~touch].max())   # the slack bound alone, where no far particle is
+        clean = big & (slack[k] == 0.0) & ~touch
         if clean.sum():
             rel = np.abs(cg[k][clean] / co[k][clean] - 1.0)
             tot_ok += int((rel <= 1.1e-5).sum())
-            assert (rel <= 1.1e-5).mean() >= 0.99, (k, rel.max())
+            bad = np.argwhere(clean)[rel > 1.1e-5]
+            assert len(bad) == 0, (k, len(bad), int(clean.sum()), rel.max(), bad[:5].tolist(), [int(no[tuple(b)]) for b in bad[:5]])
         rel_all = np.abs(cg[k][big] / co[k][big] - 1.0)
         # the paper's figure of merit (~90 % of the cells differ by < 2.5 % on its hardware)
         assert (rel_all < 0.025).mean() >= 0.999, (k, (rel_all < 0.025).mean())
@@ -103,7 +125,8 @@ def test_concentration_field_end_to_end(lpm, orc, name, scale, stride, steps, nt
     # counts: equal except where a particle sits within the position tolerance of a face
     assert abs(int(ng.sum()) - int(no.sum())) <= 2 + 1e-4 * no.sum()
     assert np.abs(ng - no)[big].sum() <= 2e-3 * no[big].sum()
-    print(f"[conc e2e {name}] cells>=100: {big.sum()}, particles {no.sum()}, count L1 diff {np.abs(ng - no).sum()}")
+    print(f"[conc e2e {name} {steps}] cells>=100: {big.sum()}, clean of them checked to 1e-5: {tot_ok}, far particles {far.sum()} of {len(far)}, "
+          f"cells they touch {touch.sum()}, particles {no.sum()}, count L1 diff {np.abs(ng - no).sum()}")
 
 
 # ------------------------------------------------------------------ c5 on its OWN domain (S§8(d): 1/100-scale full-rate run)
@@ -405,3 +428,57 @@ def test_fused_binning_equals_the_standalone_kernel(lpm, orc, name, scale, nt):
     oc = o.concentration()
     nz = oc > 0
     assert np.array_equal(nz, conc_f > 0) and np.abs(conc_f[nz] / oc[nz] - 1).max() <= 1e-5
+
+
+# ------------------------------------------------------------------ S 8(e): two shards of the CUDA path, summed, equal the unsharded CUDA run
+def test_two_cuda_shards_sum_to_the_unsharded_run(lpm, orc):
+    """P:L63 "each particle can be handled independently": rank r of N simulates the ids r, r + N, ... (lpm_release's
+    pid_offset / pid_stride) and the ranks' grids are summed (one all-reduce per grid; bench.py).  Here both shards run on this
+    one device, one after the other - they share nothing, so this is what two GPUs compute.  Philox is keyed by the global id:
+    the union of the shards' particles is the unsharded run's set bit for bit; counts add up exactly; concentration,
+    totals to 1e-6, cells to the fixed-point rounding of the tile tables.  And the summed field equals the oracle's unsharded one."""
+    steps = 720
+    w = make("c3", scale=0.02, n_steps=steps).replace(nt=4, bin_every=360)
+    N = w.release.n_particles
+    full = lpm.Simulation(w)
+    full.step(steps)
+    fp = gpu_state(full)
+    c_full, n_full = full.concentration().cpu().numpy().astype(np.float64), full.counts().cpu().numpy().astype(np.int64)
+    d_full, l_full = full.deposition(f64=True).cpu().numpy(), np.array(full.ledger())
+    conc, cnt, dep, led = 0.0, 0, 0.0, 0.0
+    seen = {}
+    for r in range(2):
+        ws = make("c3", scale=0.02, n_steps=steps)
+        ws.release.pid_offset, ws.release.pid_stride = r, 2
+        ws = ws.replace(nt=4, bin_every=360, capacity=len(range(r, N, 2)))
+        sh = lpm.Simulation(ws)
+        sh.step(steps)
+        sp = gpu_state(sh)
+        assert np.array_equal(sp["pid"], np.arange(r, N, 2)[:len(sp["pid"])])
+        for key in ("x", "y", "z", "status"):
+            np.testing.assert_array_equal(sp[key], fp[key][sp["pid"].astype(np.int64)], err_msg=f"shard {r} {key}")
+        np.testing.assert_array_equal(sp["q"], fp["q"][:, sp["pid"].astype(np.int64)])
+        seen[r] = len(sp["pid"])
+        conc = conc + sh.concentration().cpu().numpy().astype(np.float64)
+        cnt = cnt + sh.counts().cpu().numpy().astype(np.int64)
+        dep = dep + sh.deposition(f64=True).cpu().numpy()
+        led = led + np.array(sh.ledger())
+    assert seen[0] + seen[1] == len(fp["pid"])
+    np.testing.assert_array_equal(cnt, n_full)
+    # totals to 1e-6.  Per cell: a particle's contribution is rounded to the tile table's fixed point (<= 3.8e-6 relative,
+    # unbiased; DESIGN.md B9 / B10) when it hits the CTA-private table and added exactly when it does not, and which of the two
+    # happens depends on the tile's other particles, i.e. on the sharding: 5e-6 per cell.  The ledger is summed from fp32
+    # per-thread partial sums: 1e-5.
+    assert abs(conc.sum() / c_full.sum() - 1.0) < 1e-6 and abs(dep.sum() / d_full.sum() - 1.0) < 1e-6
+    np.testing.assert_allclose(conc, c_full, rtol=5e-6, atol=1e-6 * c_full.max())
+    np.testing.assert_allclose(dep, d_full, rtol=5e-6, atol=1e-9 * d_full.max())
+    np.testing.assert_allclose(led, l_full, rtol=1e-5, atol=1e-6 * l_full.max())
+    o = orc.OracleSim(w)
+    o.step(steps)
+    co, no = o.concentration(), o.counts().astype(np.int64)
+    assert abs(int(cnt.sum()) - int(no.sum())) <= 2 + 1e-4 * no.sum()
+    big = no >= 100
+    assert big.sum() >= 10
+    for k in range(w.K):
+        assert abs(conc[k].sum() / co[k].sum() - 1.0) < 1e-5
+        assert np.median(np.abs(conc[k][big] / co[k][big] - 1.0)) < 1e-5
