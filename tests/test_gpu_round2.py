@@ -61,13 +61,17 @@ def _conc_face_slack(p, g, K, delta):
     return slack
 
 
-@pytest.mark.parametrize("name,scale,stride,steps,nt", [
-    ("c2", 0.1, 1, 1440, 3),            # the whole 2 h run, 1e5 particles
-    ("c3", 1.0, 10, 2520, 9),           # 7 h: dry deposition, the first hour of rain, particles leaving the domain
-    ("c4", 1.0, 20, 1440, 3),           # 2 h on the 1000 x 1000 x 30 grid of 100 m cells
-    ("c4", 1.0, 100, 8640, 13),         # the WHOLE 12 h of BASELINE config 4 on every 100th id: rain, exits, all 13 snapshots
+@pytest.mark.parametrize("name,scale,stride,steps,nt,min_count", [
+    ("c2", 0.1, 1, 1440, 3, 100),       # the whole 2 h run, 1e5 particles
+    ("c3", 1.0, 10, 2520, 9, 100),      # 7 h: dry deposition, the first hour of rain, particles leaving the domain
+    ("c4", 1.0, 20, 1440, 3, 100),      # 2 h on the 1000 x 1000 x 30 grid of 100 m cells
+    # the WHOLE 12 h of BASELINE config 4 on every 100th id: rain, exits, all 13 snapshots.  231 particles are born per step and
+    # the release lasts the 12 h, so only the 3 cells next to the source ever hold 100 of them: cells from 20 particles on are
+    # compared (the count threshold masks sampling noise in the paper's comparison of two random runs; here both runs
+    # draw the same numbers, and a cell of n in-tolerance particles agrees to 1e-5 whatever n is)
+    ("c4", 1.0, 100, 8640, 13, 20),
 ])
-def test_concentration_field_end_to_end(lpm, orc, name, scale, stride, steps, nt):
+def test_concentration_field_end_to_end(lpm, orc, name, scale, stride, steps, nt, min_count):
     """The paper's own comparison (Fig. 4: relative difference per cell, poorly populated cells masked out):
     after N steps the concentration field of the CUDA path equals the oracle's on every cell with count >= 100 to
     1e-5 relative + face slack (activity of oracle particles within 1.5 m of a cell face: 1e-5 of the 100 km domain
@@ -88,7 +92,7 @@ def test_concentration_field_end_to_end(lpm, orc, name, scale, stride, steps, nt
     cg, co = sim.concentration().cpu().numpy().astype(np.float64) * V, o.concentration() * V      # activity per cell
     ng, no = sim.counts().cpu().numpy().astype(np.int64), o.counts().astype(np.int64)
     slack = _conc_face_slack(o.particles(), g, w.K, 1.5)
-    big = no >= 100
+    big = no >= min_count
     assert big.sum() >= 10, big.sum()
     # far particles, and the cells they touch in either run
     gp, p = gpu_state(sim), o.particles()
