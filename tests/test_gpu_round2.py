@@ -115,7 +115,10 @@ def test_concentration_field_end_to_end(lpm, orc, name, scale, stride, steps, nt
         tol = 1e-5 * co[k] + 1.0001 * slack[k] + 3e-7 * co[k]                  # (+ the fp32 read-out of the CUDA path)
         excess = np.maximum(np.abs(cg[k] - co[k]) - tol, 0.0)
         assert excess[big].sum() <= 2e-3 * co[k][big].sum(), (k, excess[big].sum() / co[k][big].sum())
-        assert excess[big & ~touch].sum() <= 1e-9 * co[k][big].sum(), (k, excess[big & ~touch].max())   # the slack bound alone, where no far particle is
+        # EVERY well-populated cell that no far particle touches: inside 1e-5 + its own face slack, no aggregate.  (Cells with no
+        # slack at all - checked to the bare 1e-5 below - hardly exist: with 100 particles in a 100 m cell one of them is within
+        # 1.5 m of a face almost surely.)
+        assert excess[big & ~touch].sum() <= 1e-9 * co[k][big].sum(), (k, excess[big & ~touch].max())
         clean = big & (slack[k] == 0.0) & ~touch
         if clean.sum():
             rel = np.abs(cg[k][clean] / co[k][clean] - 1.0)
@@ -123,13 +126,16 @@ def test_concentration_field_end_to_end(lpm, orc, name, scale, stride, steps, nt
             bad = np.argwhere(clean)[rel > 1.1e-5]
             assert len(bad) == 0, (k, len(bad), int(clean.sum()), rel.max(), bad[:5].tolist(), [int(no[tuple(b)]) for b in bad[:5]])
         rel_all = np.abs(cg[k][big] / co[k][big] - 1.0)
-        # the paper's figure of merit (~90 % of the cells differ by < 2.5 % on its hardware)
-        assert (rel_all < 0.025).mean() >= 0.999, (k, (rel_all < 0.025).mean())
+        # the paper's figure of merit (~90 % of the cells differ by < 2.5 % on its hardware).  One particle that sits in the
+        # neighbouring cell changes a cell of 20 by 5 %: with the low count threshold of the 12 h case the paper's own 90 % is the bar
+        fom = 0.999 if min_count >= 100 else 0.9
+        assert (rel_all < 0.025).mean() >= fom, (k, (rel_all < 0.025).mean())
         assert abs(cg[k].sum() / co[k].sum() - 1.0) < 1e-5
     # counts: equal except where a particle sits within the position tolerance of a face
     assert abs(int(ng.sum()) - int(no.sum())) <= 2 + 1e-4 * no.sum()
     assert np.abs(ng - no)[big].sum() <= 2e-3 * no[big].sum()
-    print(f"[conc e2e {name} {steps}] cells>=100: {big.sum()}, clean of them checked to 1e-5: {tot_ok}, far particles {far.sum()} of {len(far)}, "
+    print(f"[conc e2e {name} {steps}] cells>={min_count}: {big.sum()}, of them checked to 1e-5 + own face slack: {(big & ~touch).sum()}, "
+          f"without any slack: {tot_ok}, far particles {far.sum()} of {len(far)}, "
           f"cells they touch {touch.sum()}, particles {no.sum()}, count L1 diff {np.abs(ng - no).sum()}")
 
 
