@@ -487,7 +487,7 @@ def test_two_cuda_shards_sum_to_the_unsharded_run(lpm, orc):
     o.step(steps)
     co, no = o.concentration(), o.counts().astype(np.int64)
     assert abs(int(cnt.sum()) - int(no.sum())) <= 2 + 1e-4 * no.sum()
-    big = no >= 100
+    big = no >= 5          # (16667 particles are born in these 2 h: few cells hold many)
     assert big.sum() >= 10
     for k in range(w.K):
         assert abs(conc[k].sum() / co[k].sum() - 1.0) < 1e-5
