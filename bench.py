@@ -571,6 +571,9 @@ def run_ours(args):
         "in_domain_fraction": in_domain, "in_domain_fraction_how": in_domain_how,
         "active_over_born": units / born_units if born_units else None,
         "born_particle_steps": born_units if born_units else None,
+        # the same run in the units of round 1 (every BORN particle x step, whether or not it is still inside the domain): keeps the
+        # rounds comparable across the OPEN -> ABSORB change of c3 / c4; not the headline
+        "born_particle_steps_per_s": born_units / (ms * 1e-3) if born_units and ms > 0 else None,
         "sim_hours_per_s": sim_hours / (ms * 1e-3),
         "e2e": {"value": units_e2e / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                 "ms_per_step": ms_e2e / K, "sim_hours_per_s": sim_hours / (ms_e2e * 1e-3)},
